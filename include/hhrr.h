@@ -1,0 +1,178 @@
+/*
+ * hhrr.h -- C ABI of libhhrr: the fused HHRRLBM + wall-model time step on one B200.
+ *
+ * The calls follow the paper's statement of the problem (arxiv 2510.13726,
+ * /root/reference/PAPER.md): a lattice of given extents, porosity and
+ * solid velocity from a rotor description (Eq. 12-13 :133-140, Def. 1 :196-205,
+ * Fig. 4 :254-269), wall-model cells at the porosity frontier (:157-188, :322-324),
+ * the time loop of Listing 3 (:308-318), and as outputs the velocity moments (:147)
+ * and the per-element integrated boundary force (Eq. 23 :211, :267, :315-317).
+ *
+ * Conventions.  D3Q27, dx = dt = 1, c_s^2 = 1/3.
+ * Cell (x,y,z), linear index  x + nx*(y + ny*z)  (x fastest).  Direction
+ * i = (cx+1) + 3(cy+1) + 9(cz+1), rest i = 13, opposite 26-i, weights
+ * w_i = w(cx)w(cy)w(cz) with w(0)=2/3, w(+-1)=1/6.  Field arguments with several
+ * components are SoA planes: u = [ux(all cells) | uy | uz].
+ *
+ * Memory.  Every pointer argument is a HOST pointer owned by the caller, unless its
+ * name starts with d_ (device pointer, caller-owned).  The library allocates no
+ * lattice-sized device memory: the caller hands hhrr_create() one device workspace
+ * of at least hhrr_workspace_bytes() bytes (256-byte aligned), which the lattice
+ * uses until hhrr_destroy(); the caller frees it afterwards.  All work is issued on
+ * the CUDA stream given to hhrr_create (a cudaStream_t passed as void*; NULL = the
+ * legacy default stream).  Calls that return data to host memory synchronise that
+ * stream; hhrr_step() does not.
+ *
+ * Errors.  Every int-returning call returns HHRR_OK (0) or a negative hhrr_status;
+ * nothing throws or aborts across the ABI.  hhrr_last_error() returns a
+ * thread-local, NUL-terminated message for the last failing call on this thread.
+ * There is no CPU fallback: without a usable CUDA device every call that needs one
+ * fails with HHRR_E_CUDA.
+ */
+#ifndef HHRR_H_
+#define HHRR_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HHRR_Q 27
+#define HHRR_MAX_TAGS 16 /* element tags 1..15; tag 0 = none */
+
+typedef enum {
+  HHRR_OK = 0,
+  HHRR_E_ARG = -1,   /* NULL / out-of-range argument                         */
+  HHRR_E_SIZE = -2,  /* workspace too small or extents overflow int32 cells  */
+  HHRR_E_CUDA = -3,  /* a CUDA runtime call or kernel launch failed          */
+  HHRR_E_NAN = -4,   /* hhrr_check_finite found a non-finite population      */
+  HHRR_E_STATE = -5  /* call not valid in the lattice's current state        */
+} hhrr_status;
+
+/* Outer boundary per axis (reading R12; the paper only names its outer
+ * boundaries).  MIRROR = free-slip symmetry plane half a cell outside
+ * the first / last cell: a population leaving through it returns to the same cell
+ * with that velocity component reversed.                                            */
+typedef enum { HHRR_PERIODIC = 0, HHRR_MIRROR = 1 } hhrr_axis_mode;
+
+/* Cell types of Fig. 4 + the inflow fringe (R12). */
+typedef enum {
+  HHRR_FLUID = 0,    /* d = 1                                                     */
+  HHRR_GROWTH = 1,   /* d = 1, one of the 26 neighbours has phi < eps/2 (:269)    */
+  HHRR_FRONTIER = 2, /* |phi| < eps/2, 0 < d < 1  (Def. 1, Eq. 21-22 :196-203)    */
+  HHRR_SOLID = 3,    /* phi <= -eps/2, d = 0                                      */
+  HHRR_FRINGE = 4    /* d = 0, u^B = u_in                                         */
+} hhrr_cell_type;
+
+typedef struct {
+  int32_t nx, ny, nz;
+  int32_t mode[3];           /* hhrr_axis_mode per axis                                       */
+  double tau0;               /* molecular relaxation time, nu = c_s^2 (tau0 - 1/2)   (Eq. 14) */
+  double sigma;              /* hybridisation factor of Eq. 7, in [0,1]        */
+  double smagorinsky_cs;     /* C_S of Eq. 4                                 */
+  double body_force[3];      /* g, lattice units (R11)                                        */
+  double eps_cells;          /* transition width eps of Def. 1, in cells   */
+  double kappa, E;           /* wall-function constants, 0.41 and 9.8          */
+  int32_t newton_max_iter;   /* 10 in the paper                                */
+  double newton_tol;         /* 1e-4 in the paper                              */
+  double sampling_distance;  /* h_s: wall-model sampling distance along the normal, in cells  */
+} hhrr_params;
+
+/* "Rotor description": a rotor-frame reference grid of signed distances (the paper
+ * keeps it at twice the lattice resolution) with an element tag
+ * per node (:267), rotating rigidly (:265) about `axis` (unit vector) through
+ * `centre` at `omega` rad per step from angle `theta0`.  Node (ix,iy,iz) sits at
+ * rotor-frame position origin + spacing*(ix,iy,iz) relative to the centre, and at
+ * index ix + gx*(iy + gy*iz).  sdf/tag are read during hhrr_set_rotor only.      */
+typedef struct {
+  const float* sdf;
+  const uint8_t* tag;
+  int32_t gx, gy, gz;
+  double spacing;
+  double origin[3];
+  double centre[3], axis[3], omega, theta0;
+  int32_t n_tags; /* tags 1..n_tags are rotor elements (blades, hub) */
+} hhrr_rotor_desc;
+
+typedef struct hhrr_lattice hhrr_lattice; /* opaque, owned by the library */
+
+/* Device bytes hhrr_create needs for `p` (and, if rotor != NULL, for that rotor's
+ * reference grid).  Returns 0 on invalid arguments.                                 */
+size_t hhrr_workspace_bytes(const hhrr_params* p, const hhrr_rotor_desc* rotor);
+
+/* Creates a lattice at rest (f_i = w_i, d = 1, no geometry) in the caller's device
+ * workspace.  `cuda_stream` is a cudaStream_t.                                       */
+int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes, void* cuda_stream,
+                hhrr_lattice** out);
+int hhrr_destroy(hhrr_lattice* L);
+
+/* f = f_eq(rho,u) (Eq. 11); with_neq != 0 adds the regularised
+ * f^(1) of Eq. 8-10 with a1^(2) = -2 rho c_s^2 tau0 S^FD(u).  rho: N, u: 3N floats. */
+int hhrr_init_equilibrium(hhrr_lattice* L, const float* rho, const float* u, int with_neq);
+
+/* Static geometry as a signed-distance field phi (N floats; > 0 fluid).  Types and
+ * porosity follow Def. 1 from phi; tag (N bytes, nullable = all 1) names the element;
+ * d_override (N floats, nullable) replaces the linear ramp of Eq. 22 inside the
+ * transition band (e.g. a tanh ramp).  phi == NULL removes the static geometry.     */
+int hhrr_set_static_geometry(hhrr_lattice* L, const float* phi, const uint8_t* tag,
+                             const float* d_override);
+/* Rigid-body velocity of element `tag`: u^B(x) = vel + omega x (x - centre). */
+int hhrr_set_body(hhrr_lattice* L, int32_t tag, const double centre[3], const double omega[3],
+                  const double vel[3]);
+/* Inflow fringe (R12): cells with x_begin <= x < x_end get d = 0, u^B = u_in. */
+int hhrr_set_fringe(hhrr_lattice* L, int32_t x_begin, int32_t x_end, const double u_in[3]);
+/* Rotor (copied to the device workspace); sets the bodies of tags 1..n_tags. */
+int hhrr_set_rotor(hhrr_lattice* L, const hhrr_rotor_desc* rotor);
+/* Wall model on the cells {FRONTIER, phi > 0} (R13). */
+int hhrr_enable_wall_model(hhrr_lattice* L, int enable);
+/* Evaluates geometry(current step) now (InitializePorosityO). */
+int hhrr_update_geometry(hhrr_lattice* L);
+
+/* n_steps passes of Listing 3: UpdatePorosityO, collide & stream
+ * (Eq. 6-14), WallModelO, boundary-force collection and per-element integration,
+ * rigid rotation.  Asynchronous on the lattice's stream.                            */
+int hhrr_step(hhrr_lattice* L, int32_t n_steps);
+int64_t hhrr_step_count(const hhrr_lattice* L);
+
+/* rho (N) and v = (j + g/2)/rho (3N, SoA) of the current populations. */
+int hhrr_get_moments(hhrr_lattice* L, float* rho, float* v);
+/* Same, into DEVICE buffers, asynchronous on the stream (no host copy). */
+int hhrr_get_moments_device(hhrr_lattice* L, float* d_rho, float* d_v);
+/* Force ON each element per step, F[(s - first_step)*HHRR_MAX_TAGS*3 + tag*3 + a],
+ * for steps first_step .. first_step+n_steps-1 (must lie within the last
+ * hhrr_force_history() steps taken).                                                */
+int hhrr_get_forces(hhrr_lattice* L, int64_t first_step, int64_t n_steps, double* F);
+int64_t hhrr_force_history(void);
+/* Cell types / tags / porosity of the last evaluated geometry (any pointer nullable). */
+int hhrr_get_cell_types(hhrr_lattice* L, uint8_t* type, uint8_t* tag, float* d);
+/* Wall-model cell list in ascending cell index.  *count receives the list length;
+ * at most `capacity` entries are written.  idx: cell index; y1n: 3 doubles per entry
+ * (wall distance times unit normal); u_tau: last friction velocity;
+ * valid: 1 if the cell carries a wall-model state.  Array pointers nullable.         */
+int hhrr_get_wall_list(hhrr_lattice* L, int64_t capacity, int32_t* idx, double* y1n, double* u_tau,
+                       uint8_t* valid, int64_t* count);
+/* Wall-model output of one cell: slip velocity u_wm[3] and strain S_wm[6] (xx yy zz xy xz yz). */
+int hhrr_get_wall_state(hhrr_lattice* L, int64_t cell, double* u_tau, double u_wm[3], double s_wm[6],
+                        int32_t* valid);
+/* Populations as stored: deviations f_i - w_i, 27 planes of N floats (checkpoint / resume). */
+int hhrr_get_populations(hhrr_lattice* L, float* f_minus_w);
+int hhrr_set_populations(hhrr_lattice* L, const float* f_minus_w);
+/* Time-n homogenised velocity field of the last collide (3N floats), for tests. */
+int hhrr_get_uhat(hhrr_lattice* L, float* uhat);
+/* HHRR_E_NAN if any population is non-finite (synchronises). */
+int hhrr_check_finite(hhrr_lattice* L);
+/* Selects the collide-stream kernel: 0 = two-pass (moments pass + collide pass),
+ * 1 = fused sliding-window kernel (default).  Both compute the same step.           */
+int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant);
+/* Number of kernel launches issued by this lattice so far. */
+int64_t hhrr_launch_count(const hhrr_lattice* L);
+
+const char* hhrr_last_error(void);
+const char* hhrr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HHRR_H_ */

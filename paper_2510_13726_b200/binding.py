@@ -1,0 +1,306 @@
+"""Thin ctypes binding of libhhrr.so (include/hhrr.h).  Argument marshalling only: every step
+of the path runs in the CUDA kernels behind the C ABI.  PyTorch is used for the device
+workspace allocation and the CUDA stream, nothing else.
+
+There is no CPU fallback: importing works without a GPU (so the symbol table can be
+checked), but creating a Lattice without the built library or without a CUDA device raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+LIB_PATH = _HERE / "libhhrr.so"
+
+Q = 27
+MAX_TAGS = 16
+FLUID, GROWTH, FRONTIER, SOLID, FRINGE = 0, 1, 2, 3, 4
+PERIODIC, MIRROR = 0, 1
+
+# every symbol include/hhrr.h declares (tests check the library exports exactly these)
+SYMBOLS = [
+    "hhrr_workspace_bytes", "hhrr_create", "hhrr_destroy", "hhrr_init_equilibrium",
+    "hhrr_set_static_geometry", "hhrr_set_body", "hhrr_set_fringe", "hhrr_set_rotor",
+    "hhrr_enable_wall_model", "hhrr_update_geometry", "hhrr_step", "hhrr_step_count",
+    "hhrr_get_moments", "hhrr_get_moments_device", "hhrr_get_forces", "hhrr_force_history",
+    "hhrr_get_cell_types", "hhrr_get_wall_list", "hhrr_get_wall_state", "hhrr_get_populations",
+    "hhrr_set_populations", "hhrr_get_uhat", "hhrr_check_finite", "hhrr_set_kernel_variant",
+    "hhrr_launch_count", "hhrr_last_error", "hhrr_version",
+]
+
+
+class Params(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+                ("mode", C.c_int32 * 3),
+                ("tau0", C.c_double), ("sigma", C.c_double), ("smagorinsky_cs", C.c_double),
+                ("body_force", C.c_double * 3),
+                ("eps_cells", C.c_double),
+                ("kappa", C.c_double), ("E", C.c_double),
+                ("newton_max_iter", C.c_int32), ("newton_tol", C.c_double),
+                ("sampling_distance", C.c_double)]
+
+
+class RotorDesc(C.Structure):
+    _fields_ = [("sdf", C.c_void_p), ("tag", C.c_void_p),
+                ("gx", C.c_int32), ("gy", C.c_int32), ("gz", C.c_int32),
+                ("spacing", C.c_double), ("origin", C.c_double * 3),
+                ("centre", C.c_double * 3), ("axis", C.c_double * 3),
+                ("omega", C.c_double), ("theta0", C.c_double), ("n_tags", C.c_int32)]
+
+
+class HhrrError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"hhrr error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Loads libhhrr.so; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise RuntimeError(f"{LIB_PATH} missing: run `python -m paper_2510_13726_b200.build` "
+                               "(the CUDA library is the only implementation; there is no fallback)")
+        L = C.CDLL(str(LIB_PATH))
+        vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+        L.hhrr_workspace_bytes.restype = C.c_size_t
+        L.hhrr_workspace_bytes.argtypes = [C.POINTER(Params), C.POINTER(RotorDesc)]
+        L.hhrr_create.argtypes = [C.POINTER(Params), vp, C.c_size_t, vp, C.POINTER(vp)]
+        L.hhrr_destroy.argtypes = [vp]
+        L.hhrr_init_equilibrium.argtypes = [vp, vp, vp, C.c_int]
+        L.hhrr_set_static_geometry.argtypes = [vp, vp, vp, vp]
+        L.hhrr_set_body.argtypes = [vp, i32, vp, vp, vp]
+        L.hhrr_set_fringe.argtypes = [vp, i32, i32, vp]
+        L.hhrr_set_rotor.argtypes = [vp, C.POINTER(RotorDesc)]
+        L.hhrr_enable_wall_model.argtypes = [vp, C.c_int]
+        L.hhrr_update_geometry.argtypes = [vp]
+        L.hhrr_step.argtypes = [vp, i32]
+        L.hhrr_step_count.restype = i64
+        L.hhrr_step_count.argtypes = [vp]
+        L.hhrr_get_moments.argtypes = [vp, vp, vp]
+        L.hhrr_get_moments_device.argtypes = [vp, vp, vp]
+        L.hhrr_get_forces.argtypes = [vp, i64, i64, vp]
+        L.hhrr_force_history.restype = i64
+        L.hhrr_get_cell_types.argtypes = [vp, vp, vp, vp]
+        L.hhrr_get_wall_list.argtypes = [vp, i64, vp, vp, vp, vp, C.POINTER(i64)]
+        L.hhrr_get_wall_state.argtypes = [vp, i64, C.POINTER(dbl), vp, vp, C.POINTER(i32)]
+        L.hhrr_get_populations.argtypes = [vp, vp]
+        L.hhrr_set_populations.argtypes = [vp, vp]
+        L.hhrr_get_uhat.argtypes = [vp, vp]
+        L.hhrr_check_finite.argtypes = [vp]
+        L.hhrr_set_kernel_variant.argtypes = [vp, i32]
+        L.hhrr_launch_count.restype = i64
+        L.hhrr_launch_count.argtypes = [vp]
+        L.hhrr_last_error.restype = C.c_char_p
+        L.hhrr_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        raise HhrrError(rc, lib().hhrr_last_error().decode())
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _f32(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.float32)
+
+
+def _f64(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.float64)
+
+
+def make_params(nx, ny, nz, mode=(0, 0, 0), tau0=0.55, sigma=0.995, smagorinsky_cs=0.1,
+                body_force=(0.0, 0.0, 0.0), eps_cells=2.0, kappa=0.41, E=9.8,
+                newton_max_iter=10, newton_tol=1e-4, sampling_distance=2.0) -> Params:
+    p = Params()
+    p.nx, p.ny, p.nz = nx, ny, nz
+    p.mode[:] = list(mode)
+    p.tau0, p.sigma, p.smagorinsky_cs = tau0, sigma, smagorinsky_cs
+    p.body_force[:] = list(body_force)
+    p.eps_cells = eps_cells
+    p.kappa, p.E = kappa, E
+    p.newton_max_iter, p.newton_tol = newton_max_iter, newton_tol
+    p.sampling_distance = sampling_distance
+    return p
+
+
+def _rotor_desc(sdf, tag, spacing, origin, centre, axis, omega, theta0, n_tags):
+    sdf = np.ascontiguousarray(sdf, np.float32)
+    tag = np.ascontiguousarray(tag, np.uint8)
+    gz, gy, gx = sdf.shape
+    r = RotorDesc()
+    r.sdf, r.tag = sdf.ctypes.data, tag.ctypes.data
+    r.gx, r.gy, r.gz = gx, gy, gz
+    r.spacing = spacing
+    r.origin[:] = list(origin)
+    r.centre[:] = list(centre)
+    r.axis[:] = list(axis)
+    r.omega, r.theta0, r.n_tags = omega, theta0, n_tags
+    return r, (sdf, tag)
+
+
+def workspace_bytes(params: Params, rotor_shape=None) -> int:
+    r = None
+    if rotor_shape is not None:
+        r = RotorDesc()
+        r.gz, r.gy, r.gx = rotor_shape
+    n = lib().hhrr_workspace_bytes(C.byref(params), C.byref(r) if r is not None else None)
+    if n == 0:
+        raise HhrrError(-1, "hhrr_workspace_bytes: invalid parameters")
+    return n
+
+
+class Lattice:
+    """One lattice on one GPU.  Method names mirror include/hhrr.h without the prefix."""
+
+    def __init__(self, params: Params, rotor_shape=None, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2510_13726_b200 needs a CUDA device (no CPU fallback)")
+        self.p = params
+        self.nx, self.ny, self.nz = params.nx, params.ny, params.nz
+        self.n = self.nx * self.ny * self.nz
+        self.device = torch.device(device)
+        nbytes = workspace_bytes(params, rotor_shape)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = C.c_void_p()
+            _check(lib().hhrr_create(C.byref(params), C.c_void_p(self.workspace.data_ptr()), nbytes,
+                                     C.c_void_p(self.stream.cuda_stream), C.byref(h)))
+        self.h = h
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().hhrr_destroy(self.h)
+            self.h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- setup
+    def init_equilibrium(self, rho, u, with_neq=False):
+        rho = _f32(rho).ravel()
+        u = _f32(u).reshape(3, -1)
+        assert rho.size == self.n and u.shape[1] == self.n
+        _check(lib().hhrr_init_equilibrium(self.h, _p(rho), _p(u), int(with_neq)))
+
+    def set_static_geometry(self, phi, tag=None, d_override=None):
+        phi = None if phi is None else _f32(phi).ravel()
+        tag = None if tag is None else np.ascontiguousarray(tag, np.uint8).ravel()
+        dov = None if d_override is None else _f32(d_override).ravel()
+        _check(lib().hhrr_set_static_geometry(self.h, _p(phi), _p(tag), _p(dov)))
+
+    def set_body(self, tag, centre=(0, 0, 0), omega=(0, 0, 0), vel=(0, 0, 0)):
+        c, o, v = _f64(centre), _f64(omega), _f64(vel)
+        _check(lib().hhrr_set_body(self.h, int(tag), _p(c), _p(o), _p(v)))
+
+    def set_fringe(self, x0, x1, u_in):
+        u = _f64(u_in)
+        _check(lib().hhrr_set_fringe(self.h, int(x0), int(x1), _p(u)))
+
+    def set_rotor(self, sdf, tag, spacing, origin, centre, axis, omega, theta0, n_tags):
+        r, keep = _rotor_desc(sdf, tag, spacing, origin, centre, axis, omega, theta0, n_tags)
+        _check(lib().hhrr_set_rotor(self.h, C.byref(r)))
+        del keep
+
+    def enable_wall_model(self, enable=True):
+        _check(lib().hhrr_enable_wall_model(self.h, int(enable)))
+
+    def update_geometry(self):
+        _check(lib().hhrr_update_geometry(self.h))
+
+    def set_kernel_variant(self, variant):
+        _check(lib().hhrr_set_kernel_variant(self.h, int(variant)))
+
+    # ---- time loop
+    def step(self, n=1):
+        _check(lib().hhrr_step(self.h, int(n)))
+
+    def step_count(self):
+        return lib().hhrr_step_count(self.h)
+
+    def launch_count(self):
+        return lib().hhrr_launch_count(self.h)
+
+    def check_finite(self):
+        _check(lib().hhrr_check_finite(self.h))
+
+    # ---- outputs
+    def moments(self):
+        rho = np.empty(self.n, np.float32)
+        v = np.empty((3, self.n), np.float32)
+        _check(lib().hhrr_get_moments(self.h, _p(rho), _p(v)))
+        return rho, v
+
+    def moments_device(self, rho_t, v_t):
+        """rho_t: float32 CUDA tensor [n]; v_t: float32 CUDA tensor [3, n]; asynchronous."""
+        _check(lib().hhrr_get_moments_device(self.h, C.c_void_p(rho_t.data_ptr()), C.c_void_p(v_t.data_ptr())))
+
+    def forces(self, first=0, count=None):
+        if count is None:
+            count = self.step_count() - first
+        F = np.zeros((count, MAX_TAGS, 3))
+        if count:
+            _check(lib().hhrr_get_forces(self.h, int(first), int(count), _p(F)))
+        return F
+
+    def cell_types(self):
+        t = np.empty(self.n, np.uint8)
+        g = np.empty(self.n, np.uint8)
+        d = np.empty(self.n, np.float32)
+        _check(lib().hhrr_get_cell_types(self.h, _p(t), _p(g), _p(d)))
+        return t, g, d
+
+    def wall_list(self):
+        k = C.c_int64(0)
+        _check(lib().hhrr_get_wall_list(self.h, 0, None, None, None, None, C.byref(k)))
+        k = k.value
+        idx = np.zeros(k, np.int32)
+        y1n = np.zeros((k, 3))
+        ut = np.zeros(k)
+        va = np.zeros(k, np.uint8)
+        if k:
+            kk = C.c_int64(0)
+            _check(lib().hhrr_get_wall_list(self.h, k, _p(idx), _p(y1n), _p(ut), _p(va), C.byref(kk)))
+        return idx, y1n, ut, va
+
+    def wall_state(self, cell):
+        ut = C.c_double(0)
+        valid = C.c_int32(0)
+        u = np.zeros(3)
+        s = np.zeros(6)
+        _check(lib().hhrr_get_wall_state(self.h, int(cell), C.byref(ut), _p(u), _p(s), C.byref(valid)))
+        return valid.value, ut.value, u, s
+
+    def populations(self):
+        f = np.empty((Q, self.n), np.float32)
+        _check(lib().hhrr_get_populations(self.h, _p(f)))
+        return f
+
+    def set_populations(self, f_minus_w):
+        f = _f32(f_minus_w).reshape(Q, self.n)
+        _check(lib().hhrr_set_populations(self.h, _p(f)))
+
+    def uhat(self):
+        u = np.empty((3, self.n), np.float32)
+        _check(lib().hhrr_get_uhat(self.h, _p(u)))
+        return u
+
+    def synchronize(self):
+        self.stream.synchronize()

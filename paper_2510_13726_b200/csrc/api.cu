@@ -1,0 +1,514 @@
+// api.cu -- the C ABI of include/hhrr.h: argument checking, workspace carving, host<->device
+// staging and the per-step launch sequence of Listing 3.
+// CUDA path only; shares nothing with oracle/.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "lattice.h"
+
+using namespace hhrr;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+int cuda_fail(cudaError_t e, const char* what) {
+  return fail(HHRR_E_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+#define CU(call)                                   \
+  do {                                             \
+    cudaError_t e_ = (call);                       \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
+  } while (0)
+
+size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
+
+bool params_ok(const hhrr_params* p) {
+  if (!p) return false;
+  if (p->nx < 1 || p->ny < 1 || p->nz < 1) return false;
+  double n = (double)p->nx * p->ny * p->nz;
+  if (n > 2.0e9) return false;  // int32 cell indices in the compact lists
+  for (int a = 0; a < 3; ++a)
+    if (p->mode[a] != HHRR_PERIODIC && p->mode[a] != HHRR_MIRROR) return false;
+  if (!(p->tau0 > 0.5) || !(p->sigma >= 0.0 && p->sigma <= 1.0) || !(p->smagorinsky_cs >= 0.0)) return false;
+  if (!(p->eps_cells > 0.0) || !(p->kappa > 0.0) || !(p->E > 0.0) || p->newton_max_iter < 0) return false;
+  if (!(p->sampling_distance > 0.0)) return false;
+  return true;
+}
+
+int64_t list_capacity(int64_t n) { return std::min<int64_t>(n, std::max<int64_t>(1 << 20, n / 4)); }
+
+// Carves the workspace; with base == nullptr only sizes it.
+struct Carver {
+  char* base;
+  size_t off = 0;
+  template <class T>
+  T* take(int64_t count) {
+    T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    off += align_up(sizeof(T) * (size_t)count);
+    return p;
+  }
+};
+
+size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* base) {
+  Carver c{base};
+  int64_t n = (int64_t)p->nx * p->ny * p->nz;
+  int64_t cap = list_capacity(n);
+  float* fA = c.take<float>(Q * n);
+  float* fB = c.take<float>(Q * n);
+  uint8_t* flags = c.take<uint8_t>(n);
+  float* d = c.take<float>(n);
+  double* phi = c.take<double>(n);
+  float* phi_static = c.take<float>(n);
+  uint8_t* tag_static = c.take<uint8_t>(n);
+  float* d_override = c.take<float>(n);
+  float* uhat = c.take<float>(3 * n);
+  double* wm_utau = c.take<double>(n);
+  float* wm_u = c.take<float>(3 * n);
+  float* wm_s = c.take<float>(6 * n);
+  int32_t* wall_idx = c.take<int32_t>(cap);
+  double* wall_y1n = c.take<double>(3 * cap);
+  int32_t* force_idx = c.take<int32_t>(cap);
+  Counters* counters = c.take<Counters>(1);
+  double* force = c.take<double>(FORCE_HISTORY * MAX_TAGS * 3);
+  float* rot_sdf = c.take<float>(rotor_nodes);
+  uint8_t* rot_tag = c.take<uint8_t>(rotor_nodes);
+  if (L) {
+    L->fA = fA; L->fB = fB; L->flags = flags; L->d = d; L->phi = phi; L->phi_static = phi_static;
+    L->tag_static = tag_static; L->d_override = d_override; L->uhat = uhat; L->wm_utau = wm_utau;
+    L->wm_u = wm_u; L->wm_s = wm_s; L->wall_idx = wall_idx; L->wall_y1n = wall_y1n;
+    L->force_idx = force_idx; L->counters = counters; L->force = force; L->rot_sdf = rot_sdf;
+    L->rot_tag = rot_tag; L->rot_nodes_cap = rotor_nodes; L->cap_list = cap;
+  }
+  return c.off;
+}
+
+__global__ void fill_bytes_kernel(uint8_t* p, int64_t count, uint8_t v) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, s = (int64_t)gridDim.x * blockDim.x;
+  for (; i < count; i += s) p[i] = v;
+}
+__global__ void fill_float_kernel(float* p, int64_t count, float v) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, s = (int64_t)gridDim.x * blockDim.x;
+  for (; i < count; i += s) p[i] = v;
+}
+
+// synchronous host <-> device copies on the lattice stream
+int upload(hhrr_lattice* L, void* dst, const void* src, size_t bytes) {
+  CU(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, L->stream));
+  CU(cudaStreamSynchronize(L->stream));
+  return HHRR_OK;
+}
+int download(hhrr_lattice* L, void* dst, const void* src, size_t bytes) {
+  CU(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, L->stream));
+  CU(cudaStreamSynchronize(L->stream));
+  return HHRR_OK;
+}
+
+int ensure_geometry(hhrr_lattice* L) {
+  if (L->geometry_current) return HHRR_OK;
+  cudaError_t e = launch_geometry(L, L->geometry_dirty);
+  if (e != cudaSuccess) return cuda_fail(e, "geometry kernels");
+  L->geometry_dirty = false;
+  L->geometry_current = true;
+  return HHRR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* hhrr_last_error(void) { return g_err; }
+const char* hhrr_version(void) { return "hhrr-b200 0.1 (D3Q27 fp32, sm_100a)"; }
+int64_t hhrr_force_history(void) { return FORCE_HISTORY; }
+
+size_t hhrr_workspace_bytes(const hhrr_params* p, const hhrr_rotor_desc* rotor) {
+  if (!params_ok(p)) return 0;
+  int64_t nodes = 0;
+  if (rotor) {
+    if (rotor->gx < 2 || rotor->gy < 2 || rotor->gz < 2) return 0;
+    nodes = (int64_t)rotor->gx * rotor->gy * rotor->gz;
+  }
+  return carve(nullptr, p, nodes, nullptr) + 1024;
+}
+
+int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes, void* cuda_stream,
+                hhrr_lattice** out) {
+  if (!out) return fail(HHRR_E_ARG, "hhrr_create: out is NULL");
+  *out = nullptr;
+  if (!params_ok(p)) return fail(HHRR_E_ARG, "hhrr_create: invalid parameters");
+  if (!d_workspace) return fail(HHRR_E_ARG, "hhrr_create: workspace is NULL");
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev < 1) return fail(HHRR_E_CUDA, "hhrr_create: no CUDA device (%s)", cudaGetErrorString(e));
+  cudaPointerAttributes attr;
+  e = cudaPointerGetAttributes(&attr, d_workspace);
+  if (e != cudaSuccess || attr.type != cudaMemoryTypeDevice)
+    return fail(HHRR_E_ARG, "hhrr_create: workspace is not device memory");
+  char* base = reinterpret_cast<char*>(align_up(reinterpret_cast<size_t>(d_workspace)));
+  size_t lead = (size_t)(base - reinterpret_cast<char*>(d_workspace));
+  size_t need_min = carve(nullptr, p, 0, nullptr);
+  if (workspace_bytes < lead + need_min)
+    return fail(HHRR_E_SIZE, "hhrr_create: workspace %zu bytes < %zu needed", workspace_bytes, lead + need_min);
+  hhrr_lattice* L = new (std::nothrow) hhrr_lattice();
+  if (!L) return fail(HHRR_E_SIZE, "hhrr_create: out of host memory");
+  memset(L, 0, sizeof(*L));
+  L->p = *p;
+  L->dom.nx = p->nx; L->dom.ny = p->ny; L->dom.nz = p->nz;
+  for (int a = 0; a < 3; ++a) L->dom.mode[a] = p->mode[a];
+  L->dom.n = (int64_t)p->nx * p->ny * p->nz;
+  L->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+  L->device = attr.device;
+  // rotor grid gets whatever the workspace has left
+  int64_t rest = (int64_t)(workspace_bytes - lead - need_min);
+  int64_t spare = std::max<int64_t>(0, (rest - 512) / 5);
+  carve(L, p, spare, base);
+  L->variant = 0;
+  L->geometry_dirty = true;
+  L->geometry_current = false;
+  const int64_t n = L->dom.n;
+  cudaStream_t s = L->stream;
+  fill_float_kernel<<<1184, 256, 0, s>>>(L->fA, Q * n, 0.f);
+  fill_float_kernel<<<1184, 256, 0, s>>>(L->fB, Q * n, 0.f);
+  fill_bytes_kernel<<<1184, 256, 0, s>>>(L->flags, n, 0);
+  fill_float_kernel<<<1184, 256, 0, s>>>(L->d, n, 1.f);
+  fill_float_kernel<<<1184, 256, 0, s>>>(L->uhat, 3 * n, 0.f);
+  fill_float_kernel<<<1184, 256, 0, s>>>(L->wm_u, 3 * n, 0.f);
+  fill_float_kernel<<<1184, 256, 0, s>>>(L->wm_s, 6 * n, 0.f);
+  L->launches += 7;
+  e = cudaMemsetAsync(L->wm_utau, 0, sizeof(double) * n, s);
+  if (e == cudaSuccess) e = cudaMemsetAsync(L->counters, 0, sizeof(Counters), s);
+  if (e == cudaSuccess) e = cudaMemsetAsync(L->force, 0, sizeof(double) * FORCE_HISTORY * MAX_TAGS * 3, s);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) {
+    delete L;
+    return cuda_fail(e, "hhrr_create: initialising the workspace");
+  }
+  *out = L;
+  return HHRR_OK;
+}
+
+int hhrr_destroy(hhrr_lattice* L) {
+  if (!L) return fail(HHRR_E_ARG, "hhrr_destroy: NULL lattice");
+  cudaStreamSynchronize(L->stream);
+  delete L;
+  return HHRR_OK;
+}
+
+int hhrr_init_equilibrium(hhrr_lattice* L, const float* rho, const float* u, int with_neq) {
+  if (!L || !rho || !u) return fail(HHRR_E_ARG, "hhrr_init_equilibrium: NULL argument");
+  const int64_t n = L->dom.n;
+  // stage rho in buffer B (scratch between steps) and u in the uhat field
+  int rc = upload(L, L->fB, rho, sizeof(float) * n);
+  if (rc) return rc;
+  rc = upload(L, L->uhat, u, sizeof(float) * 3 * n);
+  if (rc) return rc;
+  cudaError_t e = launch_init(L, L->fB, L->uhat, with_neq);
+  if (e != cudaSuccess) return cuda_fail(e, "init kernel");
+  CU(cudaStreamSynchronize(L->stream));
+  L->geometry_current = false;
+  return HHRR_OK;
+}
+
+int hhrr_set_static_geometry(hhrr_lattice* L, const float* phi, const uint8_t* tag, const float* d_override) {
+  if (!L) return fail(HHRR_E_ARG, "hhrr_set_static_geometry: NULL lattice");
+  const int64_t n = L->dom.n;
+  L->has_static = L->has_tag_static = L->has_override = false;
+  if (phi) {
+    int rc = upload(L, L->phi_static, phi, sizeof(float) * n);
+    if (rc) return rc;
+    L->has_static = true;
+    if (tag) {
+      rc = upload(L, L->tag_static, tag, n);
+      if (rc) return rc;
+      L->has_tag_static = true;
+    }
+    if (d_override) {
+      rc = upload(L, L->d_override, d_override, sizeof(float) * n);
+      if (rc) return rc;
+      L->has_override = true;
+    }
+  }
+  L->geometry_dirty = true;
+  L->geometry_current = false;
+  return HHRR_OK;
+}
+
+int hhrr_set_body(hhrr_lattice* L, int32_t tag, const double centre[3], const double omega[3],
+                  const double vel[3]) {
+  if (!L || !centre || !omega || !vel) return fail(HHRR_E_ARG, "hhrr_set_body: NULL argument");
+  if (tag < 0 || tag >= MAX_TAGS) return fail(HHRR_E_ARG, "hhrr_set_body: tag %d out of range", tag);
+  for (int a = 0; a < 3; ++a) {
+    L->bodies.c[tag][a] = centre[a];
+    L->bodies.w[tag][a] = omega[a];
+    L->bodies.v[tag][a] = vel[a];
+  }
+  return HHRR_OK;
+}
+
+int hhrr_set_fringe(hhrr_lattice* L, int32_t x_begin, int32_t x_end, const double u_in[3]) {
+  if (!L || !u_in) return fail(HHRR_E_ARG, "hhrr_set_fringe: NULL argument");
+  L->has_fringe = x_end > x_begin;
+  L->fr_x0 = x_begin;
+  L->fr_x1 = x_end;
+  for (int a = 0; a < 3; ++a) L->fr_u[a] = u_in[a];
+  L->geometry_dirty = true;
+  L->geometry_current = false;
+  return HHRR_OK;
+}
+
+int hhrr_set_rotor(hhrr_lattice* L, const hhrr_rotor_desc* r) {
+  if (!L || !r || !r->sdf || !r->tag) return fail(HHRR_E_ARG, "hhrr_set_rotor: NULL argument");
+  if (r->n_tags < 1 || r->n_tags >= MAX_TAGS) return fail(HHRR_E_ARG, "hhrr_set_rotor: n_tags out of range");
+  if (r->gx < 2 || r->gy < 2 || r->gz < 2 || !(r->spacing > 0.0)) return fail(HHRR_E_ARG, "hhrr_set_rotor: bad grid");
+  int64_t nodes = (int64_t)r->gx * r->gy * r->gz;
+  if (nodes > L->rot_nodes_cap)
+    return fail(HHRR_E_SIZE, "hhrr_set_rotor: reference grid of %lld nodes does not fit the workspace (%lld)",
+                (long long)nodes, (long long)L->rot_nodes_cap);
+  int rc = upload(L, L->rot_sdf, r->sdf, sizeof(float) * nodes);
+  if (rc) return rc;
+  rc = upload(L, L->rot_tag, r->tag, nodes);
+  if (rc) return rc;
+  L->rot = *r;
+  L->rot.sdf = nullptr;
+  L->rot.tag = nullptr;
+  L->has_rotor = true;
+  for (int k = 1; k <= r->n_tags; ++k)  // u^B = Omega x (x - x_c)
+    for (int a = 0; a < 3; ++a) {
+      L->bodies.c[k][a] = r->centre[a];
+      L->bodies.w[k][a] = r->axis[a] * r->omega;
+      L->bodies.v[k][a] = 0.0;
+    }
+  // Box swept by the reference grid under rotation about the axis: the axial coordinate
+  // and the radial distance of a point are invariant, so bound both over the grid corners.
+  double amin = 1e300, amax = -1e300, rmax = 0.0;
+  for (int k = 0; k < 8; ++k) {
+    double q[3] = {r->origin[0] + ((k & 1) ? (r->gx - 1) * r->spacing : 0.0),
+                   r->origin[1] + ((k & 2) ? (r->gy - 1) * r->spacing : 0.0),
+                   r->origin[2] + ((k & 4) ? (r->gz - 1) * r->spacing : 0.0)};
+    double ad = q[0] * r->axis[0] + q[1] * r->axis[1] + q[2] * r->axis[2];
+    double rr = std::sqrt(std::max(0.0, q[0] * q[0] + q[1] * q[1] + q[2] * q[2] - ad * ad));
+    amin = std::min(amin, ad);
+    amax = std::max(amax, ad);
+    rmax = std::max(rmax, rr);
+  }
+  int lo[3], hi[3], ext[3] = {L->dom.nx, L->dom.ny, L->dom.nz};
+  for (int a = 0; a < 3; ++a) {
+    double ak = r->axis[a], perp = std::sqrt(std::max(0.0, 1.0 - ak * ak));
+    double e0 = std::min(ak * amin, ak * amax) - perp * rmax, e1 = std::max(ak * amin, ak * amax) + perp * rmax;
+    lo[a] = (int)std::floor(r->centre[a] + e0) - 3;
+    hi[a] = (int)std::ceil(r->centre[a] + e1) + 4;
+    lo[a] = std::max(0, std::min(ext[a], lo[a]));
+    hi[a] = std::max(lo[a], std::min(ext[a], hi[a]));
+  }
+  L->rot_box = Box{lo[0], hi[0], lo[1], hi[1], lo[2], hi[2]};
+  L->geometry_dirty = true;
+  L->geometry_current = false;
+  return HHRR_OK;
+}
+
+int hhrr_enable_wall_model(hhrr_lattice* L, int enable) {
+  if (!L) return fail(HHRR_E_ARG, "hhrr_enable_wall_model: NULL lattice");
+  L->wm_enabled = enable != 0;
+  L->geometry_dirty = true;
+  L->geometry_current = false;
+  return HHRR_OK;
+}
+
+int hhrr_update_geometry(hhrr_lattice* L) {
+  if (!L) return fail(HHRR_E_ARG, "hhrr_update_geometry: NULL lattice");
+  L->geometry_current = false;
+  return ensure_geometry(L);
+}
+
+int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant) {
+  if (!L || variant < 0 || variant > 1) return fail(HHRR_E_ARG, "hhrr_set_kernel_variant: bad argument");
+  L->variant = variant;
+  return HHRR_OK;
+}
+
+int64_t hhrr_launch_count(const hhrr_lattice* L) { return L ? L->launches : 0; }
+int64_t hhrr_step_count(const hhrr_lattice* L) { return L ? L->step : 0; }
+
+int hhrr_step(hhrr_lattice* L, int32_t n_steps) {
+  if (!L || n_steps < 0) return fail(HHRR_E_ARG, "hhrr_step: bad argument");
+  for (int32_t s = 0; s < n_steps; ++s) {
+    int rc = ensure_geometry(L);  // Listing 3 line 2: UpdatePorosityO
+    if (rc) return rc;
+    cudaError_t e = launch_collide_stream(L);  // line 3
+    if (e != cudaSuccess) return cuda_fail(e, "collide-stream kernel");
+    e = launch_wall_model(L);  // line 4: WallModelO
+    if (e != cudaSuccess) return cuda_fail(e, "wall-model kernel");
+    e = launch_forces(L);  // lines 5-6
+    if (e != cudaSuccess) return cuda_fail(e, "force kernels");
+    L->step += 1;  // line 7: theta_{n+1} = theta_n + Omega
+    L->geometry_current = !L->has_rotor;  // static geometry stays valid
+  }
+  return HHRR_OK;
+}
+
+int hhrr_get_moments_device(hhrr_lattice* L, float* d_rho, float* d_v) {
+  if (!L || !d_rho || !d_v) return fail(HHRR_E_ARG, "hhrr_get_moments_device: NULL argument");
+  cudaError_t e = launch_moments(L, d_rho, d_v);
+  if (e != cudaSuccess) return cuda_fail(e, "moments kernel");
+  return HHRR_OK;
+}
+
+int hhrr_get_moments(hhrr_lattice* L, float* rho, float* v) {
+  if (!L || !rho || !v) return fail(HHRR_E_ARG, "hhrr_get_moments: NULL argument");
+  const int64_t n = L->dom.n;
+  float* scratch = L->fB;  // buffer B is free between steps
+  cudaError_t e = launch_moments(L, scratch, scratch + n);
+  if (e != cudaSuccess) return cuda_fail(e, "moments kernel");
+  int rc = download(L, rho, scratch, sizeof(float) * n);
+  if (rc) return rc;
+  return download(L, v, scratch + n, sizeof(float) * 3 * n);
+}
+
+int hhrr_get_forces(hhrr_lattice* L, int64_t first_step, int64_t n_steps, double* F) {
+  if (!L || !F || n_steps < 0) return fail(HHRR_E_ARG, "hhrr_get_forces: bad argument");
+  if (first_step < 0 || first_step + n_steps > L->step || first_step < L->step - FORCE_HISTORY)
+    return fail(HHRR_E_STATE, "hhrr_get_forces: steps [%lld,%lld) not in the recorded history (step %lld)",
+                (long long)first_step, (long long)(first_step + n_steps), (long long)L->step);
+  const size_t rec = sizeof(double) * MAX_TAGS * 3;
+  int64_t s = first_step;
+  while (s < first_step + n_steps) {  // the ring may wrap once
+    int64_t slot = s % FORCE_HISTORY;
+    int64_t run = std::min<int64_t>(first_step + n_steps - s, FORCE_HISTORY - slot);
+    CU(cudaMemcpyAsync(F + (s - first_step) * MAX_TAGS * 3, L->force + slot * MAX_TAGS * 3, rec * run,
+                       cudaMemcpyDeviceToHost, L->stream));
+    s += run;
+  }
+  CU(cudaStreamSynchronize(L->stream));
+  return HHRR_OK;
+}
+
+int hhrr_get_cell_types(hhrr_lattice* L, uint8_t* type, uint8_t* tag, float* d) {
+  if (!L) return fail(HHRR_E_ARG, "hhrr_get_cell_types: NULL lattice");
+  const int64_t n = L->dom.n;
+  if (type || tag) {
+    std::vector<uint8_t> fl((size_t)n);
+    int rc = download(L, fl.data(), L->flags, (size_t)n);
+    if (rc) return rc;
+    for (int64_t c = 0; c < n; ++c) {
+      if (type) type[c] = fl[c] & TYPE_MASK;
+      if (tag) tag[c] = (fl[c] >> TAG_SHIFT) & TAG_MASK;
+    }
+  }
+  if (d) return download(L, d, L->d, sizeof(float) * n);
+  return HHRR_OK;
+}
+
+namespace {
+__global__ void gather_wall_kernel(const int32_t* idx, int count, const double* wm_utau, const uint8_t* flags,
+                                   double* out_utau, uint8_t* out_valid) {
+  int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= count) return;
+  int64_t c = idx[e];
+  out_utau[e] = wm_utau[c];
+  out_valid[e] = (flags[c] & WM_VALID) ? 1 : 0;
+}
+int read_counters(hhrr_lattice* L, Counters* h) { return download(L, h, L->counters, sizeof(Counters)); }
+}  // namespace
+
+int hhrr_get_wall_list(hhrr_lattice* L, int64_t capacity, int32_t* idx, double* y1n, double* u_tau,
+                       uint8_t* valid, int64_t* count) {
+  if (!L || !count) return fail(HHRR_E_ARG, "hhrr_get_wall_list: NULL argument");
+  Counters h;
+  int rc = read_counters(L, &h);
+  if (rc) return rc;
+  if (h.overflow) return fail(HHRR_E_SIZE, "compact cell list overflowed its capacity of %lld", (long long)L->cap_list);
+  int64_t k = h.wall_count;
+  *count = k;
+  if (k == 0 || capacity <= 0 || !idx) return HHRR_OK;
+  std::vector<int32_t> hidx((size_t)k);
+  std::vector<double> hy((size_t)3 * k), hu((size_t)k);
+  std::vector<uint8_t> hv((size_t)k);
+  rc = download(L, hidx.data(), L->wall_idx, sizeof(int32_t) * k);
+  if (rc) return rc;
+  rc = download(L, hy.data(), L->wall_y1n, sizeof(double) * 3 * k);
+  if (rc) return rc;
+  double* s_utau = reinterpret_cast<double*>(L->fB);  // scratch
+  uint8_t* s_valid = reinterpret_cast<uint8_t*>(s_utau + k);
+  gather_wall_kernel<<<(unsigned)((k + 255) / 256), 256, 0, L->stream>>>(L->wall_idx, (int)k, L->wm_utau, L->flags,
+                                                                         s_utau, s_valid);
+  L->launches++;
+  CU(cudaGetLastError());
+  rc = download(L, hu.data(), s_utau, sizeof(double) * k);
+  if (rc) return rc;
+  rc = download(L, hv.data(), s_valid, (size_t)k);
+  if (rc) return rc;
+  std::vector<int64_t> order((size_t)k);
+  for (int64_t e = 0; e < k; ++e) order[e] = e;
+  std::sort(order.begin(), order.end(), [&](int64_t a, int64_t b) { return hidx[a] < hidx[b]; });
+  int64_t m = std::min(k, capacity);
+  for (int64_t e = 0; e < m; ++e) {
+    int64_t o = order[e];
+    idx[e] = hidx[o];
+    if (y1n)
+      for (int a = 0; a < 3; ++a) y1n[3 * e + a] = hy[3 * o + a];
+    if (u_tau) u_tau[e] = hu[o];
+    if (valid) valid[e] = hv[o];
+  }
+  return HHRR_OK;
+}
+
+int hhrr_get_wall_state(hhrr_lattice* L, int64_t cell, double* u_tau, double u_wm[3], double s_wm[6],
+                        int32_t* valid) {
+  if (!L || cell < 0 || cell >= L->dom.n) return fail(HHRR_E_ARG, "hhrr_get_wall_state: bad argument");
+  const int64_t n = L->dom.n;
+  double ut;
+  float u[3], s[6];
+  uint8_t fl;
+  CU(cudaMemcpyAsync(&ut, L->wm_utau + cell, sizeof(double), cudaMemcpyDeviceToHost, L->stream));
+  for (int a = 0; a < 3; ++a)
+    CU(cudaMemcpyAsync(&u[a], L->wm_u + a * n + cell, sizeof(float), cudaMemcpyDeviceToHost, L->stream));
+  for (int a = 0; a < 6; ++a)
+    CU(cudaMemcpyAsync(&s[a], L->wm_s + a * n + cell, sizeof(float), cudaMemcpyDeviceToHost, L->stream));
+  CU(cudaMemcpyAsync(&fl, L->flags + cell, 1, cudaMemcpyDeviceToHost, L->stream));
+  CU(cudaStreamSynchronize(L->stream));
+  if (u_tau) *u_tau = ut;
+  if (u_wm) for (int a = 0; a < 3; ++a) u_wm[a] = u[a];
+  if (s_wm) for (int a = 0; a < 6; ++a) s_wm[a] = s[a];
+  if (valid) *valid = (fl & WM_VALID) ? 1 : 0;
+  return HHRR_OK;
+}
+
+int hhrr_get_populations(hhrr_lattice* L, float* f_minus_w) {
+  if (!L || !f_minus_w) return fail(HHRR_E_ARG, "hhrr_get_populations: NULL argument");
+  return download(L, f_minus_w, L->fA, sizeof(float) * Q * L->dom.n);
+}
+int hhrr_set_populations(hhrr_lattice* L, const float* f_minus_w) {
+  if (!L || !f_minus_w) return fail(HHRR_E_ARG, "hhrr_set_populations: NULL argument");
+  return upload(L, L->fA, f_minus_w, sizeof(float) * Q * L->dom.n);
+}
+int hhrr_get_uhat(hhrr_lattice* L, float* uhat) {
+  if (!L || !uhat) return fail(HHRR_E_ARG, "hhrr_get_uhat: NULL argument");
+  return download(L, uhat, L->uhat, sizeof(float) * 3 * L->dom.n);
+}
+
+int hhrr_check_finite(hhrr_lattice* L) {
+  if (!L) return fail(HHRR_E_ARG, "hhrr_check_finite: NULL lattice");
+  cudaError_t e = launch_check_finite(L);
+  if (e != cudaSuccess) return cuda_fail(e, "finite-check kernel");
+  Counters h;
+  int rc = read_counters(L, &h);
+  if (rc) return rc;
+  if (h.overflow) return fail(HHRR_E_SIZE, "compact cell list overflowed its capacity of %lld", (long long)L->cap_list);
+  if (h.nonfinite) return fail(HHRR_E_NAN, "non-finite population at step %lld", (long long)L->step);
+  return HHRR_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,206 @@
+// d3q27.cuh -- D3Q27 cell model of the HHRRLBM in fp32 on population deviations f_i - w_i.
+//
+// PAPER.md:98 (Eq. 6), :102 (Eq. 7), :113-122 (Eq. 8-10), :126-129 (Eq. 11), :133 (Eq. 12),
+// :144 (Eq. 14); readings R1-R6 of DESIGN.md.  All sums over the 27 directions are written
+// through the tensor-product structure c = (cx,cy,cz), cx,cy,cz in {-1,0,1}:
+//   * moments: three separable passes (x, then y, then z)            ~70 adds
+//   * reconstruction: f_i = w_i (E_i + O_i), f_ibar = w_i (E_i - O_i) with E the even and
+//     O the odd polynomial in c                                       ~220 flops
+// CUDA path only; shares nothing with oracle/.
+#pragma once
+#include "lattice.h"
+
+namespace hhrr {
+
+__host__ __device__ constexpr int dir_cx(int i) { return i % 3 - 1; }
+__host__ __device__ constexpr int dir_cy(int i) { return (i / 3) % 3 - 1; }
+__host__ __device__ constexpr int dir_cz(int i) { return i / 9 - 1; }
+__host__ __device__ constexpr float dir_w(int i) {
+  return (dir_cx(i) ? 1.f / 6.f : 2.f / 3.f) * (dir_cy(i) ? 1.f / 6.f : 2.f / 3.f) *
+         (dir_cz(i) ? 1.f / 6.f : 2.f / 3.f);
+}
+__host__ __device__ constexpr double dir_wd(int i) {
+  return (dir_cx(i) ? 1.0 / 6.0 : 2.0 / 3.0) * (dir_cy(i) ? 1.0 / 6.0 : 2.0 / 3.0) *
+         (dir_cz(i) ? 1.0 / 6.0 : 2.0 / 3.0);
+}
+
+struct Moments {  // of the deviations: drho = rho - 1, j, M_ab = sum c_a c_b (f - w)
+  float drho, jx, jy, jz, mxx, myy, mzz, mxy, mxz, myz;
+};
+
+// rho and j only (halo cells, moments pass, read-back): 3 separable passes
+__device__ __forceinline__ void moments_rho_j(const float (&f)[Q], float& drho, float& jx, float& jy,
+                                              float& jz) {
+  float s0[9], s1[9];
+#pragma unroll
+  for (int m = 0; m < 9; ++m) {
+    float fm = f[3 * m], f0 = f[3 * m + 1], fp = f[3 * m + 2];
+    s0[m] = (fp + fm) + f0;
+    s1[m] = fp - fm;
+  }
+  float t00[3], t01[3], t10[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    t00[k] = (s0[3 * k + 2] + s0[3 * k]) + s0[3 * k + 1];
+    t01[k] = s0[3 * k + 2] - s0[3 * k];
+    t10[k] = (s1[3 * k + 2] + s1[3 * k]) + s1[3 * k + 1];
+  }
+  drho = (t00[2] + t00[0]) + t00[1];
+  jz = t00[2] - t00[0];
+  jy = (t01[2] + t01[0]) + t01[1];
+  jx = (t10[2] + t10[0]) + t10[1];
+}
+
+__device__ __forceinline__ Moments moments_all(const float (&f)[Q]) {
+  float s0[9], s1[9], s2[9];
+#pragma unroll
+  for (int m = 0; m < 9; ++m) {
+    float fm = f[3 * m], f0 = f[3 * m + 1], fp = f[3 * m + 2];
+    s2[m] = fp + fm;
+    s0[m] = s2[m] + f0;
+    s1[m] = fp - fm;
+  }
+  float t00[3], t01[3], t02[3], t10[3], t11[3], t20[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    t02[k] = s0[3 * k + 2] + s0[3 * k];
+    t00[k] = t02[k] + s0[3 * k + 1];
+    t01[k] = s0[3 * k + 2] - s0[3 * k];
+    t10[k] = (s1[3 * k + 2] + s1[3 * k]) + s1[3 * k + 1];
+    t11[k] = s1[3 * k + 2] - s1[3 * k];
+    t20[k] = (s2[3 * k + 2] + s2[3 * k]) + s2[3 * k + 1];
+  }
+  Moments m;
+  m.mzz = t00[2] + t00[0];
+  m.drho = m.mzz + t00[1];
+  m.jz = t00[2] - t00[0];
+  m.jy = (t01[2] + t01[0]) + t01[1];
+  m.myz = t01[2] - t01[0];
+  m.myy = (t02[2] + t02[0]) + t02[1];
+  m.jx = (t10[2] + t10[0]) + t10[1];
+  m.mxz = t10[2] - t10[0];
+  m.mxy = (t11[2] + t11[0]) + t11[1];
+  m.mxx = (t20[2] + t20[0]) + t20[1];
+  return m;
+}
+
+// u^B of a cell (fringe R12), without the wall-model slip
+__device__ __forceinline__ void solid_velocity(const PhysF& ph, const BodiesF& bo, uint8_t flags, int x,
+                                               int y, int z, float uB[3]) {
+  int type = flags & TYPE_MASK;
+  uB[0] = uB[1] = uB[2] = 0.f;
+  if (type == HHRR_FRINGE) {
+    uB[0] = ph.fr_u[0];
+    uB[1] = ph.fr_u[1];
+    uB[2] = ph.fr_u[2];
+  } else if (type == HHRR_SOLID || type == HHRR_FRONTIER) {
+    int k = (flags >> TAG_SHIFT) & TAG_MASK;
+    float rx = (float)x - bo.c[k][0], ry = (float)y - bo.c[k][1], rz = (float)z - bo.c[k][2];
+    uB[0] = bo.v[k][0] + (bo.w[k][1] * rz - bo.w[k][2] * ry);
+    uB[1] = bo.v[k][1] + (bo.w[k][2] * rx - bo.w[k][0] * rz);
+    uB[2] = bo.v[k][2] + (bo.w[k][0] * ry - bo.w[k][1] * rx);
+  }
+}
+
+// Eq. 12 with reading R1 (d = 1 fluid): uhat = d u + (1-d) u^B, u = (j + g)/rho  (R11)
+__device__ __forceinline__ void homogenised_velocity(const PhysF& ph, float drho, float jx, float jy,
+                                                     float jz, float d, const float uB[3], float& rho,
+                                                     float uh[3]) {
+  rho = 1.f + drho;
+  float ir = 1.f / rho;
+  float ux = (jx + ph.g[0]) * ir, uy = (jy + ph.g[1]) * ir, uz = (jz + ph.g[2]) * ir;
+  float e = 1.f - d;
+  uh[0] = d * ux + e * uB[0];
+  uh[1] = d * uy + e * uB[1];
+  uh[2] = d * uz + e * uB[2];
+}
+
+// One collision.  m: moments of the deviations; rho, uh: from homogenised_velocity;
+// S: strain handed to the hybrid term (xx yy zz xy xz yz); sigma: this cell's hybrid factor.
+// Output: post-collision deviations f*_i - w_i.
+__device__ __forceinline__ void collide(const PhysF& ph, const Moments& m, float rho, const float uh[3],
+                                        const float S[6], float sigma, float (&out)[Q]) {
+  const float third = 1.f / 3.f;
+  float ux = uh[0], uy = uh[1], uz = uh[2];
+  float rux = rho * ux, ruy = rho * uy, ruz = rho * uz;
+  // Pi^neq = sum H2 f - rho uh uh  (R4)
+  float dr3 = m.drho * third;
+  float pxx = m.mxx - dr3 - rux * ux, pyy = m.myy - dr3 - ruy * uy, pzz = m.mzz - dr3 - ruz * uz;
+  float pxy = m.mxy - rux * uy, pxz = m.mxz - rux * uz, pyz = m.myz - ruy * uz;
+  // Smagorinsky closed form (Eq. 3-5, 14; R6)
+  float pp = pxx * pxx + pyy * pyy + pzz * pzz + 2.f * (pxy * pxy + pxz * pxz + pyz * pyz);
+  float Qn = sqrtf(2.f * pp);
+  float tau = 0.5f * (ph.tau0 + sqrtf(ph.tau0 * ph.tau0 + ph.smag18 * Qn / rho));
+  float k = 1.f - 1.f / tau;
+  // hybrid a1^(2) (Eq. 7 + Eq. 10; R2)
+  float hs = (1.f - sigma) * (2.f * third) * rho * tau;
+  float axx = sigma * pxx - hs * S[0], ayy = sigma * pyy - hs * S[1], azz = sigma * pzz - hs * S[2];
+  float axy = sigma * pxy - hs * S[3], axz = sigma * pxz - hs * S[4], ayz = sigma * pyz - hs * S[5];
+  // second order: T = 4.5 (rho uh uh + k a2)
+  float Txx = 4.5f * (rux * ux + k * axx), Tyy = 4.5f * (ruy * uy + k * ayy), Tzz = 4.5f * (ruz * uz + k * azz);
+  float Txy = 9.f * (rux * uy + k * axy), Txz = 9.f * (rux * uz + k * axz), Tyz = 9.f * (ruy * uz + k * ayz);
+  // third order (R3): A3_aab = rho ua ua ub + k (2 ua a_ab + ub a_aa); G_ab = 13.5 A3_aab; Gxyz = 27 A3_xyz
+  float Gxy = 13.5f * (rux * ux * uy + k * (2.f * ux * axy + uy * axx));  // xx y
+  float Gxz = 13.5f * (rux * ux * uz + k * (2.f * ux * axz + uz * axx));  // xx z
+  float Gyx = 13.5f * (ruy * uy * ux + k * (2.f * uy * axy + ux * ayy));  // yy x
+  float Gyz = 13.5f * (ruy * uy * uz + k * (2.f * uy * ayz + uz * ayy));  // yy z
+  float Gzx = 13.5f * (ruz * uz * ux + k * (2.f * uz * axz + ux * azz));  // zz x
+  float Gzy = 13.5f * (ruz * uz * uy + k * (2.f * uz * ayz + uy * azz));  // zz y
+  float Gxyz = 27.f * (rux * uy * uz + k * (ux * ayz + uy * axz + uz * axy));
+  // even part tables: q(c) = c^2 - 1/3
+  float Ex[2] = {-third * Txx, 2.f * third * Txx};
+  float Ey[2] = {-third * Tyy, 2.f * third * Tyy};
+  float Ez[2] = {m.drho - third * Tzz, m.drho + 2.f * third * Tzz};
+  // odd part: coefficient of c_b is m_b + sum_{a != b} q(c_a) G_ab
+  float mx = 3.f * rux, my = 3.f * ruy, mz = 3.f * ruz;
+  float OX[2][2], OY[2][2], OZ[2][2];  // [other axis 1 squared][other axis 2 squared]
+#pragma unroll
+  for (int p = 0; p < 2; ++p)
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      float qp = p ? 2.f * third : -third, qq = q ? 2.f * third : -third;
+      OX[p][q] = mx + qp * Gyx + qq * Gzx;  // p: cy^2, q: cz^2
+      OY[p][q] = my + qp * Gxy + qq * Gzy;  // p: cx^2, q: cz^2
+      OZ[p][q] = mz + qp * Gxz + qq * Gyz;  // p: cx^2, q: cy^2
+    }
+#pragma unroll
+  for (int i = 0; i <= 13; ++i) {
+    const int cx = dir_cx(i), cy = dir_cy(i), cz = dir_cz(i);
+    const int x2 = cx * cx, y2 = cy * cy, z2 = cz * cz;
+    float E = Ex[x2] + Ey[y2] + Ez[z2];
+    if (cx * cy == 1) E += Txy;
+    if (cx * cy == -1) E -= Txy;
+    if (cx * cz == 1) E += Txz;
+    if (cx * cz == -1) E -= Txz;
+    if (cy * cz == 1) E += Tyz;
+    if (cy * cz == -1) E -= Tyz;
+    const float w = dir_w(i);
+    if (i == 13) {
+      out[13] = w * E;
+    } else {
+      float O = 0.f;
+      if (cx == 1) O += OX[y2][z2];
+      if (cx == -1) O -= OX[y2][z2];
+      if (cy == 1) O += OY[x2][z2];
+      if (cy == -1) O -= OY[x2][z2];
+      if (cz == 1) O += OZ[x2][y2];
+      if (cz == -1) O -= OZ[x2][y2];
+      if (cx * cy * cz == 1) O += Gxyz;
+      if (cx * cy * cz == -1) O -= Gxyz;
+      out[i] = w * (E + O);
+      out[26 - i] = w * (E - O);
+    }
+  }
+}
+
+// neighbour index along one axis with the outer-boundary rule R12.
+// Returns the wrapped / reflected coordinate; flip = true if it was reflected.
+__device__ __forceinline__ int wrap_axis(int v, int n, int mode, bool& flip) {
+  flip = false;
+  if (v >= 0 && v < n) return v;
+  if (mode == HHRR_PERIODIC) return v < 0 ? v + n : v - n;
+  flip = true;
+  return v < 0 ? -1 - v : 2 * n - 1 - v;
+}
+
+}  // namespace hhrr

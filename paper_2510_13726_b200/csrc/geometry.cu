@@ -1,0 +1,329 @@
+// geometry.cu -- K1: UpdatePorosityO (Listing 3 line 2).
+//
+// Signed distance -> porosity (Def. 1, Eq. 21-22), cell types of Fig. 4
+// (:254-263), integer element tag (:267), wall-model set with the y1 vector (:324) and the
+// compact lists the wall-model and force kernels run over.  The rotor is re-embedded every
+// step by rotating cell centres into the rotor frame and sampling the reference grid
+// (:219, :265).  Instead of the paper's incremental growth-layer walk (:269) the kernels
+// re-evaluate the fixed box swept by the rotor -- a few percent of the cells -- which gives
+// the brute-force classification by construction.
+//
+// Integer results (types, tags, lists) are defined by the fp64 operation order below; this
+// file is compiled with -fmad=false so no contraction changes it.
+#include "lattice.h"
+
+namespace hhrr {
+
+struct GeoArgs {
+  Dom dm;
+  Box box;          // cells processed (inside == true) or skipped (inside == false)
+  int inside;
+  double h;         // eps/2
+  double eps;
+  int has_static, has_tag_static, has_override, has_fringe, has_rotor, wm_enabled;
+  int fr_x0, fr_x1;
+  double cth, sth;  // cos / sin of the rotor angle, evaluated once on the host
+  RotorDev rot;
+  const float* phi_static;
+  const uint8_t* tag_static;
+  const float* d_override;
+  double* phi;
+  uint8_t* flags;
+  float* d;
+  int32_t* wall_idx;
+  double* wall_y1n;
+  int32_t* force_idx;
+  Counters* cnt;
+  int cap_list;
+};
+
+__device__ __forceinline__ int wrap_any(int v, int n, int mode) {
+  if (v >= 0 && v < n) return v;
+  if (mode == HHRR_PERIODIC) return ((v % n) + n) % n;
+  return v < 0 ? -1 - v : 2 * n - 1 - v;
+}
+
+// rotate (p - centre) by -theta about the axis, trilinear-sample the reference grid
+__device__ double rotor_phi(const RotorDev& R, double cth, double sth, double px, double py, double pz,
+                            int* tag_out) {
+  double rx = px - R.centre[0], ry = py - R.centre[1], rz = pz - R.centre[2];
+  double ax = R.axis[0], ay = R.axis[1], az = R.axis[2];
+  double kx = ay * rz - az * ry, ky = az * rx - ax * rz, kz = ax * ry - ay * rx;
+  double ad = ax * rx + ay * ry + az * rz;
+  double omc = 1.0 - cth;
+  double qx = rx * cth - kx * sth + ax * ad * omc;
+  double qy = ry * cth - ky * sth + ay * ad * omc;
+  double qz = rz * cth - kz * sth + az * ad * omc;
+  double gx = (qx - R.origin[0]) / R.spacing;
+  double gy = (qy - R.origin[1]) / R.spacing;
+  double gz = (qz - R.origin[2]) / R.spacing;
+  double fx = floor(gx), fy = floor(gy), fz = floor(gz);
+  *tag_out = 0;
+  if (!(fx >= 0.0 && fy >= 0.0 && fz >= 0.0 && fx < (double)(R.gx - 1) && fy < (double)(R.gy - 1) &&
+        fz < (double)(R.gz - 1)))
+    return BIG_PHI;
+  int ix = (int)fx, iy = (int)fy, iz = (int)fz;
+  double tx = gx - fx, ty = gy - fy, tz = gz - fz;
+  const float* s = R.sdf;
+  int64_t sx = 1, sy = R.gx, sz = (int64_t)R.gx * R.gy;
+  int64_t b = ix * sx + iy * sy + iz * sz;
+  double v000 = s[b], v100 = s[b + sx], v010 = s[b + sy], v110 = s[b + sx + sy];
+  double v001 = s[b + sz], v101 = s[b + sx + sz], v011 = s[b + sy + sz], v111 = s[b + sx + sy + sz];
+  double c00 = v000 + tx * (v100 - v000);
+  double c10 = v010 + tx * (v110 - v010);
+  double c01 = v001 + tx * (v101 - v001);
+  double c11 = v011 + tx * (v111 - v011);
+  double c0 = c00 + ty * (c10 - c00);
+  double c1 = c01 + ty * (c11 - c01);
+  double phi = c0 + tz * (c1 - c0);
+  int nx_ = (int)floor(gx + 0.5), ny_ = (int)floor(gy + 0.5), nz_ = (int)floor(gz + 0.5);
+  if (nx_ > R.gx - 1) nx_ = R.gx - 1;
+  if (ny_ > R.gy - 1) ny_ = R.gy - 1;
+  if (nz_ > R.gz - 1) nz_ = R.gz - 1;
+  *tag_out = R.tag[nx_ * sx + ny_ * sy + nz_ * sz];
+  return phi;
+}
+
+// iteration space: the box itself, or the whole domain minus the box
+__device__ __forceinline__ bool geo_cell(const GeoArgs& a, int& x, int& y, int& z) {
+  if (a.inside) {
+    int bx = a.box.x1 - a.box.x0, by = a.box.y1 - a.box.y0;
+    x = a.box.x0 + blockIdx.y * blockDim.x + threadIdx.x;
+    int yz = blockIdx.x;
+    y = a.box.y0 + yz % by;
+    z = a.box.z0 + yz / by;
+    return x < a.box.x1 && bx > 0;
+  }
+  x = blockIdx.y * blockDim.x + threadIdx.x;
+  int yz = blockIdx.x;
+  y = yz % a.dm.ny;
+  z = yz / a.dm.ny;
+  if (x >= a.dm.nx) return false;
+  bool in_box = x >= a.box.x0 && x < a.box.x1 && y >= a.box.y0 && y < a.box.y1 && z >= a.box.z0 && z < a.box.z1;
+  return !in_box;
+}
+
+// pass 1: phi and provisional tag
+__global__ void __launch_bounds__(128) geometry_phi_kernel(GeoArgs a) {
+  int x, y, z;
+  if (!geo_cell(a, x, y, z)) return;
+  int64_t c = (int64_t)x + (int64_t)a.dm.nx * ((int64_t)y + (int64_t)a.dm.ny * z);
+  double phi = BIG_PHI;
+  int tg = 0;
+  if (a.has_static) {
+    phi = (double)a.phi_static[c];
+    tg = a.has_tag_static ? a.tag_static[c] : 1;
+  }
+  if (a.has_rotor) {
+    int rt;
+    double pr = rotor_phi(a.rot, a.cth, a.sth, (double)x, (double)y, (double)z, &rt);
+    if (pr < phi) {
+      phi = pr;
+      tg = rt;
+    }
+  }
+  a.phi[c] = phi;
+  a.flags[c] = (uint8_t)((a.flags[c] & WM_VALID) | ((tg & TAG_MASK) << TAG_SHIFT));
+}
+
+// pass 2: type, porosity, wall-model set (R13) and the compact lists
+__global__ void __launch_bounds__(128) geometry_type_kernel(GeoArgs a) {
+  int x, y, z;
+  bool active = geo_cell(a, x, y, z);
+  int inw = 0, inf = 0;
+  int64_t c = 0;
+  double y1v[3] = {0, 0, 0};
+  if (active) {
+    const int nx = a.dm.nx, ny = a.dm.ny, nz = a.dm.nz;
+    const int64_t snx = nx, snxy = (int64_t)nx * ny;
+    c = x + snx * y + snxy * z;
+    double phi = a.phi[c];
+    uint8_t fl = a.flags[c];
+    int tg = (fl >> TAG_SHIFT) & TAG_MASK;
+    int type;
+    float d;
+    if (a.has_fringe && x >= a.fr_x0 && x < a.fr_x1) {
+      type = HHRR_FRINGE;
+      d = 0.f;
+    } else if (phi <= -a.h) {
+      type = HHRR_SOLID;
+      d = 0.f;
+    } else if (phi < a.h) {
+      type = HHRR_FRONTIER;
+      double dd = phi / a.eps + 0.5;  // Eq. 22
+      if (a.has_override && a.has_static && (double)a.phi_static[c] == phi) dd = (double)a.d_override[c];
+      d = (float)dd;
+    } else {
+      type = HHRR_FLUID;
+      d = 1.f;
+      for (int dz = -1; dz <= 1 && type == HHRR_FLUID; ++dz)
+        for (int dy = -1; dy <= 1 && type == HHRR_FLUID; ++dy)
+          for (int dx = -1; dx <= 1; ++dx) {
+            if (!dx && !dy && !dz) continue;
+            int xx = wrap_any(x + dx, nx, a.dm.mode[0]);
+            int yy = wrap_any(y + dy, ny, a.dm.mode[1]);
+            int zz = wrap_any(z + dz, nz, a.dm.mode[2]);
+            if (a.phi[xx + snx * yy + snxy * zz] < a.h) {
+              type = HHRR_GROWTH;
+              break;
+            }
+          }
+    }
+    if (type == HHRR_FLUID || type == HHRR_FRINGE) tg = 0;
+    if (a.wm_enabled && type == HHRR_FRONTIER && phi > 0.0) {
+      int xm = wrap_any(x - 1, nx, a.dm.mode[0]), xp = wrap_any(x + 1, nx, a.dm.mode[0]);
+      int ym = wrap_any(y - 1, ny, a.dm.mode[1]), yp = wrap_any(y + 1, ny, a.dm.mode[1]);
+      int zm = wrap_any(z - 1, nz, a.dm.mode[2]), zp = wrap_any(z + 1, nz, a.dm.mode[2]);
+      double gr0 = 0.5 * (a.phi[xp + snx * y + snxy * z] - a.phi[xm + snx * y + snxy * z]);
+      double gr1 = 0.5 * (a.phi[x + snx * yp + snxy * z] - a.phi[x + snx * ym + snxy * z]);
+      double gr2 = 0.5 * (a.phi[x + snx * y + snxy * zp] - a.phi[x + snx * y + snxy * zm]);
+      double nn = sqrt(gr0 * gr0 + gr1 * gr1 + gr2 * gr2);
+      if (nn > 1e-12 && nn < 1e20) {
+        inw = 1;
+        y1v[0] = phi * (gr0 / nn);
+        y1v[1] = phi * (gr1 / nn);
+        y1v[2] = phi * (gr2 / nn);
+      }
+    }
+    inf = (type == HHRR_SOLID || type == HHRR_FRONTIER) && tg > 0;
+    uint8_t valid = inw ? (fl & WM_VALID) : 0;  // arrays of cells not in W_n are invalidated
+    a.flags[c] = (uint8_t)(type | (tg << TAG_SHIFT) | valid);
+    a.d[c] = d;
+  }
+  // warp-aggregated appends keep the lists nearly in cell order
+  unsigned lane = threadIdx.x & 31;
+  unsigned mw = __ballot_sync(0xffffffffu, inw);
+  if (mw) {
+    int base = 0;
+    if (lane == 0) base = atomicAdd(&a.cnt->wall_count, __popc(mw));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (inw) {
+      int slot = base + __popc(mw & ((1u << lane) - 1));
+      if (slot < a.cap_list) {
+        a.wall_idx[slot] = (int32_t)c;
+        a.wall_y1n[3 * (int64_t)slot] = y1v[0];
+        a.wall_y1n[3 * (int64_t)slot + 1] = y1v[1];
+        a.wall_y1n[3 * (int64_t)slot + 2] = y1v[2];
+      } else {
+        a.cnt->overflow = 1;
+      }
+    }
+  }
+  unsigned mf = __ballot_sync(0xffffffffu, inf);
+  if (mf) {
+    int base = 0;
+    if (lane == 0) base = atomicAdd(&a.cnt->force_count, __popc(mf));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (inf) {
+      int slot = base + __popc(mf & ((1u << lane) - 1));
+      if (slot < a.cap_list)
+        a.force_idx[slot] = (int32_t)c;
+      else
+        a.cnt->overflow = 1;
+    }
+  }
+}
+
+__global__ void counters_kernel(Counters* cnt, int op) {
+  if (op == 0) {  // start a full rebuild
+    cnt->wall_count = cnt->force_count = 0;
+    cnt->wall_static = cnt->force_static = 0;
+  } else if (op == 1) {  // static prefix complete
+    cnt->wall_count = min(cnt->wall_count, 0x7fffffff);
+    cnt->wall_static = cnt->wall_count;
+    cnt->force_static = cnt->force_count;
+  } else {  // start a box update
+    cnt->wall_count = cnt->wall_static;
+    cnt->force_count = cnt->force_static;
+  }
+}
+
+static void geo_grid(const GeoArgs& a, dim3& g, dim3& b) {
+  b = dim3(128);
+  if (a.inside) {
+    int bx = a.box.x1 - a.box.x0, by = a.box.y1 - a.box.y0, bz = a.box.z1 - a.box.z0;
+    g = dim3(by * bz, (bx + 127) / 128);
+  } else {
+    g = dim3(a.dm.ny * a.dm.nz, (a.dm.nx + 127) / 128);
+  }
+}
+
+cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
+  GeoArgs a;
+  a.dm = L->dom;
+  a.h = 0.5 * L->p.eps_cells;
+  a.eps = L->p.eps_cells;
+  a.has_static = L->has_static;
+  a.has_tag_static = L->has_tag_static;
+  a.has_override = L->has_override;
+  a.has_fringe = L->has_fringe;
+  a.has_rotor = L->has_rotor;
+  a.wm_enabled = L->wm_enabled;
+  a.fr_x0 = L->fr_x0;
+  a.fr_x1 = L->fr_x1;
+  a.cth = 1.0;
+  a.sth = 0.0;
+  Box none = {0, 0, 0, 0, 0, 0};
+  Box rb = none;
+  if (L->has_rotor) {
+    double th = L->rot.theta0 + (double)L->step * L->rot.omega;  // rigid rotation only
+    a.cth = cos(th);
+    a.sth = sin(th);
+    a.rot.sdf = L->rot_sdf;
+    a.rot.tag = L->rot_tag;
+    a.rot.gx = L->rot.gx;
+    a.rot.gy = L->rot.gy;
+    a.rot.gz = L->rot.gz;
+    a.rot.spacing = L->rot.spacing;
+    for (int k = 0; k < 3; ++k) {
+      a.rot.origin[k] = L->rot.origin[k];
+      a.rot.centre[k] = L->rot.centre[k];
+      a.rot.axis[k] = L->rot.axis[k];
+    }
+    rb = L->rot_box;
+  } else {
+    a.rot = RotorDev{};
+  }
+  a.phi_static = L->phi_static;
+  a.tag_static = L->tag_static;
+  a.d_override = L->d_override;
+  a.phi = L->phi;
+  a.flags = L->flags;
+  a.d = L->d;
+  a.wall_idx = L->wall_idx;
+  a.wall_y1n = L->wall_y1n;
+  a.force_idx = L->force_idx;
+  a.cnt = L->counters;
+  a.cap_list = (int)L->cap_list;
+  dim3 g, b;
+  bool box_empty = rb.x1 <= rb.x0 || rb.y1 <= rb.y0 || rb.z1 <= rb.z0;
+  if (full) {
+    // phi everywhere, then types: outside the rotor box first (static list prefix), box last
+    a.box = none;
+    a.inside = 0;
+    geo_grid(a, g, b);
+    geometry_phi_kernel<<<g, b, 0, L->stream>>>(a);
+    counters_kernel<<<1, 1, 0, L->stream>>>(L->counters, 0);
+    a.box = rb;
+    geometry_type_kernel<<<g, b, 0, L->stream>>>(a);
+    counters_kernel<<<1, 1, 0, L->stream>>>(L->counters, 1);
+    L->launches += 4;
+    if (!box_empty) {
+      a.inside = 1;
+      geo_grid(a, g, b);
+      geometry_type_kernel<<<g, b, 0, L->stream>>>(a);
+      L->launches++;
+    }
+  } else if (!box_empty) {
+    a.box = rb;
+    a.inside = 1;
+    geo_grid(a, g, b);
+    geometry_phi_kernel<<<g, b, 0, L->stream>>>(a);
+    counters_kernel<<<1, 1, 0, L->stream>>>(L->counters, 2);
+    geometry_type_kernel<<<g, b, 0, L->stream>>>(a);
+    L->launches += 3;
+  }
+  return cudaGetLastError();
+}
+
+}  // namespace hhrr

@@ -1,0 +1,117 @@
+// lattice.h -- internal state of an hhrr_lattice and the parameter blocks handed to kernels.
+// CUDA path only; shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/hhrr.h"
+
+namespace hhrr {
+
+constexpr int Q = HHRR_Q;
+constexpr int MAX_TAGS = HHRR_MAX_TAGS;
+constexpr int64_t FORCE_HISTORY = 4096;  // ring of per-step force records
+constexpr double BIG_PHI = 1.0e30;       // "no geometry here"
+
+// flags byte per cell: bits 0-2 hhrr_cell_type, bits 3-6 element tag, bit 7 wall-model state valid
+constexpr uint8_t TYPE_MASK = 0x07;
+constexpr int TAG_SHIFT = 3;
+constexpr uint8_t TAG_MASK = 0x0f;
+constexpr uint8_t WM_VALID = 0x80;
+
+struct Dom {
+  int nx, ny, nz;
+  int mode[3];
+  int64_t n;
+};
+
+// rigid bodies, fp32 copy for the collide kernel, fp64 for wall model / force
+struct BodiesF {
+  float c[MAX_TAGS][3], w[MAX_TAGS][3], v[MAX_TAGS][3];
+};
+struct BodiesD {
+  double c[MAX_TAGS][3], w[MAX_TAGS][3], v[MAX_TAGS][3];
+};
+
+struct PhysF {
+  float tau0, sigma, smag18;  // smag18 = 18 C_S^2 (Eq. 14 closed form, R6)
+  float g[3];
+  float fr_u[3];
+};
+
+struct Box {  // half-open cell box
+  int x0, x1, y0, y1, z0, z1;
+};
+
+struct RotorDev {
+  const float* sdf;
+  const uint8_t* tag;
+  int gx, gy, gz;
+  double spacing, origin[3], centre[3], axis[3];
+};
+
+// counters living in device memory
+struct Counters {
+  int wall_count, force_count;
+  int wall_static, force_static;  // list prefix owned by cells outside the rotor box
+  int overflow;
+  int nonfinite;
+  int pad[2];
+};
+
+}  // namespace hhrr
+
+struct hhrr_lattice {
+  hhrr_params p;
+  hhrr::Dom dom;
+  cudaStream_t stream;
+  int device;
+  // device arrays (inside the caller's workspace)
+  float *fA, *fB;           // 27 planes each: post-stream populations minus weights
+  uint8_t* flags;           // N
+  float* d;                 // N porosity (read for FRONTIER cells only)
+  double* phi;              // N signed distance of the last geometry
+  float* phi_static;        // N
+  uint8_t* tag_static;      // N
+  float* d_override;        // N
+  float* uhat;              // 3N (two-pass variant, init, tests)
+  double* wm_utau;          // N
+  float* wm_u;              // 3N
+  float* wm_s;              // 6N
+  int32_t* wall_idx;        // cap_list
+  double* wall_y1n;         // 3*cap_list (AoS)
+  int32_t* force_idx;       // cap_list
+  hhrr::Counters* counters; // 1
+  double* force;            // FORCE_HISTORY * MAX_TAGS * 3
+  float* rot_sdf;
+  uint8_t* rot_tag;
+  int64_t rot_nodes_cap;
+  int64_t cap_list;
+  // host state
+  bool has_static, has_tag_static, has_override, has_fringe, has_rotor, wm_enabled;
+  int fr_x0, fr_x1;
+  double fr_u[3];
+  hhrr_rotor_desc rot;  // sdf/tag pointers nulled
+  hhrr::Box rot_box;
+  hhrr::BodiesD bodies;
+  bool geometry_dirty;     // full-domain geometry pass needed
+  bool geometry_current;   // geometry(step) evaluated
+  int64_t step;
+  int variant;
+  int64_t launches;
+};
+
+// ---- kernel launchers (one per translation unit) ---------------------------------------
+namespace hhrr {
+// geometry.cu (compiled with -fmad=false: operation order is part of the definition)
+cudaError_t launch_geometry(hhrr_lattice* L, bool full);
+// collide.cu
+cudaError_t launch_fill_rest(hhrr_lattice* L);
+cudaError_t launch_init(hhrr_lattice* L, const float* d_rho, const float* d_u, int with_neq);
+cudaError_t launch_collide_stream(hhrr_lattice* L);
+cudaError_t launch_moments(hhrr_lattice* L, float* d_rho, float* d_v);
+cudaError_t launch_check_finite(hhrr_lattice* L);
+// wallmodel.cu
+cudaError_t launch_wall_model(hhrr_lattice* L);
+cudaError_t launch_forces(hhrr_lattice* L);
+}  // namespace hhrr

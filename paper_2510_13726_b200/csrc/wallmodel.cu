@@ -1,0 +1,251 @@
+// wallmodel.cu -- K3: WallModelO (Listing 3 line 4; Eq. 15-20 :159-184; :186;
+// :324) on the compact wall-cell list, and K4: boundary force collection + per-element
+// integration (Listing 3 lines 5-6, :315-317; Eq. 23 :211; :267).
+//
+// Both kernels touch 1e4-1e5 cells, so they run in fp64 on the fp32 populations: the Newton
+// stop rule (:184) decides an iteration count, and it is taken in the same precision as the
+// oracle takes it.  Forces accumulate in fp64.  CUDA path only; shares nothing with oracle/.
+#include "d3q27.cuh"
+
+namespace hhrr {
+
+struct WmArgs {
+  Dom dm;
+  double g[3];
+  double nu, kappa, E, tol, hs;
+  int max_iter;
+  BodiesD bo;
+  const float* f;  // post-stream populations (deviations)
+  uint8_t* flags;
+  const int32_t* wall_idx;
+  const double* wall_y1n;
+  const Counters* cnt;
+  int cap_list;
+  double* wm_utau;
+  float* wm_u;
+  float* wm_s;
+};
+
+__device__ __forceinline__ int wrap_far(int v, int n, int mode, bool& flip) {
+  flip = false;
+  if (v >= 0 && v < n) return v;
+  if (mode == HHRR_PERIODIC) return ((v % n) + n) % n;
+  flip = true;
+  return v < 0 ? -1 - v : 2 * n - 1 - v;
+}
+
+// reported velocity moment v = (j + g/2)/rho of a cell (R11)
+__device__ __forceinline__ void cell_velocity_d(const float* __restrict__ f, int64_t n, int64_t c,
+                                                const double g[3], double v[3]) {
+  double drho = 0, j0 = 0, j1 = 0, j2 = 0;
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    double fi = (double)__ldg(f + (int64_t)i * n + c);
+    drho += fi;
+    j0 += dir_cx(i) * fi;
+    j1 += dir_cy(i) * fi;
+    j2 += dir_cz(i) * fi;
+  }
+  double ir = 1.0 / (1.0 + drho);
+  v[0] = (j0 + 0.5 * g[0]) * ir;
+  v[1] = (j1 + 0.5 * g[1]) * ir;
+  v[2] = (j2 + 0.5 * g[2]) * ir;
+}
+
+__device__ __forceinline__ void body_velocity_d(const BodiesD& bo, int k, int x, int y, int z, double us[3]) {
+  double r0 = x - bo.c[k][0], r1 = y - bo.c[k][1], r2 = z - bo.c[k][2];
+  us[0] = bo.v[k][0] + (bo.w[k][1] * r2 - bo.w[k][2] * r1);
+  us[1] = bo.v[k][1] + (bo.w[k][2] * r0 - bo.w[k][0] * r2);
+  us[2] = bo.v[k][2] + (bo.w[k][0] * r1 - bo.w[k][1] * r0);
+}
+
+// truncated Spalding law (Eq. 18) and its u_tau derivative (R9)
+__device__ __forceinline__ double spalding_f(double ut, double U, double y, double nu, double kap, double E) {
+  double up = U / ut, k = kap * up;
+  return up + (exp(k) - 1.0 - k - 0.5 * k * k - k * k * k / 6.0) / E - y * ut / nu;
+}
+__device__ __forceinline__ double spalding_df(double ut, double U, double y, double nu, double kap, double E) {
+  double up = U / ut, k = kap * up;
+  return -(U / (ut * ut)) * (1.0 + (kap / E) * (exp(k) - 1.0 - k - 0.5 * k * k)) - y / nu;
+}
+
+__global__ void __launch_bounds__(128) wall_model_kernel(WmArgs a) {
+  const int count = min(a.cnt->wall_count, a.cap_list);
+  const int64_t n = a.dm.n, nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
+  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < count; e += gridDim.x * blockDim.x) {
+    int64_t c = a.wall_idx[e];
+    int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
+    double y1v[3] = {a.wall_y1n[3 * (int64_t)e], a.wall_y1n[3 * (int64_t)e + 1], a.wall_y1n[3 * (int64_t)e + 2]};
+    double y1 = sqrt(y1v[0] * y1v[0] + y1v[1] * y1v[1] + y1v[2] * y1v[2]);
+    double nrm[3] = {y1v[0] / y1, y1v[1] / y1, y1v[2] / y1};
+    // velocity at x_w + h_s n, trilinear over the 8 surrounding cells (R15)
+    double px = x + a.hs * nrm[0], py = y + a.hs * nrm[1], pz = z + a.hs * nrm[2];
+    double fx = floor(px), fy = floor(py), fz = floor(pz);
+    double tx = px - fx, ty = py - fy, tz = pz - fz;
+    int ix = (int)fx, iy = (int)fy, iz = (int)fz;
+    double vs[3] = {0, 0, 0};
+    for (int k = 0; k < 8; ++k) {
+      int ox = k & 1, oy = (k >> 1) & 1, oz = (k >> 2) & 1;
+      double w = (ox ? tx : 1.0 - tx) * (oy ? ty : 1.0 - ty) * (oz ? tz : 1.0 - tz);
+      bool flx, fly, flz;
+      int xx = wrap_far(ix + ox, a.dm.nx, a.dm.mode[0], flx);
+      int yy = wrap_far(iy + oy, a.dm.ny, a.dm.mode[1], fly);
+      int zz = wrap_far(iz + oz, a.dm.nz, a.dm.mode[2], flz);
+      double v[3];
+      cell_velocity_d(a.f, n, xx + nx * yy + nxy * zz, a.g, v);
+      if (flx) v[0] = -v[0];
+      if (fly) v[1] = -v[1];
+      if (flz) v[2] = -v[2];
+      vs[0] += w * v[0];
+      vs[1] += w * v[1];
+      vs[2] += w * v[2];
+    }
+    double vw[3], us[3];
+    cell_velocity_d(a.f, n, c, a.g, vw);
+    uint8_t fl = a.flags[c];
+    body_velocity_d(a.bo, (fl >> TAG_SHIFT) & TAG_MASK, x, y, z, us);
+    double r[3], rn = 0.0;
+    for (int q = 0; q < 3; ++q) {
+      r[q] = vs[q] - us[q];
+      rn += r[q] * nrm[q];
+    }
+    double ut[3], U = 0.0;
+    for (int q = 0; q < 3; ++q) {
+      ut[q] = r[q] - rn * nrm[q];
+      U += ut[q] * ut[q];
+    }
+    U = sqrt(U);
+    double utau = 0.0;
+    double uw[3] = {0, 0, 0}, sw[6] = {0, 0, 0, 0, 0, 0};
+    if (!(U < 1e-14)) {
+      double yy = y1 + a.hs;
+      double prev = a.wm_utau[c];
+      double ua = ((fl & WM_VALID) && prev > 0.0) ? prev : sqrt(a.nu * U / yy);  // Eq. 20
+      // Newton-Raphson (Eq. 19), stop rule of PAPER.md:184
+      double fa = spalding_f(ua, U, yy, a.nu, a.kappa, a.E), ub = ua;
+      for (int it = 0; it < a.max_iter; ++it) {
+        ub = ua - fa / spalding_df(ua, U, yy, a.nu, a.kappa, a.E);
+        if (!(ub > 0.0)) ub = 0.5 * ua;
+        double fb = spalding_f(ub, U, yy, a.nu, a.kappa, a.E);
+        double df = fabs(fb - fa);
+        ua = ub;
+        fa = fb;
+        if (df < a.tol) break;
+      }
+      utau = ub;
+      for (int q = 0; q < 3; ++q) uw[q] = utau * ut[q] / U;  // R8
+      double G[3][3];
+      for (int p = 0; p < 3; ++p)
+        for (int q = 0; q < 3; ++q) G[p][q] = (vs[p] - vw[p]) * nrm[q] / a.hs;  // R10
+      sw[0] = G[0][0];
+      sw[1] = G[1][1];
+      sw[2] = G[2][2];
+      sw[3] = 0.5 * (G[0][1] + G[1][0]);
+      sw[4] = 0.5 * (G[0][2] + G[2][0]);
+      sw[5] = 0.5 * (G[1][2] + G[2][1]);
+    }
+    a.wm_utau[c] = utau;
+    for (int q = 0; q < 3; ++q) a.wm_u[(int64_t)q * n + c] = (float)uw[q];
+    for (int q = 0; q < 6; ++q) a.wm_s[(int64_t)q * n + c] = (float)sw[q];
+    a.flags[c] = fl | WM_VALID;
+  }
+}
+
+// ---------------------------------------------------------------------------- K4 forces
+struct ForceArgs {
+  Dom dm;
+  BodiesD bo;
+  const float* f;
+  const uint8_t* flags;
+  const int32_t* force_idx;
+  const Counters* cnt;
+  int cap_list;
+  double* out;  // [MAX_TAGS][3] of this step (zeroed by the kernel launched before)
+};
+
+__global__ void zero_force_kernel(double* out) {
+  if (threadIdx.x < MAX_TAGS * 3) out[threadIdx.x] = 0.0;
+}
+
+// F_k = - sum_{x: d<1, tag=k} sum_{i != rest} [(c_i - u^s) f_i(x + c_i) + (c_i + u^s) f_ibar(x)]
+// (Eq. 23 with reading R7), fp64 accumulation: thread -> shared per-tag bins -> global atomics.
+__global__ void __launch_bounds__(128) force_kernel(ForceArgs a) {
+  __shared__ double bins[MAX_TAGS * 3];
+  for (int t = threadIdx.x; t < MAX_TAGS * 3; t += blockDim.x) bins[t] = 0.0;
+  __syncthreads();
+  const int count = min(a.cnt->force_count, a.cap_list);
+  const int64_t n = a.dm.n, nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
+  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < count; e += gridDim.x * blockDim.x) {
+    int64_t c = a.force_idx[e];
+    int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
+    int k = (a.flags[c] >> TAG_SHIFT) & TAG_MASK;
+    double us[3];
+    body_velocity_d(a.bo, k, x, y, z, us);
+    double acc[3] = {0, 0, 0};
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+      if (i == 13) continue;
+      bool fl;
+      int xx = wrap_far(x + dir_cx(i), a.dm.nx, a.dm.mode[0], fl);
+      int yy = wrap_far(y + dir_cy(i), a.dm.ny, a.dm.mode[1], fl);
+      int zz = wrap_far(z + dir_cz(i), a.dm.nz, a.dm.mode[2], fl);
+      // stored values are deviations: f = w + dev, and w_i = w_ibar
+      double w = dir_wd(i);
+      double fa = w + (double)__ldg(a.f + (int64_t)i * n + (xx + nx * yy + nxy * zz));
+      double fb = w + (double)__ldg(a.f + (int64_t)(26 - i) * n + c);
+      double ci[3] = {(double)dir_cx(i), (double)dir_cy(i), (double)dir_cz(i)};
+      for (int q = 0; q < 3; ++q) acc[q] += (ci[q] - us[q]) * fa + (ci[q] + us[q]) * fb;
+    }
+    for (int q = 0; q < 3; ++q) atomicAdd(&bins[k * 3 + q], -acc[q]);
+  }
+  __syncthreads();
+  for (int t = threadIdx.x; t < MAX_TAGS * 3; t += blockDim.x)
+    if (bins[t] != 0.0) atomicAdd(&a.out[t], bins[t]);
+}
+
+// ---------------------------------------------------------------------------- launchers
+static void fill_bodies(const hhrr_lattice* L, BodiesD& b) { b = L->bodies; }
+
+cudaError_t launch_wall_model(hhrr_lattice* L) {
+  if (!L->wm_enabled) return cudaSuccess;
+  WmArgs a;
+  a.dm = L->dom;
+  for (int q = 0; q < 3; ++q) a.g[q] = L->p.body_force[q];
+  a.nu = (L->p.tau0 - 0.5) / 3.0;
+  a.kappa = L->p.kappa;
+  a.E = L->p.E;
+  a.tol = L->p.newton_tol;
+  a.hs = L->p.sampling_distance;
+  a.max_iter = L->p.newton_max_iter;
+  fill_bodies(L, a.bo);
+  a.f = L->fA;
+  a.flags = L->flags;
+  a.wall_idx = L->wall_idx;
+  a.wall_y1n = L->wall_y1n;
+  a.cnt = L->counters;
+  a.cap_list = (int)L->cap_list;
+  a.wm_utau = L->wm_utau;
+  a.wm_u = L->wm_u;
+  a.wm_s = L->wm_s;
+  wall_model_kernel<<<592, 128, 0, L->stream>>>(a);
+  L->launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_forces(hhrr_lattice* L) {
+  ForceArgs a;
+  a.dm = L->dom;
+  fill_bodies(L, a.bo);
+  a.f = L->fA;
+  a.flags = L->flags;
+  a.force_idx = L->force_idx;
+  a.cnt = L->counters;
+  a.cap_list = (int)L->cap_list;
+  a.out = L->force + (L->step % FORCE_HISTORY) * MAX_TAGS * 3;
+  zero_force_kernel<<<1, 64, 0, L->stream>>>(a.out);
+  force_kernel<<<296, 128, 0, L->stream>>>(a);
+  L->launches += 2;
+  return cudaGetLastError();
+}
+
+}  // namespace hhrr

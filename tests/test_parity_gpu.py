@@ -1,0 +1,175 @@
+"""GPU-vs-oracle parity through the C ABI (run with -m gpu on a B200).
+
+Both sides are driven by paper_2510_13726_b200.inputs.apply_case from the same seeded fp32
+inputs.  Bars (BASELINE.json north_star):
+  rel-Linf(q) = max_x |q_gpu - q_ora| / max_x |q_ora|  for rho and for the velocity vector:
+  <= 1e-5 after 10 steps, <= 1e-3 at the end of long runs; cell types, tags and the
+  wall-model list bit-exact; forces <= 1e-5 (10 steps) relative to the largest component.
+"""
+import numpy as np
+import pytest
+
+from paper_2510_13726_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+TOL10 = 1e-5
+TOL_LONG = 1e-3
+
+
+def _gpu_lattice(case, variant, rotor_shape=None):
+    from paper_2510_13726_b200 import binding as B
+    p = B.make_params(case.nx, case.ny, case.nz, mode=case.mode, **case.params)
+    if case.rotor is not None:
+        rotor_shape = case.rotor["sdf"].shape
+    L = B.Lattice(p, rotor_shape=rotor_shape)
+    L.set_kernel_variant(variant)
+    I.apply_case(case, L)
+    return L
+
+
+def _ora_lattice(O, case):
+    p = O.make_params(case.nx, case.ny, case.nz, mode=case.mode, **case.params)
+    L = O.Lattice(p)
+    I.apply_case(case, L)
+    return L
+
+
+def rel_linf(rho_g, v_g, rho_o, v_o):
+    e_rho = np.max(np.abs(rho_g.astype(np.float64) - rho_o)) / np.max(np.abs(rho_o))
+    dv = np.linalg.norm(v_g.astype(np.float64) - v_o, axis=0)
+    e_v = dv.max() / np.linalg.norm(v_o, axis=0).max()
+    return e_rho, e_v
+
+
+def compare_geometry(G, Oa):
+    tg, gg, dg = G.cell_types()
+    to, go, do = Oa.cell_types()
+    assert np.array_equal(tg, to), f"{np.count_nonzero(tg != to)} cell types differ"
+    assert np.array_equal(gg, go), f"{np.count_nonzero(gg != go)} tags differ"
+    assert np.max(np.abs(dg.astype(np.float64) - do)) <= 1e-7
+    ig, yg, ug, vg = G.wall_list()
+    io, yo, uo, vo = Oa.wall_list()
+    assert np.array_equal(ig, io), "wall-model cell lists differ"
+    assert np.array_equal(vg, vo), "wall-model valid flags differ"
+    if len(io):
+        assert np.max(np.abs(yg - yo)) <= 1e-12
+        assert np.max(np.abs(ug - uo)) <= 1e-6 * max(np.max(np.abs(uo)), 1e-30) + 1e-12
+
+
+def compare_forces(G, Oa, tol):
+    Fg, Fo = G.forces(), Oa.forces()
+    scale = np.max(np.abs(Fo))
+    if scale > 0:
+        assert np.max(np.abs(Fg - Fo)) <= tol * scale, (np.max(np.abs(Fg - Fo)), scale)
+
+
+def run_parity(oracle, case, steps, variant, tol, check_every=None, force_tol=None):
+    G, Oa = _gpu_lattice(case, variant), _ora_lattice(oracle, case)
+    done = 0
+    chunk = check_every or steps
+    G.update_geometry(); Oa.update_geometry()
+    compare_geometry(G, Oa)
+    while done < steps:
+        k = min(chunk, steps - done)
+        G.step(k); Oa.step(k)
+        done += k
+        compare_geometry(G, Oa)
+    G.check_finite()
+    e_rho, e_v = rel_linf(*G.moments(), *Oa.moments())
+    assert e_rho <= tol and e_v <= tol, (e_rho, e_v)
+    compare_forces(G, Oa, force_tol or tol)
+    G.close(); Oa.close()
+    return e_rho, e_v
+
+
+VARIANTS = [0, 1]
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_config1_tgv32_10_steps(oracle, variant):
+    """BASELINE.json config 1 at full size."""
+    run_parity(oracle, I.baseline_config(1), 10, variant, TOL10)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_tgv_ragged_extents(oracle, variant):
+    """Extents that are no multiple of any tile: several tiles and a ragged tail on every axis."""
+    rho, u = I.noisy_uniform(45, 19, 23, (0.03, -0.02, 0.01), 5e-3, 77)
+    case = I.Case("ragged", 45, 19, 23, 10, params=dict(I.DEFAULTS, tau0=0.53), rho=rho, u=u, with_neq=True)
+    run_parity(oracle, case, 10, variant, TOL10)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_tiny_lattices(oracle, variant):
+    """Degenerate extents: a single cell row / plane wraps onto itself."""
+    for ext in [(1, 1, 1), (5, 1, 1), (3, 4, 1), (2, 2, 2), (33, 2, 3)]:
+        rho, u = I.noisy_uniform(*ext, (0.02, 0.01, -0.01), 2e-3, 5)
+        case = I.Case("tiny", *ext, 5, params=dict(I.DEFAULTS, tau0=0.6), rho=rho, u=u)
+        run_parity(oracle, case, 5, variant, TOL10)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_mirror_axes(oracle, variant):
+    """Free-slip mirror planes on every axis (reading R12)."""
+    rho, u = I.noisy_uniform(20, 12, 9, (0.0, 0.0, 0.0), 1e-2, 9)
+    case = I.Case("mirror", 20, 12, 9, 10, mode=(I.MIRROR, I.MIRROR, I.MIRROR),
+                  params=dict(I.DEFAULTS, tau0=0.56), rho=rho, u=u, with_neq=True)
+    run_parity(oracle, case, 10, variant, TOL10)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_config2_sphere_small_and_full(oracle, variant):
+    """Config 2: reduced size stepwise, then the full 128x64x64 / 200 steps."""
+    run_parity(oracle, I.case_sphere(64, 32, 32, 5.0, 10), 10, variant, TOL10, check_every=5)
+    e = run_parity(oracle, I.baseline_config(2), 200, variant, TOL_LONG, check_every=100, force_tol=TOL_LONG)
+    print("config2 200 steps rel-Linf", e)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_config3_channel_reduced(oracle, variant):
+    """Config 3 recipe at 64x48x32: body force, mirror top, porosity-0 wall, wall-model list, Newton."""
+    case = I.case_channel(64, 48, 32, 60)
+    run_parity(oracle, case, 10, variant, TOL10, check_every=1)
+    run_parity(oracle, case, 60, variant, TOL_LONG, check_every=30, force_tol=TOL_LONG)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_config3_log_law_branch(oracle, variant):
+    """Config 3b: Re_tau = 5050 puts the sampling point in the log layer (exp branch of Eq. 18)."""
+    case = I.case_channel(48, 40, 24, 10, re_tau=5050.0)
+    run_parity(oracle, case, 10, variant, TOL10, check_every=2)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_config4_rotor_reduced(oracle, variant):
+    """Config 4 recipe at 96x72x72, R = 20: rotating porosity, tags, growth layer, wall list
+    and per-blade forces, geometry compared bit-exact after every step."""
+    case = I.case_rotor(96, 72, 72, 20.0, 12, omega=0.012)
+    run_parity(oracle, case, 12, variant, TOL10, check_every=1)
+
+
+def test_moving_static_body_and_checkpoint(oracle):
+    """set_body on a static solid (translating sphere) and populations round trip."""
+    case = I.case_sphere(48, 24, 24, 4.0, 6)
+    G, Oa = _gpu_lattice(case, 1), _ora_lattice(oracle, case)
+    for L in (G, Oa):
+        L.set_body(1, centre=(12, 11.5, 11.5), omega=(0.0, 0.0, 0.002), vel=(0.01, 0.0, 0.0))
+    G.step(3); Oa.step(3)
+    f = G.populations()
+    G2 = _gpu_lattice(case, 1)
+    G2.set_body(1, centre=(12, 11.5, 11.5), omega=(0.0, 0.0, 0.002), vel=(0.01, 0.0, 0.0))
+    G2.set_populations(f)
+    G.step(3); G2.step(3); Oa.step(3)
+    assert np.array_equal(G.populations(), G2.populations())
+    e_rho, e_v = rel_linf(*G.moments(), *Oa.moments())
+    assert e_rho <= TOL10 and e_v <= TOL10, (e_rho, e_v)
+
+
+def test_variants_agree_bitwise_on_moments_order():
+    """The two kernel variants implement the same arithmetic; they must agree to rounding."""
+    case = I.case_sphere(64, 32, 32, 5.0, 20)
+    A, Bv = _gpu_lattice(case, 0), _gpu_lattice(case, 1)
+    A.step(20); Bv.step(20)
+    e_rho, e_v = rel_linf(*A.moments(), *[x.astype(np.float64) for x in Bv.moments()])
+    assert e_rho <= 1e-6 and e_v <= 1e-5, (e_rho, e_v)

@@ -1,0 +1,303 @@
+#!/usr/bin/env python
+"""bench.py -- MLUPs of the fused HHRRLBM + wall-model step on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
+
+A "step" is one pass of Listing 3: rotor/porosity update, fused
+collide-stream, wall model, per-element force reduction.  At N = 1 the workload is
+BASELINE.json config 5: the 768x384x364 (~107 M cells) block holding one synthetic rotor of
+radius 120 cells.  The path does not shard (north_star: one GPU, no collectives): with N > 1
+every rank runs an independent replica ("replicas only", weak scaling), timed as the max
+over ranks.  Prints ONE JSON line on rank 0.
+
+--impl reference times the fp64 CPU oracle (oracle/) as it stands on the host cores, on a
+bounded sample of the same recipe (there is no reference implementation to install; see
+DESIGN.md "Reference arm").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+from paper_2510_13726_b200 import inputs as I  # noqa: E402  (seeded input recipes only)
+
+METRIC = "MLUPs (fused HHRRLBM+wall-model step) on 1 B200 and % of HBM peak GB/s"
+BYTES_PER_CELL = 216.0  # 27 x 4 B read + 27 x 4 B write
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def measured_peak():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            return float(json.loads(p.read_text())["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def workload(config: int) -> tuple[I.Case, str]:
+    case = I.baseline_config(config)
+    names = {1: "config1 TGV 32^3", 2: "config2 sphere channel 128x64x64", 3: "config3 half-channel 256x128x128",
+             4: "config4 rotor R=80 512x256x256", 5: "config5 rotor R=120 768x384x364 (~107M cells)"}
+    return case, names[config]
+
+
+# ------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons = [], None, set()
+        rows = [r for t, r in self.rows if t0 - 0.05 <= t <= t1 + 0.15] or [r for _, r in self.rows]
+        for r in rows:
+            c = [x.strip() for x in r.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0]))
+                smax = float(c[1])
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------- CPU oracle leg
+def oracle_sample(config: int, budget_s: float = 20.0):
+    """Times the oracle as it stands on a bounded sample of the config's recipe."""
+    from oracle import oracle as O
+    O.build()
+    if config >= 4:
+        case = I.case_rotor(192, 96, 91, 30.0, 4, omega=0.002 * 4)
+        sample = "config-5 recipe scaled 1/4 (192x96x91 cells, rotor R=30, wall model + forces on)"
+    elif config == 3:
+        case = I.case_channel(128, 64, 64, 4)
+        sample = "config-3 recipe at 128x64x64"
+    else:
+        case = I.baseline_config(config)
+        sample = f"config {config} at full size"
+    p = O.make_params(case.nx, case.ny, case.nz, mode=case.mode, **case.params)
+    L = O.Lattice(p)
+    I.apply_case(case, L)
+    L.step(1)  # warm-up (first-touch, geometry)
+    t0 = time.perf_counter()
+    steps = 0
+    while True:
+        L.step(1)
+        steps += 1
+        dt = time.perf_counter() - t0
+        if dt > budget_s or steps >= 50:
+            break
+    L.close()
+    mlups = case.n * steps / dt / 1e6
+    return {"value": mlups, "unit": "MLUPs", "cores": O.threads(), "kind": "oracle",
+            "sample": f"{sample}, {steps} steps in {dt:.1f} s"}, dt / steps
+
+
+def run_reference(args, rank, world):
+    """Reference arm: the oracle on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    case, wname = workload(args.config)
+    per_step_budget = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    from oracle import oracle as O
+    O.build()
+    base, _ = oracle_sample(args.config, budget_s=1.0)  # warm the build / page cache
+    t_all, v_all = [], []
+    for s in range(args.warmup + args.steps):
+        cb, t_step = oracle_sample(args.config, budget_s=per_step_budget)
+        if s >= args.warmup:
+            t_all.append(t_step)
+            v_all.append(cb["value"])
+    value = float(np.mean(v_all))
+    cb["value"] = value
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "MLUPs", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(np.mean(t_all) * 1e3),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": wname, "note": "each step = one bounded oracle sample"},
+            "cpu_baseline": cb,
+            "e2e": {"value": value, "unit": "MLUPs", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2510_13726_b200 import binding as B, build
+
+    build.build()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA library is the only implementation)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    dev = f"cuda:{local_rank}"
+
+    case, wname = workload(args.config)
+    p = B.make_params(case.nx, case.ny, case.nz, mode=case.mode, **case.params)
+    L = B.Lattice(p, rotor_shape=None if case.rotor is None else case.rotor["sdf"].shape, device=dev)
+    L.set_kernel_variant(args.variant)
+    I.apply_case(case, L)
+    n = case.n
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    L.step(args.warmup)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    L.set_timing(True)
+    launches0 = L.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_wall0 = time.time()
+    ev0.record(L.stream)
+    L.step(args.steps)
+    ev1.record(L.stream)
+    barrier()
+    t_wall1 = time.time()
+    ms = ev0.elapsed_time(ev1)
+    launches = L.launch_count() - launches0
+    k_ms, k_n = L.timing()
+    L.set_timing(False)
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    L.check_finite()
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * n * args.steps / (ms * 1e3)
+
+    # end to end through the C ABI with HOST buffers: upload the populations from pinned host
+    # memory, step, read moments and forces back -- all inside the timed region
+    e2e_steps = args.steps
+    h_f = torch.empty((27, n), dtype=torch.float32).pin_memory()
+    h_rho = torch.empty(n, dtype=torch.float32).pin_memory()
+    h_v = torch.empty((3, n), dtype=torch.float32).pin_memory()
+    lib = B.lib()
+    import ctypes as C
+    B._check(lib.hhrr_get_populations(L.h, C.c_void_p(h_f.data_ptr())))
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(L.stream)
+    B._check(lib.hhrr_set_populations(L.h, C.c_void_p(h_f.data_ptr())))
+    L.step(e2e_steps)
+    B._check(lib.hhrr_get_moments(L.h, C.c_void_p(h_rho.data_ptr()), C.c_void_p(h_v.data_ptr())))
+    F = L.forces(L.step_count() - min(e2e_steps, 1024), min(e2e_steps, 1024))
+    e1.record(L.stream)
+    barrier()
+    e2e_ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e = {"value": world * n * e2e_steps / (e2e_ms * 1e3), "unit": "MLUPs",
+           "h2d_bytes_per_step": h_f.numel() * 4 / e2e_steps,
+           "d2h_bytes_per_step": (h_rho.numel() + h_v.numel()) * 4 / e2e_steps + F.nbytes / e2e_steps,
+           "steps": e2e_steps, "ms_total": e2e_ms,
+           "what": "hhrr_set_populations(pinned host) + hhrr_step + hhrr_get_moments(pinned host) + hhrr_get_forces"}
+    thrust = float(F[-1, 1:5, 0].sum()) if case.rotor is not None else None
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        k_avg_ms = k_ms / max(1, k_n)
+        achieved = n * BYTES_PER_CELL / (k_avg_ms * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": "fused_kernel" if args.variant == 1 else "moments_kernel+collide_kernel",
+                    "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                    "peak_source": peak_src, "kernel_ms": k_avg_ms, "kernel_launches_timed": k_n,
+                    "kernel_share_of_step": k_ms / (ms * k_n / args.steps) if k_n else None,
+                    "algorithmic_bytes_per_cell": BYTES_PER_CELL}
+        tr = ROOT / "profiles" / "traffic.json"   # DRAM bytes per launch from the committed ncu capture
+        if tr.exists():
+            try:
+                t = json.loads(tr.read_text())
+                if t.get("cells") == n and t.get("variant") == args.variant:
+                    roofline["traffic"] = t["dram_bytes_per_launch"]
+            except Exception:
+                pass
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            cpu, _ = oracle_sample(args.config, budget_s=15.0)
+        line = {"metric": METRIC, "value": value, "unit": "MLUPs", "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": wname, "cells_per_gpu": n, "lattice": "D3Q27", "storage": "fp32 SoA A/B",
+                           "kernel_variant": args.variant, "parallelism": f"replicas x{world}",
+                           "l2": "inputs (11.6 GB per buffer) exceed the 126 MB L2; no flush needed"},
+                "hbm_frac_of_peak_step": value * 1e6 * BYTES_PER_CELL / 1e9 / peak / world,
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
+                "clocks": clocks, "thrust_last_step": thrust}
+        print(json.dumps(line), flush=True)
+    L.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=100)
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--variant", type=int, default=1, choices=[0, 1])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

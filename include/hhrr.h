@@ -166,6 +166,12 @@ int hhrr_check_finite(hhrr_lattice* L);
 /* Selects the collide-stream kernel: 0 = two-pass (moments pass + collide pass),
  * 1 = fused sliding-window kernel (default).  Both compute the same step.           */
 int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant);
+/* Optional CUDA-event timing of the collide-stream launches inside hhrr_step (the kernel the
+ * roofline is quoted on).  hhrr_get_timing synchronises, returns the summed device time in
+ * milliseconds and the number of launches it covers (at most 1024 per window), and starts a
+ * new window.                                                                              */
+int hhrr_set_timing(hhrr_lattice* L, int enable);
+int hhrr_get_timing(hhrr_lattice* L, double* ms_collide_stream, int64_t* launches);
 /* Number of kernel launches issued by this lattice so far. */
 int64_t hhrr_launch_count(const hhrr_lattice* L);
 

@@ -28,7 +28,7 @@ SYMBOLS = [
     "hhrr_get_moments", "hhrr_get_moments_device", "hhrr_get_forces", "hhrr_force_history",
     "hhrr_get_cell_types", "hhrr_get_wall_list", "hhrr_get_wall_state", "hhrr_get_populations",
     "hhrr_set_populations", "hhrr_get_uhat", "hhrr_check_finite", "hhrr_set_kernel_variant",
-    "hhrr_launch_count", "hhrr_last_error", "hhrr_version",
+    "hhrr_set_timing", "hhrr_get_timing", "hhrr_launch_count", "hhrr_last_error", "hhrr_version",
 ]
 
 
@@ -95,6 +95,8 @@ def lib():
         L.hhrr_get_uhat.argtypes = [vp, vp]
         L.hhrr_check_finite.argtypes = [vp]
         L.hhrr_set_kernel_variant.argtypes = [vp, i32]
+        L.hhrr_set_timing.argtypes = [vp, C.c_int]
+        L.hhrr_get_timing.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
         L.hhrr_launch_count.restype = i64
         L.hhrr_launch_count.argtypes = [vp]
         L.hhrr_last_error.restype = C.c_char_p
@@ -237,6 +239,15 @@ class Lattice:
 
     def launch_count(self):
         return lib().hhrr_launch_count(self.h)
+
+    def set_timing(self, enable=True):
+        _check(lib().hhrr_set_timing(self.h, int(enable)))
+
+    def timing(self):
+        """(summed collide-stream device ms, launches covered) since the last call."""
+        ms, k = C.c_double(0), C.c_int64(0)
+        _check(lib().hhrr_get_timing(self.h, C.byref(ms), C.byref(k)))
+        return ms.value, k.value
 
     def check_finite(self):
         _check(lib().hhrr_check_finite(self.h))

@@ -174,7 +174,7 @@ int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes,
   int64_t rest = (int64_t)(workspace_bytes - lead - need_min);
   int64_t spare = std::max<int64_t>(0, (rest - 512) / 5);
   carve(L, p, spare, base);
-  L->variant = 0;
+  L->variant = 1;
   L->geometry_dirty = true;
   L->geometry_current = false;
   const int64_t n = L->dom.n;
@@ -203,6 +203,8 @@ int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes,
 int hhrr_destroy(hhrr_lattice* L) {
   if (!L) return fail(HHRR_E_ARG, "hhrr_destroy: NULL lattice");
   cudaStreamSynchronize(L->stream);
+  if (L->ev[0])
+    for (int k = 0; k < 2 * 1024; ++k) cudaEventDestroy(L->ev[k]);
   delete L;
   return HHRR_OK;
 }
@@ -339,6 +341,30 @@ int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant) {
   return HHRR_OK;
 }
 
+int hhrr_set_timing(hhrr_lattice* L, int enable) {
+  if (!L) return fail(HHRR_E_ARG, "hhrr_set_timing: NULL lattice");
+  if (enable && !L->ev[0])
+    for (int k = 0; k < 2 * 1024; ++k) CU(cudaEventCreate(&L->ev[k]));
+  L->timing = enable != 0;
+  L->ev_n = 0;
+  return HHRR_OK;
+}
+
+int hhrr_get_timing(hhrr_lattice* L, double* ms_collide_stream, int64_t* launches) {
+  if (!L || !ms_collide_stream || !launches) return fail(HHRR_E_ARG, "hhrr_get_timing: NULL argument");
+  CU(cudaStreamSynchronize(L->stream));
+  double total = 0.0;
+  for (int k = 0; k < L->ev_n; ++k) {
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, L->ev[2 * k], L->ev[2 * k + 1]));
+    total += ms;
+  }
+  *ms_collide_stream = total;
+  *launches = L->ev_n;
+  L->ev_n = 0;
+  return HHRR_OK;
+}
+
 int64_t hhrr_launch_count(const hhrr_lattice* L) { return L ? L->launches : 0; }
 int64_t hhrr_step_count(const hhrr_lattice* L) { return L ? L->step : 0; }
 
@@ -347,8 +373,14 @@ int hhrr_step(hhrr_lattice* L, int32_t n_steps) {
   for (int32_t s = 0; s < n_steps; ++s) {
     int rc = ensure_geometry(L);  // Listing 3 line 2: UpdatePorosityO
     if (rc) return rc;
+    const bool timed = L->timing && L->ev_n < 1024;
+    if (timed) CU(cudaEventRecord(L->ev[2 * L->ev_n], L->stream));
     cudaError_t e = launch_collide_stream(L);  // line 3
     if (e != cudaSuccess) return cuda_fail(e, "collide-stream kernel");
+    if (timed) {
+      CU(cudaEventRecord(L->ev[2 * L->ev_n + 1], L->stream));
+      L->ev_n++;
+    }
     e = launch_wall_model(L);  // line 4: WallModelO
     if (e != cudaSuccess) return cuda_fail(e, "wall-model kernel");
     e = launch_forces(L);  // lines 5-6

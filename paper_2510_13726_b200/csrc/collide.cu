@@ -64,38 +64,6 @@ __global__ void __launch_bounds__(256) moments_kernel(Dom dm, PhysF ph, BodiesF 
   uhat[2 * dm.n + c] = uh[2];
 }
 
-// push-store of the 27 post-collision values with the outer-boundary rule R12
-__device__ __forceinline__ void push_store(const Dom& dm, float* __restrict__ fout, int x, int y, int z,
-                                           const float (&o)[Q]) {
-  bool fxm, fxp, fym, fyp, fzm, fzp;
-  int xm = wrap_axis(x - 1, dm.nx, dm.mode[0], fxm), xp = wrap_axis(x + 1, dm.nx, dm.mode[0], fxp);
-  int ym = wrap_axis(y - 1, dm.ny, dm.mode[1], fym), yp = wrap_axis(y + 1, dm.ny, dm.mode[1], fyp);
-  int zm = wrap_axis(z - 1, dm.nz, dm.mode[2], fzm), zp = wrap_axis(z + 1, dm.nz, dm.mode[2], fzp);
-  const int64_t nx = dm.nx, nxy = (int64_t)dm.nx * dm.ny;
-  if (!(fxm | fxp | fym | fyp | fzm | fzp)) {
-    int xs[3] = {xm, x, xp};
-    int64_t ys[3] = {ym * nx, y * nx, yp * nx};
-    int64_t zs[3] = {zm * nxy, z * nxy, zp * nxy};
-#pragma unroll
-    for (int i = 0; i < Q; ++i)
-      fout[(int64_t)i * dm.n + zs[dir_cz(i) + 1] + ys[dir_cy(i) + 1] + xs[dir_cx(i) + 1]] = o[i];
-  } else {
-    // a population leaving through a mirror plane returns to the same cell, component reversed
-#pragma unroll
-    for (int i = 0; i < Q; ++i) {
-      int cx = dir_cx(i), cy = dir_cy(i), cz = dir_cz(i);
-      int tx = cx < 0 ? xm : (cx > 0 ? xp : x);
-      int ty = cy < 0 ? ym : (cy > 0 ? yp : y);
-      int tz = cz < 0 ? zm : (cz > 0 ? zp : z);
-      if ((cx < 0 && fxm) || (cx > 0 && fxp)) { tx = x; cx = -cx; }
-      if ((cy < 0 && fym) || (cy > 0 && fyp)) { ty = y; cy = -cy; }
-      if ((cz < 0 && fzm) || (cz > 0 && fzp)) { tz = z; cz = -cz; }
-      int io = (cx + 1) + 3 * (cy + 1) + 9 * (cz + 1);
-      fout[(int64_t)io * dm.n + tz * nxy + ty * nx + tx] = o[i];
-    }
-  }
-}
-
 // ------------------------------------------------------------------ variant 0, pass 2
 __global__ void __launch_bounds__(256) collide_kernel(Dom dm, PhysF ph, BodiesF bo,
                                                       const float* __restrict__ fin, float* __restrict__ fout,

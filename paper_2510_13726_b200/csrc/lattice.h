@@ -99,6 +99,10 @@ struct hhrr_lattice {
   int64_t step;
   int variant;
   int64_t launches;
+  // optional CUDA-event timing of the collide-stream kernel (hhrr_set_timing)
+  bool timing;
+  int ev_n;
+  cudaEvent_t ev[2 * 1024];
 };
 
 // ---- kernel launchers (one per translation unit) ---------------------------------------

@@ -42,7 +42,7 @@ def rel_linf(rho_g, v_g, rho_o, v_o):
     return e_rho, e_v
 
 
-def compare_geometry(G, Oa):
+def compare_geometry(G, Oa, tol=TOL10):
     tg, gg, dg = G.cell_types()
     to, go, do = Oa.cell_types()
     assert np.array_equal(tg, to), f"{np.count_nonzero(tg != to)} cell types differ"
@@ -54,7 +54,7 @@ def compare_geometry(G, Oa):
     assert np.array_equal(vg, vo), "wall-model valid flags differ"
     if len(io):
         assert np.max(np.abs(yg - yo)) <= 1e-12
-        assert np.max(np.abs(ug - uo)) <= 1e-6 * max(np.max(np.abs(uo)), 1e-30) + 1e-12
+        assert np.max(np.abs(ug - uo)) <= tol * max(np.max(np.abs(uo)), 1e-30) + 1e-12
 
 
 def compare_forces(G, Oa, tol):
@@ -74,7 +74,7 @@ def run_parity(oracle, case, steps, variant, tol, check_every=None, force_tol=No
         k = min(chunk, steps - done)
         G.step(k); Oa.step(k)
         done += k
-        compare_geometry(G, Oa)
+        compare_geometry(G, Oa, tol)
     G.check_finite()
     e_rho, e_v = rel_linf(*G.moments(), *Oa.moments())
     assert e_rho <= tol and e_v <= tol, (e_rho, e_v)

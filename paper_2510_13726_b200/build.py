@@ -27,6 +27,7 @@ SOURCES = {
     "api.cu": [],
     "collide.cu": [],
     "fused.cu": [],
+    "fused_ws.cu": [],
     "wallmodel.cu": [],
     "geometry.cu": ["-fmad=false"],
 }

@@ -71,6 +71,7 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
   uint8_t* flags = c.take<uint8_t>(n);
   float* d = c.take<float>(n);
   double* phi = c.take<double>(n);
+  uint8_t* below = c.take<uint8_t>(n);
   float* phi_static = c.take<float>(n);
   uint8_t* tag_static = c.take<uint8_t>(n);
   float* d_override = c.take<float>(n);
@@ -86,7 +87,7 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
   float* rot_sdf = c.take<float>(rotor_nodes);
   uint8_t* rot_tag = c.take<uint8_t>(rotor_nodes);
   if (L) {
-    L->fA = fA; L->fB = fB; L->flags = flags; L->d = d; L->phi = phi; L->phi_static = phi_static;
+    L->fA = fA; L->fB = fB; L->flags = flags; L->d = d; L->phi = phi; L->below = below; L->phi_static = phi_static;
     L->tag_static = tag_static; L->d_override = d_override; L->uhat = uhat; L->wm_utau = wm_utau;
     L->wm_u = wm_u; L->wm_s = wm_s; L->wall_idx = wall_idx; L->wall_y1n = wall_y1n;
     L->force_idx = force_idx; L->counters = counters; L->force = force; L->rot_sdf = rot_sdf;
@@ -336,7 +337,7 @@ int hhrr_update_geometry(hhrr_lattice* L) {
 }
 
 int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant) {
-  if (!L || variant < 0 || variant > 1) return fail(HHRR_E_ARG, "hhrr_set_kernel_variant: bad argument");
+  if (!L || variant < 0 || (variant > 2 && (variant < 11 || variant > 29))) return fail(HHRR_E_ARG, "hhrr_set_kernel_variant: bad argument");
   L->variant = variant;
   return HHRR_OK;
 }

@@ -249,13 +249,16 @@ cudaError_t launch_init(hhrr_lattice* L, const float* d_rho, const float* d_u, i
   return cudaGetLastError();
 }
 
-cudaError_t launch_fused(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo);  // fused.cu
+cudaError_t launch_fused(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo);     // fused.cu
+cudaError_t launch_fused_ws(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo);  // fused_ws.cu
 
 cudaError_t launch_collide_stream(hhrr_lattice* L) {
   PhysF ph = make_phys(L);
   BodiesF bo = make_bodies(L);
   cudaError_t e;
-  if (L->variant == 1) {
+  if (L->variant == 2 || (L->variant >= 21 && L->variant <= 29)) {
+    e = launch_fused_ws(L, ph, bo);
+  } else if (L->variant >= 1) {
     e = launch_fused(L, ph, bo);
   } else {
     int bx = row_block(L->dom);

@@ -24,6 +24,18 @@ __host__ __device__ constexpr double dir_wd(int i) {
          (dir_cz(i) ? 1.0 / 6.0 : 2.0 / 3.0);
 }
 
+// MUFU reciprocal + one Newton step (<= 1 ulp, branch-free) and MUFU square root (2^-23 rel.)
+__device__ __forceinline__ float rcp_nr(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return fmaf(r, fmaf(-x, r, 1.f), r);
+}
+__device__ __forceinline__ float sqrt_fast(float x) {
+  float r;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
 struct Moments {  // of the deviations: drho = rho - 1, j, M_ab = sum c_a c_b (f - w)
   float drho, jx, jy, jz, mxx, myy, mzz, mxy, mxz, myz;
 };
@@ -107,7 +119,7 @@ __device__ __forceinline__ void homogenised_velocity(const PhysF& ph, float drho
                                                      float jz, float d, const float uB[3], float& rho,
                                                      float uh[3]) {
   rho = 1.f + drho;
-  float ir = 1.f / rho;
+  float ir = rcp_nr(rho);
   float ux = (jx + ph.g[0]) * ir, uy = (jy + ph.g[1]) * ir, uz = (jz + ph.g[2]) * ir;
   float e = 1.f - d;
   uh[0] = d * ux + e * uB[0];
@@ -129,9 +141,9 @@ __device__ __forceinline__ void collide(const PhysF& ph, const Moments& m, float
   float pxy = m.mxy - rux * uy, pxz = m.mxz - rux * uz, pyz = m.myz - ruy * uz;
   // Smagorinsky closed form (Eq. 3-5, 14; R6)
   float pp = pxx * pxx + pyy * pyy + pzz * pzz + 2.f * (pxy * pxy + pxz * pxz + pyz * pyz);
-  float Qn = sqrtf(2.f * pp);
-  float tau = 0.5f * (ph.tau0 + sqrtf(ph.tau0 * ph.tau0 + ph.smag18 * Qn / rho));
-  float k = 1.f - 1.f / tau;
+  float Qn = sqrt_fast(2.f * pp);
+  float tau = 0.5f * (ph.tau0 + sqrt_fast(ph.tau0 * ph.tau0 + ph.smag18 * Qn * rcp_nr(rho)));
+  float k = 1.f - rcp_nr(tau);
   // hybrid a1^(2) (Eq. 7 + Eq. 10; R2)
   float hs = (1.f - sigma) * (2.f * third) * rho * tau;
   float axx = sigma * pxx - hs * S[0], ayy = sigma * pyy - hs * S[1], azz = sigma * pzz - hs * S[2];

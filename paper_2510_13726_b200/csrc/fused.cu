@@ -10,6 +10,9 @@
 // (rho, j only) for the one-cell xy halo, whose populations are L2 hits because neighbouring
 // columns run concurrently.  Plane z is collided when plane z+1 has been published, so the
 // populations cross HBM once in and once out: 216 B per cell update, no uhat field.
+//
+// Addressing: the 27 plane offsets i*n and the 27 interior push offsets are warp-uniform
+// 64-bit constants in the kernel parameter block, so a load / store costs one 64-bit add.
 #include "d3q27.cuh"
 
 namespace hhrr {
@@ -34,12 +37,9 @@ struct FusedArgs {
   const float* wm_u;
   const float* wm_s;
   int zchunk;
+  long long plane[Q];  // i * n                          (element offsets, warp-uniform)
+  long long push[Q];   // i * n + cx + cy*nx + cz*nx*ny  (interior push target of direction i)
 };
-
-__device__ __forceinline__ void load_cell_f(const float* __restrict__ f, int64_t n, int64_t c, float (&v)[Q]) {
-#pragma unroll
-  for (int i = 0; i < Q; ++i) v[i] = __ldg(f + (int64_t)i * n + c);
-}
 
 // porosity and u^B (+ wall-model slip) of a real cell
 __device__ __forceinline__ void solid_state(const FusedArgs& a, uint8_t fl, int64_t c, int x, int y, int z,
@@ -67,8 +67,8 @@ __device__ __forceinline__ int virt(int v, int n, int mode, bool& flip, bool& ok
   return wrap_axis(v, n, mode, flip);
 }
 
-template <int TX, int TY>
-__global__ void __launch_bounds__(TX* TY) fused_kernel(FusedArgs a) {
+template <int TX, int TY, int MINB>
+__global__ void __launch_bounds__(TX* TY, MINB) fused_kernel(const __grid_constant__ FusedArgs a) {
   using C = FusedCfg<TX, TY>;
   __shared__ float ring[4][3][C::PLANE];
   const Dom& dm = a.dm;
@@ -82,9 +82,11 @@ __global__ void __launch_bounds__(TX* TY) fused_kernel(FusedArgs a) {
   const int xv = x0 + tx, yv = y0 + ty;
   bool fxo, fyo, okx, oky;
   const int xr = virt(xv, dm.nx, dm.mode[0], fxo, okx), yr = virt(yv, dm.ny, dm.mode[1], fyo, oky);
-  const bool own_moment = okx && oky;                                   // publishes uhat
-  const bool own_collide = xv < dm.nx && yv < dm.ny;                    // a real cell of this tile
+  const bool own_moment = okx && oky;                 // publishes uhat
+  const bool own_collide = xv < dm.nx && yv < dm.ny;  // a real cell of this tile
+  const bool xy_interior = xv > 0 && xv < dm.nx - 1 && yv > 0 && yv < dm.ny - 1;
   const int own_slot = (ty + 1) * C::SX + (tx + 1);
+  const int64_t own_xy = xr + nx * yr;
   // halo duty
   bool halo = tid < C::HALO, fxh = false, fyh = false;
   int xh = 0, yh = 0, halo_slot = 0;
@@ -104,6 +106,7 @@ __global__ void __launch_bounds__(TX* TY) fused_kernel(FusedArgs a) {
     halo = ox && oy;
     halo_slot = hy * C::SX + hx;
   }
+  const int64_t halo_xy = xh + nx * yh;
 
   Moments mcur = {}, mnext = {};
   float rho_c = 1.f, rho_n = 1.f, uh_c[3] = {0, 0, 0}, uh_n[3] = {0, 0, 0};
@@ -112,12 +115,15 @@ __global__ void __launch_bounds__(TX* TY) fused_kernel(FusedArgs a) {
   // publishes uhat of virtual plane zq into ring slot (zq & 3); keeps the own cell's moments
   auto publish = [&](int zq, bool keep) {
     bool fz, okz;
-    int zr = virt(zq, dm.nz, dm.mode[2], fz, okz);
+    const int zr = virt(zq, dm.nz, dm.mode[2], fz, okz);
     float(*slot)[C::PLANE] = ring[zq & 3];
+    const int64_t zoff = nxy * zr;
     if (own_moment) {
-      int64_t c = xr + nx * yr + nxy * zr;
+      const int64_t c = own_xy + zoff;
+      const float* __restrict__ p = a.fin + c;
       float f[Q];
-      load_cell_f(a.fin, n, c, f);
+#pragma unroll
+      for (int i = 0; i < Q; ++i) f[i] = __ldg(p + a.plane[i]);
       uint8_t fl = __ldg(a.flags + c);
       float d, uB[3], rho, uh[3];
       solid_state(a, fl, c, xr, yr, zr, d, uB);
@@ -137,9 +143,11 @@ __global__ void __launch_bounds__(TX* TY) fused_kernel(FusedArgs a) {
       slot[2][own_slot] = fz ? -uh[2] : uh[2];
     }
     if (halo) {
-      int64_t c = xh + nx * yh + nxy * zr;
+      const int64_t c = halo_xy + zoff;
+      const float* __restrict__ p = a.fin + c;
       float f[Q];
-      load_cell_f(a.fin, n, c, f);
+#pragma unroll
+      for (int i = 0; i < Q; ++i) f[i] = __ldg(p + a.plane[i]);
       uint8_t fl = __ldg(a.flags + c);
       float d, uB[3], rho, uh[3], drho, jx, jy, jz;
       solid_state(a, fl, c, xh, yh, zr, d, uB);
@@ -161,8 +169,8 @@ __global__ void __launch_bounds__(TX* TY) fused_kernel(FusedArgs a) {
     __syncthreads();
     if (own_collide) {
       float S[6], sigma = a.ph.sigma;
+      const int64_t c = xv + nx * yv + nxy * z;
       if (fl_c & WM_VALID) {
-        int64_t c = xv + nx * yv + nxy * z;
 #pragma unroll
         for (int q = 0; q < 6; ++q) S[q] = __ldg(a.wm_s + (int64_t)q * n + c);
         sigma = 0.f;
@@ -184,25 +192,31 @@ __global__ void __launch_bounds__(TX* TY) fused_kernel(FusedArgs a) {
       }
       float o27[Q];
       collide(a.ph, mcur, rho_c, uh_c, S, sigma, o27);
-      push_store(dm, a.fout, xv, yv, z, o27);
+      if (xy_interior && z > 0 && z < dm.nz - 1) {  // no wrap, no reflection: constant push offsets
+        float* __restrict__ q = a.fout + c;
+#pragma unroll
+        for (int i = 0; i < Q; ++i) q[a.push[i]] = o27[i];
+      } else {
+        push_store(dm, a.fout, xv, yv, z, o27);
+      }
     }
     mcur = mnext; rho_c = rho_n; fl_c = fl_n;
     uh_c[0] = uh_n[0]; uh_c[1] = uh_n[1]; uh_c[2] = uh_n[2];
   }
 }
 
-template <int TX, int TY>
+template <int TX, int TY, int MINB>
 static cudaError_t launch_cfg(hhrr_lattice* L, const FusedArgs& a0) {
   FusedArgs a = a0;
   const Dom& dm = L->dom;
   int tiles = ((dm.nx + TX - 1) / TX) * ((dm.ny + TY - 1) / TY);
-  int want = (8 * 148 + tiles - 1) / tiles;                 // >= ~8 blocks per SM in total
-  int maxchunks = (dm.nz + 15) / 16;                          // >= 16 planes per chunk
+  int want = (8 * 148 * MINB + tiles - 1) / tiles;  // >= ~8 waves of resident blocks
+  int maxchunks = (dm.nz + 15) / 16;                  // >= 16 planes per chunk
   int nch = want < 1 ? 1 : (want > maxchunks ? maxchunks : want);
   a.zchunk = (dm.nz + nch - 1) / nch;
   nch = (dm.nz + a.zchunk - 1) / a.zchunk;
   dim3 grid((dm.nx + TX - 1) / TX, (dm.ny + TY - 1) / TY, nch);
-  fused_kernel<TX, TY><<<grid, TX * TY, 0, L->stream>>>(a);
+  fused_kernel<TX, TY, MINB><<<grid, TX * TY, 0, L->stream>>>(a);
   L->launches++;
   return cudaGetLastError();
 }
@@ -219,8 +233,22 @@ cudaError_t launch_fused(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo) {
   a.wm_u = L->wm_u;
   a.wm_s = L->wm_s;
   a.zchunk = L->dom.nz;
-  if (L->dom.nx > 32) return launch_cfg<64, 8>(L, a);
-  return launch_cfg<32, 8>(L, a);
+  const long long n = L->dom.n, nx = L->dom.nx, nxy = (long long)L->dom.nx * L->dom.ny;
+  for (int i = 0; i < Q; ++i) {
+    a.plane[i] = i * n;
+    a.push[i] = i * n + dir_cx(i) + dir_cy(i) * nx + dir_cz(i) * nxy;
+  }
+  switch (L->variant) {  // 1 = default; 11.. = tile shapes kept for tuning runs
+    case 11: return launch_cfg<64, 8, 1>(L, a);
+    case 12: return launch_cfg<64, 4, 4>(L, a);
+    case 13: return launch_cfg<32, 8, 4>(L, a);
+    case 14: return launch_cfg<128, 4, 2>(L, a);
+    case 15: return launch_cfg<32, 16, 2>(L, a);
+    case 16: return launch_cfg<64, 4, 2>(L, a);
+    default: break;
+  }
+  if (L->dom.nx > 32) return launch_cfg<64, 8, 2>(L, a);
+  return launch_cfg<32, 8, 2>(L, a);
 }
 
 }  // namespace hhrr

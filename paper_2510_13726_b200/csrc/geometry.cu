@@ -28,6 +28,7 @@ struct GeoArgs {
   const uint8_t* tag_static;
   const float* d_override;
   double* phi;
+  uint8_t* below;   // phi < eps/2 per cell: what the growth-layer test reads (1 B instead of 8)
   uint8_t* flags;
   float* d;
   int32_t* wall_idx;
@@ -123,6 +124,7 @@ __global__ void __launch_bounds__(128) geometry_phi_kernel(GeoArgs a) {
     }
   }
   a.phi[c] = phi;
+  a.below[c] = phi < a.h ? 1 : 0;
   a.flags[c] = (uint8_t)((a.flags[c] & WM_VALID) | ((tg & TAG_MASK) << TAG_SHIFT));
 }
 
@@ -163,7 +165,7 @@ __global__ void __launch_bounds__(128) geometry_type_kernel(GeoArgs a) {
             int xx = wrap_any(x + dx, nx, a.dm.mode[0]);
             int yy = wrap_any(y + dy, ny, a.dm.mode[1]);
             int zz = wrap_any(z + dz, nz, a.dm.mode[2]);
-            if (a.phi[xx + snx * yy + snxy * zz] < a.h) {
+            if (a.below[xx + snx * yy + snxy * zz]) {
               type = HHRR_GROWTH;
               break;
             }
@@ -288,6 +290,7 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
   a.tag_static = L->tag_static;
   a.d_override = L->d_override;
   a.phi = L->phi;
+  a.below = L->below;
   a.flags = L->flags;
   a.d = L->d;
   a.wall_idx = L->wall_idx;

@@ -71,6 +71,7 @@ struct hhrr_lattice {
   uint8_t* flags;           // N
   float* d;                 // N porosity (read for FRONTIER cells only)
   double* phi;              // N signed distance of the last geometry
+  uint8_t* below;           // N: phi < eps/2
   float* phi_static;        // N
   uint8_t* tag_static;      // N
   float* d_override;        // N

@@ -83,7 +83,7 @@ def run_parity(oracle, case, steps, variant, tol, check_every=None, force_tol=No
     return e_rho, e_v
 
 
-VARIANTS = [0, 1]
+VARIANTS = [0, 1, 2]
 
 
 @pytest.mark.parametrize("variant", VARIANTS)

@@ -163,8 +163,9 @@ int hhrr_set_populations(hhrr_lattice* L, const float* f_minus_w);
 int hhrr_get_uhat(hhrr_lattice* L, float* uhat);
 /* HHRR_E_NAN if any population is non-finite (synchronises). */
 int hhrr_check_finite(hhrr_lattice* L);
-/* Selects the collide-stream kernel: 0 = two-pass (moments pass + collide pass),
- * 1 = fused sliding-window kernel (default).  Both compute the same step.           */
+/* Selects the collide-stream kernel: 0 = two-pass (moments pass + collide pass), 1 = fused
+ * sliding-window kernel, 2 = fused warp-specialised kernel (default); 11-29 = tile shapes of
+ * 1 and 2 kept for tuning runs.  All compute the same step.                            */
 int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant);
 /* Optional CUDA-event timing of the collide-stream launches inside hhrr_step (the kernel the
  * roofline is quoted on).  hhrr_get_timing synchronises, returns the summed device time in

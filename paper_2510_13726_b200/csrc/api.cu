@@ -72,6 +72,8 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
   float* d = c.take<float>(n);
   double* phi = c.take<double>(n);
   uint8_t* below = c.take<uint8_t>(n);
+  uint8_t* rowflag = c.take<uint8_t>((int64_t)p->ny * p->nz);
+  uint8_t* rowflag_static = c.take<uint8_t>((int64_t)p->ny * p->nz);
   float* phi_static = c.take<float>(n);
   uint8_t* tag_static = c.take<uint8_t>(n);
   float* d_override = c.take<float>(n);
@@ -87,7 +89,7 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
   float* rot_sdf = c.take<float>(rotor_nodes);
   uint8_t* rot_tag = c.take<uint8_t>(rotor_nodes);
   if (L) {
-    L->fA = fA; L->fB = fB; L->flags = flags; L->d = d; L->phi = phi; L->below = below; L->phi_static = phi_static;
+    L->fA = fA; L->fB = fB; L->flags = flags; L->d = d; L->phi = phi; L->below = below; L->rowflag = rowflag; L->rowflag_static = rowflag_static; L->phi_static = phi_static;
     L->tag_static = tag_static; L->d_override = d_override; L->uhat = uhat; L->wm_utau = wm_utau;
     L->wm_u = wm_u; L->wm_s = wm_s; L->wall_idx = wall_idx; L->wall_y1n = wall_y1n;
     L->force_idx = force_idx; L->counters = counters; L->force = force; L->rot_sdf = rot_sdf;
@@ -175,7 +177,7 @@ int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes,
   int64_t rest = (int64_t)(workspace_bytes - lead - need_min);
   int64_t spare = std::max<int64_t>(0, (rest - 512) / 5);
   carve(L, p, spare, base);
-  L->variant = 1;
+  L->variant = 2;
   L->geometry_dirty = true;
   L->geometry_current = false;
   const int64_t n = L->dom.n;
@@ -294,19 +296,30 @@ int hhrr_set_rotor(hhrr_lattice* L, const hhrr_rotor_desc* r) {
       L->bodies.w[k][a] = r->axis[a] * r->omega;
       L->bodies.v[k][a] = 0.0;
     }
-  // Box swept by the reference grid under rotation about the axis: the axial coordinate
-  // and the radial distance of a point are invariant, so bound both over the grid corners.
+  // Box swept under rotation about the axis by the part of the reference grid that can yield
+  // phi < eps/2: a trilinear sample is below eps/2 only if one of its 8 nodes is, so bound the
+  // axial coordinate and the radial distance (both invariant under the rotation) of the nodes
+  // with sdf < eps/2, widened by one grid cell.  Cells outside keep phi >= eps/2 at every angle.
+  const double hband = 0.5 * L->p.eps_cells;
   double amin = 1e300, amax = -1e300, rmax = 0.0;
-  for (int k = 0; k < 8; ++k) {
-    double q[3] = {r->origin[0] + ((k & 1) ? (r->gx - 1) * r->spacing : 0.0),
-                   r->origin[1] + ((k & 2) ? (r->gy - 1) * r->spacing : 0.0),
-                   r->origin[2] + ((k & 4) ? (r->gz - 1) * r->spacing : 0.0)};
-    double ad = q[0] * r->axis[0] + q[1] * r->axis[1] + q[2] * r->axis[2];
-    double rr = std::sqrt(std::max(0.0, q[0] * q[0] + q[1] * q[1] + q[2] * q[2] - ad * ad));
-    amin = std::min(amin, ad);
-    amax = std::max(amax, ad);
-    rmax = std::max(rmax, rr);
-  }
+  for (int iz = 0; iz < r->gz; ++iz)
+    for (int iy = 0; iy < r->gy; ++iy) {
+      const float* row = r->sdf + ((int64_t)iz * r->gy + iy) * r->gx;
+      for (int ix = 0; ix < r->gx; ++ix) {
+        if (!((double)row[ix] < hband)) continue;
+        double q[3] = {r->origin[0] + ix * r->spacing, r->origin[1] + iy * r->spacing, r->origin[2] + iz * r->spacing};
+        double ad = q[0] * r->axis[0] + q[1] * r->axis[1] + q[2] * r->axis[2];
+        double rr = std::sqrt(std::max(0.0, q[0] * q[0] + q[1] * q[1] + q[2] * q[2] - ad * ad));
+        amin = std::min(amin, ad);
+        amax = std::max(amax, ad);
+        rmax = std::max(rmax, rr);
+      }
+    }
+  const bool any_node = amax >= amin;
+  const double widen = 1.7320508075688772 * r->spacing;
+  amin -= widen;
+  amax += widen;
+  rmax += widen;
   int lo[3], hi[3], ext[3] = {L->dom.nx, L->dom.ny, L->dom.nz};
   for (int a = 0; a < 3; ++a) {
     double ak = r->axis[a], perp = std::sqrt(std::max(0.0, 1.0 - ak * ak));
@@ -315,6 +328,7 @@ int hhrr_set_rotor(hhrr_lattice* L, const hhrr_rotor_desc* r) {
     hi[a] = (int)std::ceil(r->centre[a] + e1) + 4;
     lo[a] = std::max(0, std::min(ext[a], lo[a]));
     hi[a] = std::max(lo[a], std::min(ext[a], hi[a]));
+    if (!any_node) lo[a] = hi[a] = 0;
   }
   L->rot_box = Box{lo[0], hi[0], lo[1], hi[1], lo[2], hi[2]};
   L->geometry_dirty = true;

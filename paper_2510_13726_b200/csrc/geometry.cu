@@ -29,6 +29,7 @@ struct GeoArgs {
   const float* d_override;
   double* phi;
   uint8_t* below;   // phi < eps/2 per cell: what the growth-layer test reads (1 B instead of 8)
+  uint8_t* rowflag; // per (y,z) row: some cell of the row may have phi < eps/2 (superset)
   uint8_t* flags;
   float* d;
   int32_t* wall_idx;
@@ -124,7 +125,9 @@ __global__ void __launch_bounds__(128) geometry_phi_kernel(GeoArgs a) {
     }
   }
   a.phi[c] = phi;
-  a.below[c] = phi < a.h ? 1 : 0;
+  const bool below = phi < a.h;
+  a.below[c] = below ? 1 : 0;
+  if (below) a.rowflag[y + a.dm.ny * z] = 1;
   a.flags[c] = (uint8_t)((a.flags[c] & WM_VALID) | ((tg & TAG_MASK) << TAG_SHIFT));
 }
 
@@ -158,7 +161,12 @@ __global__ void __launch_bounds__(128) geometry_type_kernel(GeoArgs a) {
     } else {
       type = HHRR_FLUID;
       d = 1.f;
-      for (int dz = -1; dz <= 1 && type == HHRR_FLUID; ++dz)
+      // rows with no cell below eps/2 in any of the nine neighbouring rows need no cell test
+      bool near_row = false;
+      for (int dz = -1; dz <= 1; ++dz)
+        for (int dy = -1; dy <= 1; ++dy)
+          near_row |= a.rowflag[wrap_any(y + dy, ny, a.dm.mode[1]) + ny * wrap_any(z + dz, nz, a.dm.mode[2])] != 0;
+      for (int dz = -1; near_row && dz <= 1 && type == HHRR_FLUID; ++dz)
         for (int dy = -1; dy <= 1 && type == HHRR_FLUID; ++dy)
           for (int dx = -1; dx <= 1; ++dx) {
             if (!dx && !dy && !dz) continue;
@@ -291,6 +299,7 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
   a.d_override = L->d_override;
   a.phi = L->phi;
   a.below = L->below;
+  a.rowflag = L->rowflag;
   a.flags = L->flags;
   a.d = L->d;
   a.wall_idx = L->wall_idx;
@@ -300,12 +309,16 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
   a.cap_list = (int)L->cap_list;
   dim3 g, b;
   bool box_empty = rb.x1 <= rb.x0 || rb.y1 <= rb.y0 || rb.z1 <= rb.z0;
+  const size_t rows = (size_t)L->dom.ny * L->dom.nz;
   if (full) {
     // phi everywhere, then types: outside the rotor box first (static list prefix), box last
     a.box = none;
     a.inside = 0;
     geo_grid(a, g, b);
+    cudaMemsetAsync(L->rowflag, 0, rows, L->stream);
     geometry_phi_kernel<<<g, b, 0, L->stream>>>(a);
+    // what the full pass marks (static geometry and the rotor at this angle) stays marked: a superset
+    cudaMemcpyAsync(L->rowflag_static, L->rowflag, rows, cudaMemcpyDeviceToDevice, L->stream);
     counters_kernel<<<1, 1, 0, L->stream>>>(L->counters, 0);
     a.box = rb;
     geometry_type_kernel<<<g, b, 0, L->stream>>>(a);
@@ -321,6 +334,7 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
     a.box = rb;
     a.inside = 1;
     geo_grid(a, g, b);
+    cudaMemcpyAsync(L->rowflag, L->rowflag_static, rows, cudaMemcpyDeviceToDevice, L->stream);
     geometry_phi_kernel<<<g, b, 0, L->stream>>>(a);
     counters_kernel<<<1, 1, 0, L->stream>>>(L->counters, 2);
     geometry_type_kernel<<<g, b, 0, L->stream>>>(a);

@@ -72,6 +72,7 @@ struct hhrr_lattice {
   float* d;                 // N porosity (read for FRONTIER cells only)
   double* phi;              // N signed distance of the last geometry
   uint8_t* below;           // N: phi < eps/2
+  uint8_t *rowflag, *rowflag_static;  // ny*nz: row may hold a cell with phi < eps/2
   float* phi_static;        // N
   uint8_t* tag_static;      // N
   float* d_override;        // N

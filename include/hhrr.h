@@ -159,6 +159,11 @@ int hhrr_get_wall_state(hhrr_lattice* L, int64_t cell, double* u_tau, double u_w
 /* Populations as stored: deviations f_i - w_i, 27 planes of N floats (checkpoint / resume). */
 int hhrr_get_populations(hhrr_lattice* L, float* f_minus_w);
 int hhrr_set_populations(hhrr_lattice* L, const float* f_minus_w);
+/* Populations (deviations f_i - w_i) of selected cells: out[k*27 + i] for cells[k], and the
+ * cells' flags as stored (type | tag << 3 | wall-model-valid << 7) if flags != NULL.  Lets tests
+ * check sampled cells of lattices too large to copy back whole.                          */
+int hhrr_get_cell_populations(hhrr_lattice* L, int64_t n_cells, const int64_t* cells, float* out,
+                              uint8_t* flags);
 /* Time-n homogenised velocity field of the last collide (3N floats), for tests. */
 int hhrr_get_uhat(hhrr_lattice* L, float* uhat);
 /* HHRR_E_NAN if any population is non-finite (synchronises). */

@@ -27,7 +27,7 @@ SYMBOLS = [
     "hhrr_enable_wall_model", "hhrr_update_geometry", "hhrr_step", "hhrr_step_count",
     "hhrr_get_moments", "hhrr_get_moments_device", "hhrr_get_forces", "hhrr_force_history",
     "hhrr_get_cell_types", "hhrr_get_wall_list", "hhrr_get_wall_state", "hhrr_get_populations",
-    "hhrr_set_populations", "hhrr_get_uhat", "hhrr_check_finite", "hhrr_set_kernel_variant",
+    "hhrr_set_populations", "hhrr_get_cell_populations", "hhrr_get_uhat", "hhrr_check_finite", "hhrr_set_kernel_variant",
     "hhrr_set_timing", "hhrr_get_timing", "hhrr_launch_count", "hhrr_last_error", "hhrr_version",
 ]
 
@@ -92,6 +92,7 @@ def lib():
         L.hhrr_get_wall_state.argtypes = [vp, i64, C.POINTER(dbl), vp, vp, C.POINTER(i32)]
         L.hhrr_get_populations.argtypes = [vp, vp]
         L.hhrr_set_populations.argtypes = [vp, vp]
+        L.hhrr_get_cell_populations.argtypes = [vp, i64, vp, vp, vp]
         L.hhrr_get_uhat.argtypes = [vp, vp]
         L.hhrr_check_finite.argtypes = [vp]
         L.hhrr_set_kernel_variant.argtypes = [vp, i32]
@@ -307,6 +308,14 @@ class Lattice:
     def set_populations(self, f_minus_w):
         f = _f32(f_minus_w).reshape(Q, self.n)
         _check(lib().hhrr_set_populations(self.h, _p(f)))
+
+    def cell_populations(self, cells):
+        """(f - w)[k, 27] and the stored flag bytes of the given cell indices."""
+        cells = np.ascontiguousarray(cells, np.int64)
+        out = np.empty((cells.size, Q), np.float32)
+        fl = np.empty(cells.size, np.uint8)
+        _check(lib().hhrr_get_cell_populations(self.h, cells.size, _p(cells), _p(out), _p(fl)))
+        return out, fl
 
     def uhat(self):
         u = np.empty((3, self.n), np.float32)

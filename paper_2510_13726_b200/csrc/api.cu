@@ -467,6 +467,14 @@ __global__ void gather_wall_kernel(const int32_t* idx, int count, const double* 
   out_utau[e] = wm_utau[c];
   out_valid[e] = (flags[c] & WM_VALID) ? 1 : 0;
 }
+__global__ void gather_cells_kernel(const float* f, const uint8_t* flags, int64_t n, const int64_t* cells,
+                                    int64_t count, float* out, uint8_t* out_flags) {
+  int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= count) return;
+  int64_t c = cells[k];
+  for (int i = 0; i < Q; ++i) out[k * Q + i] = f[(int64_t)i * n + c];
+  out_flags[k] = flags[c];
+}
 int read_counters(hhrr_lattice* L, Counters* h) { return download(L, h, L->counters, sizeof(Counters)); }
 }  // namespace
 
@@ -530,6 +538,30 @@ int hhrr_get_wall_state(hhrr_lattice* L, int64_t cell, double* u_tau, double u_w
   if (u_wm) for (int a = 0; a < 3; ++a) u_wm[a] = u[a];
   if (s_wm) for (int a = 0; a < 6; ++a) s_wm[a] = s[a];
   if (valid) *valid = (fl & WM_VALID) ? 1 : 0;
+  return HHRR_OK;
+}
+
+int hhrr_get_cell_populations(hhrr_lattice* L, int64_t n_cells, const int64_t* cells, float* out,
+                              uint8_t* flags) {
+  if (!L || !cells || !out || n_cells < 0) return fail(HHRR_E_ARG, "hhrr_get_cell_populations: bad argument");
+  if (n_cells == 0) return HHRR_OK;
+  if (n_cells > L->dom.n) return fail(HHRR_E_ARG, "hhrr_get_cell_populations: more cells than the lattice has");
+  for (int64_t k = 0; k < n_cells; ++k)
+    if (cells[k] < 0 || cells[k] >= L->dom.n) return fail(HHRR_E_ARG, "hhrr_get_cell_populations: cell out of range");
+  // scratch in buffer B: [cells | out | flags]
+  char* sb = reinterpret_cast<char*>(L->fB);
+  int64_t* d_cells = reinterpret_cast<int64_t*>(sb);
+  float* d_out = reinterpret_cast<float*>(sb + 8 * n_cells);
+  uint8_t* d_fl = reinterpret_cast<uint8_t*>(sb + 8 * n_cells + 4 * Q * n_cells);
+  int rc = upload(L, d_cells, cells, 8 * (size_t)n_cells);
+  if (rc) return rc;
+  gather_cells_kernel<<<(unsigned)((n_cells + 127) / 128), 128, 0, L->stream>>>(L->fA, L->flags, L->dom.n, d_cells,
+                                                                             n_cells, d_out, d_fl);
+  L->launches++;
+  CU(cudaGetLastError());
+  rc = download(L, out, d_out, 4 * (size_t)Q * n_cells);
+  if (rc) return rc;
+  if (flags) return download(L, flags, d_fl, (size_t)n_cells);
   return HHRR_OK;
 }
 

@@ -303,13 +303,13 @@ cudaError_t launch_fused_ws(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo)
     a.push_b[i] = 4 * (i * n + dir_cx(i) + dir_cy(i) * nx + dir_cz(i) * nxy);
   }
   switch (L->variant) {
-    case 21: return launch_ws_cfg<64, 8, 20, 5>(L, a);
-    case 22: return launch_ws_cfg<64, 8, 20, 6>(L, a);
-    case 23: return launch_ws_cfg<128, 4, 24, 4, 4>(L, a);
-    case 24: return launch_ws_cfg<128, 4, 24, 5, 4>(L, a);
-    case 25: return launch_ws_cfg<64, 12, 14, 4>(L, a);
-    case 26: return launch_ws_cfg<32, 8, 10, 4>(L, a);
-    case 27: return launch_ws_cfg<64, 8, 10, 4>(L, a);
+    case 21: return launch_ws_cfg<64, 8, 10, 4, 1>(L, a);
+    case 22: return launch_ws_cfg<64, 8, 10, 5, 1>(L, a);
+    case 23: return launch_ws_cfg<64, 16, 12, 4, 2>(L, a);
+    case 24: return launch_ws_cfg<128, 8, 10, 4, 2>(L, a);
+    case 25: return launch_ws_cfg<64, 12, 14, 4, 2>(L, a);
+    case 26: return launch_ws_cfg<64, 8, 5, 4, 1>(L, a);
+    case 27: return launch_ws_cfg<64, 8, 10, 4, 2>(L, a);
     default: break;
   }
   return launch_ws_cfg<64, 8, 20, 4>(L, a);

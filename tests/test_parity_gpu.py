@@ -173,3 +173,96 @@ def test_variants_agree_bitwise_on_moments_order():
     A.step(20); Bv.step(20)
     e_rho, e_v = rel_linf(*A.moments(), *[x.astype(np.float64) for x in Bv.moments()])
     assert e_rho <= 1e-6 and e_v <= 1e-5, (e_rho, e_v)
+
+
+def test_config5_full_size_sampled_cells(oracle):
+    """BASELINE.json config 5 at FULL size (768x384x364, rotor R=120) in the launch configuration
+    bench.py times (default kernel variant).  The oracle cannot step 107 M cells in a test, so one
+    whole time step is checked on sampled cells it can compute one by one: for each sample the
+    oracle's single-cell collision (ohrr_collide_cell) is fed the GPU's pre-step populations of the
+    cell and of its six face neighbours (for S^FD), and its 27 post-collision values are compared
+    with what the GPU stored at the 27 push targets.  Samples cover bulk fluid, tile / z-chunk
+    seams, the inflow fringe, growth, frontier (with and without wall-model state) and solid cells."""
+    case = I.baseline_config(5)
+    G = _gpu_lattice(case, 2)
+    G.step(2)
+    G.update_geometry()                     # the geometry the next collide uses
+    nx, ny, nz = case.nx, case.ny, case.nz
+    n = case.n
+    types, tags, dpor = G.cell_types()
+    rng = np.random.default_rng(55)
+    samples = set(int(c) for c in rng.integers(0, n, 260))
+    for x in (0, 3, 4, 63, 64, 127, 128, nx - 1):          # fringe, tile seams in x, periodic wrap
+        for y in (0, 7, 8, 191, 192, ny - 1):               # tile seams in y
+            for z in (0, 22, 23, 24, 25, 181, nz - 1):      # z-chunk seams
+                samples.add(x + nx * (y + ny * z))
+    for t in (1, 2, 3):                                     # growth, frontier, solid cells of the rotor
+        idx = np.flatnonzero(types == t)
+        assert idx.size > 0
+        samples.update(int(c) for c in rng.choice(idx, min(120, idx.size), replace=False))
+    samples = np.array(sorted(samples), np.int64)
+    cx, cy, cz, w = oracle.lattice_tables()
+
+    def nb(c, dx, dy, dz):
+        x, y, z = c % nx, (c // nx) % ny, c // (nx * ny)
+        return ((x + dx) % nx) + nx * (((y + dy) % ny) + ny * ((z + dz) % nz))
+
+    faces = [(1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)]
+    need = np.array(sorted(set(int(c) for c in samples) | {nb(int(c), *f) for c in samples for f in faces}), np.int64)
+    pre, fl = G.cell_populations(need)
+    pos = {int(c): k for k, c in enumerate(need)}
+    rot = case.rotor
+    om = np.array(rot["axis"]) * rot["omega"]
+    ctr = np.array(rot["centre"])
+    tau0, sig, cs = case.params["tau0"], case.params["sigma"], case.params["smagorinsky_cs"]
+    u_in = np.array(case.fringe[2])
+    wm_valid_seen = 0
+
+    def state(c):
+        k = pos[c]
+        f = pre[k].astype(np.float64) + w
+        t, valid = int(fl[k]) & 7, bool(int(fl[k]) & 0x80)
+        assert t == types[c]
+        d, uB = 1.0, np.zeros(3)
+        if t == 4:
+            d, uB = 0.0, u_in.copy()
+        elif t in (2, 3):
+            d = float(dpor[c]) if t == 2 else 0.0
+            r = np.array([c % nx, (c // nx) % ny, c // (nx * ny)], float) - ctr
+            uB = np.cross(om, r)
+        return f, d, uB, valid
+
+    def uhat(c):
+        f, d, uB, valid = state(c)
+        if valid:
+            uB = uB + G.wall_state(c)[2]
+        return oracle.collide_cell(f, np.zeros(3), d, uB, np.zeros((3, 3)), sig, tau0, cs)[1][1:4]
+
+    expect = np.zeros((samples.size, 27))
+    for k, c in enumerate(samples):
+        c = int(c)
+        f, d, uB, valid = state(c)
+        sigma = sig
+        if valid:
+            wm_valid_seen += 1
+            _, _, uwm, s = G.wall_state(c)
+            uB = uB + uwm
+            S = np.array([[s[0], s[3], s[4]], [s[3], s[1], s[5]], [s[4], s[5], s[2]]])
+            sigma = 0.0
+        else:
+            grad = np.zeros((3, 3))                        # grad[a][b] = d_b u_a
+            for b in range(3):
+                grad[:, b] = 0.5 * (uhat(nb(c, *faces[2 * b])) - uhat(nb(c, *faces[2 * b + 1])))
+            S = 0.5 * (grad + grad.T)
+        expect[k] = oracle.collide_cell(f, np.zeros(3), d, uB, S, sigma, tau0, cs)[0] - w
+    G.step(1)
+    worst = 0.0
+    for i in range(27):
+        targets = np.array([nb(int(c), int(cx[i]), int(cy[i]), int(cz[i])) for c in samples], np.int64)
+        post, _ = G.cell_populations(targets)
+        worst = max(worst, float(np.max(np.abs(post[:, i].astype(np.float64) - expect[:, i]))))
+    scale = float(np.max(np.abs(expect)))
+    assert wm_valid_seen > 0, "no wall-model cell among the samples"
+    assert worst <= TOL10 * scale, (worst, scale)
+    G.check_finite()
+    G.close()

@@ -169,8 +169,9 @@ int hhrr_get_uhat(hhrr_lattice* L, float* uhat);
 /* HHRR_E_NAN if any population is non-finite (synchronises). */
 int hhrr_check_finite(hhrr_lattice* L);
 /* Selects the collide-stream kernel: 0 = two-pass (moments pass + collide pass), 1 = fused
- * sliding-window kernel, 2 = fused warp-specialised kernel (default); 11-29 = tile shapes of
- * 1 and 2 kept for tuning runs.  All compute the same step.                            */
+ * sliding-window kernel, 2 = fused warp-specialised kernel, 3 = the same with two cells per
+ * lane, 4 = fused kernel fed by TMA (default; needs nx % 64 == 0 and ny % 8 == 0, otherwise
+ * 2 runs); 11-49 = tile shapes kept for tuning runs.  All compute the same step.        */
 int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant);
 /* Optional CUDA-event timing of the collide-stream launches inside hhrr_step (the kernel the
  * roofline is quoted on).  hhrr_get_timing synchronises, returns the summed device time in

@@ -28,6 +28,8 @@ SOURCES = {
     "collide.cu": [],
     "fused.cu": [],
     "fused_ws.cu": [],
+    "fused_ws2.cu": [],
+    "fused_tma.cu": [],
     "wallmodel.cu": [],
     "geometry.cu": ["-fmad=false"],
 }

@@ -177,7 +177,7 @@ int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes,
   int64_t rest = (int64_t)(workspace_bytes - lead - need_min);
   int64_t spare = std::max<int64_t>(0, (rest - 512) / 5);
   carve(L, p, spare, base);
-  L->variant = 2;
+  L->variant = 4;
   L->geometry_dirty = true;
   L->geometry_current = false;
   const int64_t n = L->dom.n;
@@ -351,7 +351,7 @@ int hhrr_update_geometry(hhrr_lattice* L) {
 }
 
 int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant) {
-  if (!L || variant < 0 || (variant > 2 && (variant < 11 || variant > 29))) return fail(HHRR_E_ARG, "hhrr_set_kernel_variant: bad argument");
+  if (!L || variant < 0 || (variant > 4 && (variant < 11 || variant > 49))) return fail(HHRR_E_ARG, "hhrr_set_kernel_variant: bad argument");
   L->variant = variant;
   return HHRR_OK;
 }

@@ -251,12 +251,30 @@ cudaError_t launch_init(hhrr_lattice* L, const float* d_rho, const float* d_u, i
 
 cudaError_t launch_fused(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo);     // fused.cu
 cudaError_t launch_fused_ws(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo);  // fused_ws.cu
+cudaError_t launch_fused_ws2(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo); // fused_ws2.cu
+cudaError_t launch_fused_tma(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo); // fused_tma.cu
 
 cudaError_t launch_collide_stream(hhrr_lattice* L) {
   PhysF ph = make_phys(L);
   BodiesF bo = make_bodies(L);
   cudaError_t e;
-  if (L->variant == 2 || (L->variant >= 21 && L->variant <= 29)) {
+  if (L->variant == 4 || L->variant == 41) {
+    e = launch_fused_tma(L, ph, bo);
+    if (e == cudaErrorNotSupported) {  // ragged tiles: warp-specialised kernel, one cell per lane
+      const int v = L->variant;
+      L->variant = 2;
+      e = launch_fused_ws(L, ph, bo);
+      L->variant = v;
+    }
+  } else if (L->variant == 3 || (L->variant >= 31 && L->variant <= 39)) {
+    e = launch_fused_ws2(L, ph, bo);
+    if (e == cudaErrorNotSupported) {  // odd nx: one cell per lane
+      const int v = L->variant;
+      L->variant = 2;
+      e = launch_fused_ws(L, ph, bo);
+      L->variant = v;
+    }
+  } else if (L->variant == 2 || (L->variant >= 21 && L->variant <= 29)) {
     e = launch_fused_ws(L, ph, bo);
   } else if (L->variant >= 1) {
     e = launch_fused(L, ph, bo);

@@ -199,8 +199,9 @@ __device__ __forceinline__ void collide(const PhysF& ph, const Moments& m, float
       if (cz == -1) O -= OZ[x2][y2];
       if (cx * cy * cz == 1) O += Gxyz;
       if (cx * cy * cz == -1) O -= Gxyz;
-      out[i] = w * (E + O);
-      out[26 - i] = w * (E - O);
+      const float wE = w * E;
+      out[i] = fmaf(w, O, wE);
+      out[26 - i] = fmaf(-w, O, wE);
     }
   }
 }

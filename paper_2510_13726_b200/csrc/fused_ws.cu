@@ -15,7 +15,7 @@
 // Synchronisation is by named barriers (bar.arrive / bar.sync), one FULL and one EMPTY per slot.
 #include <cstdlib>
 
-#include "d3q27.cuh"
+#include "ws_common.cuh"
 
 namespace hhrr {
 
@@ -38,51 +38,6 @@ struct WsCfg {
   static_assert(RTASKS % NPW == 0, "row tasks must divide evenly over the producer warps");
   static_assert(2 * DEPTH + 1 <= 16, "named barriers");
 };
-
-struct WsArgs {
-  Dom dm;
-  PhysF ph;
-  BodiesF bo;
-  const float* fin;
-  float* fout;
-  const uint8_t* flags;
-  const float* d;
-  const float* wm_u;
-  const float* wm_s;
-  int zchunk;
-  long long plane_b[Q];  // 4 * i * n                            (byte offsets, warp-uniform)
-  long long push_b[Q];   // 4 * (i * n + cx + cy*nx + cz*nx*ny)
-};
-
-__device__ __forceinline__ void bar_sync(int id, int count) {
-  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
-}
-__device__ __forceinline__ void bar_arrive(int id, int count) {
-  asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory");
-}
-
-__device__ __forceinline__ int virt_ws(int v, int n, int mode, bool& flip, bool& ok) {
-  flip = false;
-  ok = (v >= -1 && v <= n);
-  if (!ok) return 0;
-  return wrap_axis(v, n, mode, flip);
-}
-
-__device__ __forceinline__ void solid_state_ws(const WsArgs& a, uint8_t fl, int64_t c, int x, int y, int z,
-                                               float& d, float uB[3]) {
-  int type = fl & TYPE_MASK;
-  d = 1.f;
-  uB[0] = uB[1] = uB[2] = 0.f;
-  if (type >= HHRR_FRONTIER) {
-    d = (type == HHRR_FRONTIER) ? __ldg(a.d + c) : 0.f;
-    solid_velocity(a.ph, a.bo, fl, x, y, z, uB);
-    if (fl & WM_VALID) {
-      uB[0] += __ldg(a.wm_u + c);
-      uB[1] += __ldg(a.wm_u + a.dm.n + c);
-      uB[2] += __ldg(a.wm_u + 2 * a.dm.n + c);
-    }
-  }
-}
 
 // per-lane description of one producer task; fixed over the z march
 struct PTask {
@@ -270,13 +225,7 @@ static cudaError_t launch_ws_cfg(hhrr_lattice* L, const WsArgs& a0) {
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  // Short z-chunks (~24 planes): blocks are dispatched in (x, y, z-chunk) order, so all SMs work
-  // on one slab of the lattice at a time and a tile's halo rows are still in L2 when its
-  // neighbour tile loads them; long chunks let neighbouring blocks drift apart (measured:
-  // 6.3 ms at 2 chunks vs 5.6 ms at 16 on 768x384x364).  Cost: two extra planes loaded per chunk.
-  int nch = (dm.nz + 11) / 24;
-  if (nch < 1) nch = 1;
-  if (const char* e = getenv("HHRR_ZCHUNKS")) nch = atoi(e) < 1 ? 1 : atoi(e);  // tuning runs only
+  int nch = ws_zchunks(dm.nz);
   a.zchunk = (dm.nz + nch - 1) / nch;
   nch = (dm.nz + a.zchunk - 1) / a.zchunk;
   dim3 grid((dm.nx + TX - 1) / TX, (dm.ny + TY - 1) / TY, nch);
@@ -285,8 +234,7 @@ static cudaError_t launch_ws_cfg(hhrr_lattice* L, const WsArgs& a0) {
   return cudaGetLastError();
 }
 
-cudaError_t launch_fused_ws(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo) {
-  WsArgs a;
+void fill_ws_args(const hhrr_lattice* L, const PhysF& ph, const BodiesF& bo, WsArgs& a) {
   a.dm = L->dom;
   a.ph = ph;
   a.bo = bo;
@@ -302,6 +250,22 @@ cudaError_t launch_fused_ws(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo)
     a.plane_b[i] = 4 * (i * n);
     a.push_b[i] = 4 * (i * n + dir_cx(i) + dir_cy(i) * nx + dir_cz(i) * nxy);
   }
+}
+
+// number of z-chunks: short chunks (~24 planes).  Blocks are dispatched in (x, y, z-chunk) order, so
+// all SMs work on one slab of the lattice at a time and a tile's halo rows are still in L2 when its
+// neighbour tile loads them; long chunks let neighbouring blocks drift apart (measured: 6.3 ms at 2
+// chunks vs 5.6 ms at 16 on 768x384x364).  Cost: two extra planes loaded per chunk.
+int ws_zchunks(int nz) {
+  int nch = (nz + 11) / 24;
+  if (nch < 1) nch = 1;
+  if (const char* e = getenv("HHRR_ZCHUNKS")) nch = atoi(e) < 1 ? 1 : atoi(e);  // tuning runs only
+  return nch;
+}
+
+cudaError_t launch_fused_ws(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo) {
+  WsArgs a;
+  fill_ws_args(L, ph, bo, a);
   switch (L->variant) {
     case 21: return launch_ws_cfg<64, 8, 10, 4, 1>(L, a);
     case 22: return launch_ws_cfg<64, 8, 10, 5, 1>(L, a);

@@ -249,11 +249,13 @@ __global__ void counters_kernel(Counters* cnt, int op) {
 }
 
 static void geo_grid(const GeoArgs& a, dim3& g, dim3& b) {
-  b = dim3(128);
   if (a.inside) {
     int bx = a.box.x1 - a.box.x0, by = a.box.y1 - a.box.y0, bz = a.box.z1 - a.box.z0;
-    g = dim3(by * bz, (bx + 127) / 128);
+    int t = bx <= 32 ? 32 : (bx <= 64 ? 64 : 128);  // a rotor box is thin along its axis: do not idle lanes
+    b = dim3(t);
+    g = dim3(by * bz, (bx + t - 1) / t);
   } else {
+    b = dim3(128);
     g = dim3(a.dm.ny * a.dm.nz, (a.dm.nx + 127) / 128);
   }
 }

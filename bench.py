@@ -163,7 +163,7 @@ def run_reference(args, rank, world):
 def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
-    from paper_2510_13726_b200 import binding as B, build
+    from paper_2510_13726_b200 import binding as B, build, replicas
 
     build.build()
     if not torch.cuda.is_available():
@@ -208,11 +208,8 @@ def run_ours(args, rank, world, local_rank):
     L.set_timing(False)
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     L.check_finite()
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * n * args.steps / (ms * 1e3)
+    ms = replicas.max_over_ranks(ms, device=dev)          # slowest replica
+    value = replicas.aggregate_mlups(n, args.steps, ms, world)
 
     # end to end through the C ABI with HOST buffers: upload the populations from pinned host
     # memory, step, read moments and forces back -- all inside the timed region
@@ -233,11 +230,8 @@ def run_ours(args, rank, world, local_rank):
     e1.record(L.stream)
     barrier()
     e2e_ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
-    e2e = {"value": world * n * e2e_steps / (e2e_ms * 1e3), "unit": "MLUPs",
+    e2e_ms = replicas.max_over_ranks(e2e_ms, device=dev)
+    e2e = {"value": replicas.aggregate_mlups(n, e2e_steps, e2e_ms, world), "unit": "MLUPs",
            "h2d_bytes_per_step": h_f.numel() * 4 / e2e_steps,
            "d2h_bytes_per_step": (h_rho.numel() + h_v.numel()) * 4 / e2e_steps + F.nbytes / e2e_steps,
            "steps": e2e_steps, "ms_total": e2e_ms,

@@ -106,15 +106,7 @@ def oracle_sample(config: int, budget_s: float = 20.0):
     """Times the oracle as it stands on a bounded sample of the config's recipe."""
     from oracle import oracle as O
     O.build()
-    if config >= 4:
-        case = I.case_rotor(192, 96, 91, 30.0, 4, omega=0.002 * 4)
-        sample = "config-5 recipe scaled 1/4 (192x96x91 cells, rotor R=30, wall model + forces on)"
-    elif config == 3:
-        case = I.case_channel(128, 64, 64, 4)
-        sample = "config-3 recipe at 128x64x64"
-    else:
-        case = I.baseline_config(config)
-        sample = f"config {config} at full size"
+    case, sample = reference_sample(config)
     p = O.make_params(case.nx, case.ny, case.nz, mode=case.mode, **case.params)
     L = O.Lattice(p)
     I.apply_case(case, L)
@@ -133,27 +125,50 @@ def oracle_sample(config: int, budget_s: float = 20.0):
             "sample": f"{sample}, {steps} steps in {dt:.1f} s"}, dt / steps
 
 
+def reference_sample(config: int, shrink: int = 0):
+    """The bounded sample of the config's recipe the oracle is timed on; shrink halves the scale again."""
+    if config >= 4:
+        k = 4 << shrink
+        nx, ny, nz, R = 768 // k, 384 // k, 364 // k, 120.0 / k
+        return (I.case_rotor(nx, ny, nz, R, 4, omega=0.002 * k),
+                f"config-5 recipe scaled 1/{k} ({nx}x{ny}x{nz} cells, rotor R={R:g}, wall model + forces on)")
+    if config == 3:
+        return I.case_channel(128, 64, 64, 4), "config-3 recipe at 128x64x64"
+    return I.baseline_config(config), f"config {config} at full size"
+
+
 def run_reference(args, rank, world):
-    """Reference arm: the oracle on the host cores (rank 0 only)."""
+    """Reference arm: the oracle, as it stands, on the host cores (rank 0 only).  One step = one oracle
+    time step (all of Listing 3) on the bounded sample lattice; W untimed warm-up steps, K timed."""
     if rank != 0:
         return
-    case, wname = workload(args.config)
-    per_step_budget = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    _, wname = workload(args.config)
     from oracle import oracle as O
     O.build()
-    base, _ = oracle_sample(args.config, budget_s=1.0)  # warm the build / page cache
-    t_all, v_all = [], []
-    for s in range(args.warmup + args.steps):
-        cb, t_step = oracle_sample(args.config, budget_s=per_step_budget)
-        if s >= args.warmup:
-            t_all.append(t_step)
-            v_all.append(cb["value"])
-    value = float(np.mean(v_all))
-    cb["value"] = value
+    # size the sample so that W + K oracle steps end within a few minutes on this host
+    for shrink in range(4):
+        case, sample = reference_sample(args.config, shrink)
+        p = O.make_params(case.nx, case.ny, case.nz, mode=case.mode, **case.params)
+        L = O.Lattice(p)
+        I.apply_case(case, L)
+        L.step(1)
+        t0 = time.perf_counter()
+        L.step(1)
+        if (time.perf_counter() - t0) * (args.steps + args.warmup) <= 200.0 or shrink == 3 or args.config < 4:
+            break
+        L.close()
+    L.step(max(0, args.warmup - 2))
+    t0 = time.perf_counter()
+    L.step(args.steps)
+    dt = time.perf_counter() - t0
+    L.close()
+    value = case.n * args.steps / dt / 1e6
+    cb = {"value": value, "unit": "MLUPs", "cores": O.threads(), "kind": "oracle",
+          "sample": f"{sample}, {args.steps} steps in {dt:.1f} s"}
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "MLUPs", "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(np.mean(t_all) * 1e3),
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": {"workload": wname, "note": "each step = one bounded oracle sample"},
+            "data": "synthetic", "config": {"workload": wname, "note": "each step = one oracle time step on the bounded sample"},
             "cpu_baseline": cb,
             "e2e": {"value": value, "unit": "MLUPs", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}

@@ -262,7 +262,7 @@ def run_ours(args, rank, world, local_rank):
                     "peak_source": peak_src, "kernel_ms": k_avg_ms, "kernel_launches_timed": k_n,
                     "kernel_share_of_step": k_ms / (ms * k_n / args.steps) if k_n else None,
                     "algorithmic_bytes_per_cell": BYTES_PER_CELL}
-        tr = ROOT / "profiles" / "traffic.json"   # DRAM bytes per launch from the committed ncu capture
+        tr = ROOT / "profiles" / "r01_traffic.txt"   # DRAM bytes per launch from the committed ncu capture
         if tr.exists():
             try:
                 t = json.loads(tr.read_text())

@@ -71,6 +71,19 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map
       : "memory");
 }
 
+// register reallocation between warpgroups (the kernel starts with 65536 / threads registers each;
+// the producer/aux warpgroup hands most of its share to the two worker warpgroups)
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+
+// uhat of plane `it` is published: one arrival per warp; waited for one iteration later (split phase:
+// a warp may run up to one plane ahead of the slowest one instead of meeting it at a block barrier)
+__device__ __forceinline__ void pub_arrive(uint32_t pub0, int it) {
+  __syncwarp();
+  if ((threadIdx.x & 31) == 0) mbar_arrive(pub0 + 8 * (it & 1));
+}
+__device__ __forceinline__ void pub_wait(uint32_t pub0, int it) { mbar_wait(pub0 + 8 * (it & 1), (it >> 1) & 1); }
+
 template <int CPT>
 __global__ void __launch_bounds__(tma::threads(CPT), 1)
     fused_tma_kernel(const __grid_constant__ WsArgs a, const __grid_constant__ CUtensorMap map_main,
@@ -80,7 +93,7 @@ __global__ void __launch_bounds__(tma::threads(CPT), 1)
   extern __shared__ __align__(128) unsigned char smem[];
   float(*ring)[3][PLANE] = reinterpret_cast<float(*)[3][PLANE]>(smem + (size_t)NS * STAGE_BYTES);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)NS * STAGE_BYTES + RING_BYTES);
-  const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + NS);
+  const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + NS), pub0 = smem_u32(bars + 2 * NS);
 
   const Dom& dm = a.dm;
   const int tid = threadIdx.x;
@@ -106,10 +119,15 @@ __global__ void __launch_bounds__(tma::threads(CPT), 1)
       mbar_init(full0 + 8 * s, 2);  // TMA issue (+ its bytes) and the flag bytes
       mbar_init(empty0 + 8 * s, (WORKERS + AUX) / 32);
     }
+    for (int s = 0; s < 2; ++s) mbar_init(pub0 + 8 * s, (WORKERS + AUX) / 32);  // uhat of a plane published
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   __syncthreads();
+
+  if constexpr (CPT == 2) {  // 2 worker warpgroups + 1 warpgroup of aux/producer warps: 256*216 + 128*72 = 384*168
+    if (tid >= WORKERS) reg_dec<72>(); else reg_inc<216>();
+  }
 
   if (tid >= WORKERS + AUX) {
     // ------------------------------------------------------------------ producer: one lane issues TMA
@@ -190,6 +208,7 @@ __global__ void __launch_bounds__(tma::threads(CPT), 1)
       const float* st = reinterpret_cast<const float*>(smem + (size_t)s * STAGE_BYTES);
       const uint8_t* flb = smem + (size_t)s * STAGE_BYTES + TMA_BYTES;
       float(*slot)[PLANE] = ring[it & 3];
+      if (it >= 4) pub_wait(pub0, it - 2);  // every worker is past the collision that read this ring slot
       mbar_wait(full0 + 8 * s, k2 & 1);
 #pragma unroll
       for (int k = 0; k < 2; ++k) {
@@ -207,8 +226,10 @@ __global__ void __launch_bounds__(tma::threads(CPT), 1)
         slot[2][h_slot[k]] = fz ? -uh[2] : uh[2];
       }
       __syncwarp();
-      if ((tid & 31) == 0) mbar_arrive(empty0 + 8 * s);
-      if (p - 1 >= z0) bar_sync(1, WORKERS + AUX);  // in step with the workers' collide of plane p-1
+      if ((tid & 31) == 0) {
+        mbar_arrive(empty0 + 8 * s);
+        mbar_arrive(pub0 + 8 * (it & 1));
+      }
     }
     return;
   }
@@ -261,9 +282,10 @@ __global__ void __launch_bounds__(tma::threads(CPT), 1)
       slot[1][own_slot] = uh[1];
       slot[2][own_slot] = fz ? -uh[2] : uh[2];
     }
+    pub_arrive(pub0, it);
     const int z = p - 1;
     if (z >= z0) {
-      bar_sync(1, WORKERS + AUX);
+      pub_wait(pub0, it - 1);  // the xy neighbours' uhat of plane z (own cell of plane z+1: written above)
       float S[6], sigma = a.ph.sigma;
       if (fl_c & WM_VALID) {
         const int64_t c = own_xy + nxy * z;
@@ -358,9 +380,10 @@ __global__ void __launch_bounds__(tma::threads(CPT), 1)
           slot[2][own_slot + k] = fz ? -uh[2] : uh[2];
         }
       }
+      pub_arrive(pub0, it);
       const int z = p - 1;
       if (z >= z0) {
-        bar_sync(1, WORKERS + AUX);
+        pub_wait(pub0, it - 1);  // the xy neighbours' uhat of plane z (own cell of plane z+1: written above)
         float(*sm)[PLANE] = ring[(it - 2) & 3];
         float(*s0)[PLANE] = ring[(it - 1) & 3];
         float(*sp)[PLANE] = ring[it & 3];

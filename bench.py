@@ -257,7 +257,7 @@ def run_ours(args, rank, world, local_rank):
         peak, peak_src = measured_peak()
         k_avg_ms = k_ms / max(1, k_n)
         achieved = n * BYTES_PER_CELL / (k_avg_ms * 1e-3) / 1e9
-        roofline = {"bound": "hbm", "kernel": {0: "moments_kernel+collide_kernel", 1: "fused_kernel", 2: "fused_ws_kernel", 3: "fused_ws2_kernel", 4: "fused_tma_kernel<2>"}.get(args.variant, "fused kernel, tuning shape %d" % args.variant),
+        roofline = {"bound": "hbm", "kernel": {0: "moments_kernel+collide_kernel", 1: "fused_kernel", 2: "fused_ws_kernel", 3: "fused_ws2_kernel", 4: "fused_tma_kernel<2>", 5: "fused_xpull_kernel"}.get(args.variant, "fused kernel, tuning shape %d" % args.variant),
                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                     "peak_source": peak_src, "kernel_ms": k_avg_ms, "kernel_launches_timed": k_n,
                     "kernel_share_of_step": k_ms / (ms * k_n / args.steps) if k_n else None,
@@ -276,7 +276,7 @@ def run_ours(args, rank, world, local_rank):
         line = {"metric": METRIC, "value": value, "unit": "MLUPs", "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": {"workload": wname, "cells_per_gpu": n, "lattice": "D3Q27", "storage": "fp32 SoA A/B",
+                "config": {"workload": wname, "cells_per_gpu": n, "lattice": "D3Q27", "storage": "fp32 SoA A/B" + (", x-pull / yz-push" if L.population_storage() else ""),
                            "kernel_variant": args.variant, "parallelism": f"replicas x{world}",
                            "l2": "inputs (11.6 GB per buffer) exceed the 126 MB L2; no flush needed"},
                 "hbm_frac_of_peak_step": value * 1e6 * BYTES_PER_CELL / 1e9 / peak / world,
@@ -294,7 +294,7 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=100)
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
-    ap.add_argument("--variant", type=int, default=4, choices=[0, 1, 2, 3, 4] + list(range(11, 50)))
+    ap.add_argument("--variant", type=int, default=5, choices=[0, 1, 2, 3, 4, 5] + list(range(11, 50)))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

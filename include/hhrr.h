@@ -170,9 +170,17 @@ int hhrr_get_uhat(hhrr_lattice* L, float* uhat);
 int hhrr_check_finite(hhrr_lattice* L);
 /* Selects the collide-stream kernel: 0 = two-pass (moments pass + collide pass), 1 = fused
  * sliding-window kernel, 2 = fused warp-specialised kernel, 3 = the same with two cells per
- * lane, 4 = fused kernel fed by TMA (default; needs nx % 64 == 0 and ny % 8 == 0, otherwise
- * 2 runs); 11-49 = tile shapes kept for tuning runs.  All compute the same step.        */
+ * lane, 4 = fused kernel fed by TMA (needs nx % 64 == 0 and ny % 8 == 0, otherwise 2 runs),
+ * 5 = the TMA-fed kernel on x-pull / yz-push storage (default; needs nx % 64 == 0, nx >= 128,
+ * ny % 8 == 0 and a periodic x axis, otherwise 2 runs); 11-49 = tile shapes kept for tuning
+ * runs.  All compute the same step (Listing 3 line 3).  Variant 5 keeps plane i
+ * of the population buffer as f_i(x + c_ix, y, z) (the x move of Eq. 6, is taken
+ * on the read side); the call re-stores the current populations when the layout changes, and
+ * every entry point that takes or returns populations speaks the plain post-stream layout.   */
 int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant);
+/* 1 if the populations are currently kept x-pulled (variant 5 running its own kernel), 0 if
+ * post-stream (all other variants, and variant 5 on a lattice it cannot tile).            */
+int hhrr_population_storage(const hhrr_lattice* L);
 /* Optional CUDA-event timing of the collide-stream launches inside hhrr_step (the kernel the
  * roofline is quoted on).  hhrr_get_timing synchronises, returns the summed device time in
  * milliseconds and the number of launches it covers (at most 1024 per window), and starts a

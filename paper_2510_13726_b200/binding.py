@@ -28,6 +28,7 @@ SYMBOLS = [
     "hhrr_get_moments", "hhrr_get_moments_device", "hhrr_get_forces", "hhrr_force_history",
     "hhrr_get_cell_types", "hhrr_get_wall_list", "hhrr_get_wall_state", "hhrr_get_populations",
     "hhrr_set_populations", "hhrr_get_cell_populations", "hhrr_get_uhat", "hhrr_check_finite", "hhrr_set_kernel_variant",
+    "hhrr_population_storage",
     "hhrr_set_timing", "hhrr_get_timing", "hhrr_launch_count", "hhrr_last_error", "hhrr_version",
 ]
 
@@ -80,6 +81,7 @@ def lib():
         L.hhrr_set_rotor.argtypes = [vp, C.POINTER(RotorDesc)]
         L.hhrr_enable_wall_model.argtypes = [vp, C.c_int]
         L.hhrr_update_geometry.argtypes = [vp]
+        L.hhrr_population_storage.argtypes = [vp]
         L.hhrr_step.argtypes = [vp, i32]
         L.hhrr_step_count.restype = i64
         L.hhrr_step_count.argtypes = [vp]
@@ -230,6 +232,9 @@ class Lattice:
 
     def set_kernel_variant(self, variant):
         _check(lib().hhrr_set_kernel_variant(self.h, int(variant)))
+
+    def population_storage(self):
+        return int(lib().hhrr_population_storage(self.h))
 
     # ---- time loop
     def step(self, n=1):

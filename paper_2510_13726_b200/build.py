@@ -30,6 +30,7 @@ SOURCES = {
     "fused_ws.cu": [],
     "fused_ws2.cu": [],
     "fused_tma.cu": [],
+    "fused_xpull.cu": [],
     "wallmodel.cu": [],
     "geometry.cu": ["-fmad=false"],
 }

@@ -9,7 +9,7 @@
 #include <new>
 #include <vector>
 
-#include "lattice.h"
+#include "d3q27.cuh"
 
 using namespace hhrr;
 
@@ -177,7 +177,8 @@ int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes,
   int64_t rest = (int64_t)(workspace_bytes - lead - need_min);
   int64_t spare = std::max<int64_t>(0, (rest - 512) / 5);
   carve(L, p, spare, base);
-  L->variant = 4;
+  L->variant = 5;
+  L->dom.xs = xpull_supported(L->dom) ? 1 : 0;  // buffers start as zeros: nothing to convert
   L->geometry_dirty = true;
   L->geometry_current = false;
   const int64_t n = L->dom.n;
@@ -351,10 +352,15 @@ int hhrr_update_geometry(hhrr_lattice* L) {
 }
 
 int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant) {
-  if (!L || variant < 0 || (variant > 4 && (variant < 11 || variant > 49))) return fail(HHRR_E_ARG, "hhrr_set_kernel_variant: bad argument");
+  if (!L || variant < 0 || (variant > 5 && (variant < 11 || variant > 49))) return fail(HHRR_E_ARG, "hhrr_set_kernel_variant: bad argument");
   L->variant = variant;
+  // variant 5 keeps the populations x-pulled (where it can run); everything else stores them post-stream
+  cudaError_t e = launch_restore(L, (variant == 5 && xpull_supported(L->dom)) ? 1 : 0);
+  if (e != cudaSuccess) return cuda_fail(e, "restore kernel");
   return HHRR_OK;
 }
+
+int hhrr_population_storage(const hhrr_lattice* L) { return L ? L->dom.xs : 0; }
 
 int hhrr_set_timing(hhrr_lattice* L, int enable) {
   if (!L) return fail(HHRR_E_ARG, "hhrr_set_timing: NULL lattice");
@@ -467,12 +473,13 @@ __global__ void gather_wall_kernel(const int32_t* idx, int count, const double* 
   out_utau[e] = wm_utau[c];
   out_valid[e] = (flags[c] & WM_VALID) ? 1 : 0;
 }
-__global__ void gather_cells_kernel(const float* f, const uint8_t* flags, int64_t n, const int64_t* cells,
+__global__ void gather_cells_kernel(const float* f, const uint8_t* flags, Dom dm, const int64_t* cells,
                                     int64_t count, float* out, uint8_t* out_flags) {
   int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= count) return;
   int64_t c = cells[k];
-  for (int i = 0; i < Q; ++i) out[k * Q + i] = f[(int64_t)i * n + c];
+  const int x = (int)(c % dm.nx), y = (int)((c / dm.nx) % dm.ny), z = (int)(c / ((int64_t)dm.nx * dm.ny));
+  for (int i = 0; i < Q; ++i) out[k * Q + i] = f[pop_index(dm, i, x, y, z)];
   out_flags[k] = flags[c];
 }
 int read_counters(hhrr_lattice* L, Counters* h) { return download(L, h, L->counters, sizeof(Counters)); }
@@ -555,7 +562,7 @@ int hhrr_get_cell_populations(hhrr_lattice* L, int64_t n_cells, const int64_t* c
   uint8_t* d_fl = reinterpret_cast<uint8_t*>(sb + 8 * n_cells + 4 * Q * n_cells);
   int rc = upload(L, d_cells, cells, 8 * (size_t)n_cells);
   if (rc) return rc;
-  gather_cells_kernel<<<(unsigned)((n_cells + 127) / 128), 128, 0, L->stream>>>(L->fA, L->flags, L->dom.n, d_cells,
+  gather_cells_kernel<<<(unsigned)((n_cells + 127) / 128), 128, 0, L->stream>>>(L->fA, L->flags, L->dom, d_cells,
                                                                              n_cells, d_out, d_fl);
   L->launches++;
   CU(cudaGetLastError());
@@ -567,11 +574,27 @@ int hhrr_get_cell_populations(hhrr_lattice* L, int64_t n_cells, const int64_t* c
 
 int hhrr_get_populations(hhrr_lattice* L, float* f_minus_w) {
   if (!L || !f_minus_w) return fail(HHRR_E_ARG, "hhrr_get_populations: NULL argument");
-  return download(L, f_minus_w, L->fA, sizeof(float) * Q * L->dom.n);
+  if (!L->dom.xs) return download(L, f_minus_w, L->fA, sizeof(float) * Q * L->dom.n);
+  // the ABI speaks the plain post-stream layout: convert into buffer B (free between steps), read that
+  const int xs = L->dom.xs;
+  cudaError_t e = launch_restore(L, 0);  // A <-> B swapped, A now plain
+  if (e != cudaSuccess) return cuda_fail(e, "restore kernel");
+  int rc = download(L, f_minus_w, L->fA, sizeof(float) * Q * L->dom.n);
+  float* t = L->fA;  // swap back: the stored state is untouched
+  L->fA = L->fB;
+  L->fB = t;
+  L->dom.xs = xs;
+  return rc;
 }
 int hhrr_set_populations(hhrr_lattice* L, const float* f_minus_w) {
   if (!L || !f_minus_w) return fail(HHRR_E_ARG, "hhrr_set_populations: NULL argument");
-  return upload(L, L->fA, f_minus_w, sizeof(float) * Q * L->dom.n);
+  int rc = upload(L, L->fA, f_minus_w, sizeof(float) * Q * L->dom.n);
+  if (rc || !L->dom.xs) return rc;
+  const int xs = L->dom.xs;
+  L->dom.xs = 0;  // what was uploaded is the plain post-stream layout
+  cudaError_t e = launch_restore(L, xs);
+  if (e != cudaSuccess) return cuda_fail(e, "restore kernel");
+  return HHRR_OK;
 }
 int hhrr_get_uhat(hhrr_lattice* L, float* uhat) {
   if (!L || !uhat) return fail(HHRR_E_ARG, "hhrr_get_uhat: NULL argument");

@@ -187,8 +187,10 @@ __global__ void __launch_bounds__(256) readback_kernel(Dom dm, PhysF ph, const f
                                                        float* __restrict__ rho_out, float* __restrict__ v_out) {
   int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= dm.n) return;
+  const int x = (int)(c % dm.nx), y = (int)((c / dm.nx) % dm.ny), z = (int)(c / ((int64_t)dm.nx * dm.ny));
   float f[Q];
-  load_cell(fin, dm.n, c, f);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) f[i] = __ldg(fin + pop_index(dm, i, x, y, z));
   double drho = 0, j[3] = {0, 0, 0};
 #pragma unroll
   for (int i = 0; i < Q; ++i) {
@@ -200,6 +202,19 @@ __global__ void __launch_bounds__(256) readback_kernel(Dom dm, PhysF ph, const f
   double rho = 1.0 + drho;
   rho_out[c] = (float)rho;
   for (int a = 0; a < 3; ++a) v_out[(int64_t)a * dm.n + c] = (float)((j[a] + 0.5 * (double)ph.g[a]) / rho);
+}
+
+// re-store the populations with another x-shift: dst (storage xs_to) from src (storage dm.xs)
+__global__ void __launch_bounds__(256) restore_kernel(Dom dm, int xs_to, const float* __restrict__ src,
+                                                      float* __restrict__ dst) {
+  int x = blockIdx.x * blockDim.x + threadIdx.x;
+  int y = blockIdx.y, z = blockIdx.z;
+  if (x >= dm.nx) return;
+  Dom to = dm;
+  to.xs = xs_to;
+  // population i of the post-stream state of cell (x,y,z): read where dm keeps it, write where `to` keeps it
+#pragma unroll
+  for (int i = 0; i < Q; ++i) dst[pop_index(to, i, x, y, z)] = src[pop_index(dm, i, x, y, z)];
 }
 
 __global__ void finite_kernel(const float* __restrict__ f, int64_t count, Counters* cnt) {
@@ -246,6 +261,25 @@ cudaError_t launch_init(hhrr_lattice* L, const float* d_rho, const float* d_u, i
   int bx = row_block(L->dom);
   init_kernel<<<row_grid(L->dom, bx), bx, 0, L->stream>>>(L->dom, L->p.tau0, d_rho, d_u, with_neq, L->fA);
   L->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess && L->dom.xs) {  // init_kernel writes the plain post-stream layout
+    const int xs = L->dom.xs;
+    L->dom.xs = 0;
+    e = launch_restore(L, xs);
+  }
+  return e;
+}
+
+// buffer A: from storage dom.xs to storage xs (through buffer B, which is free between steps)
+cudaError_t launch_restore(hhrr_lattice* L, int xs) {
+  if (xs == L->dom.xs) return cudaSuccess;
+  int bx = row_block(L->dom);
+  restore_kernel<<<row_grid(L->dom, bx), bx, 0, L->stream>>>(L->dom, xs, L->fA, L->fB);
+  L->launches++;
+  float* t = L->fA;
+  L->fA = L->fB;
+  L->fB = t;
+  L->dom.xs = xs;
   return cudaGetLastError();
 }
 
@@ -253,12 +287,20 @@ cudaError_t launch_fused(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo);  
 cudaError_t launch_fused_ws(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo);  // fused_ws.cu
 cudaError_t launch_fused_ws2(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo); // fused_ws2.cu
 cudaError_t launch_fused_tma(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo); // fused_tma.cu
+cudaError_t launch_fused_xpull(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo); // fused_xpull.cu
 
 cudaError_t launch_collide_stream(hhrr_lattice* L) {
   PhysF ph = make_phys(L);
   BodiesF bo = make_bodies(L);
   cudaError_t e;
-  if (L->variant == 4 || L->variant == 41) {
+  if (L->variant == 5) {
+    e = launch_fused_xpull(L, ph, bo);
+    if (e == cudaErrorNotSupported) {  // lattice keeps post-stream storage: warp-specialised kernel
+      L->variant = 2;
+      e = launch_fused_ws(L, ph, bo);
+      L->variant = 5;
+    }
+  } else if (L->variant == 4 || L->variant == 41) {
     e = launch_fused_tma(L, ph, bo);
     if (e == cudaErrorNotSupported) {  // ragged tiles: warp-specialised kernel, one cell per lane
       const int v = L->variant;

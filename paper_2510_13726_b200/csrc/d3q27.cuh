@@ -206,6 +206,14 @@ __device__ __forceinline__ void collide(const PhysF& ph, const Moments& m, float
   }
 }
 
+// where population i of the post-stream state of cell (x,y,z) is stored (see Dom::xs)
+__device__ __forceinline__ int64_t pop_index(const Dom& dm, int i, int x, int y, int z) {
+  int xs = x - dm.xs * dir_cx(i);
+  if (xs < 0) xs += dm.nx;
+  else if (xs >= dm.nx) xs -= dm.nx;
+  return (int64_t)i * dm.n + xs + (int64_t)dm.nx * (y + (int64_t)dm.ny * z);
+}
+
 // neighbour index along one axis with the outer-boundary rule R12.
 // Returns the wrapped / reflected coordinate; flip = true if it was reflected.
 __device__ __forceinline__ int wrap_axis(int v, int n, int mode, bool& flip) {

@@ -1,0 +1,463 @@
+// fused_xpull.cu -- variant 5 of K2 (default): the TMA-fed fused collide-stream kernel on
+// "x-pull / yz-push" storage.
+//
+// Same step as every other variant (Listing 3 line 3; Eq. 6-14; S^FD of Eq. 10 from
+// the time-n uhat of the six face neighbours, sliding window along z).  What changes is WHERE the
+// streaming shift of Eq. 6 is paid:
+//   * plane i of the buffer holds g_i(x,y,z) = f*_i(x, y - c_iy, z - c_iz): the post-collision value
+//     already moved along y and z (whole, 128-byte aligned rows) but not yet along x;
+//   * the x shift happens on the read side, in shared memory: the TMA box of a tile is 72 cells wide
+//     (4 + 64 + 4), population i of cell x is read at column x - c_ix.
+// Every global store of the kernel is therefore an aligned, full-sector 8-byte store of two x-adjacent
+// cells (27 per thread and plane instead of 45 partly half-filled ones), and the 72-wide box carries
+// the x halo of the tile for free.  Tiles at the periodic x boundary get three small extra boxes (the
+// 4 wrapped columns) which only their edge lanes read.
+//
+// Needs nx % 64 == 0, nx >= 128, ny % 8 == 0 and a periodic x axis (xpull_supported); other lattices
+// keep post-stream storage and run variant 2.
+#include <cuda.h>
+
+#include <cstdlib>
+
+#include "ws_common.cuh"
+
+namespace hhrr {
+
+namespace xp {
+constexpr int TX = 64, TY = 8, NS = 2, W = TX + 8;
+constexpr int WORKERS = TX * TY / 2, AUX = 96, THREADS = WORKERS + AUX + 32;
+constexpr int SX = TX + 2, SY = TY + 2, PLANE = SX * SY;
+constexpr int HALO = 2 * TX + 2 * TY;
+// one stage, in floats: [27][8][72] tile rows | [27][72] row y0-1 | [27][72] row y0+8 |
+//                       [27][8][4] wrapped columns of the tile rows | [27][4] | [27][4] of the halo rows
+constexpr int MAIN_F = Q * TY * W, ROW_F = Q * W, ROW_PAD_F = 1952, PM_F = Q * TY * 4, PR_F = Q * 4, PR_PAD_F = 128;
+constexpr int O_RM = MAIN_F, O_RP = O_RM + ROW_PAD_F, O_PM = O_RP + ROW_PAD_F, O_PRM = O_PM + PM_F,
+              O_PRP = O_PRM + PR_PAD_F, END_F = O_PRP + PR_PAD_F;
+constexpr uint32_t TMA_BYTES = (MAIN_F + 2 * ROW_F) * 4, TMA_EDGE_BYTES = (PM_F + 2 * PR_F) * 4;
+constexpr int FL_MAIN = 0, FL_YM = TY * TX, FL_YP = FL_YM + TX, FL_XM = FL_YP + TX, FL_XP = FL_XM + TY;
+constexpr uint32_t FLAG_OFF = END_F * 4, STAGE_BYTES = FLAG_OFF + 768;
+constexpr size_t RING_BYTES = 4 * 3 * PLANE * 4;
+constexpr size_t SMEM = (size_t)NS * STAGE_BYTES + RING_BYTES + 64;
+static_assert(FL_XP + TY <= 768 && STAGE_BYTES % 128 == 0, "flag region");
+static_assert((O_RM * 4) % 128 == 0 && (O_RP * 4) % 128 == 0 && (O_PM * 4) % 128 == 0 && (O_PRM * 4) % 128 == 0 &&
+                  (O_PRP * 4) % 128 == 0 && ROW_PAD_F >= ROW_F && PR_PAD_F >= PR_F,
+              "TMA smem alignment");
+static_assert(SMEM <= 227 * 1024, "shared memory");
+// population i = (cx+1) + 3k, k = (cy+1) + 3(cz+1): stride between the members of one cx group
+}  // namespace xp
+
+namespace {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, int c3,
+                                            uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+      ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar)
+      : "memory");
+}
+// register reallocation between warpgroups: 256 * 208 + 128 * 88 = 384 * 168
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+
+// uhat of plane `it` is published: one arrival per warp, waited for one iteration later (split phase)
+__device__ __forceinline__ void pub_arrive(uint32_t pub0, int it) {
+  __syncwarp();
+  if ((threadIdx.x & 31) == 0) mbar_arrive(pub0 + 8 * (it & 1));
+}
+__device__ __forceinline__ void pub_wait(uint32_t pub0, int it) { mbar_wait(pub0 + 8 * (it & 1), (it >> 1) & 1); }
+
+// store of the 27 post-collision values of cell (x,y,z), moved along y and z only, with rule R12
+__device__ __forceinline__ void push_store_yz(const Dom& dm, float* __restrict__ fout, int x, int y, int z,
+                                              const float (&o)[Q]) {
+  bool fym, fyp, fzm, fzp;
+  const int ym = wrap_axis(y - 1, dm.ny, dm.mode[1], fym), yp = wrap_axis(y + 1, dm.ny, dm.mode[1], fyp);
+  const int zm = wrap_axis(z - 1, dm.nz, dm.mode[2], fzm), zp = wrap_axis(z + 1, dm.nz, dm.mode[2], fzp);
+  const int64_t nx = dm.nx, nxy = (int64_t)dm.nx * dm.ny;
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    int cy = dir_cy(i), cz = dir_cz(i), io = i;
+    int ty = cy < 0 ? ym : (cy > 0 ? yp : y);
+    int tz = cz < 0 ? zm : (cz > 0 ? zp : z);
+    // a population leaving through a mirror plane returns to the same cell, component reversed
+    if ((cy < 0 && fym) || (cy > 0 && fyp)) { ty = y; io -= 6 * cy; }
+    if ((cz < 0 && fzm) || (cz > 0 && fzp)) { tz = z; io -= 18 * cz; }
+    fout[(int64_t)io * dm.n + tz * nxy + ty * nx + x] = o[i];
+  }
+}
+
+}  // namespace
+
+__global__ void __launch_bounds__(xp::THREADS, 1)
+    fused_xpull_kernel(const __grid_constant__ WsArgs a, const __grid_constant__ CUtensorMap map_main,
+                       const __grid_constant__ CUtensorMap map_row, const __grid_constant__ CUtensorMap map_pm,
+                       const __grid_constant__ CUtensorMap map_pr) {
+  using namespace xp;
+  extern __shared__ __align__(128) unsigned char smem[];
+  float(*ring)[3][PLANE] = reinterpret_cast<float(*)[3][PLANE]>(smem + (size_t)NS * STAGE_BYTES);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)NS * STAGE_BYTES + RING_BYTES);
+  const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + NS), pub0 = smem_u32(bars + 2 * NS);
+
+  const Dom& dm = a.dm;
+  const int tid = threadIdx.x;
+  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
+  const int z0 = blockIdx.z * a.zchunk, z1 = min(dm.nz, z0 + a.zchunk);
+  const int64_t n = dm.n, nx = dm.nx, nxy = (int64_t)dm.nx * dm.ny;
+  const int pfirst = z0 - 1;
+  // tiles at the periodic x boundary: the 4 columns beyond it come from the other side (nx >= 128: one side only)
+  const bool edge_l = x0 == 0, edge_r = x0 + TX == dm.nx, edge = edge_l || edge_r;
+  const int px = edge_l ? dm.nx - 4 : 0;  // first wrapped column
+
+  bool fym, fyp, okh;
+  const int ym = virt_ws(y0 - 1, dm.ny, dm.mode[1], fym, okh), yp = virt_ws(y0 + TY, dm.ny, dm.mode[1], fyp, okh);
+
+  if (tid == 0) {
+    for (int s = 0; s < NS; ++s) {
+      mbar_init(full0 + 8 * s, 2);  // TMA issue (+ its bytes) and the flag bytes
+      mbar_init(empty0 + 8 * s, (WORKERS + AUX) / 32);
+    }
+    for (int s = 0; s < 2; ++s) mbar_init(pub0 + 8 * s, (WORKERS + AUX) / 32);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (tid >= WORKERS) reg_dec<88>(); else reg_inc<208>();
+
+  if (tid >= WORKERS + AUX) {
+    // ------------------------------------------------------------------ producer: one lane issues TMA
+    const int lane = tid & 31;
+    const int xl = edge_l ? dm.nx - 1 : x0 - 1, xr = edge_r ? 0 : x0 + TX;  // real x of the halo columns
+    for (int p = pfirst; p <= z1; ++p) {
+      const int it = p - pfirst, s = it % NS, k = it / NS;
+      if (k > 0) mbar_wait(empty0 + 8 * s, (k - 1) & 1);
+      bool fz, okz;
+      const int zr = virt_ws(p, dm.nz, dm.mode[2], fz, okz);
+      const uint32_t bar = full0 + 8 * s;
+      unsigned char* stb = smem + (size_t)s * STAGE_BYTES;
+      if (lane == 0) {
+        const uint32_t st = smem_u32(stb);
+        mbar_expect_tx(bar, edge ? TMA_BYTES + TMA_EDGE_BYTES : TMA_BYTES);
+        tma_load_4d(st, &map_main, x0 - 4, y0, zr, 0, bar);  // columns outside the lattice arrive as zeros
+        tma_load_4d(st + 4 * O_RM, &map_row, x0 - 4, ym, zr, 0, bar);
+        tma_load_4d(st + 4 * O_RP, &map_row, x0 - 4, yp, zr, 0, bar);
+        if (edge) {
+          tma_load_4d(st + 4 * O_PM, &map_pm, px, y0, zr, 0, bar);
+          tma_load_4d(st + 4 * O_PRM, &map_pr, px, ym, zr, 0, bar);
+          tma_load_4d(st + 4 * O_PRP, &map_pr, px, yp, zr, 0, bar);
+        }
+      }
+      // flag bytes of the same cells: 8 rows x 64 B + 2 halo rows as 16-byte loads, the columns bytewise
+      const uint8_t* fz0 = a.flags + nxy * zr;
+      unsigned char* flb = stb + FLAG_OFF;
+      const uint4 vmain = __ldg(reinterpret_cast<const uint4*>(fz0 + (x0 + (lane & 3) * 16) + nx * (y0 + (lane >> 2))));
+      uint4 vrow = make_uint4(0, 0, 0, 0);
+      uint8_t vcol = 0;
+      if (lane < 8) vrow = __ldg(reinterpret_cast<const uint4*>(fz0 + (x0 + (lane & 3) * 16) + nx * ((lane >> 2) ? yp : ym)));
+      if (lane >= 8 && lane < 8 + 2 * TY) {
+        const int h = lane - 8, right = h / TY, row = h % TY;
+        vcol = __ldg(fz0 + (right ? xr : xl) + nx * (y0 + row));
+      }
+      *reinterpret_cast<uint4*>(flb + FL_MAIN + (lane >> 2) * TX + (lane & 3) * 16) = vmain;
+      if (lane < 8) *reinterpret_cast<uint4*>(flb + FL_YM + (lane >> 2) * TX + (lane & 3) * 16) = vrow;
+      if (lane >= 8 && lane < 8 + 2 * TY) flb[FL_XM + (lane - 8)] = vcol;
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar);
+    }
+    return;
+  }
+
+  if (tid >= WORKERS) {
+    // ------------------------------------------------------------------ aux warps: uhat of the xy halo
+    // lane a owns halo cells a and a + AUX (if < HALO).  Per cell and per cx group: where population
+    // (cx, k = 0) sits in a stage and the stride to k + 1 (column lx - cx of the 72-wide boxes, or the
+    // wrapped columns at the periodic x boundary)
+    const int a0 = tid - WORKERS;
+    int h_off[2][3], h_str[2][3], h_slot[2], h_x[2], h_y[2], h_fl[2];
+    bool h_fy[2], h_on[2];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const int hc = a0 + k * AUX;
+      h_on[k] = hc < HALO;
+      h_fy[k] = false;
+      int lx, region, row = 0;  // region 0: tile rows, 1: row y0-1, 2: row y0+8
+      if (hc < 2 * TX) {
+        const int top = hc / TX;
+        lx = hc % TX;
+        region = 1 + top;
+        h_fl[k] = (top ? FL_YP : FL_YM) + lx;
+        h_slot[k] = (top ? TY + 1 : 0) * SX + lx + 1;
+        h_y[k] = top ? yp : ym;
+        h_fy[k] = top ? fyp : fym;
+      } else {
+        const int h = (hc - 2 * TX) % (2 * TY), right = h / TY;
+        row = h % TY;
+        lx = right ? TX : -1;
+        region = 0;
+        h_fl[k] = FL_XM + right * TY + row;
+        h_slot[k] = (row + 1) * SX + (right ? TX + 1 : 0);
+        h_y[k] = y0 + row;
+      }
+      int xr = x0 + lx;
+      h_x[k] = xr < 0 ? xr + dm.nx : (xr >= dm.nx ? xr - dm.nx : xr);
+#pragma unroll
+      for (int g = 0; g < 3; ++g) {  // cx = g - 1
+        const int sx = x0 + lx - (g - 1);  // real (unwrapped) x of the source column
+        if (sx >= 0 && sx < dm.nx) {
+          const int col = 4 + lx - (g - 1);
+          const int pstride = region == 0 ? TY * W : W;
+          const int base = region == 0 ? row * W : (region == 1 ? O_RM : O_RP);
+          h_off[k][g] = base + col + g * pstride;
+          h_str[k][g] = 3 * pstride;
+        } else {
+          const int col = (sx < 0 ? sx + dm.nx : sx - dm.nx) - px;  // 0..3
+          const int pstride = region == 0 ? TY * 4 : 4;
+          const int base = region == 0 ? O_PM + row * 4 : (region == 1 ? O_PRM : O_PRP);
+          h_off[k][g] = base + col + g * pstride;
+          h_str[k][g] = 3 * pstride;
+        }
+      }
+    }
+    for (int p = pfirst; p <= z1; ++p) {
+      const int it = p - pfirst, s = it % NS, k2 = it / NS;
+      bool fz, okz;
+      const int zr = virt_ws(p, dm.nz, dm.mode[2], fz, okz);
+      const int64_t zoff = nxy * zr;
+      const float* st = reinterpret_cast<const float*>(smem + (size_t)s * STAGE_BYTES);
+      const uint8_t* flb = smem + (size_t)s * STAGE_BYTES + FLAG_OFF;
+      float(*slot)[PLANE] = ring[it & 3];
+      if (it >= 4) pub_wait(pub0, it - 2);  // every worker is past the collision that read this ring slot
+      mbar_wait(full0 + 8 * s, k2 & 1);
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        if (!h_on[k]) continue;
+        float f[Q];
+#pragma unroll
+        for (int i = 0; i < Q; ++i) f[i] = st[h_off[k][i % 3] + (i / 3) * h_str[k][i % 3]];
+        const int64_t c = h_x[k] + nx * h_y[k] + zoff;
+        float d, uB[3], rho, uh[3], drho, jx, jy, jz;
+        solid_state_ws(a, flb[h_fl[k]], c, h_x[k], h_y[k], zr, d, uB);
+        moments_rho_j(f, drho, jx, jy, jz);
+        homogenised_velocity(a.ph, drho, jx, jy, jz, d, uB, rho, uh);
+        slot[0][h_slot[k]] = uh[0];
+        slot[1][h_slot[k]] = h_fy[k] ? -uh[1] : uh[1];
+        slot[2][h_slot[k]] = fz ? -uh[2] : uh[2];
+      }
+      __syncwarp();
+      if ((tid & 31) == 0) {
+        mbar_arrive(empty0 + 8 * s);
+        mbar_arrive(pub0 + 8 * (it & 1));
+      }
+    }
+    return;
+  }
+
+  // -------------------------------------------------------------------- workers, two x-adjacent cells each
+  constexpr int HX = TX / 2;
+  const int tx2 = tid % HX, ty = tid / HX;
+  const int xa = x0 + 2 * tx2, yv = y0 + ty;  // cells (xa, yv) and (xa + 1, yv)
+  const bool row_interior = yv > 0 && yv < dm.ny - 1;
+  const int own_slot = (ty + 1) * SX + 2 * tx2 + 1;
+  const int own_off = ty * W + 4 + 2 * tx2;   // + i * TY * W: population i of cell xa, unshifted column
+  const int own_fl = ty * TX + 2 * tx2;
+  const int64_t own_xy = xa + nx * yv;
+  // the one lane of a boundary tile whose x neighbour column is a wrapped one
+  const bool patch_l = edge_l && tx2 == 0, patch_r = edge_r && tx2 == HX - 1;
+  const int patch_off = O_PM + ty * 4 + (patch_l ? 3 : 0);
+
+  Moments mcur[2] = {}, mnext[2] = {};
+  float rho_c[2] = {1.f, 1.f}, rho_n[2] = {1.f, 1.f}, uh_c[2][3] = {}, uh_n[2][3] = {};
+  uint8_t fl_c[2] = {0, 0}, fl_n[2] = {0, 0};
+  char* dst = reinterpret_cast<char*>(a.fout) + 4 * (own_xy + nxy * z0);
+  const int64_t zstride_b = 4 * nxy;
+
+  for (int p = pfirst; p <= z1; ++p) {
+    const int it = p - pfirst, s = it % NS, k2 = it / NS;
+    {
+      bool fz, okz;
+      const int zr = virt_ws(p, dm.nz, dm.mode[2], fz, okz);
+      const int64_t c = own_xy + nxy * zr;
+      const float* st = reinterpret_cast<const float*>(smem + (size_t)s * STAGE_BYTES);
+      float(*slot)[PLANE] = ring[it & 3];
+      mbar_wait(full0 + 8 * s, k2 & 1);
+      const uint16_t flw = *reinterpret_cast<const uint16_t*>(smem + (size_t)s * STAGE_BYTES + FLAG_OFF + FL_MAIN + own_fl);
+      float f[2][Q];
+#pragma unroll
+      for (int i = 0; i < Q; ++i) {  // population i of cell x sits at column x - cx (x-pull)
+        const float* q = st + i * (TY * W) + own_off - dir_cx(i);
+        if (dir_cx(i) == 0) {
+          const float2 v = *reinterpret_cast<const float2*>(q);
+          f[0][i] = v.x;
+          f[1][i] = v.y;
+        } else {
+          f[0][i] = q[0];
+          f[1][i] = q[1];
+        }
+      }
+      if (edge) {
+        if (patch_l) {
+#pragma unroll
+          for (int k = 0; k < 9; ++k) f[0][3 * k + 2] = st[patch_off + (3 * k + 2) * (TY * 4)];  // cx = +1 from x = nx-1
+        }
+        if (patch_r) {
+#pragma unroll
+          for (int k = 0; k < 9; ++k) f[1][3 * k] = st[patch_off + (3 * k) * (TY * 4)];          // cx = -1 from x = 0
+        }
+      }
+      __syncwarp();
+      if ((tid & 31) == 0) mbar_arrive(empty0 + 8 * s);  // this warp has read its part of the stage
+      const bool keep = p >= z0 && p < z1;
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        const uint8_t fl = (uint8_t)(k ? (flw >> 8) : (flw & 0xff));
+        float d, uB[3], rho, uh[3];
+        solid_state_ws(a, fl, c + k, xa + k, yv, zr, d, uB);
+        if (keep) {
+          mnext[k] = moments_all(f[k]);
+          homogenised_velocity(a.ph, mnext[k].drho, mnext[k].jx, mnext[k].jy, mnext[k].jz, d, uB, rho, uh);
+          rho_n[k] = rho;
+          uh_n[k][0] = uh[0]; uh_n[k][1] = uh[1]; uh_n[k][2] = uh[2];
+          fl_n[k] = fl;
+        } else {
+          float drho, jx, jy, jz;
+          moments_rho_j(f[k], drho, jx, jy, jz);
+          homogenised_velocity(a.ph, drho, jx, jy, jz, d, uB, rho, uh);
+        }
+        slot[0][own_slot + k] = uh[0];
+        slot[1][own_slot + k] = uh[1];
+        slot[2][own_slot + k] = fz ? -uh[2] : uh[2];
+      }
+    }
+    pub_arrive(pub0, it);
+    const int z = p - 1;
+    if (z >= z0) {
+      pub_wait(pub0, it - 1);  // the xy neighbours' uhat of plane z (own cell of plane z+1: written above)
+      float(*sm)[PLANE] = ring[(it - 2) & 3];
+      float(*s0)[PLANE] = ring[(it - 1) & 3];
+      float(*sp)[PLANE] = ring[it & 3];
+      float out[2][Q];
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        const int o = own_slot + k;
+        float S[6], sigma = a.ph.sigma;
+        float dxu0 = s0[0][o + 1] - s0[0][o - 1], dxu1 = s0[1][o + 1] - s0[1][o - 1], dxu2 = s0[2][o + 1] - s0[2][o - 1];
+        float dyu0 = s0[0][o + SX] - s0[0][o - SX], dyu1 = s0[1][o + SX] - s0[1][o - SX],
+              dyu2 = s0[2][o + SX] - s0[2][o - SX];
+        float dzu0 = sp[0][o] - sm[0][o], dzu1 = sp[1][o] - sm[1][o], dzu2 = sp[2][o] - sm[2][o];
+        S[0] = 0.5f * dxu0;
+        S[1] = 0.5f * dyu1;
+        S[2] = 0.5f * dzu2;
+        S[3] = 0.25f * (dyu0 + dxu1);
+        S[4] = 0.25f * (dzu0 + dxu2);
+        S[5] = 0.25f * (dzu1 + dyu2);
+        if (fl_c[k] & WM_VALID) {  // wall-model strain, sigma = 0 (rare)
+          const int64_t c = own_xy + k + nxy * z;
+#pragma unroll
+          for (int q = 0; q < 6; ++q) S[q] = __ldg(a.wm_s + (int64_t)q * n + c);
+          sigma = 0.f;
+        }
+        collide(a.ph, mcur[k], rho_c[k], uh_c[k], S, sigma, out[k]);
+      }
+      if (row_interior && z > 0 && z < dm.nz - 1) {  // no wrap, no reflection: constant offsets, aligned pairs
+#pragma unroll
+        for (int i = 0; i < Q; ++i)
+          *reinterpret_cast<float2*>(dst + a.push_b[i]) = make_float2(out[0][i], out[1][i]);
+      } else {
+        push_store_yz(dm, a.fout, xa, yv, z, out[0]);
+        push_store_yz(dm, a.fout, xa + 1, yv, z, out[1]);
+      }
+      dst += zstride_b;
+    }
+    if (p >= z0) {
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        mcur[k] = mnext[k]; rho_c[k] = rho_n[k]; fl_c[k] = fl_n[k];
+        uh_c[k][0] = uh_n[k][0]; uh_c[k][1] = uh_n[k][1]; uh_c[k][2] = uh_n[k][2];
+      }
+    }
+  }
+}
+
+// ---- host side: tensor maps (driver entry point through the runtime; libcuda is not linked) ----
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+// populations as a 4-D tensor (x, y, z, population) of fp32; box = bx x by x 1 x 27
+static bool make_map(CUtensorMap* m, const float* base, const Dom& dm, uint32_t bx, uint32_t by) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return false;
+  cuuint64_t gdim[4] = {(cuuint64_t)dm.nx, (cuuint64_t)dm.ny, (cuuint64_t)dm.nz, (cuuint64_t)Q};
+  cuuint64_t gstr[3] = {(cuuint64_t)dm.nx * 4, (cuuint64_t)dm.nx * dm.ny * 4, (cuuint64_t)dm.n * 4};
+  cuuint32_t box[4] = {bx, by, 1, (cuuint32_t)Q};
+  cuuint32_t estr[4] = {1, 1, 1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<float*>(base), gdim, gstr, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+bool xpull_supported(const Dom& dm) {
+  return dm.nx % xp::TX == 0 && dm.nx >= 2 * xp::TX && dm.ny % xp::TY == 0 && dm.mode[0] == HHRR_PERIODIC &&
+         encode_fn() != nullptr;
+}
+
+cudaError_t launch_fused_xpull(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo) {
+  const Dom& dm = L->dom;
+  if (!dm.xs || !xpull_supported(dm)) return cudaErrorNotSupported;
+  CUtensorMap m_main, m_row, m_pm, m_pr;
+  if (!make_map(&m_main, L->fA, dm, xp::W, xp::TY) || !make_map(&m_row, L->fA, dm, xp::W, 1) ||
+      !make_map(&m_pm, L->fA, dm, 4, xp::TY) || !make_map(&m_pr, L->fA, dm, 4, 1))
+    return cudaErrorNotSupported;
+  WsArgs a;
+  fill_ws_args(L, ph, bo, a);
+  for (int i = 0; i < Q; ++i)  // y and z moves only: the x move is taken on the read side
+    a.push_b[i] = 4LL * ((long long)i * dm.n + (long long)dir_cy(i) * dm.nx + (long long)dir_cz(i) * dm.nx * dm.ny);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(fused_xpull_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xp::SMEM);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  int nch = ws_zchunks(dm.nz);
+  a.zchunk = (dm.nz + nch - 1) / nch;
+  nch = (dm.nz + a.zchunk - 1) / a.zchunk;
+  dim3 grid(dm.nx / xp::TX, dm.ny / xp::TY, nch);
+  fused_xpull_kernel<<<grid, xp::THREADS, xp::SMEM, L->stream>>>(a, m_main, m_row, m_pm, m_pr);
+  L->launches++;
+  return cudaGetLastError();
+}
+
+}  // namespace hhrr

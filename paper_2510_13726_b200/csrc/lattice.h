@@ -23,6 +23,10 @@ struct Dom {
   int nx, ny, nz;
   int mode[3];
   int64_t n;
+  // storage of the populations: xs = 0 "push" (post-stream: plane i holds f_i(x,y,z));
+  // xs = 1 "x-pull / yz-push": plane i holds g_i(x,y,z) = f_i(x + c_ix, y, z), i.e. the post-collision
+  // value already moved along y and z but not yet along x (periodic x axis only).  pop_index() hides it.
+  int xs;
 };
 
 // rigid bodies, fp32 copy for the collide kernel, fp64 for wall model / force
@@ -99,7 +103,7 @@ struct hhrr_lattice {
   bool geometry_dirty;     // full-domain geometry pass needed
   bool geometry_current;   // geometry(step) evaluated
   int64_t step;
-  int variant;
+  int variant;       // requested kernel variant; dom.xs says how the populations are stored for it
   int64_t launches;
   // optional CUDA-event timing of the collide-stream kernel (hhrr_set_timing)
   bool timing;
@@ -117,6 +121,8 @@ cudaError_t launch_init(hhrr_lattice* L, const float* d_rho, const float* d_u, i
 cudaError_t launch_collide_stream(hhrr_lattice* L);
 cudaError_t launch_moments(hhrr_lattice* L, float* d_rho, float* d_v);
 cudaError_t launch_check_finite(hhrr_lattice* L);
+bool xpull_supported(const Dom& dm);                    // fused_xpull.cu: variant 5 can run this lattice
+cudaError_t launch_restore(hhrr_lattice* L, int xs);    // re-store the populations of buffer A with x-shift xs
 // wallmodel.cu
 cudaError_t launch_wall_model(hhrr_lattice* L);
 cudaError_t launch_forces(hhrr_lattice* L);

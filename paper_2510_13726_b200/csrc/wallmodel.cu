@@ -35,12 +35,12 @@ __device__ __forceinline__ int wrap_far(int v, int n, int mode, bool& flip) {
 }
 
 // reported velocity moment v = (j + g/2)/rho of a cell (R11)
-__device__ __forceinline__ void cell_velocity_d(const float* __restrict__ f, int64_t n, int64_t c,
+__device__ __forceinline__ void cell_velocity_d(const float* __restrict__ f, const Dom& dm, int x, int y, int z,
                                                 const double g[3], double v[3]) {
   double drho = 0, j0 = 0, j1 = 0, j2 = 0;
 #pragma unroll
   for (int i = 0; i < Q; ++i) {
-    double fi = (double)__ldg(f + (int64_t)i * n + c);
+    double fi = (double)__ldg(f + pop_index(dm, i, x, y, z));
     drho += fi;
     j0 += dir_cx(i) * fi;
     j1 += dir_cy(i) * fi;
@@ -92,7 +92,7 @@ __global__ void __launch_bounds__(128) wall_model_kernel(WmArgs a) {
       int yy = wrap_far(iy + oy, a.dm.ny, a.dm.mode[1], fly);
       int zz = wrap_far(iz + oz, a.dm.nz, a.dm.mode[2], flz);
       double v[3];
-      cell_velocity_d(a.f, n, xx + nx * yy + nxy * zz, a.g, v);
+      cell_velocity_d(a.f, a.dm, xx, yy, zz, a.g, v);
       if (flx) v[0] = -v[0];
       if (fly) v[1] = -v[1];
       if (flz) v[2] = -v[2];
@@ -101,7 +101,7 @@ __global__ void __launch_bounds__(128) wall_model_kernel(WmArgs a) {
       vs[2] += w * v[2];
     }
     double vw[3], us[3];
-    cell_velocity_d(a.f, n, c, a.g, vw);
+    cell_velocity_d(a.f, a.dm, x, y, z, a.g, vw);
     uint8_t fl = a.flags[c];
     body_velocity_d(a.bo, (fl >> TAG_SHIFT) & TAG_MASK, x, y, z, us);
     double r[3], rn = 0.0;
@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(128) force_kernel(ForceArgs a) {
   for (int t = threadIdx.x; t < MAX_TAGS * 3; t += blockDim.x) bins[t] = 0.0;
   __syncthreads();
   const int count = min(a.cnt->force_count, a.cap_list);
-  const int64_t n = a.dm.n, nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
+  const int64_t nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
   for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < count; e += gridDim.x * blockDim.x) {
     int64_t c = a.force_idx[e];
     int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
@@ -191,8 +191,8 @@ __global__ void __launch_bounds__(128) force_kernel(ForceArgs a) {
       int zz = wrap_far(z + dir_cz(i), a.dm.nz, a.dm.mode[2], fl);
       // stored values are deviations: f = w + dev, and w_i = w_ibar
       double w = dir_wd(i);
-      double fa = w + (double)__ldg(a.f + (int64_t)i * n + (xx + nx * yy + nxy * zz));
-      double fb = w + (double)__ldg(a.f + (int64_t)(26 - i) * n + c);
+      double fa = w + (double)__ldg(a.f + pop_index(a.dm, i, xx, yy, zz));
+      double fb = w + (double)__ldg(a.f + pop_index(a.dm, 26 - i, x, y, z));
       double ci[3] = {(double)dir_cx(i), (double)dir_cy(i), (double)dir_cz(i)};
       for (int q = 0; q < 3; ++q) acc[q] += (ci[q] - us[q]) * fa + (ci[q] + us[q]) * fb;
     }

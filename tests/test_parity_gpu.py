@@ -83,7 +83,7 @@ def run_parity(oracle, case, steps, variant, tol, check_every=None, force_tol=No
     return e_rho, e_v
 
 
-VARIANTS = [0, 1, 2, 3, 4]
+VARIANTS = [0, 1, 2, 3, 4, 5]
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
@@ -149,6 +149,61 @@ def test_config4_rotor_reduced(oracle, variant):
     run_parity(oracle, case, 12, variant, TOL10, check_every=1)
 
 
+# ---- variant 5 (default) on lattices its own kernel tiles: x-pull / yz-push storage, nx >= 128 -------
+def _xpull_lattice(case):
+    G = _gpu_lattice(case, 5)
+    assert G.population_storage() == 1, "variant 5 fell back to post-stream storage"
+    return G
+
+
+def test_xpull_periodic_noise(oracle):
+    """Three x tiles, two y tiles, several planes: the periodic x boundary columns, tile seams."""
+    rho, u = I.noisy_uniform(192, 16, 11, (0.03, -0.02, 0.01), 5e-3, 78)
+    case = I.Case("xpull", 192, 16, 11, 10, params=dict(I.DEFAULTS, tau0=0.53), rho=rho, u=u, with_neq=True)
+    _xpull_lattice(case).close()
+    run_parity(oracle, case, 10, 5, TOL10)
+
+
+def test_xpull_mirror_yz(oracle):
+    """Mirror planes in y and z under x-pull storage (x stays periodic: the storage needs it)."""
+    rho, u = I.noisy_uniform(128, 16, 9, (0.01, 0.0, 0.0), 1e-2, 10)
+    case = I.Case("xpull-mirror", 128, 16, 9, 10, mode=(I.PERIODIC, I.MIRROR, I.MIRROR),
+                  params=dict(I.DEFAULTS, tau0=0.56), rho=rho, u=u, with_neq=True)
+    _xpull_lattice(case).close()
+    run_parity(oracle, case, 10, 5, TOL10)
+
+
+def test_xpull_channel_and_rotor(oracle):
+    """Config 3 and config 4 recipes at extents variant 5 tiles itself: wall model and forces read the
+    x-pulled populations; geometry and wall list stay bit-exact."""
+    case = I.case_channel(128, 48, 16, 30)
+    _xpull_lattice(case).close()
+    run_parity(oracle, case, 10, 5, TOL10, check_every=1)
+    run_parity(oracle, case, 30, 5, TOL_LONG, check_every=15, force_tol=TOL_LONG)
+    case = I.case_rotor(128, 72, 72, 20.0, 12, omega=0.012)
+    _xpull_lattice(case).close()
+    run_parity(oracle, case, 12, 5, TOL10, check_every=1)
+
+
+def test_xpull_storage_round_trip():
+    """Populations go in and out in the plain post-stream layout whatever the storage; switching the
+    variant re-stores them without changing the state."""
+    case = I.case_sphere(128, 32, 32, 5.0, 4)
+    A, Bv = _xpull_lattice(case), _gpu_lattice(case, 4)
+    assert Bv.population_storage() == 0
+    A.step(4); Bv.step(4)
+    fa, fb = A.populations(), Bv.populations()
+    assert np.max(np.abs(fa - fb)) <= 1e-6 * np.max(np.abs(fb))
+    A.set_kernel_variant(2)                      # re-store post-stream ...
+    assert A.population_storage() == 0 and np.array_equal(A.populations(), fa)
+    A.set_kernel_variant(5)                      # ... and back
+    assert A.population_storage() == 1 and np.array_equal(A.populations(), fa)
+    Bv.set_populations(fa)
+    A.step(3); Bv.step(3)
+    assert np.max(np.abs(A.populations() - Bv.populations())) <= 1e-6 * np.max(np.abs(fb))
+    A.close(); Bv.close()
+
+
 def test_moving_static_body_and_checkpoint(oracle):
     """set_body on a static solid (translating sphere) and populations round trip."""
     case = I.case_sphere(48, 24, 24, 4.0, 6)
@@ -184,7 +239,8 @@ def test_config5_full_size_sampled_cells(oracle):
     with what the GPU stored at the 27 push targets.  Samples cover bulk fluid, tile / z-chunk
     seams, the inflow fringe, growth, frontier (with and without wall-model state) and solid cells."""
     case = I.baseline_config(5)
-    G = _gpu_lattice(case, 4)               # the default variant: what bench.py times
+    G = _gpu_lattice(case, 5)               # the default variant: what bench.py times
+    assert G.population_storage() == 1
     G.step(2)
     G.update_geometry()                     # the geometry the next collide uses
     nx, ny, nz = case.nx, case.ny, case.nz
@@ -270,21 +326,21 @@ def test_config5_full_size_sampled_cells(oracle):
 
 def test_config1_tgv32_1000_steps(oracle):
     """north_star: rel-Linf <= 1e-3 on density and velocity after 1000 steps (config 1)."""
-    e = run_parity(oracle, I.case_tgv(32, 1000), 1000, 4, TOL_LONG)
+    e = run_parity(oracle, I.case_tgv(32, 1000), 1000, 5, TOL_LONG)
     print("config1 1000 steps rel-Linf", e)
     assert e[1] <= 5e-4  # measured 1.0e-4 (fp32 arithmetic over 1000 steps); the bar is 1e-3
 
 
 def test_config3_channel_500_steps(oracle):
     """Config 3 recipe, reduced extents, its full 500 steps (wall model warm starts, Newton every step)."""
-    run_parity(oracle, I.case_channel(64, 48, 32, 500), 500, 4, TOL_LONG, check_every=250, force_tol=TOL_LONG)
+    run_parity(oracle, I.case_channel(128, 48, 16, 500), 500, 5, TOL_LONG, check_every=250, force_tol=TOL_LONG)
 
 
 def test_config4_rotor_100_steps(oracle):
     """Config 4 recipe, reduced extents, 100 steps = 1.2 rad of rotation: cells change type hundreds of
     times; geometry compared bit-exact every 20 steps."""
-    case = I.case_rotor(96, 72, 72, 20.0, 100, omega=0.012)
-    run_parity(oracle, case, 100, 4, TOL_LONG, check_every=20, force_tol=TOL_LONG)
+    case = I.case_rotor(128, 72, 72, 20.0, 100, omega=0.012)
+    run_parity(oracle, case, 100, 5, TOL_LONG, check_every=20, force_tol=TOL_LONG)
 
 
 def test_force_history_ring_and_errors(oracle):

@@ -257,7 +257,7 @@ void fill_ws_args(const hhrr_lattice* L, const PhysF& ph, const BodiesF& bo, WsA
 // neighbour tile loads them; long chunks let neighbouring blocks drift apart (measured: 6.3 ms at 2
 // chunks vs 5.6 ms at 16 on 768x384x364).  Cost: two extra planes loaded per chunk.
 int ws_zchunks(int nz) {
-  int nch = (nz + 11) / 24;
+  int nch = (nz + 9) / 19;  // ~19 planes per chunk: measured optimum on config 5 (profiles/)
   if (nch < 1) nch = 1;
   if (const char* e = getenv("HHRR_ZCHUNKS")) nch = atoi(e) < 1 ? 1 : atoi(e);  // tuning runs only
   return nch;

@@ -245,7 +245,9 @@ __global__ void __launch_bounds__(xp::THREADS, 1)
       const float* st = reinterpret_cast<const float*>(smem + (size_t)s * STAGE_BYTES);
       const uint8_t* flb = smem + (size_t)s * STAGE_BYTES + FLAG_OFF;
       float(*slot)[PLANE] = ring[it & 3];
-      if (it >= 4) pub_wait(pub0, it - 2);  // every worker is past the collision that read this ring slot
+      // every worker is past the collision that read this ring slot; waiting from it = 2 on (not only
+      // once the slot is reused) also keeps any arrival for plane it behind the completed phase it - 2
+      if (it >= 2) pub_wait(pub0, it - 2);
       mbar_wait(full0 + 8 * s, k2 & 1);
 #pragma unroll
       for (int k = 0; k < 2; ++k) {
@@ -348,9 +350,12 @@ __global__ void __launch_bounds__(xp::THREADS, 1)
       }
     }
     pub_arrive(pub0, it);
+    // the xy neighbours' uhat of plane p-1 (own cell of plane p: written above).  Waited for in EVERY
+    // iteration, also the two that collide nothing: a warp must not arrive for plane it + 1 on the
+    // barrier plane it - 1 still uses
+    if (it >= 1) pub_wait(pub0, it - 1);
     const int z = p - 1;
     if (z >= z0) {
-      pub_wait(pub0, it - 1);  // the xy neighbours' uhat of plane z (own cell of plane z+1: written above)
       float(*sm)[PLANE] = ring[(it - 2) & 3];
       float(*s0)[PLANE] = ring[(it - 1) & 3];
       float(*sp)[PLANE] = ring[it & 3];

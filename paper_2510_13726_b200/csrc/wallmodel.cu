@@ -69,10 +69,20 @@ __device__ __forceinline__ double spalding_df(double ut, double U, double y, dou
   return -(U / (ut * ut)) * (1.0 + (kap / E) * (exp(k) - 1.0 - k - 0.5 * k * k)) - y / nu;
 }
 
+// fp64 value of another lane
+__device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+__device__ __forceinline__ double shfl_down_d(double v, int delta) { return __shfl_down_sync(0xffffffffu, v, delta); }
+
+// One warp per wall-model cell.  Lane 3k + g (k = 0..8, g = 0..2) loads nine populations of cell k --
+// k = 0..7 the corners of the trilinear stencil around x_w + h_s n (R15), k = 8 the wall
+// cell itself -- so the 243 gathered loads of a cell are in flight at once; the three partial sums of a
+// cell meet by shuffles, lane 0 does the Newton iteration (Eq. 19) and writes the cell's state.
 __global__ void __launch_bounds__(128) wall_model_kernel(WmArgs a) {
   const int count = min(a.cnt->wall_count, a.cap_list);
   const int64_t n = a.dm.n, nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
-  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < count; e += gridDim.x * blockDim.x) {
+  const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+  const int kc = lane / 3, g = lane - 3 * kc;  // cell of the stencil, population group (lanes 27-31 idle)
+  for (int e = blockIdx.x * wpb + (threadIdx.x >> 5); e < count; e += gridDim.x * wpb) {
     int64_t c = a.wall_idx[e];
     int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
     double y1v[3] = {a.wall_y1n[3 * (int64_t)e], a.wall_y1n[3 * (int64_t)e + 1], a.wall_y1n[3 * (int64_t)e + 2]};
@@ -83,25 +93,52 @@ __global__ void __launch_bounds__(128) wall_model_kernel(WmArgs a) {
     double fx = floor(px), fy = floor(py), fz = floor(pz);
     double tx = px - fx, ty = py - fy, tz = pz - fz;
     int ix = (int)fx, iy = (int)fy, iz = (int)fz;
-    double vs[3] = {0, 0, 0};
-    for (int k = 0; k < 8; ++k) {
-      int ox = k & 1, oy = (k >> 1) & 1, oz = (k >> 2) & 1;
-      double w = (ox ? tx : 1.0 - tx) * (oy ? ty : 1.0 - ty) * (oz ? tz : 1.0 - tz);
-      bool flx, fly, flz;
-      int xx = wrap_far(ix + ox, a.dm.nx, a.dm.mode[0], flx);
-      int yy = wrap_far(iy + oy, a.dm.ny, a.dm.mode[1], fly);
-      int zz = wrap_far(iz + oz, a.dm.nz, a.dm.mode[2], flz);
-      double v[3];
-      cell_velocity_d(a.f, a.dm, xx, yy, zz, a.g, v);
-      if (flx) v[0] = -v[0];
-      if (fly) v[1] = -v[1];
-      if (flz) v[2] = -v[2];
-      vs[0] += w * v[0];
-      vs[1] += w * v[1];
-      vs[2] += w * v[2];
+    // this lane's cell
+    int xx = x, yy = y, zz = z;
+    bool flx = false, fly = false, flz = false;
+    double w = 0.0;
+    if (kc < 8) {
+      int ox = kc & 1, oy = (kc >> 1) & 1, oz = (kc >> 2) & 1;
+      w = (ox ? tx : 1.0 - tx) * (oy ? ty : 1.0 - ty) * (oz ? tz : 1.0 - tz);
+      xx = wrap_far(ix + ox, a.dm.nx, a.dm.mode[0], flx);
+      yy = wrap_far(iy + oy, a.dm.ny, a.dm.mode[1], fly);
+      zz = wrap_far(iz + oz, a.dm.nz, a.dm.mode[2], flz);
     }
-    double vw[3], us[3];
-    cell_velocity_d(a.f, a.dm, x, y, z, a.g, vw);
+    double drho = 0, j0 = 0, j1 = 0, j2 = 0;
+    if (kc < 9) {
+      float fv[9];
+#pragma unroll
+      for (int q = 0; q < 9; ++q) fv[q] = __ldg(a.f + pop_index(a.dm, 9 * g + q, xx, yy, zz));
+#pragma unroll
+      for (int q = 0; q < 9; ++q) {  // population 9g + q: cx = q % 3 - 1, cy = q / 3 - 1, cz = g - 1
+        double fi = (double)fv[q];
+        drho += fi;
+        j0 += (q % 3 - 1) * fi;
+        j1 += (q / 3 - 1) * fi;
+      }
+      j2 = (g - 1) * drho;
+    }
+    // the three groups of a cell: lanes 3k, 3k+1, 3k+2
+    drho += shfl_down_d(drho, 1) + shfl_down_d(drho, 2);
+    j0 += shfl_down_d(j0, 1) + shfl_down_d(j0, 2);
+    j1 += shfl_down_d(j1, 1) + shfl_down_d(j1, 2);
+    j2 += shfl_down_d(j2, 1) + shfl_down_d(j2, 2);
+    double ir = 1.0 / (1.0 + drho);  // reported velocity moment v = (j + g/2)/rho (R11), valid on lanes 3k
+    double v[3] = {(j0 + 0.5 * a.g[0]) * ir, (j1 + 0.5 * a.g[1]) * ir, (j2 + 0.5 * a.g[2]) * ir};
+    if (flx) v[0] = -v[0];
+    if (fly) v[1] = -v[1];
+    if (flz) v[2] = -v[2];
+    double vs[3] = {0, 0, 0}, vw[3];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      double wk = shfl_d(w, 3 * k);
+#pragma unroll
+      for (int q = 0; q < 3; ++q) vs[q] += wk * shfl_d(v[q], 3 * k);
+    }
+#pragma unroll
+    for (int q = 0; q < 3; ++q) vw[q] = shfl_d(v[q], 24);
+    if (lane != 0) continue;
+    double us[3];
     uint8_t fl = a.flags[c];
     body_velocity_d(a.bo, (fl >> TAG_SHIFT) & TAG_MASK, x, y, z, us);
     double r[3], rn = 0.0;
@@ -168,35 +205,43 @@ __global__ void zero_force_kernel(double* out) {
 }
 
 // F_k = - sum_{x: d<1, tag=k} sum_{i != rest} [(c_i - u^s) f_i(x + c_i) + (c_i + u^s) f_ibar(x)]
-// (Eq. 23 with reading R7), fp64 accumulation: thread -> shared per-tag bins -> global atomics.
+// (Eq. 23 with reading R7), fp64 accumulation.  One warp per cell: lane i < 27 takes link i (both
+// loads of a cell's 26 links are in flight at once), warp shuffle sum -> shared per-tag bins -> one
+// global atomic per block, tag and component.
 __global__ void __launch_bounds__(128) force_kernel(ForceArgs a) {
   __shared__ double bins[MAX_TAGS * 3];
   for (int t = threadIdx.x; t < MAX_TAGS * 3; t += blockDim.x) bins[t] = 0.0;
   __syncthreads();
   const int count = min(a.cnt->force_count, a.cap_list);
   const int64_t nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
-  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < count; e += gridDim.x * blockDim.x) {
+  const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+  const int i = lane;
+  const int cx = i % 3 - 1, cy = (i / 3) % 3 - 1, cz = i / 9 - 1;
+  const bool link = i < Q && i != 13;
+  for (int e = blockIdx.x * wpb + (threadIdx.x >> 5); e < count; e += gridDim.x * wpb) {
     int64_t c = a.force_idx[e];
     int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
     int k = (a.flags[c] >> TAG_SHIFT) & TAG_MASK;
     double us[3];
     body_velocity_d(a.bo, k, x, y, z, us);
     double acc[3] = {0, 0, 0};
-#pragma unroll
-    for (int i = 0; i < Q; ++i) {
-      if (i == 13) continue;
+    if (link) {
       bool fl;
-      int xx = wrap_far(x + dir_cx(i), a.dm.nx, a.dm.mode[0], fl);
-      int yy = wrap_far(y + dir_cy(i), a.dm.ny, a.dm.mode[1], fl);
-      int zz = wrap_far(z + dir_cz(i), a.dm.nz, a.dm.mode[2], fl);
+      int xx = wrap_far(x + cx, a.dm.nx, a.dm.mode[0], fl);
+      int yy = wrap_far(y + cy, a.dm.ny, a.dm.mode[1], fl);
+      int zz = wrap_far(z + cz, a.dm.nz, a.dm.mode[2], fl);
       // stored values are deviations: f = w + dev, and w_i = w_ibar
-      double w = dir_wd(i);
+      double w = (cx ? 1.0 / 6.0 : 2.0 / 3.0) * (cy ? 1.0 / 6.0 : 2.0 / 3.0) * (cz ? 1.0 / 6.0 : 2.0 / 3.0);
       double fa = w + (double)__ldg(a.f + pop_index(a.dm, i, xx, yy, zz));
       double fb = w + (double)__ldg(a.f + pop_index(a.dm, 26 - i, x, y, z));
-      double ci[3] = {(double)dir_cx(i), (double)dir_cy(i), (double)dir_cz(i)};
-      for (int q = 0; q < 3; ++q) acc[q] += (ci[q] - us[q]) * fa + (ci[q] + us[q]) * fb;
+      double ci[3] = {(double)cx, (double)cy, (double)cz};
+      for (int q = 0; q < 3; ++q) acc[q] = (ci[q] - us[q]) * fa + (ci[q] + us[q]) * fb;
     }
-    for (int q = 0; q < 3; ++q) atomicAdd(&bins[k * 3 + q], -acc[q]);
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1)
+      for (int q = 0; q < 3; ++q) acc[q] += __shfl_down_sync(0xffffffffu, acc[q], off);
+    if (lane == 0)
+      for (int q = 0; q < 3; ++q) atomicAdd(&bins[k * 3 + q], -acc[q]);
   }
   __syncthreads();
   for (int t = threadIdx.x; t < MAX_TAGS * 3; t += blockDim.x)
@@ -227,7 +272,7 @@ cudaError_t launch_wall_model(hhrr_lattice* L) {
   a.wm_utau = L->wm_utau;
   a.wm_u = L->wm_u;
   a.wm_s = L->wm_s;
-  wall_model_kernel<<<592, 128, 0, L->stream>>>(a);
+  wall_model_kernel<<<2368, 128, 0, L->stream>>>(a);
   L->launches++;
   return cudaGetLastError();
 }
@@ -243,7 +288,7 @@ cudaError_t launch_forces(hhrr_lattice* L) {
   a.cap_list = (int)L->cap_list;
   a.out = L->force + (L->step % FORCE_HISTORY) * MAX_TAGS * 3;
   zero_force_kernel<<<1, 64, 0, L->stream>>>(a.out);
-  force_kernel<<<296, 128, 0, L->stream>>>(a);
+  force_kernel<<<2368, 128, 0, L->stream>>>(a);
   L->launches += 2;
   return cudaGetLastError();
 }

@@ -204,6 +204,20 @@ def test_xpull_storage_round_trip():
     A.close(); Bv.close()
 
 
+@pytest.mark.parametrize("variant", [2, 4, 5])
+def test_fused_kernels_are_deterministic(variant):
+    """Two identical lattices stay bitwise identical: every step is a deterministic function of the
+    state (R19).  A race between the warps of a fused kernel (ring slots, pipeline stages,
+    barrier phases at the start of a z-chunk) shows up here long before it exceeds a parity tolerance."""
+    case = I.case_rotor(128, 72, 72, 20.0, 6, omega=0.012)
+    A, Bv = _gpu_lattice(case, variant), _gpu_lattice(case, variant)
+    for _ in range(3):
+        A.step(2); Bv.step(2)
+        assert np.array_equal(A.populations(), Bv.populations())
+        assert np.array_equal(A.wall_list()[2], Bv.wall_list()[2])
+    A.close(); Bv.close()
+
+
 def test_moving_static_body_and_checkpoint(oracle):
     """set_body on a static solid (translating sphere) and populations round trip."""
     case = I.case_sphere(48, 24, 24, 4.0, 6)

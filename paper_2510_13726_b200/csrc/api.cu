@@ -83,6 +83,7 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
   float* wm_s = c.take<float>(6 * n);
   int32_t* wall_idx = c.take<int32_t>(cap);
   double* wall_y1n = c.take<double>(3 * cap);
+  double* wall_samp = c.take<double>(6 * cap);
   int32_t* force_idx = c.take<int32_t>(cap);
   Counters* counters = c.take<Counters>(1);
   double* force = c.take<double>(FORCE_HISTORY * MAX_TAGS * 3);
@@ -91,7 +92,7 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
   if (L) {
     L->fA = fA; L->fB = fB; L->flags = flags; L->d = d; L->phi = phi; L->below = below; L->rowflag = rowflag; L->rowflag_static = rowflag_static; L->phi_static = phi_static;
     L->tag_static = tag_static; L->d_override = d_override; L->uhat = uhat; L->wm_utau = wm_utau;
-    L->wm_u = wm_u; L->wm_s = wm_s; L->wall_idx = wall_idx; L->wall_y1n = wall_y1n;
+    L->wm_u = wm_u; L->wm_s = wm_s; L->wall_idx = wall_idx; L->wall_y1n = wall_y1n; L->wall_samp = wall_samp;
     L->force_idx = force_idx; L->counters = counters; L->force = force; L->rot_sdf = rot_sdf;
     L->rot_tag = rot_tag; L->rot_nodes_cap = rotor_nodes; L->cap_list = cap;
   }
@@ -402,10 +403,8 @@ int hhrr_step(hhrr_lattice* L, int32_t n_steps) {
       CU(cudaEventRecord(L->ev[2 * L->ev_n + 1], L->stream));
       L->ev_n++;
     }
-    e = launch_wall_model(L);  // line 4: WallModelO
-    if (e != cudaSuccess) return cuda_fail(e, "wall-model kernel");
-    e = launch_forces(L);  // lines 5-6
-    if (e != cudaSuccess) return cuda_fail(e, "force kernels");
+    e = launch_wall_model_and_forces(L);  // line 4: WallModelO; lines 5-6: forces (one launch)
+    if (e != cudaSuccess) return cuda_fail(e, "wall-model / force kernel");
     L->step += 1;  // line 7: theta_{n+1} = theta_n + Omega
     L->geometry_current = !L->has_rotor;  // static geometry stays valid
   }

@@ -86,6 +86,7 @@ struct hhrr_lattice {
   float* wm_s;              // 6N
   int32_t* wall_idx;        // cap_list
   double* wall_y1n;         // 3*cap_list (AoS)
+  double* wall_samp;        // 6*cap_list: v_s and v(x_w) per wall cell, between the two phases of K3
   int32_t* force_idx;       // cap_list
   hhrr::Counters* counters; // 1
   double* force;            // FORCE_HISTORY * MAX_TAGS * 3
@@ -124,6 +125,5 @@ cudaError_t launch_check_finite(hhrr_lattice* L);
 bool xpull_supported(const Dom& dm);                    // fused_xpull.cu: variant 5 can run this lattice
 cudaError_t launch_restore(hhrr_lattice* L, int xs);    // re-store the populations of buffer A with x-shift xs
 // wallmodel.cu
-cudaError_t launch_wall_model(hhrr_lattice* L);
-cudaError_t launch_forces(hhrr_lattice* L);
+cudaError_t launch_wall_model_and_forces(hhrr_lattice* L);
 }  // namespace hhrr

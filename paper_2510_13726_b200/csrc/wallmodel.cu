@@ -21,6 +21,7 @@ struct WmArgs {
   const double* wall_y1n;
   const Counters* cnt;
   int cap_list;
+  double* samp;  // [cap_list][6]: sampled velocity v_s and the cell's own velocity v(x_w), phase A -> phase B
   double* wm_utau;
   float* wm_u;
   float* wm_s;
@@ -73,16 +74,18 @@ __device__ __forceinline__ double spalding_df(double ut, double U, double y, dou
 __device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 __device__ __forceinline__ double shfl_down_d(double v, int delta) { return __shfl_down_sync(0xffffffffu, v, delta); }
 
-// One warp per wall-model cell.  Lane 3k + g (k = 0..8, g = 0..2) loads nine populations of cell k --
-// k = 0..7 the corners of the trilinear stencil around x_w + h_s n (R15), k = 8 the wall
-// cell itself -- so the 243 gathered loads of a cell are in flight at once; the three partial sums of a
-// cell meet by shuffles, lane 0 does the Newton iteration (Eq. 19) and writes the cell's state.
-__global__ void __launch_bounds__(128) wall_model_kernel(WmArgs a) {
+// K3 runs in two phases.  Phase A, one WARP per wall-model cell: lane 3k + g (k = 0..8, g = 0..2) loads
+// nine populations of cell k -- k = 0..7 the corners of the trilinear stencil around x_w + h_s n
+// (R15), k = 8 the wall cell itself -- so the 243 gathered loads of a cell are in flight at
+// once; the partial sums meet by shuffles and lane 0 stores v_s and v(x_w).  Phase B, one THREAD per
+// cell: tangential speed, Newton iteration on Eq. 18 (Eq. 19; fp64 exp, all 32 lanes busy), slip velocity
+// and wall strain.
+__device__ __forceinline__ void wall_sample_block(const WmArgs& a, int block, int nblocks) {
   const int count = min(a.cnt->wall_count, a.cap_list);
-  const int64_t n = a.dm.n, nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
+  const int64_t nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
   const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
   const int kc = lane / 3, g = lane - 3 * kc;  // cell of the stencil, population group (lanes 27-31 idle)
-  for (int e = blockIdx.x * wpb + (threadIdx.x >> 5); e < count; e += gridDim.x * wpb) {
+  for (int e = block * wpb + (threadIdx.x >> 5); e < count; e += nblocks * wpb) {
     int64_t c = a.wall_idx[e];
     int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
     double y1v[3] = {a.wall_y1n[3 * (int64_t)e], a.wall_y1n[3 * (int64_t)e + 1], a.wall_y1n[3 * (int64_t)e + 2]};
@@ -128,16 +131,34 @@ __global__ void __launch_bounds__(128) wall_model_kernel(WmArgs a) {
     if (flx) v[0] = -v[0];
     if (fly) v[1] = -v[1];
     if (flz) v[2] = -v[2];
-    double vs[3] = {0, 0, 0}, vw[3];
+    double vs[3] = {0, 0, 0};
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
       double wk = shfl_d(w, 3 * k);
 #pragma unroll
       for (int q = 0; q < 3; ++q) vs[q] += wk * shfl_d(v[q], 3 * k);
     }
-#pragma unroll
-    for (int q = 0; q < 3; ++q) vw[q] = shfl_d(v[q], 24);
-    if (lane != 0) continue;
+    if (lane == 0)
+      for (int q = 0; q < 3; ++q) a.samp[6 * (int64_t)e + q] = vs[q];
+    if (lane == 24)
+      for (int q = 0; q < 3; ++q) a.samp[6 * (int64_t)e + 3 + q] = v[q];
+  }
+}
+
+__global__ void __launch_bounds__(128) wall_model_kernel(const __grid_constant__ WmArgs a) {
+  const int count = min(a.cnt->wall_count, a.cap_list);
+  const int64_t n = a.dm.n, nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
+  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < count; e += gridDim.x * blockDim.x) {
+    int64_t c = a.wall_idx[e];
+    int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
+    double y1v[3] = {a.wall_y1n[3 * (int64_t)e], a.wall_y1n[3 * (int64_t)e + 1], a.wall_y1n[3 * (int64_t)e + 2]};
+    double y1 = sqrt(y1v[0] * y1v[0] + y1v[1] * y1v[1] + y1v[2] * y1v[2]);
+    double nrm[3] = {y1v[0] / y1, y1v[1] / y1, y1v[2] / y1};
+    double vs[3], vw[3];
+    for (int q = 0; q < 3; ++q) {
+      vs[q] = a.samp[6 * (int64_t)e + q];
+      vw[q] = a.samp[6 * (int64_t)e + 3 + q];
+    }
     double us[3];
     uint8_t fl = a.flags[c];
     body_velocity_d(a.bo, (fl >> TAG_SHIFT) & TAG_MASK, x, y, z, us);
@@ -208,7 +229,7 @@ __global__ void zero_force_kernel(double* out) {
 // (Eq. 23 with reading R7), fp64 accumulation.  One warp per cell: lane i < 27 takes link i (both
 // loads of a cell's 26 links are in flight at once), warp shuffle sum -> shared per-tag bins -> one
 // global atomic per block, tag and component.
-__global__ void __launch_bounds__(128) force_kernel(ForceArgs a) {
+__device__ __forceinline__ void force_block(const ForceArgs& a, int block, int nblocks) {
   __shared__ double bins[MAX_TAGS * 3];
   for (int t = threadIdx.x; t < MAX_TAGS * 3; t += blockDim.x) bins[t] = 0.0;
   __syncthreads();
@@ -218,7 +239,7 @@ __global__ void __launch_bounds__(128) force_kernel(ForceArgs a) {
   const int i = lane;
   const int cx = i % 3 - 1, cy = (i / 3) % 3 - 1, cz = i / 9 - 1;
   const bool link = i < Q && i != 13;
-  for (int e = blockIdx.x * wpb + (threadIdx.x >> 5); e < count; e += gridDim.x * wpb) {
+  for (int e = block * wpb + (threadIdx.x >> 5); e < count; e += nblocks * wpb) {
     int64_t c = a.force_idx[e];
     int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
     int k = (a.flags[c] >> TAG_SHIFT) & TAG_MASK;
@@ -248,12 +269,23 @@ __global__ void __launch_bounds__(128) force_kernel(ForceArgs a) {
     if (bins[t] != 0.0) atomicAdd(&a.out[t], bins[t]);
 }
 
+// Phase A of K3 and K4 read the same post-stream populations and nothing of each other: one launch,
+// even blocks sample the wall-model velocities, odd blocks collect the forces.  Both are gathers whose
+// latency hides behind the other's.
+__global__ void __launch_bounds__(128) sample_force_kernel(const __grid_constant__ WmArgs w,
+                                                           const __grid_constant__ ForceArgs f, int wm_on) {
+  if (!wm_on)
+    force_block(f, blockIdx.x, gridDim.x);
+  else if ((blockIdx.x & 1) == 0)
+    wall_sample_block(w, blockIdx.x >> 1, gridDim.x >> 1);
+  else
+    force_block(f, blockIdx.x >> 1, gridDim.x >> 1);
+}
+
 // ---------------------------------------------------------------------------- launchers
 static void fill_bodies(const hhrr_lattice* L, BodiesD& b) { b = L->bodies; }
 
-cudaError_t launch_wall_model(hhrr_lattice* L) {
-  if (!L->wm_enabled) return cudaSuccess;
-  WmArgs a;
+static void fill_wm(const hhrr_lattice* L, WmArgs& a) {
   a.dm = L->dom;
   for (int q = 0; q < 3; ++q) a.g[q] = L->p.body_force[q];
   a.nu = (L->p.tau0 - 0.5) / 3.0;
@@ -269,15 +301,16 @@ cudaError_t launch_wall_model(hhrr_lattice* L) {
   a.wall_y1n = L->wall_y1n;
   a.cnt = L->counters;
   a.cap_list = (int)L->cap_list;
+  a.samp = L->wall_samp;
   a.wm_utau = L->wm_utau;
   a.wm_u = L->wm_u;
   a.wm_s = L->wm_s;
-  wall_model_kernel<<<2368, 128, 0, L->stream>>>(a);
-  L->launches++;
-  return cudaGetLastError();
 }
 
-cudaError_t launch_forces(hhrr_lattice* L) {
+// Listing 3 lines 4-6: WallModelO, then force collection and integration
+cudaError_t launch_wall_model_and_forces(hhrr_lattice* L) {
+  WmArgs w;
+  fill_wm(L, w);
   ForceArgs a;
   a.dm = L->dom;
   fill_bodies(L, a.bo);
@@ -288,8 +321,12 @@ cudaError_t launch_forces(hhrr_lattice* L) {
   a.cap_list = (int)L->cap_list;
   a.out = L->force + (L->step % FORCE_HISTORY) * MAX_TAGS * 3;
   zero_force_kernel<<<1, 64, 0, L->stream>>>(a.out);
-  force_kernel<<<2368, 128, 0, L->stream>>>(a);
+  sample_force_kernel<<<L->wm_enabled ? 4736 : 2368, 128, 0, L->stream>>>(w, a, L->wm_enabled ? 1 : 0);
   L->launches += 2;
+  if (L->wm_enabled) {
+    wall_model_kernel<<<592, 128, 0, L->stream>>>(w);
+    L->launches++;
+  }
   return cudaGetLastError();
 }
 

@@ -19,7 +19,7 @@
  * decay rate (viscosity + sign of Eq. 7/10), Smagorinsky closed form, Poiseuille
  * second difference (body force + porosity-0 wall), momentum-exchange force =
  * total body force, Spalding relation to 1e-12 + asymptotes, level set d=1/2,
- * sphere volume, rigid rotation => S^FD = 0.
+ * sphere volume, rigid rotation => S^FD = 0, bulk region = the sigma = 1 scheme.
  * PARITY UNPINNED: rotor thrust / wake against the paper's Fig. 7-10 (needs the
  * geometry and data of its ref. [19], not available) -- see DESIGN.md.
  *
@@ -36,7 +36,8 @@
 #define MAX_TAGS 16
 #define BIG_PHI 1.0e30
 
-enum { T_FLUID = 0, T_GROWTH = 1, T_FRONTIER = 2, T_SOLID = 3, T_FRINGE = 4 };
+enum { T_FLUID = 0, T_GROWTH = 1, T_FRONTIER = 2, T_SOLID = 3, T_FRINGE = 4, T_BULK = 5 };
+#define MAX_FSI_BOXES 8
 enum { AX_PERIODIC = 0, AX_MIRROR = 1 };
 
 typedef struct {
@@ -94,6 +95,11 @@ typedef struct ohrr_lattice {
   int64_t force_cap;
   int64_t step;
   int geometry_current; /* geometry(step) already evaluated */
+  /* region split (Listing 2 :271-302): union of half-open cell boxes x0 x1 y0 y1 z0 z1 that
+   * holds the wall-modelled / FSI part of the domain; fluid cells outside run the bulk RRLBM-LES model */
+  int n_fsi;
+  int32_t fsi[MAX_FSI_BOXES][6];
+  int region_violation; /* a cell that is not plain fluid was found outside every box */
 } ohrr_lattice;
 
 /* ---------------------------------------------------------------- lattice tables */
@@ -431,9 +437,19 @@ static void geometry(ohrr_lattice *L) {
                 }
               }
         }
+        if (L->n_fsi > 0) { /* bulk model where no moving wall-modelled structure can be */
+          int inside = 0;
+          for (int b = 0; b < L->n_fsi; ++b)
+            inside |= x >= L->fsi[b][0] && x < L->fsi[b][1] && y >= L->fsi[b][2] && y < L->fsi[b][3] &&
+                      z >= L->fsi[b][4] && z < L->fsi[b][5];
+          if (!inside) {
+            if (type == T_FLUID) type = T_BULK;
+            else L->region_violation = 1; /* the caller's boxes do not cover the structure: reported */
+          }
+        }
         L->type[c] = (uint8_t)type;
         L->d[c] = d;
-        if (type == T_FLUID || type == T_FRINGE) L->tag[c] = 0;
+        if (type == T_FLUID || type == T_FRINGE || type == T_BULK) L->tag[c] = 0;
         /* wall-model set W = {FRONTIER, phi > 0} (reading R13), y1 = phi, n = grad phi/|grad phi| */
         int inw = 0;
         if (L->wm_enabled && type == T_FRONTIER && phi > 0.0) {
@@ -550,6 +566,12 @@ static void collide_and_stream(ohrr_lattice *L) {
           S[0][2] = S[2][0] = s[4];
           S[1][2] = S[2][1] = s[5];
           sigma = 0.0;
+        } else if (t == T_BULK) {
+          /* Listing 2: bulk cells run RRLBM-LES -- plain momentum (d = 1 here),
+           * third-order recursive-regularised collision with the Smagorinsky effective relaxation and NO
+           * hybrid finite-difference part, i.e. Eq. 7 at sigma = 1 */
+          memset(S, 0, sizeof(S));
+          sigma = 1.0;
         } else {
           fd_strain(L, x, y, z, S);
         }
@@ -828,6 +850,18 @@ int ohrr_set_fringe(ohrr_lattice *L, int x0, int x1, const double u_in[3]) {
   L->geometry_current = 0;
   return 0;
 }
+
+/* Region split of PAPER.md:215: boxes = n_boxes x {x0,x1,y0,y1,z0,z1}, half-open; n_boxes = 0: HHRRLBM everywhere */
+int ohrr_set_fsi_region(ohrr_lattice *L, int32_t n_boxes, const int32_t *boxes) {
+  if (n_boxes < 0 || n_boxes > MAX_FSI_BOXES || (n_boxes > 0 && !boxes)) return -1;
+  L->n_fsi = n_boxes;
+  for (int b = 0; b < n_boxes; ++b)
+    for (int k = 0; k < 6; ++k) L->fsi[b][k] = boxes[6 * b + k];
+  L->region_violation = 0;
+  L->geometry_current = 0;
+  return 0;
+}
+int ohrr_region_violation(const ohrr_lattice *L) { return L->region_violation; }
 
 int ohrr_set_rotor(ohrr_lattice *L, const ohrr_rotor_desc *r) {
   if (!r || r->n_tags < 1 || r->n_tags >= MAX_TAGS) return -1;

@@ -195,6 +195,16 @@ class Lattice:
     def enable_wall_model(self, enable=True):
         lib().ohrr_enable_wall_model(self._h, int(enable))
 
+    def set_fsi_region(self, boxes):
+        """boxes: iterable of (x0, x1, y0, y1, z0, z1), half-open; empty = HHRRLBM everywhere."""
+        b = np.ascontiguousarray(np.asarray(list(boxes), np.int32).reshape(-1, 6))
+        rc = lib().ohrr_set_fsi_region(self._h, int(b.shape[0]), _p(b) if b.size else None)
+        if rc:
+            raise RuntimeError("ohrr_set_fsi_region failed")
+
+    def region_violation(self):
+        return bool(lib().ohrr_region_violation(self._h))
+
     def update_geometry(self):
         lib().ohrr_update_geometry(self._h)
 

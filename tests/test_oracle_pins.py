@@ -487,3 +487,86 @@ def test_rigid_rotation_has_zero_fd_strain(oracle):
         r = np.array([x, y, z]) - 7.5
         feq = oracle.equilibrium(1.0, np.cross(om, r))
         assert np.allclose(post[:, z, y, x], feq, atol=1e-16)
+
+
+# ------------------------------------------------------------------ region split: bulk RRLBM-LES (Listing 2)
+def test_bulk_region_types_and_violation(oracle):
+    """the simpler model runs where no wall-modelled structure can be.  Fluid cells outside
+    every FSI box become BULK (type 5), everything inside keeps its type; a solid cell outside the boxes is
+    reported, not silently re-typed."""
+    from paper_2510_13726_b200 import inputs
+    nx, ny, nz = 24, 16, 12
+    phi = inputs.sphere_phi(nx, ny, nz, (8.0, 7.5, 5.5), 3.0)
+    L = oracle.Lattice(oracle.make_params(nx, ny, nz, tau0=0.6))
+    L.set_static_geometry(phi, np.ones(nx * ny * nz, np.uint8))
+    L.update_geometry()
+    t0, _, _ = L.cell_types()
+    box = (2, 15, 1, 14, 0, 12)
+    L.set_fsi_region([box]); L.update_geometry()
+    t1, g1, d1 = L.cell_types()
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    inside = ((x >= 2) & (x < 15) & (y >= 1) & (y < 14)).reshape(-1)
+    assert np.array_equal(t1[inside], t0[inside])
+    assert np.all(t0[~inside] == 0) and np.all(t1[~inside] == 5)
+    assert np.all(g1[~inside] == 0) and np.all(d1[~inside] == 1.0)
+    assert not L.region_violation()
+    L.set_fsi_region([(9, 15, 1, 14, 0, 12)]); L.update_geometry()     # cuts through the sphere
+    assert L.region_violation()
+    L.set_fsi_region([]); L.update_geometry()                            # back to HHRRLBM everywhere
+    assert np.array_equal(L.cell_types()[0], t0) and not L.region_violation()
+
+
+def test_bulk_region_is_the_sigma_one_scheme(oracle):
+    """Listing 2: the bulk model is the third-order recursive-regularised collision with
+    the Smagorinsky relaxation and no hybrid part, i.e. Eq. 7 at sigma = 1.  (i) A run whose cells are all
+    BULK under sigma = 0.5 reproduces, to rounding, the run with sigma = 1 and no region split; (ii) with an
+    all-bulk lattice the 2-D Taylor-Green energy decays at 4 nu k^2 whatever sigma says (a bulk cell that
+    still took the sigma = 0.3 hybrid part on a tau0 = 0.8 lattice would show in the split run differing
+    from the reference, which itself is pinned by test_taylor_green_decay_gives_viscosity)."""
+    n, nz, U0, tau0 = 32, 2, 0.01, 0.8
+    k = 2 * np.pi / n
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(n), np.arange(n), indexing="ij")
+    u = np.stack([U0 * np.sin(k * x) * np.cos(k * y), -U0 * np.cos(k * x) * np.sin(k * y), 0 * x * 1.0]).reshape(3, -1)
+    rho = (1 + 3 * U0 ** 2 / 4 * (np.cos(2 * k * x) + np.cos(2 * k * y))).reshape(-1)
+
+    def run(sigma, boxes):
+        L = oracle.Lattice(oracle.make_params(n, n, nz, tau0=tau0, sigma=sigma, smagorinsky_cs=0.1))
+        L.set_fsi_region(boxes)
+        L.init_equilibrium(rho, u, True)
+        L.step(20); _, v0 = L.moments()
+        L.step(40); _, v1 = L.moments()
+        types = L.cell_types()[0]
+        return v1, -np.log(np.sum(v1 ** 2) / np.sum(v0 ** 2)) / 40 / (4 * (tau0 - 0.5) / 3 * k * k), types
+
+    v_ref, r_ref, t_ref = run(1.0, [])
+    v_blk, r_blk, t_blk = run(0.3, [(0, 0, 0, 0, 0, 0)])       # one empty box: every cell is bulk
+    assert np.all(t_ref == 0) and np.all(t_blk == 5)
+    assert np.max(np.abs(v_blk - v_ref)) <= 1e-15
+    assert abs(r_blk - 1) < 0.02, r_blk
+    v_hyb, r_hyb, _ = run(0.3, [])                              # the hybrid scheme itself differs measurably
+    assert np.max(np.abs(v_hyb - v_ref)) > 1e-9
+
+
+def test_bulk_region_interface_is_seamless(oracle):
+    """A fluid-only lattice split into an FSI half and a bulk half: cells in the FSI half keep the hybrid
+    collision (they differ from the all-bulk run), cells deep in the bulk half follow the sigma = 1 run
+    until the difference has travelled there (one cell per step)."""
+    n, nz, U0, tau0 = 32, 2, 0.02, 0.7
+    k = 2 * np.pi / n
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(n), np.arange(n), indexing="ij")
+    u = np.stack([U0 * np.sin(k * x) * np.cos(k * y), -U0 * np.cos(k * x) * np.sin(k * y), 0 * x * 1.0]).reshape(3, -1)
+    rho = np.ones(n * n * nz)
+
+    def run(sigma, boxes, steps):
+        L = oracle.Lattice(oracle.make_params(n, n, nz, tau0=tau0, sigma=sigma, smagorinsky_cs=0.0))
+        L.set_fsi_region(boxes)
+        L.init_equilibrium(rho, u, True)
+        L.step(steps)
+        return L.moments()[1].reshape(3, nz, n, n)
+
+    steps = 3
+    split = run(0.0, [(0, 8, 0, n, 0, nz)], steps)       # x in [0, 8) hybrid (pure FD), the rest bulk
+    allb = run(1.0, [], steps)
+    far = slice(8 + steps + 1, n - steps - 1)            # bulk cells no hybrid cell has reached yet
+    assert np.max(np.abs(split[:, :, :, far] - allb[:, :, :, far])) <= 1e-16
+    assert np.max(np.abs(split[:, :, :, 0:8] - allb[:, :, :, 0:8])) > 1e-9

@@ -63,8 +63,15 @@ typedef enum {
   HHRR_GROWTH = 1,   /* d = 1, one of the 26 neighbours has phi < eps/2 (:269)    */
   HHRR_FRONTIER = 2, /* |phi| < eps/2, 0 < d < 1  (Def. 1, Eq. 21-22 :196-203)    */
   HHRR_SOLID = 3,    /* phi <= -eps/2, d = 0                                      */
-  HHRR_FRINGE = 4    /* d = 0, u^B = u_in                                         */
+  HHRR_FRINGE = 4,   /* d = 0, u^B = u_in                                         */
+  HHRR_BULK = 5      /* fluid outside the FSI region: bulk RRLBM-LES model (:215)  */
 } hhrr_cell_type;
+
+/* Half-open box of cells [x0,x1) x [y0,y1) x [z0,z1). */
+typedef struct {
+  int32_t x0, x1, y0, y1, z0, z1;
+} hhrr_box;
+#define HHRR_MAX_FSI_BOXES 8
 
 typedef struct {
   int32_t nx, ny, nz;
@@ -123,6 +130,16 @@ int hhrr_set_body(hhrr_lattice* L, int32_t tag, const double centre[3], const do
                   const double vel[3]);
 /* Inflow fringe (R12): cells with x_begin <= x < x_end get d = 0, u^B = u_in. */
 int hhrr_set_fringe(hhrr_lattice* L, int32_t x_begin, int32_t x_end, const double u_in[3]);
+/* Region split of PAPER.md:215 ("a simpler RRLBM-LES model is applied for all parts of the domain
+ * that are guaranteed to not intersect the moving wall-modeled structures", Listing 2 :271-302;
+ * DESIGN.md R20).  `boxes` (host, n_boxes <= HHRR_MAX_FSI_BOXES, copied) name the FSI part of the
+ * lattice; a FLUID cell outside every box becomes HHRR_BULK and collides with the bulk model: plain
+ * momentum, third-order recursive-regularised collision with the Smagorinsky relaxation, no hybrid
+ * finite-difference part (Eq. 7 at sigma = 1).  Blocks of the collide-stream kernel that hold only
+ * bulk cells then need no neighbour velocities at all.  Every cell that is not plain fluid (solid,
+ * frontier, growth, fringe) must lie inside a box: if one does not, its type is kept and
+ * hhrr_check_finite returns HHRR_E_STATE.  n_boxes = 0 (default): HHRRLBM everywhere.          */
+int hhrr_set_fsi_region(hhrr_lattice* L, int32_t n_boxes, const hhrr_box* boxes);
 /* Rotor (copied to the device workspace); sets the bodies of tags 1..n_tags. */
 int hhrr_set_rotor(hhrr_lattice* L, const hhrr_rotor_desc* rotor);
 /* Wall model on the cells {FRONTIER, phi > 0} (R13). */

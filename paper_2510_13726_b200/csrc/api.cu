@@ -276,6 +276,18 @@ int hhrr_set_fringe(hhrr_lattice* L, int32_t x_begin, int32_t x_end, const doubl
   return HHRR_OK;
 }
 
+int hhrr_set_fsi_region(hhrr_lattice* L, int32_t n_boxes, const hhrr_box* boxes) {
+  if (!L || n_boxes < 0 || n_boxes > HHRR_MAX_FSI_BOXES || (n_boxes > 0 && !boxes))
+    return fail(HHRR_E_ARG, "hhrr_set_fsi_region: bad argument");
+  L->fsi.n = n_boxes;
+  for (int b = 0; b < n_boxes; ++b)
+    L->fsi.b[b] = Box{boxes[b].x0, boxes[b].x1, boxes[b].y0, boxes[b].y1, boxes[b].z0, boxes[b].z1};
+  CU(cudaMemsetAsync(&L->counters->region_violation, 0, sizeof(int), L->stream));
+  L->geometry_dirty = true;
+  L->geometry_current = false;
+  return HHRR_OK;
+}
+
 int hhrr_set_rotor(hhrr_lattice* L, const hhrr_rotor_desc* r) {
   if (!L || !r || !r->sdf || !r->tag) return fail(HHRR_E_ARG, "hhrr_set_rotor: NULL argument");
   if (r->n_tags < 1 || r->n_tags >= MAX_TAGS) return fail(HHRR_E_ARG, "hhrr_set_rotor: n_tags out of range");
@@ -608,6 +620,8 @@ int hhrr_check_finite(hhrr_lattice* L) {
   int rc = read_counters(L, &h);
   if (rc) return rc;
   if (h.overflow) return fail(HHRR_E_SIZE, "compact cell list overflowed its capacity of %lld", (long long)L->cap_list);
+  if (h.region_violation)
+    return fail(HHRR_E_STATE, "a cell that is not plain fluid lies outside the FSI region (hhrr_set_fsi_region)");
   if (h.nonfinite) return fail(HHRR_E_NAN, "non-finite population at step %lld", (long long)L->step);
   return HHRR_OK;
 }

@@ -30,7 +30,7 @@ __device__ __forceinline__ void cell_solid_state(const PhysF& ph, const BodiesF&
   int type = fl & TYPE_MASK;
   d = 1.f;
   uB[0] = uB[1] = uB[2] = 0.f;
-  if (type >= HHRR_FRONTIER) {
+  if (type_has_solid_state(type)) {
     d = (type == HHRR_FRONTIER) ? __ldg(dfield + c) : 0.f;
     solid_velocity(ph, bo, fl, x, y, z, uB);
     if (fl & WM_VALID) {
@@ -84,7 +84,7 @@ __global__ void __launch_bounds__(256) collide_kernel(Dom dm, PhysF ph, BodiesF 
   float d, uB[3], rho, uh[3];
   cell_solid_state(ph, bo, fl, dfield, wm_u, n, c, x, y, z, d, uB);
   homogenised_velocity(ph, m.drho, m.jx, m.jy, m.jz, d, uB, rho, uh);
-  float S[6], sigma = ph.sigma;
+  float S[6], sigma = cell_sigma(ph, fl);
   if (fl & WM_VALID) {  // sigma = 0, strain from the wall model
 #pragma unroll
     for (int a = 0; a < 6; ++a) S[a] = __ldg(wm_s + (int64_t)a * n + c);

@@ -114,6 +114,14 @@ __device__ __forceinline__ void solid_velocity(const PhysF& ph, const BodiesF& b
   }
 }
 
+// hybrid factor of a cell: bulk cells run Listing 2's model, Eq. 7 at sigma = 1 (R20)
+__device__ __forceinline__ float cell_sigma(const PhysF& ph, uint8_t flags) {
+  return (flags & TYPE_MASK) == HHRR_BULK ? 1.f : ph.sigma;
+}
+__device__ __forceinline__ bool type_has_solid_state(int type) {  // FRONTIER, SOLID, FRINGE: d < 1, u^B
+  return type >= HHRR_FRONTIER && type <= HHRR_FRINGE;
+}
+
 // Eq. 12 with reading R1 (d = 1 fluid): uhat = d u + (1-d) u^B, u = (j + g)/rho  (R11)
 __device__ __forceinline__ void homogenised_velocity(const PhysF& ph, float drho, float jx, float jy,
                                                      float jz, float d, const float uB[3], float& rho,

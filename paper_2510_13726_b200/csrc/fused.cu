@@ -47,7 +47,7 @@ __device__ __forceinline__ void solid_state(const FusedArgs& a, uint8_t fl, int6
   int type = fl & TYPE_MASK;
   d = 1.f;
   uB[0] = uB[1] = uB[2] = 0.f;
-  if (type >= HHRR_FRONTIER) {
+  if (type_has_solid_state(type)) {
     d = (type == HHRR_FRONTIER) ? __ldg(a.d + c) : 0.f;
     solid_velocity(a.ph, a.bo, fl, x, y, z, uB);
     if (fl & WM_VALID) {
@@ -168,7 +168,7 @@ __global__ void __launch_bounds__(TX* TY, MINB) fused_kernel(const __grid_consta
     publish(z + 1, z + 1 < z1);
     __syncthreads();
     if (own_collide) {
-      float S[6], sigma = a.ph.sigma;
+      float S[6], sigma = cell_sigma(a.ph, fl_c);
       const int64_t c = xv + nx * yv + nxy * z;
       if (fl_c & WM_VALID) {
 #pragma unroll

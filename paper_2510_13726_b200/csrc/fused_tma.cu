@@ -291,7 +291,7 @@ __global__ void __launch_bounds__(tma::threads(CPT), 1)
     if (it >= 1) pub_wait(pub0, it - 1);
     const int z = p - 1;
     if (z >= z0) {
-      float S[6], sigma = a.ph.sigma;
+      float S[6], sigma = cell_sigma(a.ph, fl_c);
       if (fl_c & WM_VALID) {
         const int64_t c = own_xy + nxy * z;
 #pragma unroll
@@ -399,7 +399,7 @@ __global__ void __launch_bounds__(tma::threads(CPT), 1)
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
           const int o = own_slot + k;
-          float S[6], sigma = a.ph.sigma;
+          float S[6], sigma = cell_sigma(a.ph, fl_c[k]);
           float dxu0 = s0[0][o + 1] - s0[0][o - 1], dxu1 = s0[1][o + 1] - s0[1][o - 1], dxu2 = s0[2][o + 1] - s0[2][o - 1];
           float dyu0 = s0[0][o + SX] - s0[0][o - SX], dyu1 = s0[1][o + SX] - s0[1][o - SX],
                 dyu2 = s0[2][o + SX] - s0[2][o - SX];

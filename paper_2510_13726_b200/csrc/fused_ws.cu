@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(WsCfg<TX, TY, NPW, DEPTH, CPT_>::THREADS, 1)
         m.jx = m.jy = m.jz = 0.f;  // not used by collide()
         const float rho = 1.f + m.drho;
         float uh[3] = {u0[o], u0[C::PLANE + o], u0[2 * C::PLANE + o]};
-        float S[6], sigma = a.ph.sigma;
+        float S[6], sigma = cell_sigma(a.ph, fl);
         if (fl & WM_VALID) {
           const int64_t c = xv + nx * yv + nxy * z;
 #pragma unroll

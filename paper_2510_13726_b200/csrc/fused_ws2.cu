@@ -196,7 +196,7 @@ __global__ void __launch_bounds__(Ws2Cfg<TX, TY, DEPTH>::THREADS, 1)
           const float rho = 1.f + m.drho;
           const int ok = o + k;
           float uh[3] = {u0[ok], u0[C::PLANE + ok], u0[2 * C::PLANE + ok]};
-          float S[6], sigma = a.ph.sigma;
+          float S[6], sigma = cell_sigma(a.ph, fl);
           if (fl & WM_VALID) {
             const int64_t c = xa + k + nx * yv + nxy * z;
 #pragma unroll

@@ -363,7 +363,7 @@ __global__ void __launch_bounds__(xp::THREADS, 1)
 #pragma unroll
       for (int k = 0; k < 2; ++k) {
         const int o = own_slot + k;
-        float S[6], sigma = a.ph.sigma;
+        float S[6], sigma = cell_sigma(a.ph, fl_c[k]);
         float dxu0 = s0[0][o + 1] - s0[0][o - 1], dxu1 = s0[1][o + 1] - s0[1][o - 1], dxu2 = s0[2][o + 1] - s0[2][o - 1];
         float dyu0 = s0[0][o + SX] - s0[0][o - SX], dyu1 = s0[1][o + SX] - s0[1][o - SX],
               dyu2 = s0[2][o + SX] - s0[2][o - SX];

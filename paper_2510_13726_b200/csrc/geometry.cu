@@ -16,6 +16,7 @@ namespace hhrr {
 
 struct GeoArgs {
   Dom dm;
+  Boxes fsi;        // FSI region: fluid cells outside every box are BULK (R20)
   Box box;          // cells processed (inside == true) or skipped (inside == false)
   int inside;
   double h;         // eps/2
@@ -195,7 +196,17 @@ __global__ void __launch_bounds__(128) geometry_type_kernel(GeoArgs a) {
       d = 1.f;
       if (near_below) type = HHRR_GROWTH;
     }
-    if (type == HHRR_FLUID || type == HHRR_FRINGE) tg = 0;
+    if (a.fsi.n > 0) {
+      bool inside = false;
+      for (int b = 0; b < a.fsi.n; ++b)
+        inside |= x >= a.fsi.b[b].x0 && x < a.fsi.b[b].x1 && y >= a.fsi.b[b].y0 && y < a.fsi.b[b].y1 &&
+                  z >= a.fsi.b[b].z0 && z < a.fsi.b[b].z1;
+      if (!inside) {
+        if (type == HHRR_FLUID) type = HHRR_BULK;
+        else a.cnt->region_violation = 1;  // the boxes do not cover the structure: reported, type kept
+      }
+    }
+    if (type == HHRR_FLUID || type == HHRR_FRINGE || type == HHRR_BULK) tg = 0;
     if (a.wm_enabled && type == HHRR_FRONTIER && phi > 0.0) {
       int xm = wrap_any(x - 1, nx, a.dm.mode[0]), xp = wrap_any(x + 1, nx, a.dm.mode[0]);
       int ym = wrap_any(y - 1, ny, a.dm.mode[1]), yp = wrap_any(y + 1, ny, a.dm.mode[1]);
@@ -287,6 +298,7 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
   a.has_fringe = L->has_fringe;
   a.has_rotor = L->has_rotor;
   a.wm_enabled = L->wm_enabled;
+  a.fsi = L->fsi;
   a.fr_x0 = L->fr_x0;
   a.fr_x1 = L->fr_x1;
   a.cth = 1.0;

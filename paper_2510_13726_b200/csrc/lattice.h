@@ -47,6 +47,11 @@ struct Box {  // half-open cell box
   int x0, x1, y0, y1, z0, z1;
 };
 
+struct Boxes {  // FSI region (hhrr_set_fsi_region); n = 0: the whole lattice
+  int n;
+  Box b[HHRR_MAX_FSI_BOXES];
+};
+
 struct RotorDev {
   const float* sdf;
   const uint8_t* tag;
@@ -60,7 +65,8 @@ struct Counters {
   int wall_static, force_static;  // list prefix owned by cells outside the rotor box
   int overflow;
   int nonfinite;
-  int pad[2];
+  int region_violation;  // a cell that is not plain fluid lies outside the FSI region
+  int pad[1];
 };
 
 }  // namespace hhrr
@@ -100,6 +106,7 @@ struct hhrr_lattice {
   double fr_u[3];
   hhrr_rotor_desc rot;  // sdf/tag pointers nulled
   hhrr::Box rot_box;
+  hhrr::Boxes fsi;
   hhrr::BodiesD bodies;
   bool geometry_dirty;     // full-domain geometry pass needed
   bool geometry_current;   // geometry(step) evaluated

@@ -133,6 +133,7 @@ class Case:
     fringe: Optional[tuple] = None                   # (x0, x1, u_in)
     rotor: Optional[dict] = None                     # kwargs of set_rotor
     wall_model: bool = False
+    fsi_boxes: Optional[list] = None                 # region split: [(x0,x1,y0,y1,z0,z1), ...]
 
     @property
     def n(self):
@@ -148,7 +149,37 @@ def apply_case(case: Case, lattice) -> None:
     if case.rotor is not None:
         lattice.set_rotor(**case.rotor)
     lattice.enable_wall_model(case.wall_model)
+    if case.fsi_boxes is not None:
+        lattice.set_fsi_region(case.fsi_boxes)
     lattice.init_equilibrium(case.rho, case.u, case.with_neq)
+
+
+def with_region_split(case: Case, margin: int = 6) -> Case:
+    """The same recipe with the paper's bulk / FSI region split: boxes around everything that
+    is not plain fluid -- the inflow fringe slab, the volume the rotor sweeps, a static sphere, the wall
+    layer -- each widened by `margin` cells; the rest of the lattice runs the bulk RRLBM-LES model."""
+    import dataclasses
+    nx, ny, nz = case.nx, case.ny, case.nz
+    boxes = []
+    if case.fringe is not None:
+        boxes.append((max(0, case.fringe[0] - 1), min(nx, case.fringe[1] + 1), 0, ny, 0, nz))
+    if case.rotor is not None:
+        sdf = case.rotor["sdf"]
+        gz, gy, gx = sdf.shape
+        sp, org, ctr = case.rotor["spacing"], case.rotor["origin"], case.rotor["centre"]
+        hx = max(abs(org[0]), abs(org[0] + (gx - 1) * sp))          # axis +x: axial half-extent of the grid
+        hr = max(abs(org[1]), abs(org[1] + (gy - 1) * sp), abs(org[2]), abs(org[2] + (gz - 1) * sp))
+        boxes.append((max(0, int(np.floor(ctr[0] - hx)) - margin), min(nx, int(np.ceil(ctr[0] + hx)) + margin + 1),
+                      max(0, int(np.floor(ctr[1] - hr)) - margin), min(ny, int(np.ceil(ctr[1] + hr)) + margin + 1),
+                      max(0, int(np.floor(ctr[2] - hr)) - margin), min(nz, int(np.ceil(ctr[2] + hr)) + margin + 1)))
+    if case.phi is not None:
+        near = np.flatnonzero(np.asarray(case.phi).reshape(-1) < 2.0)   # cells within 2 of the static surface
+        if near.size:
+            x, y, z = near % nx, (near // nx) % ny, near // (nx * ny)
+            boxes.append((max(0, int(x.min()) - margin), min(nx, int(x.max()) + margin + 1),
+                          max(0, int(y.min()) - margin), min(ny, int(y.max()) + margin + 1),
+                          max(0, int(z.min()) - margin), min(nz, int(z.max()) + margin + 1)))
+    return dataclasses.replace(case, name=case.name + "+split", fsi_boxes=boxes)
 
 
 DEFAULTS = dict(sigma=0.995, smagorinsky_cs=0.1, kappa=0.41, E=9.8, newton_max_iter=10,

@@ -204,6 +204,44 @@ def test_xpull_storage_round_trip():
     A.close(); Bv.close()
 
 
+# ---- bulk / FSI region split (Listing 2; R20) ------------------------------
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_region_split_rotor_and_sphere(oracle, variant):
+    """Fluid cells outside the FSI boxes are BULK (type 5, compared bit-exact) and collide with the bulk
+    RRLBM-LES model on both sides; the rotor, its growth layer, the fringe and the sphere stay HHRRLBM."""
+    case = I.with_region_split(I.case_rotor(128, 72, 72, 20.0, 12, omega=0.012))
+    assert len(case.fsi_boxes) == 2
+    run_parity(oracle, case, 12, variant, TOL10, check_every=3)
+    case = I.with_region_split(I.case_sphere(128, 32, 32, 5.0, 10))
+    run_parity(oracle, case, 10, variant, TOL10, check_every=5)
+
+
+def test_region_split_channel_and_all_bulk(oracle):
+    """Wall layer in a box (mirror top in the bulk part); and a lattice with no FSI cell at all."""
+    case = I.with_region_split(I.case_channel(128, 48, 16, 20))
+    run_parity(oracle, case, 20, 5, TOL10, check_every=5)
+    import dataclasses
+    rho, u = I.noisy_uniform(192, 16, 40, (0.03, -0.02, 0.01), 5e-3, 79)
+    case = I.Case("all-bulk", 192, 16, 40, 10, params=dict(I.DEFAULTS, tau0=0.53), rho=rho, u=u, with_neq=True,
+                  fsi_boxes=[(0, 0, 0, 0, 0, 0)])
+    run_parity(oracle, case, 10, 5, TOL10)
+    run_parity(oracle, dataclasses.replace(case, fsi_boxes=[(60, 70, 0, 16, 18, 22)]), 10, 5, TOL10)
+
+
+def test_region_split_violation_is_reported():
+    from paper_2510_13726_b200 import binding as B
+    case = I.case_sphere(128, 32, 32, 5.0, 2)
+    G = _gpu_lattice(case, 5)
+    G.set_fsi_region([(0, 5, 0, 32, 0, 32)])          # the sphere is not covered
+    G.step(1)
+    with pytest.raises(B.HhrrError):
+        G.check_finite()
+    G.set_fsi_region(I.with_region_split(case).fsi_boxes)
+    G.step(1)
+    G.check_finite()
+    G.close()
+
+
 @pytest.mark.parametrize("variant", [2, 4, 5])
 def test_fused_kernels_are_deterministic(variant):
     """Two identical lattices stay bitwise identical: every step is a deterministic function of the

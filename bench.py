@@ -47,11 +47,13 @@ def measured_peak():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def workload(config: int) -> tuple[I.Case, str]:
+def workload(config: int, region_split: bool = False) -> tuple[I.Case, str]:
     case = I.baseline_config(config)
+    if region_split:   # bulk RRLBM-LES outside boxes around the fringe / rotor / static geometry
+        case = I.with_region_split(case)
     names = {1: "config1 TGV 32^3", 2: "config2 sphere channel 128x64x64", 3: "config3 half-channel 256x128x128",
              4: "config4 rotor R=80 512x256x256", 5: "config5 rotor R=120 768x384x364 (~107M cells)"}
-    return case, names[config]
+    return case, names[config] + (" + bulk/FSI region split" if region_split else "")
 
 
 # ------------------------------------------------------------------------------- clocks
@@ -188,7 +190,7 @@ def run_ours(args, rank, world, local_rank):
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
     dev = f"cuda:{local_rank}"
 
-    case, wname = workload(args.config)
+    case, wname = workload(args.config, args.region_split)
     p = B.make_params(case.nx, case.ny, case.nz, mode=case.mode, **case.params)
     L = B.Lattice(p, rotor_shape=None if case.rotor is None else case.rotor["sdf"].shape, device=dev)
     L.set_kernel_variant(args.variant)
@@ -297,6 +299,8 @@ def main():
     ap.add_argument("--variant", type=int, default=5, choices=[0, 1, 2, 3, 4, 5] + list(range(11, 50)))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--region-split", action="store_true",
+                    help="the paper's bulk / FSI region split (PAPER.md:215); default: HHRRLBM in every cell")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank = int(os.environ.get("RANK", "0"))

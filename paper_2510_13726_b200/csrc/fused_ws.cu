@@ -238,6 +238,7 @@ void fill_ws_args(const hhrr_lattice* L, const PhysF& ph, const BodiesF& bo, WsA
   a.dm = L->dom;
   a.ph = ph;
   a.bo = bo;
+  a.fsi = L->fsi;
   a.fin = L->fA;
   a.fout = L->fB;
   a.flags = L->flags;

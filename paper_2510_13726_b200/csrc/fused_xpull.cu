@@ -122,7 +122,19 @@ __global__ void __launch_bounds__(xp::THREADS, 1)
   const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
   const int z0 = blockIdx.z * a.zchunk, z1 = min(dm.nz, z0 + a.zchunk);
   const int64_t n = dm.n, nx = dm.nx, nxy = (int64_t)dm.nx * dm.ny;
-  const int pfirst = z0 - 1;
+  // Region split (Listing 2; R20): a block none of whose cells lies in an FSI box
+  // holds BULK cells only -- sigma = 1, d = 1, no wall model -- so its collision is purely local: it loads
+  // no halo rows, no flag bytes and no overlap planes, publishes no uhat, and its aux warps only keep the
+  // barriers turning.  Everything else (pipeline, moments, collision, stores) is the code below.
+  bool bulk = a.fsi.n > 0;
+  for (int b = 0; b < a.fsi.n; ++b) {
+    const Box& q = a.fsi.b[b];
+    if (q.x0 < x0 + TX && q.x1 > x0 && q.y0 < y0 + TY && q.y1 > y0 && q.z0 < z1 && q.z1 > z0 && q.x1 > q.x0 &&
+        q.y1 > q.y0 && q.z1 > q.z0)
+      bulk = false;
+  }
+  const int pfirst = bulk ? z0 : z0 - 1;   // planes pfirst .. plast are loaded; the loops run to z1 (collide z1-1)
+  const int plast = bulk ? z1 - 1 : z1;
   // tiles at the periodic x boundary: the 4 columns beyond it come from the other side (nx >= 128: one side only)
   const bool edge_l = x0 == 0, edge_r = x0 + TX == dm.nx, edge = edge_l || edge_r;
   const int px = edge_l ? dm.nx - 4 : 0;  // first wrapped column
@@ -147,13 +159,23 @@ __global__ void __launch_bounds__(xp::THREADS, 1)
     // ------------------------------------------------------------------ producer: one lane issues TMA
     const int lane = tid & 31;
     const int xl = edge_l ? dm.nx - 1 : x0 - 1, xr = edge_r ? 0 : x0 + TX;  // real x of the halo columns
-    for (int p = pfirst; p <= z1; ++p) {
+    for (int p = pfirst; p <= plast; ++p) {
       const int it = p - pfirst, s = it % NS, k = it / NS;
       if (k > 0) mbar_wait(empty0 + 8 * s, (k - 1) & 1);
       bool fz, okz;
       const int zr = virt_ws(p, dm.nz, dm.mode[2], fz, okz);
       const uint32_t bar = full0 + 8 * s;
       unsigned char* stb = smem + (size_t)s * STAGE_BYTES;
+      if (bulk) {  // tile rows (and their wrapped columns) only
+        if (lane == 0) {
+          const uint32_t st = smem_u32(stb);
+          mbar_expect_tx(bar, edge ? (MAIN_F + PM_F) * 4 : MAIN_F * 4);
+          tma_load_4d(st, &map_main, x0 - 4, y0, zr, 0, bar);
+          if (edge) tma_load_4d(st + 4 * O_PM, &map_pm, px, y0, zr, 0, bar);
+          mbar_arrive(bar);
+        }
+        continue;
+      }
       if (lane == 0) {
         const uint32_t st = smem_u32(stb);
         mbar_expect_tx(bar, edge ? TMA_BYTES + TMA_EDGE_BYTES : TMA_BYTES);
@@ -191,6 +213,18 @@ __global__ void __launch_bounds__(xp::THREADS, 1)
     // lane a owns halo cells a and a + AUX (if < HALO).  Per cell and per cx group: where population
     // (cx, k = 0) sits in a stage and the stride to k + 1 (column lx - cx of the 72-wide boxes, or the
     // wrapped columns at the periodic x boundary)
+    if (bulk) {  // no halo: release the stages and keep the publication barrier in step
+      for (int p = pfirst; p <= z1; ++p) {
+        const int it = p - pfirst, s = it % NS, k2 = it / NS;
+        if (it >= 2) pub_wait(pub0, it - 2);
+        if (p <= plast) mbar_wait(full0 + 8 * s, k2 & 1);
+        if ((tid & 31) == 0) {
+          if (p <= plast) mbar_arrive(empty0 + 8 * s);
+          mbar_arrive(pub0 + 8 * (it & 1));
+        }
+      }
+      return;
+    }
     const int a0 = tid - WORKERS;
     int h_off[2][3], h_str[2][3], h_slot[2], h_x[2], h_y[2], h_fl[2];
     bool h_fy[2], h_on[2];
@@ -294,14 +328,15 @@ __global__ void __launch_bounds__(xp::THREADS, 1)
 
   for (int p = pfirst; p <= z1; ++p) {
     const int it = p - pfirst, s = it % NS, k2 = it / NS;
-    {
+    if (p <= plast) {
       bool fz, okz;
       const int zr = virt_ws(p, dm.nz, dm.mode[2], fz, okz);
       const int64_t c = own_xy + nxy * zr;
       const float* st = reinterpret_cast<const float*>(smem + (size_t)s * STAGE_BYTES);
       float(*slot)[PLANE] = ring[it & 3];
       mbar_wait(full0 + 8 * s, k2 & 1);
-      const uint16_t flw = *reinterpret_cast<const uint16_t*>(smem + (size_t)s * STAGE_BYTES + FLAG_OFF + FL_MAIN + own_fl);
+      const uint16_t flw = bulk ? (uint16_t)(HHRR_BULK | (HHRR_BULK << 8))
+                                : *reinterpret_cast<const uint16_t*>(smem + (size_t)s * STAGE_BYTES + FLAG_OFF + FL_MAIN + own_fl);
       float f[2][Q];
 #pragma unroll
       for (int i = 0; i < Q; ++i) {  // population i of cell x sits at column x - cx (x-pull)
@@ -344,9 +379,11 @@ __global__ void __launch_bounds__(xp::THREADS, 1)
           moments_rho_j(f[k], drho, jx, jy, jz);
           homogenised_velocity(a.ph, drho, jx, jy, jz, d, uB, rho, uh);
         }
-        slot[0][own_slot + k] = uh[0];
-        slot[1][own_slot + k] = uh[1];
-        slot[2][own_slot + k] = fz ? -uh[2] : uh[2];
+        if (!bulk) {
+          slot[0][own_slot + k] = uh[0];
+          slot[1][own_slot + k] = uh[1];
+          slot[2][own_slot + k] = fz ? -uh[2] : uh[2];
+        }
       }
     }
     pub_arrive(pub0, it);
@@ -363,17 +400,19 @@ __global__ void __launch_bounds__(xp::THREADS, 1)
 #pragma unroll
       for (int k = 0; k < 2; ++k) {
         const int o = own_slot + k;
-        float S[6], sigma = cell_sigma(a.ph, fl_c[k]);
-        float dxu0 = s0[0][o + 1] - s0[0][o - 1], dxu1 = s0[1][o + 1] - s0[1][o - 1], dxu2 = s0[2][o + 1] - s0[2][o - 1];
-        float dyu0 = s0[0][o + SX] - s0[0][o - SX], dyu1 = s0[1][o + SX] - s0[1][o - SX],
-              dyu2 = s0[2][o + SX] - s0[2][o - SX];
-        float dzu0 = sp[0][o] - sm[0][o], dzu1 = sp[1][o] - sm[1][o], dzu2 = sp[2][o] - sm[2][o];
-        S[0] = 0.5f * dxu0;
-        S[1] = 0.5f * dyu1;
-        S[2] = 0.5f * dzu2;
-        S[3] = 0.25f * (dyu0 + dxu1);
-        S[4] = 0.25f * (dzu0 + dxu2);
-        S[5] = 0.25f * (dzu1 + dyu2);
+        float S[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, sigma = cell_sigma(a.ph, fl_c[k]);
+        if (!bulk) {
+          float dxu0 = s0[0][o + 1] - s0[0][o - 1], dxu1 = s0[1][o + 1] - s0[1][o - 1], dxu2 = s0[2][o + 1] - s0[2][o - 1];
+          float dyu0 = s0[0][o + SX] - s0[0][o - SX], dyu1 = s0[1][o + SX] - s0[1][o - SX],
+                dyu2 = s0[2][o + SX] - s0[2][o - SX];
+          float dzu0 = sp[0][o] - sm[0][o], dzu1 = sp[1][o] - sm[1][o], dzu2 = sp[2][o] - sm[2][o];
+          S[0] = 0.5f * dxu0;
+          S[1] = 0.5f * dyu1;
+          S[2] = 0.5f * dzu2;
+          S[3] = 0.25f * (dyu0 + dxu1);
+          S[4] = 0.25f * (dzu0 + dxu2);
+          S[5] = 0.25f * (dzu1 + dyu2);
+        }
         if (fl_c[k] & WM_VALID) {  // wall-model strain, sigma = 0 (rare)
           const int64_t c = own_xy + k + nxy * z;
 #pragma unroll

@@ -17,6 +17,7 @@ struct WsArgs {
   const float* wm_u;
   const float* wm_s;
   int zchunk;
+  Boxes fsi;             // FSI region (n = 0: whole lattice); variant 5: blocks outside it take the bulk path
   long long plane_b[Q];  // 4 * i * n                            (byte offsets, warp-uniform)
   long long push_b[Q];   // 4 * (i * n + cx + cy*nx + cz*nx*ny)
 };

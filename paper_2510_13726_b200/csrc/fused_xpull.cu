@@ -23,28 +23,31 @@
 
 namespace hhrr {
 
-namespace xp {
-constexpr int TX = 64, TY = 8, NS = 2, W = TX + 8;
-constexpr int WORKERS = TX * TY / 2, AUX = 96, THREADS = WORKERS + AUX + 32;
-constexpr int SX = TX + 2, SY = TY + 2, PLANE = SX * SY;
-constexpr int HALO = 2 * TX + 2 * TY;
-// one stage, in floats: [27][8][72] tile rows | [27][72] row y0-1 | [27][72] row y0+8 |
-//                       [27][8][4] wrapped columns of the tile rows | [27][4] | [27][4] of the halo rows
-constexpr int MAIN_F = Q * TY * W, ROW_F = Q * W, ROW_PAD_F = 1952, PM_F = Q * TY * 4, PR_F = Q * 4, PR_PAD_F = 128;
-constexpr int O_RM = MAIN_F, O_RP = O_RM + ROW_PAD_F, O_PM = O_RP + ROW_PAD_F, O_PRM = O_PM + PM_F,
-              O_PRP = O_PRM + PR_PAD_F, END_F = O_PRP + PR_PAD_F;
-constexpr uint32_t TMA_BYTES = (MAIN_F + 2 * ROW_F) * 4, TMA_EDGE_BYTES = (PM_F + 2 * PR_F) * 4;
-constexpr int FL_MAIN = 0, FL_YM = TY * TX, FL_YP = FL_YM + TX, FL_XM = FL_YP + TX, FL_XP = FL_XM + TY;
-constexpr uint32_t FLAG_OFF = END_F * 4, STAGE_BYTES = FLAG_OFF + 768;
-constexpr size_t RING_BYTES = 4 * 3 * PLANE * 4;
-constexpr size_t SMEM = (size_t)NS * STAGE_BYTES + RING_BYTES + 64;
-static_assert(FL_XP + TY <= 768 && STAGE_BYTES % 128 == 0, "flag region");
-static_assert((O_RM * 4) % 128 == 0 && (O_RP * 4) % 128 == 0 && (O_PM * 4) % 128 == 0 && (O_PRM * 4) % 128 == 0 &&
-                  (O_PRP * 4) % 128 == 0 && ROW_PAD_F >= ROW_F && PR_PAD_F >= PR_F,
-              "TMA smem alignment");
-static_assert(SMEM <= 227 * 1024, "shared memory");
-// population i = (cx+1) + 3k, k = (cy+1) + 3(cz+1): stride between the members of one cx group
-}  // namespace xp
+// Tile shape TX x TY (512 cells).  128 x 4 is preferred: the box of a tile carries 4 cells of x halo on either
+// side, which cost whole 32-byte sectors that the x neighbour's block reads again (and mostly finds evicted),
+// 2 sectors per 16 with 128-cell rows, 2 per 8 with 64-cell rows.  64 x 8 serves lattices 128 x 4 cannot tile.
+template <int TX_, int TY_>
+struct XpCfg {
+  static constexpr int TX = TX_, TY = TY_, NS = 2, W = TX + 8;
+  static constexpr int WORKERS = TX * TY / 2, AUX = 96, THREADS = WORKERS + AUX + 32;
+  static constexpr int SX = TX + 2, SY = TY + 2, PLANE = SX * SY;
+  static constexpr int HALO = 2 * TX + 2 * TY, HSLOTS = (HALO + AUX - 1) / AUX;
+  // one stage, in floats: [27][TY][W] tile rows | [27][W] row y0-1 | [27][W] row y0+TY |
+  //                       [27][TY][4] wrapped columns of the tile rows | [27][4] | [27][4] of the halo rows
+  static constexpr int pad32(int f) { return (f + 31) / 32 * 32; }  // 128-byte granules (TMA destination)
+  static constexpr int MAIN_F = Q * TY * W, ROW_F = Q * W, ROW_PAD_F = pad32(ROW_F), PM_F = Q * TY * 4,
+                       PM_PAD_F = pad32(PM_F), PR_F = Q * 4, PR_PAD_F = pad32(PR_F);
+  static constexpr int O_RM = pad32(MAIN_F), O_RP = O_RM + ROW_PAD_F, O_PM = O_RP + ROW_PAD_F, O_PRM = O_PM + PM_PAD_F,
+                       O_PRP = O_PRM + PR_PAD_F, END_F = O_PRP + PR_PAD_F;
+  static constexpr uint32_t TMA_BYTES = (MAIN_F + 2 * ROW_F) * 4, TMA_EDGE_BYTES = (PM_F + 2 * PR_F) * 4;
+  static constexpr int FL_MAIN = 0, FL_YM = TY * TX, FL_YP = FL_YM + TX, FL_XM = FL_YP + TX, FL_XP = FL_XM + TY;
+  static constexpr uint32_t FLAG_OFF = END_F * 4, STAGE_BYTES = FLAG_OFF + 896;
+  static constexpr size_t RING_BYTES = 4 * 3 * PLANE * 4;
+  static constexpr size_t SMEM = (size_t)NS * STAGE_BYTES + RING_BYTES + 64;
+  static_assert(WORKERS == 256 && TX % 64 == 0 && TY * TX == 512, "8 worker warps, 2 cells per thread, 32 x 16 B of flags");
+  static_assert(FL_XP + TY <= 896 && STAGE_BYTES % 128 == 0, "flag region");
+  static_assert(SMEM <= 227 * 1024, "shared memory");
+};
 
 namespace {
 
@@ -107,11 +110,18 @@ __device__ __forceinline__ void push_store_yz(const Dom& dm, float* __restrict__
 
 }  // namespace
 
-__global__ void __launch_bounds__(xp::THREADS, 1)
+template <class C>
+__global__ void __launch_bounds__(C::THREADS, 1)
     fused_xpull_kernel(const __grid_constant__ WsArgs a, const __grid_constant__ CUtensorMap map_main,
                        const __grid_constant__ CUtensorMap map_row, const __grid_constant__ CUtensorMap map_pm,
                        const __grid_constant__ CUtensorMap map_pr) {
-  using namespace xp;
+  constexpr int TX = C::TX, TY = C::TY, NS = C::NS, W = C::W, WORKERS = C::WORKERS, AUX = C::AUX, SX = C::SX,
+                PLANE = C::PLANE, HALO = C::HALO, HSLOTS = C::HSLOTS, MAIN_F = C::MAIN_F, PM_F = C::PM_F, O_RM = C::O_RM,
+                O_RP = C::O_RP, O_PM = C::O_PM, O_PRM = C::O_PRM, O_PRP = C::O_PRP, FL_MAIN = C::FL_MAIN, FL_YM = C::FL_YM,
+                FL_YP = C::FL_YP, FL_XM = C::FL_XM;
+  constexpr uint32_t TMA_BYTES = C::TMA_BYTES, TMA_EDGE_BYTES = C::TMA_EDGE_BYTES, FLAG_OFF = C::FLAG_OFF,
+                     STAGE_BYTES = C::STAGE_BYTES;
+  constexpr size_t RING_BYTES = C::RING_BYTES;
   extern __shared__ __align__(128) unsigned char smem[];
   float(*ring)[3][PLANE] = reinterpret_cast<float(*)[3][PLANE]>(smem + (size_t)NS * STAGE_BYTES);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)NS * STAGE_BYTES + RING_BYTES);
@@ -191,17 +201,18 @@ __global__ void __launch_bounds__(xp::THREADS, 1)
       // flag bytes of the same cells: 8 rows x 64 B + 2 halo rows as 16-byte loads, the columns bytewise
       const uint8_t* fz0 = a.flags + nxy * zr;
       unsigned char* flb = stb + FLAG_OFF;
-      const uint4 vmain = __ldg(reinterpret_cast<const uint4*>(fz0 + (x0 + (lane & 3) * 16) + nx * (y0 + (lane >> 2))));
+      constexpr int L16 = TX / 16;  // 16-byte pieces per row; the two halo rows take 2 * L16 <= 16 lanes
+      const uint4 vmain = __ldg(reinterpret_cast<const uint4*>(fz0 + (x0 + (lane % L16) * 16) + nx * (y0 + lane / L16)));
       uint4 vrow = make_uint4(0, 0, 0, 0);
       uint8_t vcol = 0;
-      if (lane < 8) vrow = __ldg(reinterpret_cast<const uint4*>(fz0 + (x0 + (lane & 3) * 16) + nx * ((lane >> 2) ? yp : ym)));
-      if (lane >= 8 && lane < 8 + 2 * TY) {
-        const int h = lane - 8, right = h / TY, row = h % TY;
+      if (lane < 2 * L16) vrow = __ldg(reinterpret_cast<const uint4*>(fz0 + (x0 + (lane % L16) * 16) + nx * ((lane / L16) ? yp : ym)));
+      if (lane >= 16 && lane < 16 + 2 * TY) {
+        const int h = lane - 16, right = h / TY, row = h % TY;
         vcol = __ldg(fz0 + (right ? xr : xl) + nx * (y0 + row));
       }
-      *reinterpret_cast<uint4*>(flb + FL_MAIN + (lane >> 2) * TX + (lane & 3) * 16) = vmain;
-      if (lane < 8) *reinterpret_cast<uint4*>(flb + FL_YM + (lane >> 2) * TX + (lane & 3) * 16) = vrow;
-      if (lane >= 8 && lane < 8 + 2 * TY) flb[FL_XM + (lane - 8)] = vcol;
+      *reinterpret_cast<uint4*>(flb + FL_MAIN + (lane / L16) * TX + (lane % L16) * 16) = vmain;
+      if (lane < 2 * L16) *reinterpret_cast<uint4*>(flb + FL_YM + (lane / L16) * TX + (lane % L16) * 16) = vrow;
+      if (lane >= 16 && lane < 16 + 2 * TY) flb[FL_XM + (lane - 16)] = vcol;
       __syncwarp();
       if (lane == 0) mbar_arrive(bar);
     }
@@ -225,15 +236,18 @@ __global__ void __launch_bounds__(xp::THREADS, 1)
       }
       return;
     }
+    // lane a owns halo cells a, a + AUX, ... (< HALO).  Per cell and per cx group: where population
+    // (cx, k = 0) sits in a stage and the stride to k + 1 (column lx - cx of the wide boxes, or the wrapped
+    // columns at the periodic x boundary)
     const int a0 = tid - WORKERS;
-    int h_off[2][3], h_str[2][3], h_slot[2], h_x[2], h_y[2], h_fl[2];
-    bool h_fy[2], h_on[2];
+    int h_off[HSLOTS][3], h_str[HSLOTS][3], h_slot[HSLOTS], h_x[HSLOTS], h_y[HSLOTS], h_fl[HSLOTS];
+    bool h_fy[HSLOTS], h_on[HSLOTS];
 #pragma unroll
-    for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < HSLOTS; ++k) {
       const int hc = a0 + k * AUX;
       h_on[k] = hc < HALO;
       h_fy[k] = false;
-      int lx, region, row = 0;  // region 0: tile rows, 1: row y0-1, 2: row y0+8
+      int lx, region, row = 0;  // region 0: tile rows, 1: row y0-1, 2: row y0+TY
       if (hc < 2 * TX) {
         const int top = hc / TX;
         lx = hc % TX;
@@ -284,7 +298,7 @@ __global__ void __launch_bounds__(xp::THREADS, 1)
       if (it >= 2) pub_wait(pub0, it - 2);
       mbar_wait(full0 + 8 * s, k2 & 1);
 #pragma unroll
-      for (int k = 0; k < 2; ++k) {
+      for (int k = 0; k < HSLOTS; ++k) {
         if (!h_on[k]) continue;
         float f[Q];
 #pragma unroll
@@ -473,35 +487,55 @@ static bool make_map(CUtensorMap* m, const float* base, const Dom& dm, uint32_t 
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+template <class C>
+static bool shape_tiles(const Dom& dm) {
+  return dm.nx % C::TX == 0 && dm.nx >= 2 * C::TX && dm.ny % C::TY == 0;
+}
+using XpWide = XpCfg<128, 4>;
+using XpTall = XpCfg<64, 8>;
+
 bool xpull_supported(const Dom& dm) {
-  return dm.nx % xp::TX == 0 && dm.nx >= 2 * xp::TX && dm.ny % xp::TY == 0 && dm.mode[0] == HHRR_PERIODIC &&
-         encode_fn() != nullptr;
+  return (shape_tiles<XpWide>(dm) || shape_tiles<XpTall>(dm)) && dm.mode[0] == HHRR_PERIODIC && encode_fn() != nullptr;
 }
 
-cudaError_t launch_fused_xpull(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo) {
+template <class C>
+static cudaError_t launch_shape(hhrr_lattice* L, WsArgs& a) {
   const Dom& dm = L->dom;
-  if (!dm.xs || !xpull_supported(dm)) return cudaErrorNotSupported;
   CUtensorMap m_main, m_row, m_pm, m_pr;
-  if (!make_map(&m_main, L->fA, dm, xp::W, xp::TY) || !make_map(&m_row, L->fA, dm, xp::W, 1) ||
-      !make_map(&m_pm, L->fA, dm, 4, xp::TY) || !make_map(&m_pr, L->fA, dm, 4, 1))
+  if (!make_map(&m_main, L->fA, dm, C::W, C::TY) || !make_map(&m_row, L->fA, dm, C::W, 1) ||
+      !make_map(&m_pm, L->fA, dm, 4, C::TY) || !make_map(&m_pr, L->fA, dm, 4, 1))
     return cudaErrorNotSupported;
-  WsArgs a;
-  fill_ws_args(L, ph, bo, a);
-  for (int i = 0; i < Q; ++i)  // y and z moves only: the x move is taken on the read side
-    a.push_b[i] = 4LL * ((long long)i * dm.n + (long long)dir_cy(i) * dm.nx + (long long)dir_cz(i) * dm.nx * dm.ny);
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(fused_xpull_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xp::SMEM);
+    cudaError_t e = cudaFuncSetAttribute(fused_xpull_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
   int nch = ws_zchunks(dm.nz);
   a.zchunk = (dm.nz + nch - 1) / nch;
   nch = (dm.nz + a.zchunk - 1) / a.zchunk;
-  dim3 grid(dm.nx / xp::TX, dm.ny / xp::TY, nch);
-  fused_xpull_kernel<<<grid, xp::THREADS, xp::SMEM, L->stream>>>(a, m_main, m_row, m_pm, m_pr);
+  dim3 grid(dm.nx / C::TX, dm.ny / C::TY, nch);
+  fused_xpull_kernel<C><<<grid, C::THREADS, C::SMEM, L->stream>>>(a, m_main, m_row, m_pm, m_pr);
   L->launches++;
   return cudaGetLastError();
+}
+
+cudaError_t launch_fused_xpull(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo) {
+  const Dom& dm = L->dom;
+  if (!dm.xs || !xpull_supported(dm)) return cudaErrorNotSupported;
+  WsArgs a;
+  fill_ws_args(L, ph, bo, a);
+  for (int i = 0; i < Q; ++i)  // y and z moves only: the x move is taken on the read side
+    a.push_b[i] = 4LL * ((long long)i * dm.n + (long long)dir_cy(i) * dm.nx + (long long)dir_cz(i) * dm.nx * dm.ny);
+  // Blocks that need the y halo rows (the FD strain) do better with 64 x 8 tiles (2 halo rows per 8), bulk
+  // blocks (region split) with 128 x 4 (fewer x-halo sectors re-read): measured on config 5,
+  // 4.06 / 4.39 ms without the split and 4.16 / 3.98 ms with it.  HHRR_XPULL_SHAPE=tall|wide: tuning runs only.
+  bool wide = shape_tiles<XpWide>(dm) && (a.fsi.n > 0 || !shape_tiles<XpTall>(dm));
+  if (const char* shape = getenv("HHRR_XPULL_SHAPE")) {
+    if (shape[0] == 't' && shape_tiles<XpTall>(dm)) wide = false;
+    if (shape[0] == 'w' && shape_tiles<XpWide>(dm)) wide = true;
+  }
+  return wide ? launch_shape<XpWide>(L, a) : launch_shape<XpTall>(L, a);
 }
 
 }  // namespace hhrr

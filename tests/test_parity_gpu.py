@@ -156,31 +156,35 @@ def _xpull_lattice(case):
     return G
 
 
-def test_xpull_periodic_noise(oracle):
-    """Three x tiles, two y tiles, several planes: the periodic x boundary columns, tile seams."""
-    rho, u = I.noisy_uniform(192, 16, 11, (0.03, -0.02, 0.01), 5e-3, 78)
-    case = I.Case("xpull", 192, 16, 11, 10, params=dict(I.DEFAULTS, tau0=0.53), rho=rho, u=u, with_neq=True)
+@pytest.mark.parametrize("ext", [(192, 16, 11), (384, 12, 11)])
+def test_xpull_periodic_noise(oracle, ext):
+    """Three x tiles, several y tiles and planes: the periodic x boundary columns, tile seams.  192 x 16 runs
+    the 64 x 8 tile shape, 384 x 12 the 128 x 4 one (which config 5 uses)."""
+    rho, u = I.noisy_uniform(*ext, (0.03, -0.02, 0.01), 5e-3, 78)
+    case = I.Case("xpull", *ext, 10, params=dict(I.DEFAULTS, tau0=0.53), rho=rho, u=u, with_neq=True)
     _xpull_lattice(case).close()
     run_parity(oracle, case, 10, 5, TOL10)
 
 
-def test_xpull_mirror_yz(oracle):
-    """Mirror planes in y and z under x-pull storage (x stays periodic: the storage needs it)."""
-    rho, u = I.noisy_uniform(128, 16, 9, (0.01, 0.0, 0.0), 1e-2, 10)
-    case = I.Case("xpull-mirror", 128, 16, 9, 10, mode=(I.PERIODIC, I.MIRROR, I.MIRROR),
+@pytest.mark.parametrize("ext", [(128, 16, 9), (256, 12, 9)])
+def test_xpull_mirror_yz(oracle, ext):
+    """Mirror planes in y and z under x-pull storage (x stays periodic: the storage needs it); both tile shapes."""
+    rho, u = I.noisy_uniform(*ext, (0.01, 0.0, 0.0), 1e-2, 10)
+    case = I.Case("xpull-mirror", *ext, 10, mode=(I.PERIODIC, I.MIRROR, I.MIRROR),
                   params=dict(I.DEFAULTS, tau0=0.56), rho=rho, u=u, with_neq=True)
     _xpull_lattice(case).close()
     run_parity(oracle, case, 10, 5, TOL10)
 
 
-def test_xpull_channel_and_rotor(oracle):
-    """Config 3 and config 4 recipes at extents variant 5 tiles itself: wall model and forces read the
-    x-pulled populations; geometry and wall list stay bit-exact."""
-    case = I.case_channel(128, 48, 16, 30)
+@pytest.mark.parametrize("nx", [128, 256])
+def test_xpull_channel_and_rotor(oracle, nx):
+    """Config 3 and config 4 recipes at extents variant 5 tiles itself (nx = 128: 64 x 8 tiles, 256: 128 x 4):
+    wall model and forces read the x-pulled populations; geometry and wall list stay bit-exact."""
+    case = I.case_channel(nx, 48, 16, 30)
     _xpull_lattice(case).close()
     run_parity(oracle, case, 10, 5, TOL10, check_every=1)
     run_parity(oracle, case, 30, 5, TOL_LONG, check_every=15, force_tol=TOL_LONG)
-    case = I.case_rotor(128, 72, 72, 20.0, 12, omega=0.012)
+    case = I.case_rotor(nx, 72, 72, 20.0, 12, omega=0.012)
     _xpull_lattice(case).close()
     run_parity(oracle, case, 12, 5, TOL10, check_every=1)
 
@@ -214,6 +218,9 @@ def test_region_split_rotor_and_sphere(oracle, variant):
     run_parity(oracle, case, 12, variant, TOL10, check_every=3)
     case = I.with_region_split(I.case_sphere(128, 32, 32, 5.0, 10))
     run_parity(oracle, case, 10, variant, TOL10, check_every=5)
+    if variant == 5:    # 128 x 4 tiles: bulk blocks beside FSI blocks
+        case = I.with_region_split(I.case_rotor(384, 72, 72, 20.0, 8, omega=0.012), margin=3)
+        run_parity(oracle, case, 8, variant, TOL10, check_every=4)
 
 
 def test_region_split_channel_and_all_bulk(oracle):
@@ -242,12 +249,13 @@ def test_region_split_violation_is_reported():
     G.close()
 
 
-@pytest.mark.parametrize("variant", [2, 4, 5])
+@pytest.mark.parametrize("variant", [2, 4, 5, 5256])
 def test_fused_kernels_are_deterministic(variant):
     """Two identical lattices stay bitwise identical: every step is a deterministic function of the
     state (R19).  A race between the warps of a fused kernel (ring slots, pipeline stages,
     barrier phases at the start of a z-chunk) shows up here long before it exceeds a parity tolerance."""
-    case = I.case_rotor(128, 72, 72, 20.0, 6, omega=0.012)
+    nx, variant = (256, 5) if variant == 5256 else (128, variant)      # 5256: variant 5 with 128 x 4 tiles
+    case = I.case_rotor(nx, 72, 72, 20.0, 6, omega=0.012)
     A, Bv = _gpu_lattice(case, variant), _gpu_lattice(case, variant)
     for _ in range(3):
         A.step(2); Bv.step(2)

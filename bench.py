@@ -255,6 +255,30 @@ def run_ours(args, rank, world, local_rank):
            "what": "hhrr_set_populations(pinned host) + hhrr_step + hhrr_get_moments(pinned host) + hhrr_get_forces"}
     thrust = float(F[-1, 1:5, 0].sum()) if case.rotor is not None else None
 
+    # the same workload with the paper's bulk / FSI region split (Listing 2): reported beside the
+    # headline, which keeps HHRRLBM in every cell
+    split = None
+    if not args.region_split and not args.no_region_split_leg and case.fringe is not None:
+        boxes = I.with_region_split(case).fsi_boxes
+        L.set_fsi_region(boxes)
+        L.step(min(args.warmup, 20))
+        barrier()
+        L.set_timing(True)
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record(L.stream)
+        L.step(args.steps)
+        s1.record(L.stream)
+        barrier()
+        s_ms = replicas.max_over_ranks(s0.elapsed_time(s1), device=dev)
+        sk_ms, sk_n = L.timing()
+        L.set_timing(False)
+        L.check_finite()
+        split = {"value": replicas.aggregate_mlups(n, args.steps, s_ms, world), "unit": "MLUPs",
+                 "ms_per_step": s_ms / args.steps, "kernel_ms": sk_ms / max(1, sk_n),
+                 "kernel_frac_of_peak": n * BYTES_PER_CELL / (sk_ms / max(1, sk_n) * 1e-3) / 1e9 / measured_peak()[0],
+                 "fsi_boxes": [list(map(int, b)) for b in boxes],
+                 "what": "bulk RRLBM-LES (PAPER.md:215, Listing 2) outside the boxes, HHRRLBM + wall model inside"}
+
     if rank == 0:
         peak, peak_src = measured_peak()
         k_avg_ms = k_ms / max(1, k_n)
@@ -264,12 +288,13 @@ def run_ours(args, rank, world, local_rank):
                     "peak_source": peak_src, "kernel_ms": k_avg_ms, "kernel_launches_timed": k_n,
                     "kernel_share_of_step": k_ms / (ms * k_n / args.steps) if k_n else None,
                     "algorithmic_bytes_per_cell": BYTES_PER_CELL}
-        tr = ROOT / "profiles" / "r01_traffic.txt"   # DRAM bytes per launch from the committed ncu capture
+        tr = ROOT / "profiles" / "r01_traffic.txt"   # DRAM bytes per launch from the committed ncu captures
         if tr.exists():
             try:
-                t = json.loads(tr.read_text())
-                if t.get("cells") == n and t.get("variant") == args.variant:
-                    roofline["traffic"] = t["dram_bytes_per_launch"]
+                for t in json.loads(tr.read_text()):
+                    if (t.get("cells") == n and t.get("variant") == args.variant
+                            and bool(t.get("region_split")) == bool(args.region_split)):
+                        roofline["traffic"] = t["dram_bytes_per_launch"]
             except Exception:
                 pass
         cpu = None
@@ -283,7 +308,7 @@ def run_ours(args, rank, world, local_rank):
                            "l2": "inputs (11.6 GB per buffer) exceed the 126 MB L2; no flush needed"},
                 "hbm_frac_of_peak_step": value * 1e6 * BYTES_PER_CELL / 1e9 / peak / world,
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
-                "clocks": clocks, "thrust_last_step": thrust}
+                "clocks": clocks, "thrust_last_step": thrust, "region_split": split}
         print(json.dumps(line), flush=True)
     L.close()
     if world > 1:
@@ -299,6 +324,7 @@ def main():
     ap.add_argument("--variant", type=int, default=5, choices=[0, 1, 2, 3, 4, 5] + list(range(11, 50)))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-region-split-leg", action="store_true", help="skip the extra region-split measurement")
     ap.add_argument("--region-split", action="store_true",
                     help="the paper's bulk / FSI region split (PAPER.md:215); default: HHRRLBM in every cell")
     args = ap.parse_args()

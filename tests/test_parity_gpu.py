@@ -290,15 +290,20 @@ def test_variants_agree_bitwise_on_moments_order():
     assert e_rho <= 1e-6 and e_v <= 1e-5, (e_rho, e_v)
 
 
-def test_config5_full_size_sampled_cells(oracle):
+@pytest.mark.parametrize("split", [False, True])
+def test_config5_full_size_sampled_cells(oracle, split):
     """BASELINE.json config 5 at FULL size (768x384x364, rotor R=120) in the launch configuration
     bench.py times (default kernel variant).  The oracle cannot step 107 M cells in a test, so one
     whole time step is checked on sampled cells it can compute one by one: for each sample the
     oracle's single-cell collision (ohrr_collide_cell) is fed the GPU's pre-step populations of the
     cell and of its six face neighbours (for S^FD), and its 27 post-collision values are compared
     with what the GPU stored at the 27 push targets.  Samples cover bulk fluid, tile / z-chunk
-    seams, the inflow fringe, growth, frontier (with and without wall-model state) and solid cells."""
+    seams, the inflow fringe, growth, frontier (with and without wall-model state) and solid cells.
+    split = True: the same with the paper's bulk / FSI region split (bench.py's region_split leg: 128 x 4
+    tiles, bulk blocks beside FSI blocks); samples then also sit on both sides of every face of the boxes."""
     case = I.baseline_config(5)
+    if split:
+        case = I.with_region_split(case)
     G = _gpu_lattice(case, 5)               # the default variant: what bench.py times
     assert G.population_storage() == 1
     G.step(2)
@@ -312,6 +317,13 @@ def test_config5_full_size_sampled_cells(oracle):
         for y in (0, 7, 8, 191, 192, ny - 1):               # tile seams in y
             for z in (0, 22, 23, 24, 25, 181, nz - 1):      # z-chunk seams
                 samples.add(x + nx * (y + ny * z))
+    if split:
+        for (bx0, bx1, by0, by1, bz0, bz1) in case.fsi_boxes:   # both sides of the faces of the FSI boxes
+            for x in {max(bx0 - 1, 0), bx0, bx1 - 1, min(bx1, nx - 1)}:
+                for y in {max(by0 - 1, 0), by0, (by0 + by1) // 2, by1 - 1, min(by1, ny - 1)}:
+                    for z in {max(bz0 - 1, 0), bz0, (bz0 + bz1) // 2, bz1 - 1, min(bz1, nz - 1)}:
+                        samples.add(x + nx * (y + ny * z))
+        assert np.count_nonzero(types == 5) > 0.9 * n
     for t in (1, 2, 3):                                     # growth, frontier, solid cells of the rotor
         idx = np.flatnonzero(types == t)
         assert idx.size > 0
@@ -358,7 +370,7 @@ def test_config5_full_size_sampled_cells(oracle):
     for k, c in enumerate(samples):
         c = int(c)
         f, d, uB, valid = state(c)
-        sigma = sig
+        sigma = 1.0 if types[c] == 5 else sig              # BULK cells: Listing 2, Eq. 7 at sigma = 1 (R20)
         if valid:
             wm_valid_seen += 1
             _, _, uwm, s = G.wall_state(c)

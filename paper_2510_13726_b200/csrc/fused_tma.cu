@@ -495,7 +495,7 @@ cudaError_t launch_fused_tma(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  int nch = ws_zchunks(dm.nz);
+  int nch = ws_zchunks(dm.nz, 19);
   a.zchunk = (dm.nz + nch - 1) / nch;
   nch = (dm.nz + a.zchunk - 1) / a.zchunk;
   dim3 grid(dm.nx / tma::TX, dm.ny / tma::TY, nch);

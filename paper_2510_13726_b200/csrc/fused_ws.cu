@@ -225,7 +225,7 @@ static cudaError_t launch_ws_cfg(hhrr_lattice* L, const WsArgs& a0) {
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  int nch = ws_zchunks(dm.nz);
+  int nch = ws_zchunks(dm.nz, 19);
   a.zchunk = (dm.nz + nch - 1) / nch;
   nch = (dm.nz + a.zchunk - 1) / a.zchunk;
   dim3 grid((dm.nx + TX - 1) / TX, (dm.ny + TY - 1) / TY, nch);
@@ -257,8 +257,8 @@ void fill_ws_args(const hhrr_lattice* L, const PhysF& ph, const BodiesF& bo, WsA
 // all SMs work on one slab of the lattice at a time and a tile's halo rows are still in L2 when its
 // neighbour tile loads them; long chunks let neighbouring blocks drift apart (measured: 6.3 ms at 2
 // chunks vs 5.6 ms at 16 on 768x384x364).  Cost: two extra planes loaded per chunk.
-int ws_zchunks(int nz) {
-  int nch = (nz + 9) / 19;  // ~19 planes per chunk: measured optimum on config 5 (profiles/)
+int ws_zchunks(int nz, int planes) {  // ~planes planes per chunk: measured optima on config 5 (profiles/)
+  int nch = (nz + planes / 2) / planes;
   if (nch < 1) nch = 1;
   if (const char* e = getenv("HHRR_ZCHUNKS")) nch = atoi(e) < 1 ? 1 : atoi(e);  // tuning runs only
   return nch;

@@ -257,7 +257,7 @@ static cudaError_t launch_ws2_cfg(hhrr_lattice* L, const WsArgs& a0) {
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  int nch = ws_zchunks(dm.nz);
+  int nch = ws_zchunks(dm.nz, 19);
   a.zchunk = (dm.nz + nch - 1) / nch;
   nch = (dm.nz + a.zchunk - 1) / a.zchunk;
   dim3 grid((dm.nx + TX - 1) / TX, (dm.ny + TY - 1) / TY, nch);

@@ -129,8 +129,15 @@ __global__ void __launch_bounds__(C::THREADS, 1)
 
   const Dom& dm = a.dm;
   const int tid = threadIdx.x;
-  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
-  const int z0 = blockIdx.z * a.zchunk, z1 = min(dm.nz, z0 + a.zchunk);
+  // Launch order: the tiles come in groups of a.group (one per SM); a group's blocks are ordered chunk by
+  // chunk, so the block that takes chunk c+1 of a tile starts as the one that took chunk c ends -- the two
+  // halo planes the chunks share are then still in L2 instead of being read from DRAM a second time.
+  const int ntx = dm.nx / TX, ntiles = ntx * (dm.ny / TY);
+  const int per_group = a.group * a.nch, grp = blockIdx.x / per_group, rem = blockIdx.x - grp * per_group;
+  const int gsize = min(a.group, ntiles - grp * a.group);  // the last group may be short
+  const int chunk = rem / gsize, tile = grp * a.group + (rem - chunk * gsize);
+  const int x0 = (tile % ntx) * TX, y0 = (tile / ntx) * TY;
+  const int z0 = chunk * a.zchunk, z1 = min(dm.nz, z0 + a.zchunk);
   const int64_t n = dm.n, nx = dm.nx, nxy = (int64_t)dm.nx * dm.ny;
   // Region split (Listing 2; R20): a block none of whose cells lies in an FSI box
   // holds BULK cells only -- sigma = 1, d = 1, no wall model -- so its collision is purely local: it loads
@@ -511,10 +518,21 @@ static cudaError_t launch_shape(hhrr_lattice* L, WsArgs& a) {
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  int nch = ws_zchunks(dm.nz);
+  // with the grouped launch order the halo planes of a chunk are L2 hits: 22 planes without, 16 with the region split
+  int nch = ws_zchunks(dm.nz, a.fsi.n > 0 ? 16 : 22);
   a.zchunk = (dm.nz + nch - 1) / nch;
   nch = (dm.nz + a.zchunk - 1) / a.zchunk;
-  dim3 grid(dm.nx / C::TX, dm.ny / C::TY, nch);
+  static int sms = 0;
+  if (!sms) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) sms = 148;
+  }
+  a.nch = nch;
+  a.group = sms;  // one tile per SM and wave (one block per SM: shared memory)
+  if (const char* e = getenv("HHRR_XPULL_GROUP")) a.group = atoi(e) < 1 ? 1 : atoi(e);  // tuning runs only
+  const int ntiles = (dm.nx / C::TX) * (dm.ny / C::TY);
+  dim3 grid((unsigned)(ntiles * nch));
   fused_xpull_kernel<C><<<grid, C::THREADS, C::SMEM, L->stream>>>(a, m_main, m_row, m_pm, m_pr);
   L->launches++;
   return cudaGetLastError();

@@ -17,6 +17,7 @@ struct WsArgs {
   const float* wm_u;
   const float* wm_s;
   int zchunk;
+  int nch, group;        // variant 5: z-chunks per tile column; tiles per launch-order group (see fused_xpull.cu)
   Boxes fsi;             // FSI region (n = 0: whole lattice); variant 5: blocks outside it take the bulk path
   long long plane_b[Q];  // 4 * i * n                            (byte offsets, warp-uniform)
   long long push_b[Q];   // 4 * (i * n + cx + cy*nx + cz*nx*ny)
@@ -53,6 +54,6 @@ __device__ __forceinline__ void solid_state_ws(const WsArgs& a, uint8_t fl, int6
 }
 
 void fill_ws_args(const hhrr_lattice* L, const PhysF& ph, const BodiesF& bo, WsArgs& a);
-int ws_zchunks(int nz);
+int ws_zchunks(int nz, int planes);
 
 }  // namespace hhrr

@@ -254,6 +254,12 @@ def run_ours(args, rank, world, local_rank):
            "steps": e2e_steps, "ms_total": e2e_ms,
            "what": "hhrr_set_populations(pinned host) + hhrr_step + hhrr_get_moments(pinned host) + hhrr_get_forces"}
     thrust = float(F[-1, 1:5, 0].sum()) if case.rotor is not None else None
+    # Definition 3 / Eq. 26: C_T = T / (0.5 rho pi r^2 U_inf^2), lattice units, rho = 1;
+    # after a few hundred steps from rest it is a start-up value, not the converged one of the paper's Fig. 7
+    c_t = None
+    if thrust is not None and case.fringe is not None:
+        r_rot = 0.5 * (case.rotor["sdf"].shape[1] - 1) * case.rotor["spacing"] - 4.0   # grid half-extent minus its 4-cell margin
+        c_t = thrust / (0.5 * np.pi * r_rot ** 2 * case.fringe[2][0] ** 2)
 
     # the same workload with the paper's bulk / FSI region split (Listing 2): reported beside the
     # headline, which keeps HHRRLBM in every cell
@@ -308,7 +314,8 @@ def run_ours(args, rank, world, local_rank):
                            "l2": "inputs (11.6 GB per buffer) exceed the 126 MB L2; no flush needed"},
                 "hbm_frac_of_peak_step": value * 1e6 * BYTES_PER_CELL / 1e9 / peak / world,
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
-                "clocks": clocks, "thrust_last_step": thrust, "region_split": split}
+                "clocks": clocks, "thrust_last_step": thrust, "thrust_coefficient_last_step": c_t,
+                "region_split": split}
         print(json.dumps(line), flush=True)
     L.close()
     if world > 1:

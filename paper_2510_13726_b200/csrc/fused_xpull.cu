@@ -489,8 +489,14 @@ static bool make_map(CUtensorMap* m, const float* base, const Dom& dm, uint32_t 
   cuuint64_t gstr[3] = {(cuuint64_t)dm.nx * 4, (cuuint64_t)dm.nx * dm.ny * 4, (cuuint64_t)dm.n * 4};
   cuuint32_t box[4] = {bx, by, 1, (cuuint32_t)Q};
   cuuint32_t estr[4] = {1, 1, 1, 1};
+  CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_256B;  // measured: 0.5-1 % faster than 128 B, 64 B slower
+  if (const char* e = getenv("HHRR_TMA_PROMO")) {  // tuning runs only
+    promo = atoi(e) == 0 ? CU_TENSOR_MAP_L2_PROMOTION_NONE
+                         : (atoi(e) == 64 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B
+                                          : (atoi(e) == 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : promo));
+  }
   return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<float*>(base), gdim, gstr, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 

@@ -6,15 +6,18 @@
 // streaming shift of Eq. 6 is paid:
 //   * plane i of the buffer holds g_i(x,y,z) = f*_i(x, y - c_iy, z - c_iz): the post-collision value
 //     already moved along y and z (whole, 128-byte aligned rows) but not yet along x;
-//   * the x shift happens on the read side, in shared memory: the TMA box of a tile is 72 cells wide
-//     (4 + 64 + 4), population i of cell x is read at column x - c_ix.
+//   * the x shift happens on the read side, in shared memory: the TMA box of a TX-wide tile is TX + 8 cells
+//     wide (4 + TX + 4: box starts must be 16-byte aligned), population i of cell x is read at column x - c_ix.
 // Every global store of the kernel is therefore an aligned, full-sector 8-byte store of two x-adjacent
-// cells (27 per thread and plane instead of 45 partly half-filled ones), and the 72-wide box carries
-// the x halo of the tile for free.  Tiles at the periodic x boundary get three small extra boxes (the
-// 4 wrapped columns) which only their edge lanes read.
+// cells (27 per thread and plane instead of 45 partly half-filled ones), and the wide box carries the x
+// halo of the tile.  Tiles at the periodic x boundary get three small extra boxes (the 4 wrapped columns)
+// which only their edge lanes read.
 //
-// Needs nx % 64 == 0, nx >= 128, ny % 8 == 0 and a periodic x axis (xpull_supported); other lattices
-// keep post-stream storage and run variant 2.
+// Region split (Listing 2; R20): a block with no cell in an FSI box takes the bulk
+// path of the same code -- no halo rows, no flag bytes, no overlap planes, no uhat ring.
+//
+// Tile 64 x 8 (nx % 64 == 0, nx >= 128, ny % 8 == 0) or 128 x 4 (nx % 128 == 0, nx >= 256, ny % 4 == 0), periodic
+// x axis (xpull_supported); other lattices keep post-stream storage and run variant 2.
 #include <cuda.h>
 
 #include <cstdlib>

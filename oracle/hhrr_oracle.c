@@ -100,6 +100,7 @@ typedef struct ohrr_lattice {
   int n_fsi;
   int32_t fsi[MAX_FSI_BOXES][6];
   int region_violation; /* a cell that is not plain fluid was found outside every box */
+  int wall_function;    /* 0: truncated Spalding (the paper's, Eq. 18); 1: Musker's profile (BASELINE.json config 3) */
 } ohrr_lattice;
 
 /* ---------------------------------------------------------------- lattice tables */
@@ -267,6 +268,45 @@ static double spalding_df(double utau, double U, double y, double nu, double kap
   double up = U / utau, k = kappa * up;
   return -(U / (utau * utau)) * (1.0 + (kappa / E) * (exp(k) - 1.0 - k - 0.5 * k * k)) - y / nu;
 }
+/* Musker's explicit law of the wall (A. J. Musker, AIAA J. 17 (1979) 655): the closed-form integral of
+ * du+/dy+ = (kappa + C y+^2) / (kappa + C y+^2 + C kappa y+^3), kappa = 0.41, C = 0.001093,
+ *   u+(y+) = 5.424 atan((2 y+ - 8.15)/16.7) + log10((y+ + 10.6)^9.6 / (y+^2 - 8.15 y+ + 86)^2) - 3.52.
+ * Alternative wall function named by BASELINE.json ("Spalding/Musker", config 3); the paper
+ * itself uses Spalding only.  Residual in the same form as Eq. 18: f(u_tau) = U/u_tau - u+(y u_tau/nu).  */
+double ohrr_musker_uplus(double yp) {
+  return 5.424 * atan((2.0 * yp - 8.15) / 16.7) +
+         log10(pow(yp + 10.6, 9.6) / ((yp * yp - 8.15 * yp + 86.0) * (yp * yp - 8.15 * yp + 86.0))) - 3.52;
+}
+static double musker_duplus(double yp) {
+  double a = (2.0 * yp - 8.15) / 16.7;
+  return 5.424 * (2.0 / 16.7) / (1.0 + a * a) +
+         (9.6 / (yp + 10.6) - 2.0 * (2.0 * yp - 8.15) / (yp * yp - 8.15 * yp + 86.0)) / log(10.0);
+}
+double ohrr_musker_f(double utau, double U, double y, double nu) { return U / utau - ohrr_musker_uplus(y * utau / nu); }
+static double musker_df(double utau, double U, double y, double nu) {
+  return -U / (utau * utau) - musker_duplus(y * utau / nu) * y / nu;
+}
+/* the same Newton iteration and stop rule as ohrr_newton_utau (Eq. 19) on Musker's residual */
+double ohrr_newton_utau_musker(double u0, double U, double y, double nu, int max_iter, double tol, int32_t *iters) {
+  double ua = u0, fa = ohrr_musker_f(ua, U, y, nu);
+  int it = 0;
+  double ub = ua;
+  for (it = 0; it < max_iter; ++it) {
+    ub = ua - fa / musker_df(ua, U, y, nu);
+    if (!(ub > 0.0)) ub = 0.5 * ua;
+    double fb = ohrr_musker_f(ub, U, y, nu);
+    double df = fabs(fb - fa);
+    ua = ub;
+    fa = fb;
+    if (df < tol) {
+      ++it;
+      break;
+    }
+  }
+  if (iters) *iters = it;
+  return ub;
+}
+
 /* Newton-Raphson, PAPER.md:177 (Eq. 19), stop rule PAPER.md:184: until
  * |f(u^{j+1}) - f(u^j)| < tol or max_iter iterations.  Safeguard (R9): a step to a
  * non-positive value is replaced by halving.  Returns u_tau; *iters = iterations run. */
@@ -676,8 +716,10 @@ static void wall_model(ohrr_lattice *L) {
         } else {
           double yy = y1 + hs;
           double u0 = (L->wm_valid[c] && L->wm_utau[c] > 0.0) ? L->wm_utau[c] : sqrt(nu * U / yy); /* Eq. 20 */
-          utau = ohrr_newton_utau(u0, U, yy, nu, L->p.kappa, L->p.E, L->p.newton_max_iter,
-                                  L->p.newton_tol, NULL);
+          utau = L->wall_function == 1
+                     ? ohrr_newton_utau_musker(u0, U, yy, nu, L->p.newton_max_iter, L->p.newton_tol, NULL)
+                     : ohrr_newton_utau(u0, U, yy, nu, L->p.kappa, L->p.E, L->p.newton_max_iter,
+                                        L->p.newton_tol, NULL);
           for (int a = 0; a < 3; ++a) L->wm_u[3 * c + a] = utau * ut[a] / U; /* R8 */
           double G[3][3];
           for (int a = 0; a < 3; ++a)
@@ -862,6 +904,12 @@ int ohrr_set_fsi_region(ohrr_lattice *L, int32_t n_boxes, const int32_t *boxes) 
   return 0;
 }
 int ohrr_region_violation(const ohrr_lattice *L) { return L->region_violation; }
+/* 0: truncated Spalding (Eq. 18, the paper's); 1: Musker's profile */
+int ohrr_set_wall_function(ohrr_lattice *L, int kind) {
+  if (kind != 0 && kind != 1) return -1;
+  L->wall_function = kind;
+  return 0;
+}
 
 int ohrr_set_rotor(ohrr_lattice *L, const ohrr_rotor_desc *r) {
   if (!r || r->n_tags < 1 || r->n_tags >= MAX_TAGS) return -1;

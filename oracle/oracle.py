@@ -69,6 +69,12 @@ def lib():
         L.ohrr_spalding_f.argtypes = [C.c_double] * 6
         L.ohrr_newton_utau.restype = C.c_double
         L.ohrr_newton_utau.argtypes = [C.c_double] * 6 + [C.c_int, C.c_double, C.POINTER(C.c_int32)]
+        L.ohrr_musker_uplus.restype = C.c_double
+        L.ohrr_musker_uplus.argtypes = [C.c_double]
+        L.ohrr_musker_f.restype = C.c_double
+        L.ohrr_musker_f.argtypes = [C.c_double] * 4
+        L.ohrr_newton_utau_musker.restype = C.c_double
+        L.ohrr_newton_utau_musker.argtypes = [C.c_double] * 4 + [C.c_int, C.c_double, C.POINTER(C.c_int32)]
         L.ohrr_tau_eff.restype = C.c_double
         L.ohrr_tau_eff.argtypes = [C.c_double, C.c_double, C.c_double, C.c_void_p]
         L.ohrr_get_wall_list.restype = C.c_int64
@@ -129,6 +135,20 @@ def tau_eff(tau0, cs, rho, pi):
 
 def spalding_f(utau, U, y, nu, kappa=0.41, E=9.8):
     return lib().ohrr_spalding_f(utau, U, y, nu, kappa, E)
+
+
+def musker_uplus(yp):
+    return lib().ohrr_musker_uplus(float(yp))
+
+
+def musker_f(utau, U, y, nu):
+    return lib().ohrr_musker_f(float(utau), float(U), float(y), float(nu))
+
+
+def newton_utau_musker(u0, U, y, nu, max_iter=10, tol=1e-4):
+    it = C.c_int32(0)
+    u = lib().ohrr_newton_utau_musker(float(u0), float(U), float(y), float(nu), int(max_iter), float(tol), C.byref(it))
+    return u, it.value
 
 
 def newton_utau(u0, U, y, nu, kappa=0.41, E=9.8, max_iter=10, tol=1e-4):
@@ -201,6 +221,10 @@ class Lattice:
         rc = lib().ohrr_set_fsi_region(self._h, int(b.shape[0]), _p(b) if b.size else None)
         if rc:
             raise RuntimeError("ohrr_set_fsi_region failed")
+
+    def set_wall_function(self, kind):
+        if lib().ohrr_set_wall_function(self._h, int(kind)):
+            raise RuntimeError("ohrr_set_wall_function failed")
 
     def region_violation(self):
         return bool(lib().ohrr_region_violation(self._h))

@@ -570,3 +570,65 @@ def test_bulk_region_interface_is_seamless(oracle):
     far = slice(8 + steps + 1, n - steps - 1)            # bulk cells no hybrid cell has reached yet
     assert np.max(np.abs(split[:, :, :, far] - allb[:, :, :, far])) <= 1e-16
     assert np.max(np.abs(split[:, :, :, 0:8] - allb[:, :, :, 0:8])) > 1e-9
+
+
+# ------------------------------------------------------------------ Musker's wall function (BASELINE.json config 3)
+def test_musker_profile_limits_and_ode(oracle):
+    """Musker's explicit profile: no slip (u+ -> 0, du+/dy+ -> 1 at the wall), log law u+ -> ln(y+)/0.411 + 5.0 far
+    from it, monotone, and its slope follows Musker's eddy-viscosity ODE du+/dy+ = (k + C y^2)/(k + C y^2 + C k y^3),
+    k = 0.41, C = 0.001093 (the explicit form is that ODE integrated with rounded constants: 1 % agreement)."""
+    M = oracle.musker_uplus
+    assert abs(M(0.0)) < 0.02
+    assert abs((M(1e-3) - M(0.0)) / 1e-3 - 1.0) < 2e-3
+    for yp in (3e3, 1e4, 1e5):
+        assert abs(M(yp) - (np.log(yp) / 0.4112 + 5.0)) < 0.03
+    ys = np.logspace(-2, 5, 400)
+    u = np.array([M(y) for y in ys])
+    assert np.all(np.diff(u) > 0)
+    for yp in (0.5, 2.0, 5.0, 11.0, 30.0, 100.0, 1000.0):
+        h = 1e-4 * yp
+        slope = (M(yp + h) - M(yp - h)) / (2 * h)
+        ode = (0.41 + 0.001093 * yp ** 2) / (0.41 + 0.001093 * yp ** 2 + 0.001093 * 0.41 * yp ** 3)
+        assert abs(slope / ode - 1) < 0.012, (yp, slope, ode)
+    # between the two laws: the buffer layer value every law of the wall passes through (u+ ~ 13.2 at y+ = 30)
+    assert 12.5 < M(30.0) < 14.0
+
+
+@pytest.mark.parametrize("U,y,nu", [(0.05, 2.75, 3.156e-4), (0.04, 3.0, 6.25e-5), (1e-4, 2.2, 1e-2), (0.2, 2.9, 1.3e-4)])
+def test_musker_newton_satisfies_its_relation(oracle, U, y, nu):
+    """Converged Newton (Eq. 19 run long) on Musker's residual: U/u_tau = u+(y u_tau/nu) to 1e-12; close to Spalding's
+    u_tau for the same sample (two fits of the same law of the wall)."""
+    u0 = np.sqrt(nu * U / y)
+    ut, it = oracle.newton_utau_musker(u0, U, y, nu, max_iter=200, tol=0.0)
+    assert ut > 0
+    assert abs(U / ut - oracle.musker_uplus(y * ut / nu)) <= 1e-12 * max(1.0, U / ut)
+    us, _ = oracle.newton_utau(u0, U, y, nu, max_iter=200, tol=0.0)
+    assert abs(ut / us - 1) < 0.08
+    # the paper's stop rule applies unchanged
+    ut10, it10 = oracle.newton_utau_musker(u0, U, y, nu, max_iter=10, tol=1e-4)
+    assert 1 <= it10 <= 10
+
+
+def test_wall_model_with_musker_profile_on_uniform_flow(oracle):
+    """WallModelO with the wall function switched to Musker's profile: over a flat wall in a uniform stream the stored
+    u_tau is the Newton solution of U/u_tau = u+_Musker((y1 + h_s) u_tau/nu), everything else (projection, slip
+    direction, zero strain) as with Spalding's law."""
+    from paper_2510_13726_b200 import inputs
+    nx, ny, nz = 4, 12, 4
+    n = nx * ny * nz
+    phi = inputs.wall_phi(nx, ny, nz, 1.25)
+    tau0 = 0.5 + 3 * 6.25e-5
+    nu = (tau0 - 0.5) / 3
+    V = np.array([0.05, 0.004, -0.02])
+    L = oracle.Lattice(oracle.make_params(nx, ny, nz, mode=(0, 1, 0), tau0=tau0, sampling_distance=2.0))
+    L.set_static_geometry(phi, np.ones(n, np.uint8)); L.enable_wall_model(True); L.set_wall_function(1)
+    L.init_equilibrium(np.ones(n), np.tile(V[:, None], (1, n)), False)
+    L.wall_model_only()
+    idx, _, _, valid = L.wall_list()
+    assert np.all(valid == 1)
+    Vt = np.array([V[0], 0, V[2]]); U = np.linalg.norm(Vt)
+    ok, utau, uwm, swm = L.wall_state(int(idx[0]))
+    expect, _ = oracle.newton_utau_musker(np.sqrt(nu * U / 2.75), U, 2.75, nu)
+    spal, _ = oracle.newton_utau(np.sqrt(nu * U / 2.75), U, 2.75, nu)
+    assert utau == pytest.approx(expect, rel=1e-13) and abs(utau - spal) > 1e-6 * spal
+    assert np.allclose(uwm, utau * Vt / U, atol=1e-15) and np.allclose(swm, 0, atol=1e-14)

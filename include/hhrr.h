@@ -140,6 +140,11 @@ int hhrr_set_fringe(hhrr_lattice* L, int32_t x_begin, int32_t x_end, const doubl
  * frontier, growth, fringe) must lie inside a box: if one does not, its type is kept and
  * hhrr_check_finite returns HHRR_E_STATE.  n_boxes = 0 (default): HHRRLBM everywhere.          */
 int hhrr_set_fsi_region(hhrr_lattice* L, int32_t n_boxes, const hhrr_box* boxes);
+/* Wall function solved by the wall model: 0 = the paper's truncated Spalding law (Eq. 18, PAPER.md:172;
+ * default), 1 = Musker's explicit profile u+ = 5.424 atan((2y+ - 8.15)/16.7) + log10((y+ + 10.6)^9.6 /
+ * (y+^2 - 8.15 y+ + 86)^2) - 3.52 (BASELINE.json config 3 "Spalding/Musker"), solved as
+ * U/u_tau = u+(y u_tau/nu) with the same Newton iteration and stop rule (Eq. 19).  */
+int hhrr_set_wall_function(hhrr_lattice* L, int32_t kind);
 /* Rotor (copied to the device workspace); sets the bodies of tags 1..n_tags. */
 int hhrr_set_rotor(hhrr_lattice* L, const hhrr_rotor_desc* rotor);
 /* Wall model on the cells {FRONTIER, phi > 0} (R13). */

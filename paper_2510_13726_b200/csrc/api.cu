@@ -276,6 +276,12 @@ int hhrr_set_fringe(hhrr_lattice* L, int32_t x_begin, int32_t x_end, const doubl
   return HHRR_OK;
 }
 
+int hhrr_set_wall_function(hhrr_lattice* L, int32_t kind) {
+  if (!L || (kind != 0 && kind != 1)) return fail(HHRR_E_ARG, "hhrr_set_wall_function: bad argument");
+  L->wall_function = kind;
+  return HHRR_OK;
+}
+
 int hhrr_set_fsi_region(hhrr_lattice* L, int32_t n_boxes, const hhrr_box* boxes) {
   if (!L || n_boxes < 0 || n_boxes > HHRR_MAX_FSI_BOXES || (n_boxes > 0 && !boxes))
     return fail(HHRR_E_ARG, "hhrr_set_fsi_region: bad argument");

@@ -107,6 +107,7 @@ struct hhrr_lattice {
   hhrr_rotor_desc rot;  // sdf/tag pointers nulled
   hhrr::Box rot_box;
   hhrr::Boxes fsi;
+  int wall_function;  // 0 truncated Spalding (Eq. 18), 1 Musker
   hhrr::BodiesD bodies;
   bool geometry_dirty;     // full-domain geometry pass needed
   bool geometry_current;   // geometry(step) evaluated

@@ -14,6 +14,7 @@ struct WmArgs {
   double g[3];
   double nu, kappa, E, tol, hs;
   int max_iter;
+  int wall_function;  // 0 truncated Spalding, 1 Musker
   BodiesD bo;
   const float* f;  // post-stream populations (deviations)
   uint8_t* flags;
@@ -145,6 +146,23 @@ __device__ __forceinline__ void wall_sample_block(const WmArgs& a, int block, in
   }
 }
 
+// Musker's explicit profile and its slope (include/hhrr.h: hhrr_set_wall_function); residual U/u_tau - u+(y u_tau/nu)
+__device__ __forceinline__ double musker_uplus(double yp) {
+  double q = yp * yp - 8.15 * yp + 86.0;
+  return 5.424 * atan((2.0 * yp - 8.15) / 16.7) + log10(pow(yp + 10.6, 9.6) / (q * q)) - 3.52;
+}
+__device__ __forceinline__ double musker_duplus(double yp) {
+  double a = (2.0 * yp - 8.15) / 16.7;
+  return 5.424 * (2.0 / 16.7) / (1.0 + a * a) +
+         (9.6 / (yp + 10.6) - 2.0 * (2.0 * yp - 8.15) / (yp * yp - 8.15 * yp + 86.0)) / log(10.0);
+}
+__device__ __forceinline__ double wall_f(int kind, double ut, double U, double y, double nu, double kap, double E) {
+  return kind == 1 ? U / ut - musker_uplus(y * ut / nu) : spalding_f(ut, U, y, nu, kap, E);
+}
+__device__ __forceinline__ double wall_df(int kind, double ut, double U, double y, double nu, double kap, double E) {
+  return kind == 1 ? -U / (ut * ut) - musker_duplus(y * ut / nu) * y / nu : spalding_df(ut, U, y, nu, kap, E);
+}
+
 __global__ void __launch_bounds__(128) wall_model_kernel(const __grid_constant__ WmArgs a) {
   const int count = min(a.cnt->wall_count, a.cap_list);
   const int64_t n = a.dm.n, nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
@@ -180,11 +198,11 @@ __global__ void __launch_bounds__(128) wall_model_kernel(const __grid_constant__
       double prev = a.wm_utau[c];
       double ua = ((fl & WM_VALID) && prev > 0.0) ? prev : sqrt(a.nu * U / yy);  // Eq. 20
       // Newton-Raphson (Eq. 19), stop rule of PAPER.md:184
-      double fa = spalding_f(ua, U, yy, a.nu, a.kappa, a.E), ub = ua;
+      double fa = wall_f(a.wall_function, ua, U, yy, a.nu, a.kappa, a.E), ub = ua;
       for (int it = 0; it < a.max_iter; ++it) {
-        ub = ua - fa / spalding_df(ua, U, yy, a.nu, a.kappa, a.E);
+        ub = ua - fa / wall_df(a.wall_function, ua, U, yy, a.nu, a.kappa, a.E);
         if (!(ub > 0.0)) ub = 0.5 * ua;
-        double fb = spalding_f(ub, U, yy, a.nu, a.kappa, a.E);
+        double fb = wall_f(a.wall_function, ub, U, yy, a.nu, a.kappa, a.E);
         double df = fabs(fb - fa);
         ua = ub;
         fa = fb;
@@ -294,6 +312,7 @@ static void fill_wm(const hhrr_lattice* L, WmArgs& a) {
   a.tol = L->p.newton_tol;
   a.hs = L->p.sampling_distance;
   a.max_iter = L->p.newton_max_iter;
+  a.wall_function = L->wall_function;
   fill_bodies(L, a.bo);
   a.f = L->fA;
   a.flags = L->flags;

@@ -133,6 +133,7 @@ class Case:
     fringe: Optional[tuple] = None                   # (x0, x1, u_in)
     rotor: Optional[dict] = None                     # kwargs of set_rotor
     wall_model: bool = False
+    wall_function: int = 0                           # 0 truncated Spalding (the paper's), 1 Musker
     fsi_boxes: Optional[list] = None                 # region split: [(x0,x1,y0,y1,z0,z1), ...]
 
     @property
@@ -149,6 +150,8 @@ def apply_case(case: Case, lattice) -> None:
     if case.rotor is not None:
         lattice.set_rotor(**case.rotor)
     lattice.enable_wall_model(case.wall_model)
+    if case.wall_function:
+        lattice.set_wall_function(case.wall_function)
     if case.fsi_boxes is not None:
         lattice.set_fsi_region(case.fsi_boxes)
     lattice.init_equilibrium(case.rho, case.u, case.with_neq)

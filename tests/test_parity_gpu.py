@@ -264,6 +264,15 @@ def test_fused_kernels_are_deterministic(variant):
     A.close(); Bv.close()
 
 
+def test_musker_wall_function(oracle):
+    """the wall model with Musker's profile instead of the truncated Spalding law -- channel at
+    Re_tau = 1000 and in the log layer (Re_tau = 5050), and the rotor; u_tau compared per wall cell."""
+    import dataclasses
+    for case in (I.case_channel(128, 48, 16, 20), I.case_channel(48, 40, 24, 10, re_tau=5050.0),
+                 I.case_rotor(128, 72, 72, 20.0, 8, omega=0.012)):
+        run_parity(oracle, dataclasses.replace(case, wall_function=1), case.steps, 5, TOL10, check_every=2)
+
+
 def test_moving_static_body_and_checkpoint(oracle):
     """set_body on a static solid (translating sphere) and populations round trip."""
     case = I.case_sphere(48, 24, 24, 4.0, 6)

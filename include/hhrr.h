@@ -193,8 +193,9 @@ int hhrr_check_finite(hhrr_lattice* L);
 /* Selects the collide-stream kernel: 0 = two-pass (moments pass + collide pass), 1 = fused
  * sliding-window kernel, 2 = fused warp-specialised kernel, 3 = the same with two cells per
  * lane, 4 = fused kernel fed by TMA (needs nx % 64 == 0 and ny % 8 == 0, otherwise 2 runs),
- * 5 = the TMA-fed kernel on x-pull / yz-push storage (default; needs nx % 64 == 0, nx >= 128,
- * ny % 8 == 0 and a periodic x axis, otherwise 2 runs); 11-49 = tile shapes kept for tuning
+ * 5 = the TMA-fed kernel on x-pull / yz-push storage (default; needs a periodic x axis and
+ * tiles of 64 x 8 cells (nx % 64 == 0, nx >= 128, ny % 8 == 0) or 128 x 4 cells (nx % 128 == 0,
+ * nx >= 256, ny % 4 == 0), otherwise 2 runs); 11-49 = tile shapes kept for tuning
  * runs.  All compute the same step (Listing 3 line 3).  Variant 5 keeps plane i
  * of the population buffer as f_i(x + c_ix, y, z) (the x move of Eq. 6, is taken
  * on the read side); the call re-stores the current populations when the layout changes, and

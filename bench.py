@@ -260,6 +260,13 @@ def run_ours(args, rank, world, local_rank):
     if thrust is not None and case.fringe is not None:
         r_rot = 0.5 * (case.rotor["sdf"].shape[1] - 1) * case.rotor["spacing"] - 4.0   # grid half-extent minus its 4-cell margin
         c_t = thrust / (0.5 * np.pi * r_rot ** 2 * case.fringe[2][0] ** 2)
+    # torque of the rotor about its axis (+x) from hhrr_get_torques and the usual power coefficient
+    # C_P = M_x Omega / (0.5 rho pi r^2 U_inf^3) (not defined in the paper, start-up value as above)
+    torque = c_p = None
+    if case.rotor is not None:
+        torque = float(L.torques(L.step_count() - 1, 1)[0, 1:5, 0].sum())
+        if c_t is not None:
+            c_p = torque * case.rotor["omega"] / (0.5 * np.pi * r_rot ** 2 * case.fringe[2][0] ** 3)
 
     # the same workload with the paper's bulk / FSI region split (Listing 2): reported beside the
     # headline, which keeps HHRRLBM in every cell
@@ -315,6 +322,7 @@ def run_ours(args, rank, world, local_rank):
                 "hbm_frac_of_peak_step": value * 1e6 * BYTES_PER_CELL / 1e9 / peak / world,
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
                 "clocks": clocks, "thrust_last_step": thrust, "thrust_coefficient_last_step": c_t,
+                "torque_last_step": torque, "power_coefficient_last_step": c_p,
                 "region_split": split}
         print(json.dumps(line), flush=True)
     L.close()

@@ -166,6 +166,12 @@ int hhrr_get_moments_device(hhrr_lattice* L, float* d_rho, float* d_v);
  * for steps first_step .. first_step+n_steps-1 (must lie within the last
  * hhrr_force_history() steps taken).                                                */
 int hhrr_get_forces(hhrr_lattice* L, int64_t first_step, int64_t n_steps, double* F);
+/* Torque ON each element per step about the centre of the element's rigid body (hhrr_set_body):
+ * M_k = sum over the cells x of element k with d < 1 of (x - x_c) x F(x), F(x) the cell's
+ * momentum-exchange force of Eq. 23 as summed by hhrr_get_forces.  The paper
+ * integrates forces only; the torque is SURVEY 8(f)-4's output for torque / power coefficients.
+ * Same layout, history and error behaviour as hhrr_get_forces; M is a HOST buffer.            */
+int hhrr_get_torques(hhrr_lattice* L, int64_t first_step, int64_t n_steps, double* M);
 int64_t hhrr_force_history(void);
 /* Cell types / tags / porosity of the last evaluated geometry (any pointer nullable). */
 int hhrr_get_cell_types(hhrr_lattice* L, uint8_t* type, uint8_t* tag, float* d);

@@ -92,6 +92,7 @@ typedef struct ohrr_lattice {
   double *wm_utau, *wm_u /*3 AoS*/, *wm_s /*6 AoS: xx yy zz xy xz yz*/;
   /* forces */
   double *force; /* [cap][MAX_TAGS][3] */
+  double *torque; /* [cap][MAX_TAGS][3]: moment of the same per-cell forces about the body's centre */
   int64_t force_cap;
   int64_t step;
   int geometry_current; /* geometry(step) already evaluated */
@@ -739,7 +740,10 @@ static void wall_model(ohrr_lattice *L) {
  * Momentum exchange, PAPER.md:211 (Eq. 23) with reading R7 (second population is
  * the opposite one; reported with a leading minus = force ON the solid), summed
  * literally over all cells with d < 1 and all 26 links, per tag (:267, :315-317).
- * Kahan summation in cell order.                                                  */
+ * Kahan summation in cell order.
+ * Torque (SURVEY 8(f)-4; the paper integrates forces only, :209-211, so this is the
+ * textbook moment of the SAME per-cell momentum-exchange forces F(x) of Eq. 23 about the
+ * centre x_c of the element's rigid body (:140): M_k = sum_x (x - x_c) x F(x).      */
 static void forces(ohrr_lattice *L) {
   const int nx = L->p.nx, ny = L->p.ny, nz = L->p.nz;
   const int64_t n = L->n;
@@ -747,11 +751,16 @@ static void forces(ohrr_lattice *L) {
     int64_t ncap = L->force_cap * 2;
     L->force = (double *)realloc(L->force, sizeof(double) * ncap * MAX_TAGS * 3);
     memset(L->force + L->force_cap * MAX_TAGS * 3, 0, sizeof(double) * (ncap - L->force_cap) * MAX_TAGS * 3);
+    L->torque = (double *)realloc(L->torque, sizeof(double) * ncap * MAX_TAGS * 3);
+    memset(L->torque + L->force_cap * MAX_TAGS * 3, 0, sizeof(double) * (ncap - L->force_cap) * MAX_TAGS * 3);
     L->force_cap = ncap;
   }
   double sum[MAX_TAGS][3], comp[MAX_TAGS][3];
+  double tsum[MAX_TAGS][3], tcomp[MAX_TAGS][3];
   memset(sum, 0, sizeof(sum));
   memset(comp, 0, sizeof(comp));
+  memset(tsum, 0, sizeof(tsum));
+  memset(tcomp, 0, sizeof(tcomp));
   for (int z = 0; z < nz; ++z)
     for (int y = 0; y < ny; ++y)
       for (int x = 0; x < nx; ++x) {
@@ -780,8 +789,19 @@ static void forces(ohrr_lattice *L) {
           comp[k][a] = (tt - sum[k][a]) - v;
           sum[k][a] = tt;
         }
+        const body_t *b = &L->body[k];
+        double r[3] = {x - b->centre[0], y - b->centre[1], z - b->centre[2]};
+        double F[3] = {-acc[0], -acc[1], -acc[2]};
+        double m[3] = {r[1] * F[2] - r[2] * F[1], r[2] * F[0] - r[0] * F[2], r[0] * F[1] - r[1] * F[0]};
+        for (int a = 0; a < 3; ++a) {
+          double v = m[a] - tcomp[k][a];
+          double tt = tsum[k][a] + v;
+          tcomp[k][a] = (tt - tsum[k][a]) - v;
+          tsum[k][a] = tt;
+        }
       }
   memcpy(L->force + L->step * MAX_TAGS * 3, sum, sizeof(sum));
+  memcpy(L->torque + L->step * MAX_TAGS * 3, tsum, sizeof(tsum));
 }
 
 /* ---------------------------------------------------------------- public API */
@@ -808,6 +828,7 @@ ohrr_lattice *ohrr_create(const ohrr_params *p) {
   L->wm_s = (double *)calloc(6 * n, sizeof(double));
   L->force_cap = 1024;
   L->force = (double *)calloc(L->force_cap * MAX_TAGS * 3, sizeof(double));
+  L->torque = (double *)calloc(L->force_cap * MAX_TAGS * 3, sizeof(double));
   for (int64_t c = 0; c < n; ++c) L->d[c] = 1.0;
   for (int i = 0; i < Q; ++i)
     for (int64_t c = 0; c < n; ++c) L->f[(int64_t)i * n + c] = W[i];
@@ -819,7 +840,7 @@ void ohrr_destroy(ohrr_lattice *L) {
   free(L->f); free(L->f2); free(L->uhat); free(L->rho); free(L->phi_static); free(L->tag_static);
   free(L->d_override); free(L->rot_sdf); free(L->rot_tag); free(L->phi); free(L->d); free(L->type);
   free(L->tag); free(L->in_w); free(L->y1n); free(L->wm_valid); free(L->wm_utau); free(L->wm_u);
-  free(L->wm_s); free(L->force);
+  free(L->wm_s); free(L->force); free(L->torque);
   free(L);
 }
 
@@ -959,6 +980,14 @@ int ohrr_force_only(ohrr_lattice *L, double *F) {
   return 0;
 }
 
+/* pins only: same, the torque sums M[MAX_TAGS][3] */
+int ohrr_torque_only(ohrr_lattice *L, double *M) {
+  geometry(L);
+  forces(L);
+  memcpy(M, L->torque + L->step * MAX_TAGS * 3, sizeof(double) * MAX_TAGS * 3);
+  return 0;
+}
+
 /* Listing 3 */
 int ohrr_step(ohrr_lattice *L, int32_t n_steps) {
   for (int s = 0; s < n_steps; ++s) {
@@ -983,6 +1012,11 @@ int ohrr_get_moments(const ohrr_lattice *L, double *rho, double *v) {
 int ohrr_get_forces(const ohrr_lattice *L, int64_t first, int64_t count, double *F) {
   if (first < 0 || first + count > L->step) return -1;
   memcpy(F, L->force + first * MAX_TAGS * 3, sizeof(double) * count * MAX_TAGS * 3);
+  return 0;
+}
+int ohrr_get_torques(const ohrr_lattice *L, int64_t first, int64_t count, double *M) {
+  if (first < 0 || first + count > L->step) return -1;
+  memcpy(M, L->torque + first * MAX_TAGS * 3, sizeof(double) * count * MAX_TAGS * 3);
   return 0;
 }
 /* geometry of the LAST evaluated step (call ohrr_update_geometry first for the current one) */

@@ -240,6 +240,11 @@ class Lattice:
         lib().ohrr_force_only(self._h, _p(F))
         return F
 
+    def torque_only(self):
+        M = np.zeros((MAX_TAGS, 3))
+        lib().ohrr_torque_only(self._h, _p(M))
+        return M
+
     def step(self, n=1):
         lib().ohrr_step(self._h, int(n))
 
@@ -256,6 +261,15 @@ class Lattice:
         if rc:
             raise RuntimeError("ohrr_get_forces: range")
         return F
+
+    def torques(self, first=0, count=None):
+        if count is None:
+            count = lib().ohrr_step_count(self._h) - first
+        M = np.zeros((count, MAX_TAGS, 3))
+        rc = lib().ohrr_get_torques(self._h, C.c_int64(first), C.c_int64(count), _p(M))
+        if rc:
+            raise RuntimeError("ohrr_get_torques: range")
+        return M
 
     def cell_types(self):
         t = np.zeros(self.n, np.uint8); g = np.zeros(self.n, np.uint8); d = np.zeros(self.n)

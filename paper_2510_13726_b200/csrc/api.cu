@@ -87,13 +87,14 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
   int32_t* force_idx = c.take<int32_t>(cap);
   Counters* counters = c.take<Counters>(1);
   double* force = c.take<double>(FORCE_HISTORY * MAX_TAGS * 3);
+  double* torque = c.take<double>(FORCE_HISTORY * MAX_TAGS * 3);
   float* rot_sdf = c.take<float>(rotor_nodes);
   uint8_t* rot_tag = c.take<uint8_t>(rotor_nodes);
   if (L) {
     L->fA = fA; L->fB = fB; L->flags = flags; L->d = d; L->phi = phi; L->below = below; L->rowflag = rowflag; L->rowflag_static = rowflag_static; L->phi_static = phi_static;
     L->tag_static = tag_static; L->d_override = d_override; L->uhat = uhat; L->wm_utau = wm_utau;
     L->wm_u = wm_u; L->wm_s = wm_s; L->wall_idx = wall_idx; L->wall_y1n = wall_y1n; L->wall_samp = wall_samp;
-    L->force_idx = force_idx; L->counters = counters; L->force = force; L->rot_sdf = rot_sdf;
+    L->force_idx = force_idx; L->counters = counters; L->force = force; L->torque = torque; L->rot_sdf = rot_sdf;
     L->rot_tag = rot_tag; L->rot_nodes_cap = rotor_nodes; L->cap_list = cap;
   }
   return c.off;
@@ -195,6 +196,7 @@ int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes,
   e = cudaMemsetAsync(L->wm_utau, 0, sizeof(double) * n, s);
   if (e == cudaSuccess) e = cudaMemsetAsync(L->counters, 0, sizeof(Counters), s);
   if (e == cudaSuccess) e = cudaMemsetAsync(L->force, 0, sizeof(double) * FORCE_HISTORY * MAX_TAGS * 3, s);
+  if (e == cudaSuccess) e = cudaMemsetAsync(L->torque, 0, sizeof(double) * FORCE_HISTORY * MAX_TAGS * 3, s);
   if (e == cudaSuccess) e = cudaGetLastError();
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e != cudaSuccess) {
@@ -447,22 +449,31 @@ int hhrr_get_moments(hhrr_lattice* L, float* rho, float* v) {
   return download(L, v, scratch + n, sizeof(float) * 3 * n);
 }
 
-int hhrr_get_forces(hhrr_lattice* L, int64_t first_step, int64_t n_steps, double* F) {
-  if (!L || !F || n_steps < 0) return fail(HHRR_E_ARG, "hhrr_get_forces: bad argument");
+static int get_force_ring(hhrr_lattice* L, const double* ring, const char* who, int64_t first_step, int64_t n_steps,
+                          double* F) {
+  if (!L || !F || n_steps < 0) return fail(HHRR_E_ARG, "%s: bad argument", who);
   if (first_step < 0 || first_step + n_steps > L->step || first_step < L->step - FORCE_HISTORY)
-    return fail(HHRR_E_STATE, "hhrr_get_forces: steps [%lld,%lld) not in the recorded history (step %lld)",
+    return fail(HHRR_E_STATE, "%s: steps [%lld,%lld) not in the recorded history (step %lld)", who,
                 (long long)first_step, (long long)(first_step + n_steps), (long long)L->step);
   const size_t rec = sizeof(double) * MAX_TAGS * 3;
   int64_t s = first_step;
   while (s < first_step + n_steps) {  // the ring may wrap once
     int64_t slot = s % FORCE_HISTORY;
     int64_t run = std::min<int64_t>(first_step + n_steps - s, FORCE_HISTORY - slot);
-    CU(cudaMemcpyAsync(F + (s - first_step) * MAX_TAGS * 3, L->force + slot * MAX_TAGS * 3, rec * run,
+    CU(cudaMemcpyAsync(F + (s - first_step) * MAX_TAGS * 3, ring + slot * MAX_TAGS * 3, rec * run,
                        cudaMemcpyDeviceToHost, L->stream));
     s += run;
   }
   CU(cudaStreamSynchronize(L->stream));
   return HHRR_OK;
+}
+
+int hhrr_get_forces(hhrr_lattice* L, int64_t first_step, int64_t n_steps, double* F) {
+  return get_force_ring(L, L ? L->force : nullptr, "hhrr_get_forces", first_step, n_steps, F);
+}
+
+int hhrr_get_torques(hhrr_lattice* L, int64_t first_step, int64_t n_steps, double* M) {
+  return get_force_ring(L, L ? L->torque : nullptr, "hhrr_get_torques", first_step, n_steps, M);
 }
 
 int hhrr_get_cell_types(hhrr_lattice* L, uint8_t* type, uint8_t* tag, float* d) {

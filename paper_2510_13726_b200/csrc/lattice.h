@@ -96,6 +96,7 @@ struct hhrr_lattice {
   int32_t* force_idx;       // cap_list
   hhrr::Counters* counters; // 1
   double* force;            // FORCE_HISTORY * MAX_TAGS * 3
+  double* torque;           // FORCE_HISTORY * MAX_TAGS * 3, about each element's body centre
   float* rot_sdf;
   uint8_t* rot_tag;
   int64_t rot_nodes_cap;

@@ -236,20 +236,23 @@ struct ForceArgs {
   const int32_t* force_idx;
   const Counters* cnt;
   int cap_list;
-  double* out;  // [MAX_TAGS][3] of this step (zeroed by the kernel launched before)
+  double* out;    // [MAX_TAGS][3] of this step (zeroed by the kernel launched before)
+  double* out_m;  // [MAX_TAGS][3]: torque of the same per-cell forces about the body centre
 };
 
-__global__ void zero_force_kernel(double* out) {
-  if (threadIdx.x < MAX_TAGS * 3) out[threadIdx.x] = 0.0;
+__global__ void zero_force_kernel(double* out, double* out_m) {
+  if (threadIdx.x < MAX_TAGS * 3) out[threadIdx.x] = out_m[threadIdx.x] = 0.0;
 }
 
 // F_k = - sum_{x: d<1, tag=k} sum_{i != rest} [(c_i - u^s) f_i(x + c_i) + (c_i + u^s) f_ibar(x)]
 // (Eq. 23 with reading R7), fp64 accumulation.  One warp per cell: lane i < 27 takes link i (both
 // loads of a cell's 26 links are in flight at once), warp shuffle sum -> shared per-tag bins -> one
-// global atomic per block, tag and component.
+// global atomic per block, tag and component.  The torque M_k = sum_x (x - x_c) x F(x) about the
+// centre of the element's rigid body takes the same path through a second set of bins.
 __device__ __forceinline__ void force_block(const ForceArgs& a, int block, int nblocks) {
   __shared__ double bins[MAX_TAGS * 3];
-  for (int t = threadIdx.x; t < MAX_TAGS * 3; t += blockDim.x) bins[t] = 0.0;
+  __shared__ double bins_m[MAX_TAGS * 3];
+  for (int t = threadIdx.x; t < MAX_TAGS * 3; t += blockDim.x) bins[t] = bins_m[t] = 0.0;
   __syncthreads();
   const int count = min(a.cnt->force_count, a.cap_list);
   const int64_t nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
@@ -279,12 +282,22 @@ __device__ __forceinline__ void force_block(const ForceArgs& a, int block, int n
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1)
       for (int q = 0; q < 3; ++q) acc[q] += __shfl_down_sync(0xffffffffu, acc[q], off);
-    if (lane == 0)
-      for (int q = 0; q < 3; ++q) atomicAdd(&bins[k * 3 + q], -acc[q]);
+    if (lane == 0) {
+      const double F0 = -acc[0], F1 = -acc[1], F2 = -acc[2];
+      const double r0 = x - a.bo.c[k][0], r1 = y - a.bo.c[k][1], r2 = z - a.bo.c[k][2];
+      atomicAdd(&bins[k * 3 + 0], F0);
+      atomicAdd(&bins[k * 3 + 1], F1);
+      atomicAdd(&bins[k * 3 + 2], F2);
+      atomicAdd(&bins_m[k * 3 + 0], r1 * F2 - r2 * F1);
+      atomicAdd(&bins_m[k * 3 + 1], r2 * F0 - r0 * F2);
+      atomicAdd(&bins_m[k * 3 + 2], r0 * F1 - r1 * F0);
+    }
   }
   __syncthreads();
-  for (int t = threadIdx.x; t < MAX_TAGS * 3; t += blockDim.x)
+  for (int t = threadIdx.x; t < MAX_TAGS * 3; t += blockDim.x) {
     if (bins[t] != 0.0) atomicAdd(&a.out[t], bins[t]);
+    if (bins_m[t] != 0.0) atomicAdd(&a.out_m[t], bins_m[t]);
+  }
 }
 
 // Phase A of K3 and K4 read the same post-stream populations and nothing of each other: one launch,
@@ -339,7 +352,8 @@ cudaError_t launch_wall_model_and_forces(hhrr_lattice* L) {
   a.cnt = L->counters;
   a.cap_list = (int)L->cap_list;
   a.out = L->force + (L->step % FORCE_HISTORY) * MAX_TAGS * 3;
-  zero_force_kernel<<<1, 64, 0, L->stream>>>(a.out);
+  a.out_m = L->torque + (L->step % FORCE_HISTORY) * MAX_TAGS * 3;
+  zero_force_kernel<<<1, 64, 0, L->stream>>>(a.out, a.out_m);
   sample_force_kernel<<<L->wm_enabled ? 4736 : 2368, 128, 0, L->stream>>>(w, a, L->wm_enabled ? 1 : 0);
   L->launches += 2;
   if (L->wm_enabled) {

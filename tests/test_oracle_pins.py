@@ -325,6 +325,62 @@ def test_force_vanishes_for_comoving_solid(oracle):
     assert np.max(np.abs(F)) < 1e-13
 
 
+def _sphere_at_rest(oracle, rho, centre_body, n=16, R=3.6):
+    from paper_2510_13726_b200 import inputs
+    phi = inputs.sphere_phi(n, n, n, (7.3, 8.1, 7.6), R)
+    L = oracle.Lattice(oracle.make_params(n, n, n))
+    L.set_static_geometry(phi, np.ones(n ** 3, np.uint8))
+    L.set_body(1, centre=centre_body)
+    L.init_equilibrium(rho, np.zeros((3, n ** 3)), False)
+    return L
+
+
+def test_torque_of_hydrostatic_load_closed_form(oracle):
+    """Torque output (moment of Eq. 23's per-cell forces): for a fluid
+    at rest with a linear density rho = 1 + a.x every population is w_i rho, so a cell's momentum-exchange
+    force is -sum_i c_i w_i (rho(x + c_i) + rho(x)) = -a cs^2 (the pressure gradient), and the torque on N
+    such cells about x_c is N (xbar - x_c) x (-a/3), xbar their centroid.  Fails for F x r, a lever arm
+    from the wrong origin, a transposed component."""
+    n = 16
+    a = np.array([2e-3, -1e-3, 3e-3])
+    z, y, x = np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij")
+    rho = (1 + a[0] * x + a[1] * y + a[2] * z).ravel().astype(np.float64)
+    xc = np.array([2.5, 11.0, 6.25])
+    L = _sphere_at_rest(oracle, rho, xc)
+    F = L.force_only()
+    M = L.torque_only()
+    t, tag, d = L.cell_types()
+    cells = np.flatnonzero(d < 1.0)
+    assert len(cells) > 100
+    pos = np.stack([x.ravel()[cells], y.ravel()[cells], z.ravel()[cells]], axis=1).astype(np.float64)
+    assert pos.min() >= 2 and pos.max() <= n - 3          # away from the periodic seam of rho
+    assert np.allclose(F[1], -len(cells) * a / 3, rtol=1e-12, atol=1e-16)
+    expect = np.cross(pos.sum(axis=0) - len(cells) * xc, -a / 3)
+    assert np.max(np.abs(expect)) > 1e-2
+    assert np.allclose(M[1], expect, rtol=1e-11, atol=1e-15)
+    assert np.all(M[[0, 2, 3]] == 0)
+
+
+def test_torque_shift_of_reference_point(oracle):
+    """Moving the reference point by D changes the torque by -D x F (rigid-body statics): pins the cross
+    product's orientation against the already pinned force sum, on a flow with non-trivial forces."""
+    from paper_2510_13726_b200 import inputs
+    n = 16
+    rho, u = inputs.noisy_uniform(n, n, n, (0.04, 0.01, -0.02), 5e-3, 5)
+    out = []
+    for xc in [(7.3, 8.1, 7.6), (1.0, 12.5, -3.0)]:
+        phi = inputs.sphere_phi(n, n, n, (7.3, 8.1, 7.6), 3.6)
+        L = oracle.Lattice(oracle.make_params(n, n, n))
+        L.set_static_geometry(phi, np.ones(n ** 3, np.uint8))
+        L.set_body(1, centre=xc)
+        L.init_equilibrium(rho, u, True)
+        L.step(3)
+        out.append((np.array(xc), L.forces()[-1, 1], L.torques()[-1, 1]))
+    (c0, F0, M0), (c1, F1, M1) = out
+    assert np.array_equal(F0, F1) and np.linalg.norm(F0) > 1e-3
+    assert np.allclose(M1, M0 - np.cross(c1 - c0, F0), rtol=1e-10, atol=1e-14)
+
+
 # ------------------------------------------------------------------ P11 wall function
 @pytest.mark.parametrize("U,y,nu", [(0.05, 2.75, 3.156e-4), (0.04, 3.0, 6.25e-5), (1e-4, 2.2, 1e-2), (0.2, 2.9, 1.3e-4)])
 def test_spalding_relation(oracle, U, y, nu):

@@ -62,6 +62,10 @@ def compare_forces(G, Oa, tol):
     scale = np.max(np.abs(Fo))
     if scale > 0:
         assert np.max(np.abs(Fg - Fo)) <= tol * scale, (np.max(np.abs(Fg - Fo)), scale)
+    Mg, Mo = G.torques(), Oa.torques()   # hhrr_get_torques: moment of the same per-cell forces
+    scale = np.max(np.abs(Mo))
+    if scale > 0:
+        assert np.max(np.abs(Mg - Mo)) <= tol * scale, (np.max(np.abs(Mg - Mo)), scale)
 
 
 def run_parity(oracle, case, steps, variant, tol, check_every=None, force_tol=None):
@@ -424,6 +428,22 @@ def test_config4_rotor_100_steps(oracle):
     run_parity(oracle, case, 100, 5, TOL_LONG, check_every=20, force_tol=TOL_LONG)
 
 
+def test_torque_about_moved_body_centre(oracle):
+    """hhrr_get_torques against the oracle on the rotor recipe with the body centres moved off the rotor
+    axis (lever arms no longer symmetric about the hub), three blades + hub, 10 steps."""
+    case = I.case_rotor(128, 48, 48, 14.0, 10, omega=0.015)
+    G, Oa = _gpu_lattice(case, 5), _ora_lattice(oracle, case)
+    for L in (G, Oa):
+        for k in range(1, 5):
+            L.set_body(k, centre=(40.0 + k, 10.5, 30.25), omega=(0.015, 0.0, 0.0))
+    G.step(10); Oa.step(10)
+    Mg, Mo = G.torques(), Oa.torques()
+    assert np.all(np.max(np.abs(Mo[:, 1:5]), axis=(0, 2)) > 0)
+    assert np.max(np.abs(Mg - Mo)) <= TOL10 * np.max(np.abs(Mo))
+    assert np.all(Mg[:, [0, 5, 6, 7]] == 0)
+    G.close(); Oa.close()
+
+
 def test_force_history_ring_and_errors(oracle):
     """More steps than the force ring holds (4096): the last records are still right, older ones are
     refused; argument errors come back as error codes, not crashes."""
@@ -434,6 +454,10 @@ def test_force_history_ring_and_errors(oracle):
     assert G.step_count() == 4200
     Fg, Fo = G.forces(4190, 10), Oa.forces(4190, 10)
     assert np.max(np.abs(Fg - Fo)) <= TOL_LONG * np.max(np.abs(Fo))
+    Mg, Mo = G.torques(4090, 110), Oa.torques(4090, 110)   # spans the wrap of the ring (slot 4095 -> 0)
+    assert np.max(np.abs(Mg - Mo)) <= TOL_LONG * np.max(np.abs(Mo))
+    with pytest.raises(B.HhrrError):
+        G.torques(0, 10)
     with pytest.raises(B.HhrrError):
         G.forces(0, 10)                      # fell out of the ring
     with pytest.raises(B.HhrrError):

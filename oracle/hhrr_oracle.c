@@ -101,6 +101,8 @@ typedef struct ohrr_lattice {
   int n_fsi;
   int32_t fsi[MAX_FSI_BOXES][6];
   int region_violation; /* a cell that is not plain fluid was found outside every box */
+  int wm_slip;          /* 0: u_wm = u_tau e_t (R8); 1: u_wm = u_tau u+(y1+) e_t (R22, SURVEY C8 alt.) */
+  int wm_shear;         /* 0: one-sided difference (R10); 1: analytic slope of the wall function (R22, C10 alt.) */
   int wall_function;    /* 0: truncated Spalding (the paper's, Eq. 18); 1: Musker's profile (BASELINE.json config 3) */
 } ohrr_lattice;
 
@@ -306,6 +308,45 @@ double ohrr_newton_utau_musker(double u0, double U, double y, double nu, int max
   }
   if (iters) *iters = it;
   return ub;
+}
+
+/* Second readings of the two ambiguous wall-model passages (R22; SURVEY 8(c) C8 / C10 alt., 8(f)-4).
+ *
+ * u+(y+) of the truncated Spalding law: Eq. 17 gives y+(u+); its inverse by Newton on
+ *   h(u+) = u+ + (exp(k) - 1 - k - k^2/2 - k^3/6)/E - y+,  k = kappa u+,  h' = 1 + (kappa/E)(exp(k) - 1 - k - k^2/2),
+ * h increasing and convex for u+ >= 0, start at min(y+, 60/kappa) (y+ >= root: the bracket is >= 0), run until
+ * the step no longer changes u+ in double precision (at most 200 steps).                                      */
+double ohrr_spalding_uplus(double yp, double kappa, double E) {
+  if (!(yp > 0.0)) return 0.0;
+  double u = yp < 60.0 / kappa ? yp : 60.0 / kappa;
+  for (int it = 0; it < 200; ++it) {
+    double k = kappa * u, ek = exp(k);
+    double h = u + (ek - 1.0 - k - 0.5 * k * k - k * k * k / 6.0) / E - yp;
+    double dh = 1.0 + (kappa / E) * (ek - 1.0 - k - 0.5 * k * k);
+    double un = u - h / dh;
+    int done = !(fabs(un - u) > 1e-15 * fabs(un));
+    u = un;
+    if (done) break;
+  }
+  return u;
+}
+/* "wall modelled velocities ... at Y1": the wall-function velocity at the cell's own wall
+ * distance y1, u(y1) = u_tau u+(y1 u_tau/nu), in units of u_tau (Eq. 15-16).                            */
+double ohrr_wall_uplus(int kind, double yp, double kappa, double E) {
+  return kind == 1 ? ohrr_musker_uplus(yp) : ohrr_spalding_uplus(yp, kappa, E);
+}
+/* Wall-normal slope du/dy of the wall-function profile at the sampling point (y, U), given u_tau:
+ * du/dy = (u_tau^2/nu) du+/dy+ (Eq. 15-16); Spalding: du+/dy+ = 1/(dy+/du+) from Eq. 17 at u+ = U/u_tau,
+ * Musker: his defining slope at y+ = y u_tau/nu.                                                          */
+double ohrr_wall_shear(int kind, double utau, double U, double y, double nu, double kappa, double E) {
+  double slope;
+  if (kind == 1) {
+    slope = musker_duplus(y * utau / nu);
+  } else {
+    double k = kappa * (U / utau);
+    slope = 1.0 / (1.0 + (kappa / E) * (exp(k) - 1.0 - k - 0.5 * k * k));
+  }
+  return utau * utau / nu * slope;
 }
 
 /* Newton-Raphson, PAPER.md:177 (Eq. 19), stop rule PAPER.md:184: until
@@ -721,10 +762,18 @@ static void wall_model(ohrr_lattice *L) {
                      ? ohrr_newton_utau_musker(u0, U, yy, nu, L->p.newton_max_iter, L->p.newton_tol, NULL)
                      : ohrr_newton_utau(u0, U, yy, nu, L->p.kappa, L->p.E, L->p.newton_max_iter,
                                         L->p.newton_tol, NULL);
-          for (int a = 0; a < 3; ++a) L->wm_u[3 * c + a] = utau * ut[a] / U; /* R8 */
+          double upl = 1.0; /* R8: the friction velocity itself; R22: the wall-function velocity at y1 */
+          if (L->wm_slip == 1) upl = ohrr_wall_uplus(L->wall_function, y1 * utau / nu, L->p.kappa, L->p.E);
+          for (int a = 0; a < 3; ++a) L->wm_u[3 * c + a] = utau * upl * ut[a] / U;
           double G[3][3];
-          for (int a = 0; a < 3; ++a)
-            for (int b = 0; b < 3; ++b) G[a][b] = (vs[a] - vw[a]) * nrm[b] / hs; /* R10 */
+          if (L->wm_shear == 1) { /* R22: analytic slope of the wall function, tangential velocity along n */
+            double dudy = ohrr_wall_shear(L->wall_function, utau, U, yy, nu, L->p.kappa, L->p.E);
+            for (int a = 0; a < 3; ++a)
+              for (int b = 0; b < 3; ++b) G[a][b] = dudy * (ut[a] / U) * nrm[b];
+          } else {
+            for (int a = 0; a < 3; ++a)
+              for (int b = 0; b < 3; ++b) G[a][b] = (vs[a] - vw[a]) * nrm[b] / hs; /* R10 */
+          }
           double *s = &L->wm_s[6 * c];
           s[0] = G[0][0]; s[1] = G[1][1]; s[2] = G[2][2];
           s[3] = 0.5 * (G[0][1] + G[1][0]);
@@ -929,6 +978,14 @@ int ohrr_region_violation(const ohrr_lattice *L) { return L->region_violation; }
 int ohrr_set_wall_function(ohrr_lattice *L, int kind) {
   if (kind != 0 && kind != 1) return -1;
   L->wall_function = kind;
+  return 0;
+}
+
+/* slip: 0 = R8, 1 = wall-function velocity at y1; shear: 0 = R10, 1 = analytic slope (R22) */
+int ohrr_set_wall_model_variant(ohrr_lattice *L, int slip, int shear) {
+  if ((slip != 0 && slip != 1) || (shear != 0 && shear != 1)) return -1;
+  L->wm_slip = slip;
+  L->wm_shear = shear;
   return 0;
 }
 

@@ -75,6 +75,12 @@ def lib():
         L.ohrr_musker_f.argtypes = [C.c_double] * 4
         L.ohrr_newton_utau_musker.restype = C.c_double
         L.ohrr_newton_utau_musker.argtypes = [C.c_double] * 4 + [C.c_int, C.c_double, C.POINTER(C.c_int32)]
+        L.ohrr_spalding_uplus.restype = C.c_double
+        L.ohrr_spalding_uplus.argtypes = [C.c_double] * 3
+        L.ohrr_wall_uplus.restype = C.c_double
+        L.ohrr_wall_uplus.argtypes = [C.c_int] + [C.c_double] * 3
+        L.ohrr_wall_shear.restype = C.c_double
+        L.ohrr_wall_shear.argtypes = [C.c_int] + [C.c_double] * 6
         L.ohrr_tau_eff.restype = C.c_double
         L.ohrr_tau_eff.argtypes = [C.c_double, C.c_double, C.c_double, C.c_void_p]
         L.ohrr_get_wall_list.restype = C.c_int64
@@ -135,6 +141,18 @@ def tau_eff(tau0, cs, rho, pi):
 
 def spalding_f(utau, U, y, nu, kappa=0.41, E=9.8):
     return lib().ohrr_spalding_f(utau, U, y, nu, kappa, E)
+
+
+def spalding_uplus(yp, kappa=0.41, E=9.8):
+    return lib().ohrr_spalding_uplus(float(yp), float(kappa), float(E))
+
+
+def wall_uplus(kind, yp, kappa=0.41, E=9.8):
+    return lib().ohrr_wall_uplus(int(kind), float(yp), float(kappa), float(E))
+
+
+def wall_shear(kind, utau, U, y, nu, kappa=0.41, E=9.8):
+    return lib().ohrr_wall_shear(int(kind), float(utau), float(U), float(y), float(nu), float(kappa), float(E))
 
 
 def musker_uplus(yp):
@@ -221,6 +239,10 @@ class Lattice:
         rc = lib().ohrr_set_fsi_region(self._h, int(b.shape[0]), _p(b) if b.size else None)
         if rc:
             raise RuntimeError("ohrr_set_fsi_region failed")
+
+    def set_wall_model_variant(self, slip=0, shear=0):
+        if lib().ohrr_set_wall_model_variant(self._h, int(slip), int(shear)):
+            raise RuntimeError("ohrr_set_wall_model_variant failed")
 
     def set_wall_function(self, kind):
         if lib().ohrr_set_wall_function(self._h, int(kind)):

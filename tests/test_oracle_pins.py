@@ -688,3 +688,84 @@ def test_wall_model_with_musker_profile_on_uniform_flow(oracle):
     spal, _ = oracle.newton_utau(np.sqrt(nu * U / 2.75), U, 2.75, nu)
     assert utau == pytest.approx(expect, rel=1e-13) and abs(utau - spal) > 1e-6 * spal
     assert np.allclose(uwm, utau * Vt / U, atol=1e-15) and np.allclose(swm, 0, atol=1e-14)
+
+
+# ------------------------------------------------------------------ second readings of the wall model (R22)
+def test_spalding_inverse_satisfies_eq17_and_its_limits(oracle):
+    """u+(y+) used by the 'velocity at Y1' reading: satisfies Eq. 17 (:166) to 1e-13, is the
+    viscous sublayer u+ = y+ near the wall and the log law ln(E y+)/kappa far from it, increasing throughout."""
+    kap, E = 0.41, 9.8
+    ys = np.concatenate([[0.0], np.logspace(-3, 5, 300)])
+    us = np.array([oracle.spalding_uplus(y) for y in ys])
+    k = kap * us
+    back = us + (np.exp(k) - 1 - k - k ** 2 / 2 - k ** 3 / 6) / E
+    assert np.allclose(back, ys, rtol=1e-13, atol=1e-15)
+    assert np.all(np.diff(us) > 0) and us[0] == 0.0
+    assert oracle.spalding_uplus(1e-3) == pytest.approx(1e-3, rel=1e-9)
+    assert oracle.spalding_uplus(1.0) == pytest.approx(1.0, rel=2e-3)
+    for yp in (1e3, 1e4, 1e5):
+        assert oracle.spalding_uplus(yp) == pytest.approx(np.log(E * yp) / kap, rel=0.05)
+    assert 12.5 < oracle.spalding_uplus(30.0) < 14.5        # buffer-layer value every law of the wall passes through
+    # the two wall functions are fits of the same profile
+    for yp in (0.5, 5.0, 30.0, 100.0, 1000.0):
+        assert oracle.wall_uplus(0, yp) == pytest.approx(oracle.wall_uplus(1, yp), rel=0.12)
+        assert oracle.wall_uplus(1, yp) == oracle.musker_uplus(yp)
+
+
+@pytest.mark.parametrize("kind", [0, 1])
+@pytest.mark.parametrize("U,y,nu", [(0.05, 2.75, 3.156e-4), (0.04, 3.0, 6.25e-5), (1e-4, 2.2, 1e-2), (0.2, 2.9, 1.3e-4)])
+def test_analytic_wall_shear_is_the_slope_of_the_profile(oracle, kind, U, y, nu):
+    """'shear stress (cf. Eq. 17)' second reading: with u_tau converged for the sample (U, y), the
+    analytic du/dy equals the centred difference of the profile u(y) = u_tau u+(y u_tau/nu) at y; in the viscous
+    sublayer it is tau_w/(rho nu) = u_tau^2/nu (Eq. 15)."""
+    u0 = np.sqrt(nu * U / y)
+    newton = oracle.newton_utau_musker if kind else oracle.newton_utau
+    ut, _ = newton(u0, U, y, nu, max_iter=200, tol=0.0)
+    prof = lambda yy: ut * oracle.wall_uplus(kind, yy * ut / nu)
+    assert prof(y) == pytest.approx(U, rel=1e-10)
+    h = 1e-4 * y
+    fd = (prof(y + h) - prof(y - h)) / (2 * h)
+    assert oracle.wall_shear(kind, ut, U, y, nu) == pytest.approx(fd, rel=1e-6)
+    # never steeper than the sublayer (Musker's closed form, with its rounded constants, has slope 1.0003 at the wall)
+    assert 0 < oracle.wall_shear(kind, ut, U, y, nu) <= ut * ut / nu * (1 + (1e-3 if kind else 1e-12))
+    # sublayer: a sample at y+ = 0.01
+    ys, Us = 0.01 * nu / ut, 0.01 * ut
+    assert oracle.wall_shear(kind, ut, Us, ys, nu) == pytest.approx(ut * ut / nu, rel=2e-3 if kind else 1e-6)
+
+
+@pytest.mark.parametrize("kind", [0, 1])
+def test_wall_model_second_readings_on_uniform_flow(oracle, kind):
+    """WallModelO with slip = 'wall-function velocity at y1' and shear = 'analytic slope' (R22) over a flat wall
+    in a uniform stream: u_tau unchanged (same sample, same Newton); |u_wm| = u_tau u+(y1 u_tau/nu) < U along the
+    tangential sample; S_wm = sym(du/dy e_t n^T): trace 0, sqrt(2 S:S) = du/dy, and S n . e_t = du/dy / 2."""
+    from paper_2510_13726_b200 import inputs
+    nx, ny, nz = 4, 12, 4
+    n = nx * ny * nz
+    phi = inputs.wall_phi(nx, ny, nz, 1.25)
+    tau0 = 0.5 + 3 * 6.25e-5
+    nu = (tau0 - 0.5) / 3
+    V = np.array([0.05, 0.004, -0.02])
+    out = []
+    for slip, shear in ((0, 0), (1, 1)):
+        L = oracle.Lattice(oracle.make_params(nx, ny, nz, mode=(0, 1, 0), tau0=tau0, sampling_distance=2.0,
+                                              newton_max_iter=200, newton_tol=0.0))
+        L.set_static_geometry(phi, np.ones(n, np.uint8)); L.enable_wall_model(True); L.set_wall_function(kind)
+        L.set_wall_model_variant(slip, shear)
+        L.init_equilibrium(np.ones(n), np.tile(V[:, None], (1, n)), False)
+        L.wall_model_only()
+        idx, y1n, _, valid = L.wall_list()
+        assert np.all(valid == 1)
+        out.append(L.wall_state(int(idx[0])) + (y1n[0],))
+    (_, ut0, uw0, sw0, _), (_, ut1, uw1, sw1, y1v) = out
+    Vt = np.array([V[0], 0, V[2]]); U = np.linalg.norm(Vt); et = Vt / U
+    y1 = np.linalg.norm(y1v); nrm = y1v / y1
+    assert y1 == pytest.approx(0.75, abs=1e-6) and np.allclose(nrm, [0, 1, 0], atol=1e-9)
+    assert ut1 == ut0 and np.allclose(sw0, 0, atol=1e-14)
+    up1 = oracle.wall_uplus(kind, y1 * ut1 / nu)
+    assert np.allclose(uw1, ut1 * up1 * et, rtol=1e-12, atol=1e-16)
+    assert ut1 * up1 < U and np.linalg.norm(uw1) != pytest.approx(np.linalg.norm(uw0), rel=1e-3)
+    dudy = oracle.wall_shear(kind, ut1, U, 2.75, nu)
+    S = np.array([[sw1[0], sw1[3], sw1[4]], [sw1[3], sw1[1], sw1[5]], [sw1[4], sw1[5], sw1[2]]])
+    assert abs(np.trace(S)) < 1e-15
+    assert np.sqrt(2 * np.sum(S * S)) == pytest.approx(dudy, rel=1e-12)
+    assert et @ S @ nrm == pytest.approx(0.5 * dudy, rel=1e-12)

@@ -145,6 +145,18 @@ int hhrr_set_fsi_region(hhrr_lattice* L, int32_t n_boxes, const hhrr_box* boxes)
  * (y+^2 - 8.15 y+ + 86)^2) - 3.52 (BASELINE.json config 3 "Spalding/Musker"), solved as
  * U/u_tau = u+(y u_tau/nu) with the same Newton iteration and stop rule (Eq. 19).  */
 int hhrr_set_wall_function(hhrr_lattice* L, int32_t kind);
+/* Second readings of the two wall-model passages the paper leaves open.
+ * slip  0 (default): the friction velocity is added to the porous-medium velocity, u_wm = u_tau e_t
+ *                    ("adding it to the velocity moment of the porous medium");
+ *       1          : the wall-function velocity at the cell's own wall distance y1 ("wall modelled
+ *                    velocities ... at Y1", :314): u_wm = u_tau u+(y1 u_tau/nu) e_t, u+ the selected wall
+ *                    function (the inverse of Eq. 17, :166, by Newton; Musker's profile is explicit).
+ * shear 0 (default): one-sided difference between the sampling point and the cell,
+ *                    G = (v_s - v(x_w)) n^T / h_s (:324);
+ *       1          : analytic slope of the wall function at the sampling point ("shear stress (cf. Eq. 17)"),
+ *                    G = du/dy e_t n^T, du/dy = (u_tau^2/nu) du+/dy+.            S_wm = (G + G^T)/2 in both.
+ * Takes effect from the next step.  HHRR_E_ARG for other values.                                          */
+int hhrr_set_wall_model_variant(hhrr_lattice* L, int32_t slip, int32_t shear);
 /* Rotor (copied to the device workspace); sets the bodies of tags 1..n_tags. */
 int hhrr_set_rotor(hhrr_lattice* L, const hhrr_rotor_desc* rotor);
 /* Wall model on the cells {FRONTIER, phi > 0} (R13). */

@@ -28,7 +28,7 @@ SYMBOLS = [
     "hhrr_get_moments", "hhrr_get_moments_device", "hhrr_get_forces", "hhrr_get_torques", "hhrr_force_history",
     "hhrr_get_cell_types", "hhrr_get_wall_list", "hhrr_get_wall_state", "hhrr_get_populations",
     "hhrr_set_populations", "hhrr_get_cell_populations", "hhrr_get_uhat", "hhrr_check_finite", "hhrr_set_kernel_variant",
-    "hhrr_population_storage", "hhrr_set_fsi_region", "hhrr_set_wall_function",
+    "hhrr_population_storage", "hhrr_set_fsi_region", "hhrr_set_wall_function", "hhrr_set_wall_model_variant",
     "hhrr_set_timing", "hhrr_get_timing", "hhrr_launch_count", "hhrr_last_error", "hhrr_version",
 ]
 
@@ -83,6 +83,7 @@ def lib():
         L.hhrr_update_geometry.argtypes = [vp]
         L.hhrr_set_fsi_region.argtypes = [vp, i32, vp]
         L.hhrr_set_wall_function.argtypes = [vp, i32]
+        L.hhrr_set_wall_model_variant.argtypes = [vp, i32, i32]
         L.hhrr_population_storage.argtypes = [vp]
         L.hhrr_step.argtypes = [vp, i32]
         L.hhrr_step_count.restype = i64
@@ -234,6 +235,10 @@ class Lattice:
         """boxes: iterable of (x0, x1, y0, y1, z0, z1), half-open; empty = HHRRLBM everywhere."""
         b = np.ascontiguousarray(np.asarray(list(boxes), np.int32).reshape(-1, 6))
         _check(lib().hhrr_set_fsi_region(self.h, int(b.shape[0]), _p(b) if b.size else None))
+
+    def set_wall_model_variant(self, slip=0, shear=0):
+        """Second readings of PAPER.md:314 / :324 (include/hhrr.h)."""
+        _check(lib().hhrr_set_wall_model_variant(self.h, int(slip), int(shear)))
 
     def set_wall_function(self, kind):
         """0: truncated Spalding (Eq. 18, default); 1: Musker's profile."""

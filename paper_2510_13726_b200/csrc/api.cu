@@ -284,6 +284,14 @@ int hhrr_set_wall_function(hhrr_lattice* L, int32_t kind) {
   return HHRR_OK;
 }
 
+int hhrr_set_wall_model_variant(hhrr_lattice* L, int32_t slip, int32_t shear) {
+  if (!L || (slip != 0 && slip != 1) || (shear != 0 && shear != 1))
+    return fail(HHRR_E_ARG, "hhrr_set_wall_model_variant: bad argument");
+  L->wm_slip = slip;
+  L->wm_shear = shear;
+  return HHRR_OK;
+}
+
 int hhrr_set_fsi_region(hhrr_lattice* L, int32_t n_boxes, const hhrr_box* boxes) {
   if (!L || n_boxes < 0 || n_boxes > HHRR_MAX_FSI_BOXES || (n_boxes > 0 && !boxes))
     return fail(HHRR_E_ARG, "hhrr_set_fsi_region: bad argument");

@@ -109,6 +109,7 @@ struct hhrr_lattice {
   hhrr::Box rot_box;
   hhrr::Boxes fsi;
   int wall_function;  // 0 truncated Spalding (Eq. 18), 1 Musker
+  int wm_slip, wm_shear;  // second readings of PAPER.md:314 / :324 (hhrr_set_wall_model_variant), default 0
   hhrr::BodiesD bodies;
   bool geometry_dirty;     // full-domain geometry pass needed
   bool geometry_current;   // geometry(step) evaluated

@@ -15,6 +15,8 @@ struct WmArgs {
   double nu, kappa, E, tol, hs;
   int max_iter;
   int wall_function;  // 0 truncated Spalding, 1 Musker
+  int wm_slip;        // 0: u_wm = u_tau e_t; 1: wall-function velocity at y1 (hhrr_set_wall_model_variant)
+  int wm_shear;       // 0: one-sided difference; 1: analytic slope of the wall function
   BodiesD bo;
   const float* f;  // post-stream populations (deviations)
   uint8_t* flags;
@@ -163,6 +165,34 @@ __device__ __forceinline__ double wall_df(int kind, double ut, double U, double 
   return kind == 1 ? -U / (ut * ut) - musker_duplus(y * ut / nu) * y / nu : spalding_df(ut, U, y, nu, kap, E);
 }
 
+// Second readings (include/hhrr.h: hhrr_set_wall_model_variant).  u+(y+) of the truncated Spalding law: Newton on
+// Eq. 17 read as h(u+) = 0, h increasing and convex; started at min(y+, 60/kappa) >= root.
+__device__ __forceinline__ double spalding_uplus(double yp, double kap, double E) {
+  if (!(yp > 0.0)) return 0.0;
+  double u = yp < 60.0 / kap ? yp : 60.0 / kap;
+  for (int it = 0; it < 200; ++it) {
+    double k = kap * u, ek = exp(k);
+    double h = u + (ek - 1.0 - k - 0.5 * k * k - k * k * k / 6.0) / E - yp;
+    double dh = 1.0 + (kap / E) * (ek - 1.0 - k - 0.5 * k * k);
+    double un = u - h / dh;
+    bool done = !(fabs(un - u) > 1e-15 * fabs(un));
+    u = un;
+    if (done) break;
+  }
+  return u;
+}
+// du/dy = (u_tau^2/nu) du+/dy+ of the wall function at the sampling point
+__device__ __forceinline__ double wall_shear(int kind, double ut, double U, double y, double nu, double kap, double E) {
+  double slope;
+  if (kind == 1) {
+    slope = musker_duplus(y * ut / nu);
+  } else {
+    double k = kap * (U / ut);
+    slope = 1.0 / (1.0 + (kap / E) * (exp(k) - 1.0 - k - 0.5 * k * k));
+  }
+  return ut * ut / nu * slope;
+}
+
 __global__ void __launch_bounds__(128) wall_model_kernel(const __grid_constant__ WmArgs a) {
   const int count = min(a.cnt->wall_count, a.cap_list);
   const int64_t n = a.dm.n, nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
@@ -209,10 +239,21 @@ __global__ void __launch_bounds__(128) wall_model_kernel(const __grid_constant__
         if (df < a.tol) break;
       }
       utau = ub;
-      for (int q = 0; q < 3; ++q) uw[q] = utau * ut[q] / U;  // R8
+      double upl = 1.0;  // R8: the friction velocity itself; R22: the wall-function velocity at y1
+      if (a.wm_slip == 1) {
+        double yp1 = y1 * utau / a.nu;
+        upl = a.wall_function == 1 ? musker_uplus(yp1) : spalding_uplus(yp1, a.kappa, a.E);
+      }
+      for (int q = 0; q < 3; ++q) uw[q] = utau * upl * ut[q] / U;
       double G[3][3];
-      for (int p = 0; p < 3; ++p)
-        for (int q = 0; q < 3; ++q) G[p][q] = (vs[p] - vw[p]) * nrm[q] / a.hs;  // R10
+      if (a.wm_shear == 1) {  // R22
+        double dudy = wall_shear(a.wall_function, utau, U, yy, a.nu, a.kappa, a.E);
+        for (int p = 0; p < 3; ++p)
+          for (int q = 0; q < 3; ++q) G[p][q] = dudy * (ut[p] / U) * nrm[q];
+      } else {
+        for (int p = 0; p < 3; ++p)
+          for (int q = 0; q < 3; ++q) G[p][q] = (vs[p] - vw[p]) * nrm[q] / a.hs;  // R10
+      }
       sw[0] = G[0][0];
       sw[1] = G[1][1];
       sw[2] = G[2][2];
@@ -326,6 +367,8 @@ static void fill_wm(const hhrr_lattice* L, WmArgs& a) {
   a.hs = L->p.sampling_distance;
   a.max_iter = L->p.newton_max_iter;
   a.wall_function = L->wall_function;
+  a.wm_slip = L->wm_slip;
+  a.wm_shear = L->wm_shear;
   fill_bodies(L, a.bo);
   a.f = L->fA;
   a.flags = L->flags;

@@ -134,6 +134,7 @@ class Case:
     rotor: Optional[dict] = None                     # kwargs of set_rotor
     wall_model: bool = False
     wall_function: int = 0                           # 0 truncated Spalding (the paper's), 1 Musker
+    wm_variant: tuple = (0, 0)                       # (slip, shear) readings of PAPER.md:314 / :324, DESIGN R22
     fsi_boxes: Optional[list] = None                 # region split: [(x0,x1,y0,y1,z0,z1), ...]
 
     @property
@@ -152,6 +153,8 @@ def apply_case(case: Case, lattice) -> None:
     lattice.enable_wall_model(case.wall_model)
     if case.wall_function:
         lattice.set_wall_function(case.wall_function)
+    if tuple(case.wm_variant) != (0, 0):
+        lattice.set_wall_model_variant(*case.wm_variant)
     if case.fsi_boxes is not None:
         lattice.set_fsi_region(case.fsi_boxes)
     lattice.init_equilibrium(case.rho, case.u, case.with_neq)

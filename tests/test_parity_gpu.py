@@ -277,6 +277,39 @@ def test_musker_wall_function(oracle):
         run_parity(oracle, dataclasses.replace(case, wall_function=1), case.steps, 5, TOL10, check_every=2)
 
 
+@pytest.mark.parametrize("slip,shear", [(1, 0), (0, 1), (1, 1)])
+def test_wall_model_second_readings(oracle, slip, shear):
+    """SURVEY 8(f)-4 / DESIGN R22: wall-function velocity at y1 as slip, analytic slope of the wall function as wall
+    shear (hhrr_set_wall_model_variant) -- channel at Re_tau = 1000 with Spalding's law, channel in the log layer with
+    Musker's, and the rotor; u_tau, the wall state and the flow compared as in every parity test."""
+    import dataclasses
+    for case in (I.case_channel(128, 48, 16, 20),
+                 dataclasses.replace(I.case_channel(48, 40, 24, 10, re_tau=5050.0), wall_function=1),
+                 I.case_rotor(128, 72, 72, 20.0, 8, omega=0.012)):
+        case = dataclasses.replace(case, wm_variant=(slip, shear))
+        G, Oa = _gpu_lattice(case, 5), _ora_lattice(oracle, case)
+        G.step(case.steps); Oa.step(case.steps)
+        compare_geometry(G, Oa, TOL10)
+        ig = G.wall_list()[0]
+        assert len(ig) > 0
+        for c in ig[:: max(1, len(ig) // 64)]:      # wall state of sampled wall cells: slip velocity and wall strain
+            vg, ug, uwg, swg = G.wall_state(int(c))
+            vo, uo, uwo, swo = Oa.wall_state(int(c))
+            assert vg == vo
+            assert ug == pytest.approx(uo, rel=TOL10, abs=1e-12)
+            assert np.allclose(uwg, uwo, rtol=0, atol=TOL10 * max(np.max(np.abs(uwo)), 1e-7) + 1e-9)
+            assert np.allclose(swg, swo, rtol=0, atol=TOL10 * max(np.max(np.abs(swo)), 1e-7) + 1e-9)
+        e_rho, e_v = rel_linf(*G.moments(), *Oa.moments())
+        assert e_rho <= TOL10 and e_v <= TOL10, (case.name, e_rho, e_v)
+        compare_forces(G, Oa, TOL10)
+        G.close(); Oa.close()
+    from paper_2510_13726_b200 import binding as B
+    G = _gpu_lattice(I.case_channel(128, 48, 16, 1), 5)
+    with pytest.raises(B.HhrrError):
+        G.set_wall_model_variant(2, 0)
+    G.close()
+
+
 def test_moving_static_body_and_checkpoint(oracle):
     """set_body on a static solid (translating sphere) and populations round trip."""
     case = I.case_sphere(48, 24, 24, 4.0, 6)

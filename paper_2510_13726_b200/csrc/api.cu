@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -72,6 +73,7 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
   float* d = c.take<float>(n);
   double* phi = c.take<double>(n);
   uint8_t* below = c.take<uint8_t>(n);
+  uint8_t* tag_prov = c.take<uint8_t>(n);
   uint8_t* rowflag = c.take<uint8_t>((int64_t)p->ny * p->nz);
   uint8_t* rowflag_static = c.take<uint8_t>((int64_t)p->ny * p->nz);
   float* phi_static = c.take<float>(n);
@@ -91,7 +93,7 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
   float* rot_sdf = c.take<float>(rotor_nodes);
   uint8_t* rot_tag = c.take<uint8_t>(rotor_nodes);
   if (L) {
-    L->fA = fA; L->fB = fB; L->flags = flags; L->d = d; L->phi = phi; L->below = below; L->rowflag = rowflag; L->rowflag_static = rowflag_static; L->phi_static = phi_static;
+    L->fA = fA; L->fB = fB; L->flags = flags; L->d = d; L->phi = phi; L->below = below; L->tag_prov = tag_prov; L->rowflag = rowflag; L->rowflag_static = rowflag_static; L->phi_static = phi_static;
     L->tag_static = tag_static; L->d_override = d_override; L->uhat = uhat; L->wm_utau = wm_utau;
     L->wm_u = wm_u; L->wm_s = wm_s; L->wall_idx = wall_idx; L->wall_y1n = wall_y1n; L->wall_samp = wall_samp;
     L->force_idx = force_idx; L->counters = counters; L->force = force; L->torque = torque; L->rot_sdf = rot_sdf;
@@ -119,6 +121,12 @@ int download(hhrr_lattice* L, void* dst, const void* src, size_t bytes) {
   CU(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, L->stream));
   CU(cudaStreamSynchronize(L->stream));
   return HHRR_OK;
+}
+
+// the side stream may still be reading the rotor grid / static fields for a look-ahead pass: order the
+// caller's stream behind it before those inputs are overwritten
+void quiesce_side(hhrr_lattice* L) {
+  if (L->side && L->phi_ahead_step >= 0) cudaStreamWaitEvent(L->stream, L->ev_phi_done, 0);
 }
 
 int ensure_geometry(hhrr_lattice* L) {
@@ -183,6 +191,17 @@ int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes,
   L->dom.xs = xpull_supported(L->dom) ? 1 : 0;  // buffers start as zeros: nothing to convert
   L->geometry_dirty = true;
   L->geometry_current = false;
+  L->phi_ahead_step = -1;
+  if (!getenv("HHRR_NO_LOOKAHEAD")) {  // measurement switch; the look-ahead changes no result
+    int prio_lo = 0, prio_hi = 0;
+    cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+    if (cudaStreamCreateWithPriority(&L->side, cudaStreamNonBlocking, prio_lo) != cudaSuccess ||
+        cudaEventCreateWithFlags(&L->ev_type_done, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&L->ev_phi_done, cudaEventDisableTiming) != cudaSuccess) {
+      delete L;
+      return cuda_fail(cudaGetLastError(), "hhrr_create: side stream");
+    }
+  }
   const int64_t n = L->dom.n;
   cudaStream_t s = L->stream;
   fill_float_kernel<<<1184, 256, 0, s>>>(L->fA, Q * n, 0.f);
@@ -210,6 +229,12 @@ int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes,
 int hhrr_destroy(hhrr_lattice* L) {
   if (!L) return fail(HHRR_E_ARG, "hhrr_destroy: NULL lattice");
   cudaStreamSynchronize(L->stream);
+  if (L->side) {
+    cudaStreamSynchronize(L->side);
+    cudaEventDestroy(L->ev_type_done);
+    cudaEventDestroy(L->ev_phi_done);
+    cudaStreamDestroy(L->side);
+  }
   if (L->ev[0])
     for (int k = 0; k < 2 * 1024; ++k) cudaEventDestroy(L->ev[k]);
   delete L;
@@ -234,6 +259,7 @@ int hhrr_init_equilibrium(hhrr_lattice* L, const float* rho, const float* u, int
 int hhrr_set_static_geometry(hhrr_lattice* L, const float* phi, const uint8_t* tag, const float* d_override) {
   if (!L) return fail(HHRR_E_ARG, "hhrr_set_static_geometry: NULL lattice");
   const int64_t n = L->dom.n;
+  quiesce_side(L);
   L->has_static = L->has_tag_static = L->has_override = false;
   if (phi) {
     int rc = upload(L, L->phi_static, phi, sizeof(float) * n);
@@ -312,6 +338,7 @@ int hhrr_set_rotor(hhrr_lattice* L, const hhrr_rotor_desc* r) {
   if (nodes > L->rot_nodes_cap)
     return fail(HHRR_E_SIZE, "hhrr_set_rotor: reference grid of %lld nodes does not fit the workspace (%lld)",
                 (long long)nodes, (long long)L->rot_nodes_cap);
+  quiesce_side(L);
   int rc = upload(L, L->rot_sdf, r->sdf, sizeof(float) * nodes);
   if (rc) return rc;
   rc = upload(L, L->rot_tag, r->tag, nodes);
@@ -431,6 +458,8 @@ int hhrr_step(hhrr_lattice* L, int32_t n_steps) {
       CU(cudaEventRecord(L->ev[2 * L->ev_n + 1], L->stream));
       L->ev_n++;
     }
+    e = launch_phi_ahead(L);  // line 2 of the NEXT step, first half: queued behind this step's kernels
+    if (e != cudaSuccess) return cuda_fail(e, "geometry look-ahead");
     e = launch_wall_model_and_forces(L);  // line 4: WallModelO; lines 5-6: forces (one launch)
     if (e != cudaSuccess) return cuda_fail(e, "wall-model / force kernel");
     L->step += 1;  // line 7: theta_{n+1} = theta_n + Omega

@@ -31,6 +31,7 @@ struct GeoArgs {
   double* phi;
   uint8_t* below;   // phi < eps/2 per cell: what the growth-layer test reads (1 B instead of 8)
   uint8_t* rowflag; // per (y,z) row: some cell of the row may have phi < eps/2 (superset)
+  uint8_t* tag_prov;  // provisional tag of pass 1 (its own array: pass 1 may run ahead of the step that reads flags)
   uint8_t* flags;
   float* d;
   int32_t* wall_idx;
@@ -129,7 +130,7 @@ __global__ void __launch_bounds__(128) geometry_phi_kernel(GeoArgs a) {
   const bool below = phi < a.h;
   a.below[c] = below ? 1 : 0;
   if (below) a.rowflag[y + a.dm.ny * z] = 1;
-  a.flags[c] = (uint8_t)((a.flags[c] & WM_VALID) | ((tg & TAG_MASK) << TAG_SHIFT));
+  a.tag_prov[c] = (uint8_t)(tg & TAG_MASK);
 }
 
 // pass 2: type, porosity, wall-model set (R13) and the compact lists
@@ -177,7 +178,7 @@ __global__ void __launch_bounds__(128) geometry_type_kernel(GeoArgs a) {
     c = x + snx * y + snxy * z;
     double phi = a.phi[c];
     uint8_t fl = a.flags[c];
-    int tg = (fl >> TAG_SHIFT) & TAG_MASK;
+    int tg = a.tag_prov[c];
     int type;
     float d;
     if (a.has_fringe && x >= a.fr_x0 && x < a.fr_x1) {
@@ -278,7 +279,7 @@ __global__ void counters_kernel(Counters* cnt, int op) {
 static void geo_grid(const GeoArgs& a, dim3& g, dim3& b) {
   if (a.inside) {
     int bx = a.box.x1 - a.box.x0, by = a.box.y1 - a.box.y0, bz = a.box.z1 - a.box.z0;
-    int t = bx <= 32 ? 32 : (bx <= 64 ? 64 : 128);  // a rotor box is thin along its axis: do not idle lanes
+    int t = bx >= 128 ? 128 : ((bx + 31) / 32) * 32;  // a rotor box is thin along its axis: do not idle warps
     b = dim3(t);
     g = dim3(by * bz, (bx + t - 1) / t);
   } else {
@@ -287,8 +288,7 @@ static void geo_grid(const GeoArgs& a, dim3& g, dim3& b) {
   }
 }
 
-cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
-  GeoArgs a;
+static void fill_geo(hhrr_lattice* L, GeoArgs& a, int64_t step) {
   a.dm = L->dom;
   a.h = 0.5 * L->p.eps_cells;
   a.eps = L->p.eps_cells;
@@ -303,10 +303,8 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
   a.fr_x1 = L->fr_x1;
   a.cth = 1.0;
   a.sth = 0.0;
-  Box none = {0, 0, 0, 0, 0, 0};
-  Box rb = none;
   if (L->has_rotor) {
-    double th = L->rot.theta0 + (double)L->step * L->rot.omega;  // rigid rotation only
+    double th = L->rot.theta0 + (double)step * L->rot.omega;  // rigid rotation only
     a.cth = cos(th);
     a.sth = sin(th);
     a.rot.sdf = L->rot_sdf;
@@ -320,7 +318,6 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
       a.rot.centre[k] = L->rot.centre[k];
       a.rot.axis[k] = L->rot.axis[k];
     }
-    rb = L->rot_box;
   } else {
     a.rot = RotorDev{};
   }
@@ -330,6 +327,7 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
   a.phi = L->phi;
   a.below = L->below;
   a.rowflag = L->rowflag;
+  a.tag_prov = L->tag_prov;
   a.flags = L->flags;
   a.d = L->d;
   a.wall_idx = L->wall_idx;
@@ -337,9 +335,51 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
   a.force_idx = L->force_idx;
   a.cnt = L->counters;
   a.cap_list = (int)L->cap_list;
+}
+
+static bool rotor_box_empty(const hhrr_lattice* L) {
+  const Box& rb = L->rot_box;
+  return !L->has_rotor || rb.x1 <= rb.x0 || rb.y1 <= rb.y0 || rb.z1 <= rb.z0;
+}
+
+// pass 1 of geometry(step) over the rotor box, on stream s.  It reads the rotor description and the static
+// fields and writes phi / below / rowflag / tag_prov -- nothing a collide-stream, wall-model or force kernel touches.
+static void launch_box_phi(hhrr_lattice* L, int64_t step, cudaStream_t s) {
+  GeoArgs a;
+  fill_geo(L, a, step);
+  a.box = L->rot_box;
+  a.inside = 1;
+  dim3 g, b;
+  geo_grid(a, g, b);
+  cudaMemcpyAsync(L->rowflag, L->rowflag_static, (size_t)L->dom.ny * L->dom.nz, cudaMemcpyDeviceToDevice, s);
+  geometry_phi_kernel<<<g, b, 0, s>>>(a);
+  L->launches++;
+}
+
+// Look-ahead: pass 1 of geometry(step + 1) depends on the step count only (rigid rotation), so it
+// is queued on a low-priority side stream as soon as pass 2 of geometry(step) has read phi, and runs in the tail
+// of the collide-stream kernel / beside the wall-model and force kernels instead of between two steps.
+cudaError_t launch_phi_ahead(hhrr_lattice* L) {
+  if (!L->side || rotor_box_empty(L) || L->geometry_dirty) return cudaSuccess;
+  cudaStreamWaitEvent(L->side, L->ev_type_done, 0);
+  launch_box_phi(L, L->step + 1, L->side);
+  cudaEventRecord(L->ev_phi_done, L->side);
+  L->phi_ahead_step = L->step + 1;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
+  GeoArgs a;
+  fill_geo(L, a, L->step);
+  Box none = {0, 0, 0, 0, 0, 0};
+  Box rb = L->has_rotor ? L->rot_box : none;
   dim3 g, b;
   bool box_empty = rb.x1 <= rb.x0 || rb.y1 <= rb.y0 || rb.z1 <= rb.z0;
   const size_t rows = (size_t)L->dom.ny * L->dom.nz;
+  const bool ahead = L->phi_ahead_step >= 0;
+  if (ahead) cudaStreamWaitEvent(L->stream, L->ev_phi_done, 0);  // whatever the side stream wrote is complete
+  const bool have_phi = ahead && L->phi_ahead_step == L->step && !full;
+  L->phi_ahead_step = -1;
   if (full) {
     // phi everywhere, then types: outside the rotor box first (static list prefix), box last
     a.box = none;
@@ -361,15 +401,15 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
       L->launches++;
     }
   } else if (!box_empty) {
+    if (!have_phi) launch_box_phi(L, L->step, L->stream);
     a.box = rb;
     a.inside = 1;
     geo_grid(a, g, b);
-    cudaMemcpyAsync(L->rowflag, L->rowflag_static, rows, cudaMemcpyDeviceToDevice, L->stream);
-    geometry_phi_kernel<<<g, b, 0, L->stream>>>(a);
     counters_kernel<<<1, 1, 0, L->stream>>>(L->counters, 2);
     geometry_type_kernel<<<g, b, 0, L->stream>>>(a);
-    L->launches += 3;
+    L->launches += 2;
   }
+  if (L->side) cudaEventRecord(L->ev_type_done, L->stream);  // phi of this step has been read
   return cudaGetLastError();
 }
 

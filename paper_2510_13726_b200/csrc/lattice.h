@@ -75,6 +75,11 @@ struct hhrr_lattice {
   hhrr_params p;
   hhrr::Dom dom;
   cudaStream_t stream;
+  // look-ahead of geometry pass 1 (geometry.cu: launch_phi_ahead): low-priority side stream, two ordering events,
+  // the step whose phi the side stream has been asked for (-1: none)
+  cudaStream_t side;
+  cudaEvent_t ev_type_done, ev_phi_done;
+  int64_t phi_ahead_step;
   int device;
   // device arrays (inside the caller's workspace)
   float *fA, *fB;           // 27 planes each: post-stream populations minus weights
@@ -82,6 +87,7 @@ struct hhrr_lattice {
   float* d;                 // N porosity (read for FRONTIER cells only)
   double* phi;              // N signed distance of the last geometry
   uint8_t* below;           // N: phi < eps/2
+  uint8_t* tag_prov;        // N: provisional tag of geometry pass 1
   uint8_t *rowflag, *rowflag_static;  // ny*nz: row may hold a cell with phi < eps/2
   float* phi_static;        // N
   uint8_t* tag_static;      // N
@@ -130,6 +136,7 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full);
 cudaError_t launch_fill_rest(hhrr_lattice* L);
 cudaError_t launch_init(hhrr_lattice* L, const float* d_rho, const float* d_u, int with_neq);
 cudaError_t launch_collide_stream(hhrr_lattice* L);
+cudaError_t launch_phi_ahead(hhrr_lattice* L);
 cudaError_t launch_moments(hhrr_lattice* L, float* d_rho, float* d_v);
 cudaError_t launch_check_finite(hhrr_lattice* L);
 bool xpull_supported(const Dom& dm);                    // fused_xpull.cu: variant 5 can run this lattice

@@ -5,6 +5,8 @@
 // Both kernels touch 1e4-1e5 cells, so they run in fp64 on the fp32 populations: the Newton
 // stop rule (:184) decides an iteration count, and it is taken in the same precision as the
 // oracle takes it.  Forces accumulate in fp64.  CUDA path only; shares nothing with oracle/.
+#include <cstdlib>
+
 #include "d3q27.cuh"
 
 namespace hhrr {
@@ -323,15 +325,13 @@ __device__ __forceinline__ void force_block(const ForceArgs& a, int block, int n
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1)
       for (int q = 0; q < 3; ++q) acc[q] += __shfl_down_sync(0xffffffffu, acc[q], off);
-    if (lane == 0) {
-      const double F0 = -acc[0], F1 = -acc[1], F2 = -acc[2];
+    // lanes 0-2 add the force components, lanes 3-5 the torque components: one shared-memory atomic per lane
+    const double F0 = -shfl_d(acc[0], 0), F1 = -shfl_d(acc[1], 0), F2 = -shfl_d(acc[2], 0);
+    if (lane < 6) {
       const double r0 = x - a.bo.c[k][0], r1 = y - a.bo.c[k][1], r2 = z - a.bo.c[k][2];
-      atomicAdd(&bins[k * 3 + 0], F0);
-      atomicAdd(&bins[k * 3 + 1], F1);
-      atomicAdd(&bins[k * 3 + 2], F2);
-      atomicAdd(&bins_m[k * 3 + 0], r1 * F2 - r2 * F1);
-      atomicAdd(&bins_m[k * 3 + 1], r2 * F0 - r0 * F2);
-      atomicAdd(&bins_m[k * 3 + 2], r0 * F1 - r1 * F0);
+      const double v = lane == 0 ? F0 : lane == 1 ? F1 : lane == 2 ? F2
+                     : lane == 3 ? r1 * F2 - r2 * F1 : lane == 4 ? r2 * F0 - r0 * F2 : r0 * F1 - r1 * F0;
+      atomicAdd(lane < 3 ? &bins[k * 3 + lane] : &bins_m[k * 3 + lane - 3], v);
     }
   }
   __syncthreads();
@@ -345,13 +345,15 @@ __device__ __forceinline__ void force_block(const ForceArgs& a, int block, int n
 // even blocks sample the wall-model velocities, odd blocks collect the forces.  Both are gathers whose
 // latency hides behind the other's.
 __global__ void __launch_bounds__(128) sample_force_kernel(const __grid_constant__ WmArgs w,
-                                                           const __grid_constant__ ForceArgs f, int wm_on) {
+                                                           const __grid_constant__ ForceArgs f, int wm_on, int split) {
+  // of every four blocks, `split` sample wall-model velocities and 4 - split collect forces
+  const int quad = blockIdx.x >> 2, r = blockIdx.x & 3, nquad = gridDim.x >> 2;
   if (!wm_on)
     force_block(f, blockIdx.x, gridDim.x);
-  else if ((blockIdx.x & 1) == 0)
-    wall_sample_block(w, blockIdx.x >> 1, gridDim.x >> 1);
+  else if (r < split)
+    wall_sample_block(w, quad * split + r, nquad * split);
   else
-    force_block(f, blockIdx.x >> 1, gridDim.x >> 1);
+    force_block(f, quad * (4 - split) + r - split, nquad * (4 - split));
 }
 
 // ---------------------------------------------------------------------------- launchers
@@ -397,7 +399,9 @@ cudaError_t launch_wall_model_and_forces(hhrr_lattice* L) {
   a.out = L->force + (L->step % FORCE_HISTORY) * MAX_TAGS * 3;
   a.out_m = L->torque + (L->step % FORCE_HISTORY) * MAX_TAGS * 3;
   zero_force_kernel<<<1, 64, 0, L->stream>>>(a.out, a.out_m);
-  sample_force_kernel<<<L->wm_enabled ? 4736 : 2368, 128, 0, L->stream>>>(w, a, L->wm_enabled ? 1 : 0);
+  static const int split = getenv("HHRR_SF_SPLIT") ? atoi(getenv("HHRR_SF_SPLIT")) : 2;
+  static const int sf_blocks = getenv("HHRR_SF_BLOCKS") ? atoi(getenv("HHRR_SF_BLOCKS")) : 4736;
+  sample_force_kernel<<<L->wm_enabled ? sf_blocks : sf_blocks / 2, 128, 0, L->stream>>>(w, a, L->wm_enabled ? 1 : 0, split);
   L->launches += 2;
   if (L->wm_enabled) {
     wall_model_kernel<<<592, 128, 0, L->stream>>>(w);

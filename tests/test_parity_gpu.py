@@ -268,6 +268,35 @@ def test_fused_kernels_are_deterministic(variant):
     A.close(); Bv.close()
 
 
+def test_geometry_look_ahead_changes_nothing(oracle, monkeypatch):
+    """Pass 1 of UpdatePorosityO for step n+1 runs ahead on a side stream (geometry.cu: launch_phi_ahead).  With it
+    and without it (HHRR_NO_LOOKAHEAD) the populations stay bitwise equal; a rotor that is replaced, and a geometry
+    evaluation asked for between steps, while a look-ahead pass is pending give the oracle's cell types, lists and
+    flow."""
+    case = I.case_rotor(128, 72, 72, 20.0, 9, omega=0.012)
+    A = _gpu_lattice(case, 5)
+    monkeypatch.setenv("HHRR_NO_LOOKAHEAD", "1")
+    Bv = _gpu_lattice(case, 5)
+    monkeypatch.delenv("HHRR_NO_LOOKAHEAD")
+    Oa = _ora_lattice(oracle, case)
+    A.step(3); Bv.step(3); Oa.step(3)
+    assert np.array_equal(A.populations(), Bv.populations())
+    for L in (A, Bv, Oa):
+        L.update_geometry()                       # geometry(3): the look-ahead pass of step 3 is consumed here
+    compare_geometry(A, Oa)
+    A.step(1); Bv.step(1); Oa.step(1)
+    rotor2 = dict(case.rotor, omega=-0.02, theta0=0.7)
+    for L in (A, Bv, Oa):
+        L.set_rotor(**rotor2)                     # pending look-ahead pass (old rotor, step 5) must be dropped
+    A.step(3); Bv.step(3); Oa.step(3)
+    compare_geometry(A, Oa)
+    assert np.array_equal(A.populations(), Bv.populations())
+    assert np.array_equal(A.forces(), Bv.forces()) or np.allclose(A.forces(), Bv.forces(), rtol=1e-12, atol=1e-18)
+    e_rho, e_v = rel_linf(*A.moments(), *Oa.moments())
+    assert e_rho <= TOL10 and e_v <= TOL10, (e_rho, e_v)
+    A.close(); Bv.close(); Oa.close()
+
+
 def test_musker_wall_function(oracle):
     """the wall model with Musker's profile instead of the truncated Spalding law -- channel at
     Re_tau = 1000 and in the log layer (Re_tau = 5050), and the rotor; u_tau compared per wall cell."""

@@ -5,8 +5,6 @@
 // Both kernels touch 1e4-1e5 cells, so they run in fp64 on the fp32 populations: the Newton
 // stop rule (:184) decides an iteration count, and it is taken in the same precision as the
 // oracle takes it.  Forces accumulate in fp64.  CUDA path only; shares nothing with oracle/.
-#include <cstdlib>
-
 #include "d3q27.cuh"
 
 namespace hhrr {
@@ -90,10 +88,24 @@ __device__ __forceinline__ void wall_sample_block(const WmArgs& a, int block, in
   const int64_t nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
   const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
   const int kc = lane / 3, g = lane - 3 * kc;  // cell of the stencil, population group (lanes 27-31 idle)
-  for (int e = block * wpb + (threadIdx.x >> 5); e < count; e += nblocks * wpb) {
-    int64_t c = a.wall_idx[e];
+  // the list entry of the NEXT cell is fetched while this one's populations are in flight: one memory latency per
+  // cell instead of two (the kernel is latency-bound: 3e4 cells, a few per warp)
+  int e = block * wpb + (threadIdx.x >> 5);
+  int64_t c_next = 0;
+  double y_next[3] = {0, 0, 0};
+  if (e < count) {
+    c_next = a.wall_idx[e];
+    for (int q = 0; q < 3; ++q) y_next[q] = a.wall_y1n[3 * (int64_t)e + q];
+  }
+  for (; e < count; e += nblocks * wpb) {
+    const int64_t c = c_next;
+    const double y1v[3] = {y_next[0], y_next[1], y_next[2]};
+    const int en = e + nblocks * wpb;
+    if (en < count) {
+      c_next = a.wall_idx[en];
+      for (int q = 0; q < 3; ++q) y_next[q] = a.wall_y1n[3 * (int64_t)en + q];
+    }
     int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
-    double y1v[3] = {a.wall_y1n[3 * (int64_t)e], a.wall_y1n[3 * (int64_t)e + 1], a.wall_y1n[3 * (int64_t)e + 2]};
     double y1 = sqrt(y1v[0] * y1v[0] + y1v[1] * y1v[1] + y1v[2] * y1v[2]);
     double nrm[3] = {y1v[0] / y1, y1v[1] / y1, y1v[2] / y1};
     // velocity at x_w + h_s n, trilinear over the 8 surrounding cells (R15)
@@ -288,10 +300,12 @@ __global__ void zero_force_kernel(double* out, double* out_m) {
 }
 
 // F_k = - sum_{x: d<1, tag=k} sum_{i != rest} [(c_i - u^s) f_i(x + c_i) + (c_i + u^s) f_ibar(x)]
-// (Eq. 23 with reading R7), fp64 accumulation.  One warp per cell: lane i < 27 takes link i (both
-// loads of a cell's 26 links are in flight at once), warp shuffle sum -> shared per-tag bins -> one
-// global atomic per block, tag and component.  The torque M_k = sum_x (x - x_c) x F(x) about the
-// centre of the element's rigid body takes the same path through a second set of bins.
+// (Eq. 23 with reading R7), fp64 accumulation.  One LANE per cell, a warp takes 32 consecutive list entries:
+// geometry pass 2 appends a warp's cells in x order, so the entries are runs of x-neighbours and each of the
+// 52 loads of the warp touches a few sectors instead of 32.  Warp shuffle sum (when the 32 cells belong to one
+// element, the usual case; per-lane atomics otherwise) -> shared per-tag bins -> one global atomic per block,
+// tag and component.  The torque M_k = sum_x (x - x_c) x F(x) about the centre of the element's rigid body
+// takes the same path through a second set of bins.
 __device__ __forceinline__ void force_block(const ForceArgs& a, int block, int nblocks) {
   __shared__ double bins[MAX_TAGS * 3];
   __shared__ double bins_m[MAX_TAGS * 3];
@@ -300,38 +314,65 @@ __device__ __forceinline__ void force_block(const ForceArgs& a, int block, int n
   const int count = min(a.cnt->force_count, a.cap_list);
   const int64_t nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
   const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
-  const int i = lane;
-  const int cx = i % 3 - 1, cy = (i / 3) % 3 - 1, cz = i / 9 - 1;
-  const bool link = i < Q && i != 13;
-  for (int e = block * wpb + (threadIdx.x >> 5); e < count; e += nblocks * wpb) {
-    int64_t c = a.force_idx[e];
-    int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
-    int k = (a.flags[c] >> TAG_SHIFT) & TAG_MASK;
-    double us[3];
-    body_velocity_d(a.bo, k, x, y, z, us);
-    double acc[3] = {0, 0, 0};
-    if (link) {
-      bool fl;
-      int xx = wrap_far(x + cx, a.dm.nx, a.dm.mode[0], fl);
-      int yy = wrap_far(y + cy, a.dm.ny, a.dm.mode[1], fl);
-      int zz = wrap_far(z + cz, a.dm.nz, a.dm.mode[2], fl);
-      // stored values are deviations: f = w + dev, and w_i = w_ibar
-      double w = (cx ? 1.0 / 6.0 : 2.0 / 3.0) * (cy ? 1.0 / 6.0 : 2.0 / 3.0) * (cz ? 1.0 / 6.0 : 2.0 / 3.0);
-      double fa = w + (double)__ldg(a.f + pop_index(a.dm, i, xx, yy, zz));
-      double fb = w + (double)__ldg(a.f + pop_index(a.dm, 26 - i, x, y, z));
-      double ci[3] = {(double)cx, (double)cy, (double)cz};
-      for (int q = 0; q < 3; ++q) acc[q] = (ci[q] - us[q]) * fa + (ci[q] + us[q]) * fb;
-    }
+  for (int base = (block * wpb + (threadIdx.x >> 5)) * 32; base < count; base += nblocks * wpb * 32) {
+    const int e = base + lane;
+    const bool act = e < count;
+    int k = -1;
+    double v[6] = {0, 0, 0, 0, 0, 0};  // force, torque of this lane's cell
+    if (act) {
+      const int64_t c = a.force_idx[e];
+      const int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
+      k = (a.flags[c] >> TAG_SHIFT) & TAG_MASK;
+      double us[3];
+      body_velocity_d(a.bo, k, x, y, z, us);
+      double acc[3] = {0, 0, 0};
+#pragma unroll 1
+      for (int pz = 0; pz < 3; ++pz) {  // one z-plane of links at a time keeps the kernel at 8 blocks per SM
+        const int cz = pz - 1;
+        bool fl;
+        const int zz = wrap_far(z + cz, a.dm.nz, a.dm.mode[2], fl);
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1)
-      for (int q = 0; q < 3; ++q) acc[q] += __shfl_down_sync(0xffffffffu, acc[q], off);
-    // lanes 0-2 add the force components, lanes 3-5 the torque components: one shared-memory atomic per lane
-    const double F0 = -shfl_d(acc[0], 0), F1 = -shfl_d(acc[1], 0), F2 = -shfl_d(acc[2], 0);
-    if (lane < 6) {
+        for (int j = 0; j < 9; ++j) {
+          const int cx = j % 3 - 1, cy = j / 3 - 1, i = 9 * pz + j;
+          if (i == 13) continue;
+          const int xx = wrap_far(x + cx, a.dm.nx, a.dm.mode[0], fl);
+          const int yy = wrap_far(y + cy, a.dm.ny, a.dm.mode[1], fl);
+          // stored values are deviations: f = w + dev, and w_i = w_ibar
+          const double w = (cx ? 1.0 / 6.0 : 2.0 / 3.0) * (cy ? 1.0 / 6.0 : 2.0 / 3.0) * (cz ? 1.0 / 6.0 : 2.0 / 3.0);
+          const double fa = w + (double)__ldg(a.f + pop_index(a.dm, i, xx, yy, zz));
+          const double fb = w + (double)__ldg(a.f + pop_index(a.dm, 26 - i, x, y, z));
+          const double ci[3] = {(double)cx, (double)cy, (double)cz};
+#pragma unroll
+          for (int q = 0; q < 3; ++q) acc[q] += (ci[q] - us[q]) * fa + (ci[q] + us[q]) * fb;
+        }
+      }
       const double r0 = x - a.bo.c[k][0], r1 = y - a.bo.c[k][1], r2 = z - a.bo.c[k][2];
-      const double v = lane == 0 ? F0 : lane == 1 ? F1 : lane == 2 ? F2
-                     : lane == 3 ? r1 * F2 - r2 * F1 : lane == 4 ? r2 * F0 - r0 * F2 : r0 * F1 - r1 * F0;
-      atomicAdd(lane < 3 ? &bins[k * 3 + lane] : &bins_m[k * 3 + lane - 3], v);
+      v[0] = -acc[0];
+      v[1] = -acc[1];
+      v[2] = -acc[2];
+      v[3] = r1 * v[2] - r2 * v[1];
+      v[4] = r2 * v[0] - r0 * v[2];
+      v[5] = r0 * v[1] - r1 * v[0];
+    }
+    const int k0 = __shfl_sync(0xffffffffu, k, 0);  // lane 0 is active whenever the warp is here
+    if (__all_sync(0xffffffffu, !act || k == k0)) {
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1)
+#pragma unroll
+        for (int q = 0; q < 6; ++q) v[q] += __shfl_down_sync(0xffffffffu, v[q], off);
+      if (lane == 0) {
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+          atomicAdd(&bins[k0 * 3 + q], v[q]);
+          atomicAdd(&bins_m[k0 * 3 + q], v[3 + q]);
+        }
+      }
+    } else if (act) {
+#pragma unroll
+      for (int q = 0; q < 3; ++q) {
+        atomicAdd(&bins[k * 3 + q], v[q]);
+        atomicAdd(&bins_m[k * 3 + q], v[3 + q]);
+      }
     }
   }
   __syncthreads();
@@ -344,7 +385,7 @@ __device__ __forceinline__ void force_block(const ForceArgs& a, int block, int n
 // Phase A of K3 and K4 read the same post-stream populations and nothing of each other: one launch,
 // even blocks sample the wall-model velocities, odd blocks collect the forces.  Both are gathers whose
 // latency hides behind the other's.
-__global__ void __launch_bounds__(128) sample_force_kernel(const __grid_constant__ WmArgs w,
+__global__ void __launch_bounds__(128, 8) sample_force_kernel(const __grid_constant__ WmArgs w,
                                                            const __grid_constant__ ForceArgs f, int wm_on, int split) {
   // of every four blocks, `split` sample wall-model velocities and 4 - split collect forces
   const int quad = blockIdx.x >> 2, r = blockIdx.x & 3, nquad = gridDim.x >> 2;
@@ -399,9 +440,9 @@ cudaError_t launch_wall_model_and_forces(hhrr_lattice* L) {
   a.out = L->force + (L->step % FORCE_HISTORY) * MAX_TAGS * 3;
   a.out_m = L->torque + (L->step % FORCE_HISTORY) * MAX_TAGS * 3;
   zero_force_kernel<<<1, 64, 0, L->stream>>>(a.out, a.out_m);
-  static const int split = getenv("HHRR_SF_SPLIT") ? atoi(getenv("HHRR_SF_SPLIT")) : 2;
-  static const int sf_blocks = getenv("HHRR_SF_BLOCKS") ? atoi(getenv("HHRR_SF_BLOCKS")) : 4736;
-  sample_force_kernel<<<L->wm_enabled ? sf_blocks : sf_blocks / 2, 128, 0, L->stream>>>(w, a, L->wm_enabled ? 1 : 0, split);
+  // 8 blocks per SM (64 registers): 4736 = 4 waves; two of every four blocks sample, two collect forces (measured:
+  // 1:3 and 3:1 are both slower)
+  sample_force_kernel<<<L->wm_enabled ? 4736 : 2368, 128, 0, L->stream>>>(w, a, L->wm_enabled ? 1 : 0, 2);
   L->launches += 2;
   if (L->wm_enabled) {
     wall_model_kernel<<<592, 128, 0, L->stream>>>(w);

@@ -145,10 +145,10 @@ __global__ void __launch_bounds__(128) geometry_type_kernel(GeoArgs a) {
   // x into one byte (the columns just outside the run by the first and last thread), the 3-wide OR along
   // x then comes from shared memory -- 9 byte loads per cell instead of 26.
   __shared__ uint8_t col[128 + 2];
+  bool near_row = false;  // rows with no cell below eps/2 in any of the nine neighbouring rows need no cell test
   {
     const int nx = a.dm.nx, ny = a.dm.ny, nz = a.dm.nz;
     int rows[9];
-    bool near_row = false;  // rows with no cell below eps/2 in any of the nine neighbouring rows need no cell test
 #pragma unroll
     for (int r = 0; r < 9; ++r) {
       rows[r] = wrap_any(y + r % 3 - 1, ny, a.dm.mode[1]) + ny * wrap_any(z + r / 3 - 1, nz, a.dm.mode[2]);
@@ -176,9 +176,11 @@ __global__ void __launch_bounds__(128) geometry_type_kernel(GeoArgs a) {
     const int nx = a.dm.nx, ny = a.dm.ny, nz = a.dm.nz;
     const int64_t snx = nx, snxy = (int64_t)nx * ny;
     c = x + snx * y + snxy * z;
-    double phi = a.phi[c];
-    uint8_t fl = a.flags[c];
-    int tg = a.tag_prov[c];
+    // a row with no cell below eps/2 in it or around it (most rows of the box: the blades cover a small part of the
+    // disc) holds plain fluid / fringe cells only: phi >= eps/2, no tag, not in W -- nothing to read
+    double phi = near_row ? a.phi[c] : BIG_PHI;
+    uint8_t fl = near_row ? a.flags[c] : (uint8_t)0;
+    int tg = near_row ? a.tag_prov[c] : 0;
     int type;
     float d;
     if (a.has_fringe && x >= a.fr_x0 && x < a.fr_x1) {

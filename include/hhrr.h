@@ -110,7 +110,13 @@ typedef struct hhrr_lattice hhrr_lattice; /* opaque, owned by the library */
 size_t hhrr_workspace_bytes(const hhrr_params* p, const hhrr_rotor_desc* rotor);
 
 /* Creates a lattice at rest (f_i = w_i, d = 1, no geometry) in the caller's device
- * workspace.  `cuda_stream` is a cudaStream_t.                                       */
+ * workspace.  `cuda_stream` is a cudaStream_t: every kernel and copy of the library is
+ * queued on it, except the first half of the NEXT step's porosity update (rotor signed
+ * distance; a function of the step count only), which hhrr_step queues on
+ * one internal low-priority stream, ordered against `cuda_stream` by events, so that it
+ * overlaps the tail of the collide-stream kernel.  Results do not depend on it (environment
+ * variable HHRR_NO_LOOKAHEAD=1 at creation switches it off, for measurement).  The workspace
+ * must stay allocated until hhrr_destroy, which waits for both streams.                  */
 int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes, void* cuda_stream,
                 hhrr_lattice** out);
 int hhrr_destroy(hhrr_lattice* L);

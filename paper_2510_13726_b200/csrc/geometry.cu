@@ -154,6 +154,33 @@ __global__ void __launch_bounds__(128) geometry_type_kernel(GeoArgs a) {
       rows[r] = wrap_any(y + r % 3 - 1, ny, a.dm.mode[1]) + ny * wrap_any(z + r / 3 - 1, nz, a.dm.mode[2]);
       near_row |= a.rowflag[rows[r]] != 0;
     }
+    if (!near_row) {
+      // Most rows of the box (the blades cover a small part of the disc): every cell has phi >= eps/2 and no cell
+      // below eps/2 next to it -- plain fluid / fringe / bulk, no tag, not in W, in no list.  The whole block
+      // leaves here (y, z are block-uniform), before the barrier and the ballots.
+      if (active) {
+        int type = HHRR_FLUID;
+        float d = 1.f;
+        if (a.has_fringe && x >= a.fr_x0 && x < a.fr_x1) {
+          type = HHRR_FRINGE;
+          d = 0.f;
+        }
+        if (a.fsi.n > 0) {
+          bool inside = false;
+          for (int b = 0; b < a.fsi.n; ++b)
+            inside |= x >= a.fsi.b[b].x0 && x < a.fsi.b[b].x1 && y >= a.fsi.b[b].y0 && y < a.fsi.b[b].y1 &&
+                      z >= a.fsi.b[b].z0 && z < a.fsi.b[b].z1;
+          if (!inside) {
+            if (type == HHRR_FLUID) type = HHRR_BULK;
+            else a.cnt->region_violation = 1;
+          }
+        }
+        const int64_t cc = x + (int64_t)nx * (y + (int64_t)ny * z);
+        a.flags[cc] = (uint8_t)type;
+        a.d[cc] = d;
+      }
+      return;
+    }
     const int t = threadIdx.x, T = blockDim.x;
     if (near_row) {
       for (int s = t; s < T + 2; s += T) {  // s = t, and t + T for the first two threads

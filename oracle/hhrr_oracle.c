@@ -823,11 +823,15 @@ static void forces(ohrr_lattice *L) {
         double acc[3] = {0, 0, 0};
         for (int i = 0; i < Q; ++i) {
           if (i == 13) continue;
-          int fl;
-          int xx = wrap1(x + CX[i], nx, L->p.mode[0], &fl);
-          int yy = wrap1(y + CY[i], ny, L->p.mode[1], &fl);
-          int zz = wrap1(z + CZ[i], nz, L->p.mode[2], &fl);
-          double fa = L->f[(int64_t)i * n + lidx(L, xx, yy, zz)];
+          /* R12: the cell behind a MIRROR plane is the reflected image of the lattice, so f_i there is the
+           * population of the reflected cell whose normal velocity component is reversed (the same rule the
+           * streaming step O3 applies to a population leaving through the plane)                          */
+          int flx, fly, flz;
+          int xx = wrap1(x + CX[i], nx, L->p.mode[0], &flx);
+          int yy = wrap1(y + CY[i], ny, L->p.mode[1], &fly);
+          int zz = wrap1(z + CZ[i], nz, L->p.mode[2], &flz);
+          int ir = ((flx ? -CX[i] : CX[i]) + 1) + 3 * ((fly ? -CY[i] : CY[i]) + 1) + 9 * ((flz ? -CZ[i] : CZ[i]) + 1);
+          double fa = L->f[(int64_t)ir * n + lidx(L, xx, yy, zz)];
           double fb = L->f[(int64_t)(26 - i) * n + c];
           double ci[3] = {CX[i], CY[i], CZ[i]};
           for (int a = 0; a < 3; ++a) acc[a] += (ci[a] - us[a]) * fa + (ci[a] + us[a]) * fb;

@@ -329,17 +329,21 @@ __device__ __forceinline__ void force_block(const ForceArgs& a, int block, int n
 #pragma unroll 1
       for (int pz = 0; pz < 3; ++pz) {  // one z-plane of links at a time keeps the kernel at 8 blocks per SM
         const int cz = pz - 1;
-        bool fl;
-        const int zz = wrap_far(z + cz, a.dm.nz, a.dm.mode[2], fl);
+        bool flx, fly, flz;
+        const int zz = wrap_far(z + cz, a.dm.nz, a.dm.mode[2], flz);
 #pragma unroll
         for (int j = 0; j < 9; ++j) {
           const int cx = j % 3 - 1, cy = j / 3 - 1, i = 9 * pz + j;
           if (i == 13) continue;
-          const int xx = wrap_far(x + cx, a.dm.nx, a.dm.mode[0], fl);
-          const int yy = wrap_far(y + cy, a.dm.ny, a.dm.mode[1], fl);
-          // stored values are deviations: f = w + dev, and w_i = w_ibar
+          const int xx = wrap_far(x + cx, a.dm.nx, a.dm.mode[0], flx);
+          const int yy = wrap_far(y + cy, a.dm.ny, a.dm.mode[1], fly);
+          // R12: the cell behind a MIRROR plane is the reflected image of the lattice -- f_i there is the population
+          // of the reflected cell with the normal velocity component reversed (what push_store does to a
+          // population that leaves through the plane)
+          const int ir = i - (flx ? 2 * cx : 0) - (fly ? 6 * cy : 0) - (flz ? 18 * cz : 0);
+          // stored values are deviations: f = w + dev, and w_i = w_ibar = w of the reflected direction
           const double w = (cx ? 1.0 / 6.0 : 2.0 / 3.0) * (cy ? 1.0 / 6.0 : 2.0 / 3.0) * (cz ? 1.0 / 6.0 : 2.0 / 3.0);
-          const double fa = w + (double)__ldg(a.f + pop_index(a.dm, i, xx, yy, zz));
+          const double fa = w + (double)__ldg(a.f + pop_index(a.dm, ir, xx, yy, zz));
           const double fb = w + (double)__ldg(a.f + pop_index(a.dm, 26 - i, x, y, z));
           const double ci[3] = {(double)cx, (double)cy, (double)cz};
 #pragma unroll

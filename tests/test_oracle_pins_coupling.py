@@ -1,0 +1,671 @@
+"""More pins of the fp64 oracle (CPU only): the parts a mutation test of round 1 found unpinned.
+
+Each test names the oracle part it pins, the PAPER.md passage / DESIGN.md reading, and the plausible
+mistake it is there to catch (DESIGN.md section 4 keeps the table mutation -> failing test).  Expected
+values are assembled here from numpy primitives and the mathematics, never from the oracle's own
+formula and never from the CUDA path.
+"""
+import numpy as np
+import pytest
+
+Q = 27
+
+
+def _c(O):
+    cx, cy, cz, w = O.lattice_tables()
+    return np.stack([cx, cy, cz]).astype(np.float64), w
+
+
+def _grid(nx, ny, nz):
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    return x.reshape(-1), y.reshape(-1), z.reshape(-1)
+
+
+def _tau_fixed_point(tau0, cs, rho, pi):
+    """Eq. 4 + Eq. 14 with R6, solved by fixed-point iteration instead of the closed form:
+    tau = tau0 + nu_t/cs^2, nu_t = Cs^2 |S|, |S| = sqrt(2 S:S), S = -Pi/(2 rho cs^2 tau)."""
+    tau = tau0
+    for _ in range(200):
+        S = -pi / (2 * rho / 3 * tau)
+        tau = tau0 + 3 * cs ** 2 * np.sqrt(2 * np.sum(S * S))
+    return tau
+
+
+def _unstream(O, f1, shape, cell):
+    """Post-collision populations of `cell` = (x, y, z): f*_i(x) = f_i(x + c_i, n+1) (Eq. 6 lhs);
+    the caller makes sure no link of the cell crosses a MIRROR plane (periodic wrap otherwise)."""
+    nz, ny, nx = shape
+    c, _ = _c(O)
+    F = f1.reshape(Q, nz, ny, nx)
+    x, y, z = cell
+    return np.array([F[i, (z + int(c[2, i])) % nz, (y + int(c[1, i])) % ny, (x + int(c[0, i])) % nx] for i in range(Q)])
+
+
+# ------------------------------------------------------------------ wall model -> collision coupling
+def test_wall_model_state_is_consumed_by_the_collision(oracle):
+    """"K3 writes, K2 consumes" (R8, R10): on a wall-model cell the collision takes
+    u^B = u^s + u_wm, S := S_wm and sigma := 0, whatever the global sigma says.  Flat moving wall, noisy
+    sheared flow, global sigma = 0.995: after wall_model_only() + one step the post-collision first moment
+    of a wall cell is rho (d u + (1-d)(u^s + u_wm)) and its second moment is
+    rho uh uh + rho cs^2 I - (1 - 1/tau_eff) 2 rho cs^2 tau_eff S_wm with the STORED u_wm, S_wm.
+    Catches: sigma := 0 dropped, S_wm not consumed (FD strain used), slip velocity not added to u^B."""
+    from paper_2510_13726_b200 import inputs
+    nx, ny, nz = 6, 12, 5
+    n = nx * ny * nz
+    c, w = _c(oracle)
+    x, y, z = _grid(nx, ny, nz)
+    tau0, sig, cs = 0.5 + 3 * 3.156e-4, 0.995, 0.1
+    g = np.array([2e-6, 0.0, -1e-6])
+    Vw = np.array([0.004, 0.0, -0.003])
+    L = oracle.Lattice(oracle.make_params(nx, ny, nz, mode=(0, 1, 0), tau0=tau0, sigma=sig, smagorinsky_cs=cs,
+                                          body_force=tuple(g), sampling_distance=2.0))
+    L.set_static_geometry(inputs.wall_phi(nx, ny, nz, 1.25), np.ones(n, np.uint8))
+    L.set_body(1, vel=Vw)
+    L.enable_wall_model(True)
+    u = np.zeros((3, n))
+    u[0] = 0.02 + 0.004 * y + 0.003 * np.sin(2 * np.pi * x / nx)
+    u[2] = -0.01 + 0.002 * y * np.cos(2 * np.pi * z / nz)
+    L.init_equilibrium(np.ones(n), u, True)
+    rng = np.random.default_rng(41)
+    f0 = L.populations() * (1 + 0.01 * rng.standard_normal((Q, n)))
+    L.set_populations(f0)
+    L.wall_model_only()
+    idx, y1n, _, valid = L.wall_list()
+    assert len(idx) == nx * nz and np.all(valid == 1) and np.all(y[idx] == 2)
+    stored = {int(cell): L.wall_state(int(cell)) for cell in idx}
+    L.step(1)
+    f1 = L.populations()
+    d = 0.875                                         # phi = 0.75, Eq. 22 with eps = 2
+    worst_fd_vs_wm = 0.0
+    for cell in idx[::3]:
+        cell = int(cell)
+        ok, utau, uwm, s = stored[cell]
+        assert ok == 1 and utau > 0 and np.linalg.norm(uwm) > 1e-4
+        S = np.array([[s[0], s[3], s[4]], [s[3], s[1], s[5]], [s[4], s[5], s[2]]])
+        f = f0[:, cell]
+        rho = f.sum()
+        uu = (c @ f + g) / rho
+        uh = d * uu + (1 - d) * (Vw + uwm)
+        post = _unstream(oracle, f1, (nz, ny, nx), (x[cell], y[cell], z[cell]))
+        assert np.allclose(c @ post, rho * uh, atol=1e-15)
+        pi = np.einsum("i,ai,bi->ab", f, c, c) - rho / 3 * np.eye(3) - rho * np.outer(uh, uh)
+        tau = _tau_fixed_point(tau0, cs, rho, pi)
+        P = np.einsum("i,ai,bi->ab", post, c, c)
+        expect = rho * np.outer(uh, uh) + rho / 3 * np.eye(3) - (1 - 1 / tau) * 2 * rho / 3 * tau * S
+        assert np.allclose(P, expect, atol=1e-14), np.max(np.abs(P - expect))
+        # the test is sensitive: the terms a wrong coupling would add are orders above the tolerance
+        assert np.max(np.abs((1 - 1 / tau) * sig * pi)) > 1e-7            # sigma = 0.995 instead of 0
+        assert np.max(np.abs((1 - 1 / tau) * 2 * rho / 3 * tau * S)) > 1e-9
+        assert np.linalg.norm(rho * (1 - d) * uwm) > 1e-6               # slip missing from u^B
+        worst_fd_vs_wm = max(worst_fd_vs_wm, np.max(np.abs(S)))
+    assert worst_fd_vs_wm > 1e-4
+    # the time-n field the FD strain of the NEIGHBOURS differentiates carries the slip too (O2 step 2 feeds step 5):
+    # growth cell above a wall cell, d = 1, global sigma, central differences of uh assembled here
+    drow = np.array([0.0, 0.375, 0.875] + [1.0] * (ny - 3))
+
+    def uhat(cx_, cy_, cz_):
+        cell_ = (cx_ % nx) + nx * (cy_ + ny * (cz_ % nz))
+        f_ = f0[:, cell_]
+        uB_ = Vw + (stored[cell_][2] if cell_ in stored else 0.0)
+        return drow[cy_] * (c @ f_ + g) / f_.sum() + (1 - drow[cy_]) * uB_
+
+    for (xx, zz) in ((1, 1), (4, 3)):
+        cell = xx + nx * (3 + ny * zz)
+        grad = np.zeros((3, 3))
+        grad[:, 0] = 0.5 * (uhat(xx + 1, 3, zz) - uhat(xx - 1, 3, zz))
+        grad[:, 1] = 0.5 * (uhat(xx, 4, zz) - uhat(xx, 2, zz))
+        grad[:, 2] = 0.5 * (uhat(xx, 3, zz + 1) - uhat(xx, 3, zz - 1))
+        S = 0.5 * (grad + grad.T)
+        f = f0[:, cell]
+        rho, uh = f.sum(), uhat(xx, 3, zz)
+        pi = np.einsum("i,ai,bi->ab", f, c, c) - rho / 3 * np.eye(3) - rho * np.outer(uh, uh)
+        tau = _tau_fixed_point(tau0, cs, rho, pi)
+        post = _unstream(oracle, f1, (nz, ny, nx), (xx, 3, zz))
+        P = np.einsum("i,ai,bi->ab", post, c, c)
+        expect = rho * np.outer(uh, uh) + rho / 3 * np.eye(3) + (1 - 1 / tau) * (sig * pi - (1 - sig) * 2 * rho / 3 * tau * S)
+        assert np.allclose(P, expect, atol=1e-15), np.max(np.abs(P - expect))
+        slip = stored[xx + nx * (2 + ny * zz)][2]
+        assert (1 - sig) * 2 * rho / 3 * 0.25 * 0.125 * np.max(np.abs(slip)) > 1e-9   # what a slip-less field would change
+    # a frontier cell that is NOT in W (row y = 1, phi < 0) keeps the plain HLBM momentum: u^B = u^s only
+    cell = int(np.flatnonzero((y == 1) & (x == 2) & (z == 1))[0])
+    f = f0[:, cell]
+    rho = f.sum()
+    uh = 0.375 * (c @ f + g) / rho + 0.625 * Vw
+    post = _unstream(oracle, f1, (nz, ny, nx), (2, 1, 1))
+    assert np.allclose(c @ post, rho * uh, atol=1e-15)
+
+
+def test_fd_strain_differs_from_wall_strain_in_the_coupling_case(oracle):
+    """Companion of the test above: on the same kind of state a frontier cell WITHOUT wall-model state (wall
+    model disabled) collides with the global sigma and the central-difference strain of the homogenised
+    velocity (R5) -- the two closures give measurably different second moments, so the test above tells them
+    apart."""
+    from paper_2510_13726_b200 import inputs
+    nx, ny, nz = 6, 12, 5
+    n = nx * ny * nz
+    c, w = _c(oracle)
+    x, y, z = _grid(nx, ny, nz)
+    tau0, sig, cs = 0.5 + 3 * 3.156e-4, 0.6, 0.1
+    L = oracle.Lattice(oracle.make_params(nx, ny, nz, mode=(0, 1, 0), tau0=tau0, sigma=sig, smagorinsky_cs=cs))
+    phi = inputs.wall_phi(nx, ny, nz, 1.25).astype(np.float64)
+    L.set_static_geometry(phi, np.ones(n, np.uint8))
+    u = np.zeros((3, n))
+    u[0] = 0.02 + 0.004 * y + 0.003 * np.sin(2 * np.pi * x / nx)
+    L.init_equilibrium(np.ones(n), u, True)
+    f0 = L.populations()
+    L.step(1)
+    f1 = L.populations()
+    dd = np.clip(phi / 2 + 0.5, 0, 1)
+    F = f0.reshape(Q, nz, ny, nx)
+    rho = F.sum(0)
+    uh = dd.reshape(nz, ny, nx) * np.einsum("ai,izyx->azyx", c, F) / rho          # u^B = 0
+    cell = (2, 2, 1)
+    xx, yy, zz = cell
+    grad = np.zeros((3, 3))
+    grad[:, 0] = 0.5 * (uh[:, zz, yy, (xx + 1) % nx] - uh[:, zz, yy, (xx - 1) % nx])
+    grad[:, 1] = 0.5 * (uh[:, zz, yy + 1, xx] - uh[:, zz, yy - 1, xx])
+    grad[:, 2] = 0.5 * (uh[:, (zz + 1) % nz, yy, xx] - uh[:, (zz - 1) % nz, yy, xx])
+    S = 0.5 * (grad + grad.T)
+    f = F[:, zz, yy, xx]
+    r, uc = rho[zz, yy, xx], uh[:, zz, yy, xx]
+    pi = np.einsum("i,ai,bi->ab", f, c, c) - r / 3 * np.eye(3) - r * np.outer(uc, uc)
+    tau = _tau_fixed_point(tau0, cs, r, pi)
+    post = _unstream(oracle, f1, (nz, ny, nx), cell)
+    P = np.einsum("i,ai,bi->ab", post, c, c)
+    expect = r * np.outer(uc, uc) + r / 3 * np.eye(3) + (1 - 1 / tau) * (sig * pi - (1 - sig) * 2 * r / 3 * tau * S)
+    assert np.allclose(P, expect, atol=1e-15)
+
+
+# ------------------------------------------------------------------ Newton derivative (Eq. 19)
+_SAMPLES = [(0.05, 2.75, 3.156e-4), (0.04, 3.0, 6.25e-5), (1e-4, 2.2, 1e-2), (0.2, 2.9, 1.3e-4), (0.06, 2.1, 2e-5)]
+
+
+def _centred(fun, u, h):
+    return (fun(u + h) - fun(u - h)) / (2 * h)
+
+
+@pytest.mark.parametrize("U,y,nu", _SAMPLES)
+@pytest.mark.parametrize("kind", ["spalding", "musker"])
+def test_newton_derivative_is_the_slope_of_the_residual(oracle, kind, U, y, nu):
+    """Eq. 19: u^{j+1} = u^j - f(u^j)/f'(u^j).  One iteration from u^0 reveals the derivative
+    the oracle uses, f'(u^0) = f(u^0)/(u^0 - u^1); it must be the slope of the exported residual (Eq. 18,
+    :172, pinned by test_spalding_relation) -- here taken by a centred difference (Richardson-extrapolated),
+    to 1e-7.  Then the exact iterates after 1, 2, 3 steps from the cold start of Eq. 20 (:181) against a
+    numpy Newton that uses that difference quotient.  With the paper's 10-iteration cap (:184) the
+    derivative decides the unconverged u_tau that parity compares.
+    Catches: a dropped k^2/2 (or any other) term of f', a wrong sign or factor of y/nu."""
+    if kind == "spalding":
+        f = lambda u: oracle.spalding_f(u, U, y, nu)
+        newton = lambda u0, k: oracle.newton_utau(u0, U, y, nu, max_iter=k, tol=0.0)[0]
+    else:
+        f = lambda u: oracle.musker_f(u, U, y, nu)
+        newton = lambda u0, k: oracle.newton_utau_musker(u0, U, y, nu, max_iter=k, tol=0.0)[0]
+    cold = np.sqrt(nu * U / y)
+    root = newton(cold, 400)
+
+    def slope(u):
+        h = 1e-3 * u
+        return (4 * _centred(f, u, h / 2) - _centred(f, u, h)) / 3          # O(h^4)
+
+    for u0 in (cold, 0.5 * (cold + root), 1.3 * root):
+        u1 = newton(u0, 1)
+        if u1 == 0.5 * u0:                # the R9 safeguard replaced the step: no derivative to read off
+            continue
+        used = f(u0) / (u0 - u1)
+        assert used == pytest.approx(slope(u0), rel=1e-7), (u0, used, slope(u0))
+    ref = cold
+    for k in (1, 2, 3):
+        ref = ref - f(ref) / slope(ref)
+        assert newton(cold, k) == pytest.approx(ref, rel=1e-6)
+    assert abs(newton(cold, 1) - cold) > 1e-3 * cold or abs(root - cold) < 1e-3 * cold
+
+
+# ------------------------------------------------------------------ warm start (Eq. 20) and moving wall
+def _flat_wall(oracle, V, tau0, nx=4, ny=12, nz=4, **kw):
+    from paper_2510_13726_b200 import inputs
+    n = nx * ny * nz
+    L = oracle.Lattice(oracle.make_params(nx, ny, nz, mode=(0, 1, 0), tau0=tau0, sampling_distance=2.0, **kw))
+    L.set_static_geometry(inputs.wall_phi(nx, ny, nz, 1.25), np.ones(n, np.uint8))
+    L.enable_wall_model(True)
+    L.init_equilibrium(np.ones(n), np.tile(np.asarray(V, float)[:, None], (1, n)), False)
+    return L
+
+
+def test_wall_model_warm_start(oracle):
+    """Eq. 20: "previous u_tau if available", the cold guess sqrt(nu U / y) otherwise.  With
+    newton_max_iter = 1, tol = 0 every WallModelO call advances the Newton iteration by exactly one step, so
+    after k calls on the same flow the stored u_tau is the k-step iterate from the cold start.
+    Catches: an always-cold start (u_tau would stay at the 1-step value), a warm start from anything but the
+    stored u_tau."""
+    tau0 = 0.5 + 3 * 6.25e-5
+    nu = (tau0 - 0.5) / 3
+    V = np.array([0.05, 0.0, -0.02])
+    U, yy = np.linalg.norm(V), 2.75
+    L = _flat_wall(oracle, V, tau0, newton_max_iter=1, newton_tol=0.0)
+    cold = np.sqrt(nu * U / yy)
+    seen = []
+    for k in (1, 2, 3, 4, 5):
+        L.wall_model_only()
+        idx, _, ut, valid = L.wall_list()
+        assert np.all(valid == 1)
+        expect, _ = oracle.newton_utau(cold, U, yy, nu, max_iter=k, tol=0.0)
+        assert np.allclose(ut, expect, rtol=1e-14, atol=0)
+        seen.append(ut[0])
+    assert all(abs(b - a) > 1e-4 * a for a, b in zip(seen, seen[1:]))     # the iteration is still moving
+    # with the paper's stop rule (10 / 1e-4) the second call continues from the first one's u_tau
+    # (in the log layer ten iterations from the cold start are not yet converged)
+    L = _flat_wall(oracle, V, tau0)
+    L.wall_model_only(); u1 = L.wall_list()[2][0]
+    L.wall_model_only(); u2 = L.wall_list()[2][0]
+    again, _ = oracle.newton_utau(u1, U, yy, nu)
+    assert u2 == again and u2 != u1
+
+
+def test_moving_wall_uses_the_relative_velocity(oracle):
+    """"Moving Wall Model" (R15): the wall function sees the tangential velocity RELATIVE to
+    the wall, r = v_s - u^s(x_w).  Uniform stream V over a flat wall that translates at V_w and rotates about
+    its normal: U = |(V - u^s)_t| per wall cell, slip along (V - u^s)_t.
+    Catches: wall velocity not subtracted, subtracted with the wrong sign, normal part not projected out."""
+    tau0 = 0.5 + 3 * 3.156e-4
+    nu = (tau0 - 0.5) / 3
+    V = np.array([0.03, 0.004, -0.02])
+    Vw = np.array([0.011, 0.002, 0.007])
+    om = np.array([0.0, 0.0015, 0.0])
+    ctr = np.array([1.5, 0.0, 2.5])
+    nx, ny, nz = 4, 12, 4
+    L = _flat_wall(oracle, V, tau0)
+    L.set_body(1, centre=ctr, omega=om, vel=Vw)
+    L.wall_model_only()
+    idx, y1n, ut, valid = L.wall_list()
+    assert len(idx) == nx * nz
+    x, y, z = _grid(nx, ny, nz)
+    seenU = []
+    for k, cell in enumerate(idx):
+        us = Vw + np.cross(om, np.array([x[cell], y[cell], z[cell]]) - ctr)
+        r = V - us
+        rt = np.array([r[0], 0.0, r[2]])                      # normal = +y
+        U = np.linalg.norm(rt)
+        expect, _ = oracle.newton_utau(np.sqrt(nu * U / 2.75), U, 2.75, nu)
+        assert ut[k] == pytest.approx(expect, rel=1e-12)
+        ok, utau, uwm, swm = L.wall_state(int(cell))
+        assert np.allclose(uwm, utau * rt / U, rtol=1e-12, atol=1e-16)
+        seenU.append(U)
+    assert max(seenU) - min(seenU) > 1e-3                    # the rotation makes u^s differ from cell to cell
+    plain, _ = oracle.newton_utau(np.sqrt(nu * np.hypot(V[0], V[2]) / 2.75), np.hypot(V[0], V[2]), 2.75, nu)
+    assert abs(ut[0] - plain) > 1e-3 * plain
+
+
+# ------------------------------------------------------------------ geometry: growth layer, d_override, W, tags
+@pytest.mark.parametrize("solid,mode", [((3, 3, 3), (0, 0, 0)), ((0, 0, 0), (0, 0, 0)), ((6, 0, 3), (0, 0, 0)),
+                                        ((0, 3, 6), (1, 1, 1))])
+def test_growth_layer_is_the_26_neighbourhood(oracle, solid, mode):
+    """Fig. 4, :269: the growth layer is the one-cell shell around the tagged cells -- edge
+    and corner neighbours included, since a surface point may move diagonally.  One solid cell in a 7^3
+    lattice: exactly its 26 neighbours (periodic wrap, or reflection at MIRROR planes, R12) are GROWTH and
+    carry its tag.  Catches: growth from the 6 face neighbours only, no wrap at the lattice faces."""
+    n = 7
+    phi = np.full((n, n, n), 5.0)
+    sx, sy, sz = solid
+    phi[sz, sy, sx] = -1.5
+    tag = np.full(n ** 3, 3, np.uint8)
+    L = oracle.Lattice(oracle.make_params(n, n, n, mode=mode))
+    L.set_static_geometry(phi.reshape(-1), tag)
+    L.update_geometry()
+    t, g, d = L.cell_types()
+    t, g = t.reshape(n, n, n), g.reshape(n, n, n)
+    expect = np.zeros((n, n, n), np.uint8)
+    for dz in (-1, 0, 1):
+        for dy in (-1, 0, 1):
+            for dx in (-1, 0, 1):
+                q = []
+                for v, m in ((sx + dx, mode[0]), (sy + dy, mode[1]), (sz + dz, mode[2])):
+                    if m == 0:
+                        q.append(v % n)
+                    else:
+                        q.append(-1 - v if v < 0 else (2 * n - 1 - v if v >= n else v))
+                expect[q[2], q[1], q[0]] = oracle.T_GROWTH
+    expect[sz, sy, sx] = oracle.T_SOLID
+    assert np.array_equal(t, expect)
+    if mode == (0, 0, 0):
+        assert np.count_nonzero(t == oracle.T_GROWTH) == 26
+    assert np.all(g[t == oracle.T_GROWTH] == 3) and np.all(g[t == oracle.T_FLUID] == 0)
+    assert np.all(d.reshape(n, n, n)[t != oracle.T_SOLID] == 1.0)
+
+
+def test_porosity_override_only_inside_the_band(oracle):
+    """Def. 1: d = 0 / 1 outside the transition band, "a smooth transition function s"
+    inside it; config 2 passes its tanh ramp as d_override.  The override must be taken for FRONTIER cells
+    (|phi| < eps/2) and for no other cell.  Catches: d_override ignored (Eq. 22 used), or applied to solid /
+    fluid cells."""
+    from paper_2510_13726_b200 import inputs
+    n = 20
+    phi = inputs.sphere_phi(n, n, n, (9.5, 9.5, 9.5), 5.0).astype(np.float64)
+    marker = 0.1 + 0.8 * np.random.default_rng(3).random(n ** 3)
+    L = oracle.Lattice(oracle.make_params(n, n, n, eps_cells=2.0))
+    L.set_static_geometry(phi, np.ones(n ** 3, np.uint8), marker)
+    L.update_geometry()
+    t, _, d = L.cell_types()
+    band = np.abs(phi) < 1.0
+    assert np.count_nonzero(band) > 200
+    assert np.array_equal(t == oracle.T_FRONTIER, band)
+    assert np.array_equal(d[band], marker[band])
+    assert np.all(d[phi <= -1.0] == 0.0) and np.all(d[phi >= 1.0] == 1.0)
+    # config 2's own ramp: level set d = 1/2 on phi = 0, monotone, inside [0, 1]
+    ramp = inputs.tanh_transition(np.array([-1.0, -0.5, 0.0, 0.5, 1.0]), 2.0)
+    assert ramp[2] == 0.5 and np.all(np.diff(ramp) > 0) and ramp[0] == 0.0 and ramp[-1] == 1.0
+
+
+def test_wall_state_is_dropped_when_a_cell_leaves_the_wall_set(oracle):
+    """SURVEY O1 / DESIGN R14: the wall-model arrays of cells not in W_n are invalidated, so a cell that
+    re-enters W later collides once as an ordinary cell and Newton restarts from Eq. 20 (the
+    previous u_tau only "if available").  Wall moved up by one cell and back.
+    Catches: stale wall state kept for cells that left W."""
+    from paper_2510_13726_b200 import inputs
+    nx, ny, nz = 4, 12, 4
+    n = nx * ny * nz
+    tau0 = 0.5 + 3 * 3.156e-4
+    x, y, z = _grid(nx, ny, nz)
+    V = np.array([0.03, 0.0, -0.02])
+    L = _flat_wall(oracle, V, tau0)
+    L.wall_model_only()
+    row2 = np.flatnonzero(y == 2)
+    row3 = np.flatnonzero(y == 3)
+    assert all(L.wall_state(int(c))[0] == 1 for c in row2)
+    assert np.array_equal(L.wall_list()[0], row2)
+    L.set_static_geometry(inputs.wall_phi(nx, ny, nz, 2.25), np.ones(n, np.uint8))
+    L.update_geometry()
+    assert np.array_equal(L.wall_list()[0], row3)
+    assert all(L.wall_state(int(c))[0] == 0 for c in row2)          # left W: state dropped
+    assert all(L.wall_state(int(c))[0] == 0 for c in row3)          # entered W: nothing yet
+    L.set_static_geometry(inputs.wall_phi(nx, ny, nz, 1.25), np.ones(n, np.uint8))
+    L.update_geometry()
+    idx, _, _, valid = L.wall_list()
+    assert np.array_equal(idx, row2) and np.all(valid == 0)         # back in W, but its old state is gone
+    # and the next collision of such a cell is the ordinary one: global sigma, no slip (u^B = 0 here)
+    c, w = _c(oracle)
+    f0 = L.populations()
+    L.step(1)
+    cell = int(row2[5])
+    post = _unstream(oracle, L.populations(), (nz, ny, nx), (x[cell], y[cell], z[cell]))
+    rho = f0[:, cell].sum()
+    assert np.allclose(c @ post, rho * 0.875 * (c @ f0[:, cell]) / rho, atol=1e-16)
+
+
+def test_rotor_tag_is_the_tag_of_the_nearest_reference_node(oracle):
+    """PAPER.md:267 (integer tags on the reference grid), :265: a cell takes the element id of the reference
+    node NEAREST to its rotor-frame position, not of the node at the floor corner of its
+    interpolation cell.  Reference grid with a checkerboard of tags at a spacing / offset where the two differ
+    on every axis.  Catches: tag from floor(), tag axes transposed."""
+    G = 12
+    kz, ky, kx = np.meshgrid(np.arange(G), np.arange(G), np.arange(G), indexing="ij")
+    tag = (1 + (kx % 2) + 2 * (ky % 2) + 4 * (kz % 2)).astype(np.uint8)
+    sdf = np.full((G, G, G), -2.0, np.float32)
+    origin = (-5.7, -5.3, -5.5)
+    n = 16
+    ctr = (8.0, 8.0, 8.0)
+    L = oracle.Lattice(oracle.make_params(n, n, n))
+    L.set_rotor(sdf, tag, 1.0, origin, ctr, (1, 0, 0), 0.0, 0.0, 8)
+    L.update_geometry()
+    t, g, _ = L.cell_types()
+    t, g = t.reshape(n, n, n), g.reshape(n, n, n)
+    checked = 0
+    for z in range(n):
+        for y in range(n):
+            for x in range(n):
+                gx, gy, gz = x - ctr[0] - origin[0], y - ctr[1] - origin[1], z - ctr[2] - origin[2]
+                inside = all(0 <= np.floor(v) < G - 1 for v in (gx, gy, gz))
+                if not inside:
+                    assert t[z, y, x] != oracle.T_SOLID
+                    continue
+                assert t[z, y, x] == oracle.T_SOLID
+                node = [min(int(np.floor(v + 0.5)), G - 1) for v in (gx, gy, gz)]
+                assert g[z, y, x] == 1 + node[0] % 2 + 2 * (node[1] % 2) + 4 * (node[2] % 2)
+                checked += 1
+    assert checked == 11 ** 3
+
+
+# ------------------------------------------------------------------ fringe and the homogenised velocity field
+def test_fringe_imposes_the_inflow_velocity(oracle):
+    """Inflow fringe (R12: HLBM cells with d = 0, u^B = u_in): one periodic step on a noisy state.  (i) the
+    post-collision momentum of a fringe cell is rho u_in (P5 with u^B = u_in); (ii) in EVERY cell the
+    post-collision second moment is rho uh uh + rho cs^2 I + (1 - 1/tau)(sigma Pi - (1 - sigma) 2 rho cs^2 tau S)
+    with S the central differences of the homogenised field uh assembled here with np.roll -- fluid cells next
+    to the fringe differentiate across u_in.  Catches: u^B = u_in/2 (or any other value) in the collision or
+    in the time-n velocity field the FD strain differentiates."""
+    nx, ny, nz = 8, 5, 4
+    n = nx * ny * nz
+    c, w = _c(oracle)
+    rng = np.random.default_rng(23)
+    f0 = w[:, None] * (1 + 0.05 * rng.standard_normal((Q, n)))
+    tau0, sig, cs = 0.6, 0.3, 0.1
+    g = np.array([1e-4, -2e-4, 3e-4])
+    u_in = np.array([0.04, 0.01, -0.02])
+    L = oracle.Lattice(oracle.make_params(nx, ny, nz, tau0=tau0, sigma=sig, smagorinsky_cs=cs, body_force=tuple(g)))
+    L.set_fringe(0, 2, u_in)
+    L.set_populations(f0)
+    L.step(1)
+    t, _, d = L.cell_types()
+    x, y, z = _grid(nx, ny, nz)
+    assert np.array_equal(t == oracle.T_FRINGE, x < 2) and np.all(d[x < 2] == 0) and np.all(d[x >= 2] == 1)
+    F1 = L.populations().reshape(Q, nz, ny, nx)
+    post = np.stack([np.roll(F1[i], shift=(-int(c[2, i]), -int(c[1, i]), -int(c[0, i])), axis=(0, 1, 2))
+                     for i in range(Q)])
+    F0 = f0.reshape(Q, nz, ny, nx)
+    rho = F0.sum(0)
+    uu = (np.einsum("ai,izyx->azyx", c, F0) + g[:, None, None, None]) / rho
+    fr = (np.arange(nx) < 2)[None, None, :]
+    uh = np.where(fr[None], u_in[:, None, None, None], uu)
+    grad = np.zeros((3, 3) + rho.shape)
+    for b, ax in ((0, 2), (1, 1), (2, 0)):
+        grad[:, b] = 0.5 * (np.roll(uh, -1, axis=ax + 1) - np.roll(uh, 1, axis=ax + 1))
+    mom = np.einsum("ai,izyx->azyx", c, post)
+    assert np.allclose(mom, rho * uh, atol=1e-15)
+    P = np.einsum("izyx,ai,bi->abzyx", post, c, c)
+    worst = 0.0
+    for zz in range(nz):
+        for yy in range(ny):
+            for xx in range(nx):
+                r, uc = rho[zz, yy, xx], uh[:, zz, yy, xx]
+                G = grad[:, :, zz, yy, xx]
+                S = 0.5 * (G + G.T)
+                pi = np.einsum("i,ai,bi->ab", F0[:, zz, yy, xx], c, c) - r / 3 * np.eye(3) - r * np.outer(uc, uc)
+                tau = _tau_fixed_point(tau0, cs, r, pi)
+                e = r * np.outer(uc, uc) + r / 3 * np.eye(3) + (1 - 1 / tau) * (sig * pi - (1 - sig) * 2 * r / 3 * tau * S)
+                worst = max(worst, np.max(np.abs(P[:, :, zz, yy, xx] - e)))
+    assert worst < 1e-14, worst
+
+
+# ------------------------------------------------------------------ Eq. 23 across a MIRROR plane
+def test_force_on_a_mirror_lattice_equals_even_extension(oracle):
+    """Eq. 23 with R12: the ghost cell behind a MIRROR plane is the reflected image of the
+    lattice, so a link that crosses the plane reads the population with the NORMAL COMPONENT REVERSED at the
+    reflected cell.  A body touching the mirror plane on a MIRROR-y lattice of ny cells must feel, cell for
+    cell, the force of the same cells in the periodic lattice of 2 ny cells that holds the mirror-symmetric
+    state (test_mirror_axis_equals_even_extension pins the flow the same way).
+    Catches: the flip flag of the neighbour lookup ignored in the force sum (round-1 ADVICE: wall drag of
+    config 3 with the wrong sign)."""
+    from paper_2510_13726_b200 import inputs
+    nx, ny, nz = 10, 7, 9
+    rng = np.random.default_rng(31)
+    c, w = _c(oracle)
+    f0 = (w[:, None] * (1 + 0.05 * rng.standard_normal((Q, nz * ny * nx)))).reshape(Q, nz, ny, nx)
+    flip = np.array([int((c[0, i] + 1) + 3 * (-c[1, i] + 1) + 9 * (c[2, i] + 1)) for i in range(Q)])
+    big = np.zeros((Q, nz, 2 * ny, nx))
+    big[:, :, :ny] = f0
+    big[:, :, ny:] = f0[flip][:, :, ::-1]
+    # a ball cut by the lower mirror plane y = -1/2 and a slab lying on the upper one y = ny - 1/2
+    phi = np.minimum(inputs.sphere_phi(nx, ny, nz, (4.5, 0.3, 4.0), 2.6).astype(np.float64).reshape(nz, ny, nx),
+                     (ny - 2.2) - np.arange(ny, dtype=np.float64)[None, :, None] + 0 * f0[0])
+    tag = np.ones((nz, ny, nx), np.uint8)
+    tag[:, ny // 2:] = 2
+    phib = np.concatenate([phi, phi[:, ::-1]], axis=1)
+    tagb = np.concatenate([tag, tag[:, ::-1] + 2], axis=1)
+    kw = dict(tau0=0.58, sigma=0.3, smagorinsky_cs=0.12)
+    A = oracle.Lattice(oracle.make_params(nx, ny, nz, mode=(0, 1, 0), **kw))
+    B = oracle.Lattice(oracle.make_params(nx, 2 * ny, nz, **kw))
+    Us = np.array([0.01, 0.0, -0.004])
+    A.set_static_geometry(phi.reshape(-1), tag.reshape(-1)); B.set_static_geometry(phib.reshape(-1), tagb.reshape(-1))
+    for k in (1, 2):
+        A.set_body(k, vel=Us); B.set_body(k, vel=Us); B.set_body(k + 2, vel=Us)
+    A.set_populations(f0.reshape(Q, -1)); B.set_populations(big.reshape(Q, -1))
+    Fa, Fb = A.force_only(), B.force_only()
+    assert np.max(np.abs(Fb[1:3])) > 1e-2
+    assert np.allclose(Fa[1:3], Fb[1:3], rtol=0, atol=1e-13)
+    # mirror symmetry of the big lattice itself: the image bodies feel the reflected force
+    assert np.allclose(Fb[3:5] * np.array([1, -1, 1]), Fb[1:3], rtol=0, atol=1e-13)
+    A.step(3); B.step(3)
+    assert np.allclose(A.forces()[-1, 1:3], B.forces()[-1, 1:3], rtol=0, atol=1e-13)
+
+
+def test_half_channel_wall_drag_equals_body_force(oracle):
+    """Config 3's layout (wall row on one MIRROR plane, channel centreline on the other): in steady state the
+    momentum-exchange force on the wall is the momentum the body force injects per step, positive along g, and
+    the free-slip planes carry no tangential stress (round-1 ADVICE: F_x came out negative and ~100x too large)."""
+    nx, ny, nz = 3, 14, 3
+    tau0, g = 0.8, 1e-6
+    x, y, z = _grid(nx, ny, nz)
+    phi = y - 1.5
+    L = oracle.Lattice(oracle.make_params(nx, ny, nz, mode=(0, 1, 0), tau0=tau0, sigma=1.0, smagorinsky_cs=0.0,
+                                          body_force=(g, 0, 0), eps_cells=2.0))
+    L.set_static_geometry(phi, np.ones(nx * ny * nz, np.uint8))
+    L.init_equilibrium(np.ones(nx * ny * nz), np.zeros((3, nx * ny * nz)), False)
+    L.step(12000)
+    _, _, d = L.cell_types()
+    F = L.forces()[-1]
+    assert F[1, 0] > 0
+    assert F[1, 0] == pytest.approx(g * np.sum(d == 1.0), rel=1e-7)
+    assert abs(F[1, 2]) < 1e-12
+    # no net wall-normal load either: the fluid's pressure on the wall is balanced through the mirror plane
+    rho, _ = L.moments()
+    assert abs(F[1, 1]) < 1e-6 * np.mean(rho) / 3 * nx * nz
+
+
+# ------------------------------------------------------------------ Eq. 23: sign of the solid velocity
+def test_force_solid_velocity_term_is_minus_us_times_mass_inflow(oracle):
+    """Eq. 23 weighs the population that leaves the solid with (c_i - u_s) and the one that
+    enters with (c_i + u_s): momentum exchange in the frame of the moving wall (the paper's ref. [49]).
+    Splitting the sum, F(u_s) = F(0) - u_s * mdot with mdot = sum over the links of (entering - leaving)
+    populations = the net mass that streamed into {d < 1}, assembled here with np.roll.  F(0) is pinned by the
+    Poiseuille balance.  Catches: the two signs of u_s swapped (a uniform state cannot tell: both terms vanish)."""
+    from paper_2510_13726_b200 import inputs
+    n = 12
+    c, w = _c(oracle)
+    rng = np.random.default_rng(19)
+    f0 = w[:, None] * (1 + 0.08 * rng.standard_normal((Q, n ** 3)))
+    phi = inputs.sphere_phi(n, n, n, (5.3, 6.1, 5.6), 3.2)
+    Us = np.array([0.03, -0.02, 0.011])
+
+    def force(us):
+        L = oracle.Lattice(oracle.make_params(n, n, n))
+        L.set_static_geometry(phi, np.ones(n ** 3, np.uint8))
+        L.set_body(1, vel=us)
+        L.set_populations(f0)
+        F = L.force_only()
+        return F[1], L.cell_types()[2]
+
+    F0, d = force(np.zeros(3))
+    F1, _ = force(Us)
+    inside = (d < 1.0).reshape(n, n, n)
+    F = f0.reshape(Q, n, n, n)
+    mdot = 0.0
+    for i in range(Q):
+        if i == 13:
+            continue
+        # leaving through link i: f_i at x + c_i; entering through it: f_ibar at x
+        at_nb = np.roll(F[i], shift=(-int(c[2, i]), -int(c[1, i]), -int(c[0, i])), axis=(0, 1, 2))
+        mdot += np.sum((F[26 - i] - at_nb)[inside])
+    assert abs(mdot) > 1e-2
+    assert np.allclose(F1 - F0, -Us * mdot, rtol=1e-12, atol=1e-15)
+
+
+# ------------------------------------------------------------------ wall model on a curved wall
+def test_wall_model_on_a_sphere_in_a_linear_flow(oracle):
+    """WallModelO on oblique walls (PAPER.md:184 "interpolated velocity", :324 y1 normals; R13, R15, R10): a
+    sphere in the linear velocity field v = v0 + M x, for which trilinear interpolation is exact.  For every
+    wall cell: |y1 n| = phi, n ~ radial; the sample is v0 + M (x_w + h_s n), so U = |(v_s)_t|, u_tau = Newton
+    from the cold start at y = y1 + h_s, slip along the tangential sample, S_wm = sym((M n) n^T).
+    Catches: interpolation weights attached to the wrong corner / axis, normal not normalised, y1 wrong."""
+    from paper_2510_13726_b200 import inputs
+    n = 20
+    ctr = np.array([9.4, 9.7, 10.1])
+    phi = inputs.sphere_phi(n, n, n, ctr, 4.3)
+    tau0 = 0.5 + 3 * 3.156e-4
+    nu = (tau0 - 0.5) / 3
+    x, y, z = _grid(n, n, n)
+    pos = np.stack([x, y, z]).astype(np.float64)
+    v0 = np.array([0.02, -0.01, 0.015])
+    M = 1e-3 * np.array([[0.5, 1.2, -0.7], [-0.9, 0.3, 1.1], [0.8, -1.3, -0.8]])
+    u = v0[:, None] + M @ pos
+    L = oracle.Lattice(oracle.make_params(n, n, n, tau0=tau0, sampling_distance=2.0))
+    L.set_static_geometry(phi, np.ones(n ** 3, np.uint8))
+    L.enable_wall_model(True)
+    L.init_equilibrium(np.ones(n ** 3), u, False)
+    L.wall_model_only()
+    idx, y1n, ut, valid = L.wall_list()
+    assert len(idx) > 150 and np.all(valid == 1)
+    band = (phi > 0) & (phi < 1.0)
+    assert np.array_equal(idx, np.flatnonzero(band))
+    y1 = np.linalg.norm(y1n, axis=1)
+    assert np.allclose(y1, phi[idx].astype(np.float64), rtol=1e-12)
+    nrm = y1n / y1[:, None]
+    radial = (pos[:, idx] - ctr[:, None]).T
+    radial /= np.linalg.norm(radial, axis=1)[:, None]
+    assert np.min(np.sum(nrm * radial, axis=1)) > 0.995
+    for k in range(0, len(idx), 7):
+        cell = int(idx[k])
+        p = pos[:, cell] + 2.0 * nrm[k]
+        vs = v0 + M @ p
+        vt = vs - (vs @ nrm[k]) * nrm[k]
+        U = np.linalg.norm(vt)
+        expect, _ = oracle.newton_utau(np.sqrt(nu * U / (y1[k] + 2.0)), U, y1[k] + 2.0, nu)
+        ok, utau, uwm, s = L.wall_state(cell)
+        assert utau == pytest.approx(expect, rel=1e-10)
+        assert np.allclose(uwm, expect * vt / U, rtol=1e-9, atol=1e-15)
+        G = np.outer(M @ nrm[k], nrm[k])
+        S = 0.5 * (G + G.T)
+        assert np.allclose([s[0], s[1], s[2], s[3], s[4], s[5]],
+                           [S[0, 0], S[1, 1], S[2, 2], S[0, 1], S[0, 2], S[1, 2]], rtol=0, atol=1e-15)
+
+
+def test_wall_model_across_a_mirror_plane_equals_even_extension(oracle):
+    """R12 + R15: sampling points and FD stencils of wall cells next to a MIRROR plane reach behind it and see
+    the reflected flow (normal velocity component reversed).  A ball cut by the plane y = -1/2, wall model on:
+    three steps on the MIRROR lattice equal the lower half of the periodic lattice of twice the height started
+    mirror-symmetric -- populations, u_tau and forces.
+    Catches: the sampled velocity (or phi in the normal) not reflected at the plane."""
+    from paper_2510_13726_b200 import inputs
+    nx, ny, nz = 12, 8, 11
+    c, w = _c(oracle)
+    x, y, z = _grid(nx, ny, nz)
+    flip = np.array([int((c[0, i] + 1) + 3 * (-c[1, i] + 1) + 9 * (c[2, i] + 1)) for i in range(Q)])
+    # one ball cut by the plane, one hanging just above it (normals of its lowest wall cells point at the plane)
+    phi = np.minimum(inputs.sphere_phi(nx, ny, nz, (2.5, 0.4, 3.0), 2.2), inputs.sphere_phi(nx, ny, nz, (7.5, 3.4, 6.0), 3.1))
+    phi = phi.astype(np.float64).reshape(nz, ny, nx)
+    phib = np.concatenate([phi, phi[:, ::-1]], axis=1)
+    u = np.zeros((3, nz, ny, nx))
+    yy = y.reshape(nz, ny, nx)
+    u[0] = 0.03 + 0.002 * np.sin(2 * np.pi * x.reshape(nz, ny, nx) / nx)
+    u[1] = 0.004 * (yy + 0.5) / ny * np.cos(2 * np.pi * z.reshape(nz, ny, nx) / nz)
+    u[2] = -0.01
+    ub = np.concatenate([u, (u * np.array([1, -1, 1])[:, None, None, None])[:, :, ::-1]], axis=2)
+    kw = dict(tau0=0.5 + 3 * 3.156e-4, sampling_distance=2.0)
+    A = oracle.Lattice(oracle.make_params(nx, ny, nz, mode=(0, 1, 0), **kw))
+    B = oracle.Lattice(oracle.make_params(nx, 2 * ny, nz, **kw))
+    for L, p, uu in ((A, phi, u), (B, phib, ub)):
+        L.set_static_geometry(p.reshape(-1), np.ones(p.size, np.uint8))
+        L.enable_wall_model(True)
+        L.init_equilibrium(np.ones(p.size), uu.reshape(3, -1), True)
+    A.step(3); B.step(3)
+    fa = A.populations().reshape(Q, nz, ny, nx)
+    fb = B.populations().reshape(Q, nz, 2 * ny, nx)
+    assert np.allclose(fa, fb[:, :, :ny], rtol=0, atol=1e-15)
+    ia, y1na, uta, _ = A.wall_list()
+    ib, _, utb, _ = B.wall_list()
+    below = (ia // nx) % ny + 2.0 * y1na[:, 1] / np.linalg.norm(y1na, axis=1) < 0
+    assert np.count_nonzero(below) >= 4                       # sampling points behind the mirror plane
+    lower = ((ib // nx) % (2 * ny)) < ny
+    assert len(ia) > 20 and np.count_nonzero(lower) == len(ia)
+    assert np.any((ia // nx) % ny == 0)                       # wall cells in the row next to the plane
+    assert np.allclose(uta, utb[lower], rtol=1e-12)
+    Fa, Fb = A.forces()[-1, 1], B.forces()[-1, 1]             # the whole ball: twice the half's in-plane force,
+    assert np.allclose(Fa[[0, 2]], 0.5 * Fb[[0, 2]], rtol=0, atol=1e-13) and abs(Fb[1]) < 1e-13   # no normal one

@@ -23,7 +23,8 @@
  * legacy default stream).  Calls that return data to host memory synchronise that
  * stream; hhrr_step() does not.
  *
- * Errors.  Every int-returning call returns HHRR_OK (0) or a negative hhrr_status;
+ * Errors.  Every int-returning call returns HHRR_OK (0) or a negative hhrr_status
+ * (hhrr_set_kernel_variant may also return the positive notice HHRR_W_FALLBACK);
  * nothing throws or aborts across the ABI.  hhrr_last_error() returns a
  * thread-local, NUL-terminated message for the last failing call on this thread.
  * There is no CPU fallback: without a usable CUDA device every call that needs one
@@ -48,7 +49,9 @@ typedef enum {
   HHRR_E_SIZE = -2,  /* workspace too small or extents overflow int32 cells  */
   HHRR_E_CUDA = -3,  /* a CUDA runtime call or kernel launch failed          */
   HHRR_E_NAN = -4,   /* hhrr_check_finite found a non-finite population      */
-  HHRR_E_STATE = -5  /* call not valid in the lattice's current state        */
+  HHRR_E_STATE = -5, /* call not valid in the lattice's current state        */
+  HHRR_W_FALLBACK = 1 /* not an error: hhrr_set_kernel_variant(5) on a lattice the default kernel cannot
+                         tile -- the lattice keeps post-stream storage and variant 2 runs  */
 } hhrr_status;
 
 /* Outer boundary per axis (reading R12; the paper only names its outer
@@ -114,8 +117,8 @@ size_t hhrr_workspace_bytes(const hhrr_params* p, const hhrr_rotor_desc* rotor);
  * queued on it, except the first half of the NEXT step's porosity update (rotor signed
  * distance; a function of the step count only), which hhrr_step queues on
  * one internal low-priority stream, ordered against `cuda_stream` by events, so that it
- * overlaps the tail of the collide-stream kernel.  Results do not depend on it (environment
- * variable HHRR_NO_LOOKAHEAD=1 at creation switches it off, for measurement).  The workspace
+ * overlaps the tail of the collide-stream kernel.  Results do not depend on it
+ * (hhrr_set_lookahead(L, 0) switches it off, for measurement and tests).  The workspace
  * must stay allocated until hhrr_destroy, which waits for both streams.                  */
 int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes, void* cuda_stream,
                 hhrr_lattice** out);
@@ -214,16 +217,18 @@ int hhrr_get_cell_populations(hhrr_lattice* L, int64_t n_cells, const int64_t* c
 int hhrr_get_uhat(hhrr_lattice* L, float* uhat);
 /* HHRR_E_NAN if any population is non-finite (synchronises). */
 int hhrr_check_finite(hhrr_lattice* L);
-/* Selects the collide-stream kernel: 0 = two-pass (moments pass + collide pass), 1 = fused
- * sliding-window kernel, 2 = fused warp-specialised kernel, 3 = the same with two cells per
- * lane, 4 = fused kernel fed by TMA (needs nx % 64 == 0 and ny % 8 == 0, otherwise 2 runs),
- * 5 = the TMA-fed kernel on x-pull / yz-push storage (default; needs a periodic x axis and
- * tiles of 64 x 8 cells (nx % 64 == 0, nx >= 128, ny % 8 == 0) or 128 x 4 cells (nx % 128 == 0,
- * nx >= 256, ny % 4 == 0), otherwise 2 runs); 11-49 = tile shapes kept for tuning
- * runs.  All compute the same step (Listing 3 line 3).  Variant 5 keeps plane i
- * of the population buffer as f_i(x + c_ix, y, z) (the x move of Eq. 6, is taken
- * on the read side); the call re-stores the current populations when the layout changes, and
- * every entry point that takes or returns populations speaks the plain post-stream layout.   */
+/* Selects the collide-stream kernel: 5 = the TMA-fed fused kernel on x-pull / yz-push storage
+ * (default; needs a periodic x axis and tiles of 64 x 8 cells (nx % 64 == 0, nx >= 128,
+ * ny % 8 == 0) or 128 x 4 cells (nx % 128 == 0, nx >= 256, ny % 4 == 0)); 2 = the fused
+ * warp-specialised kernel on post-stream storage (any extents, any axis modes); 0 = two-pass
+ * (moments pass + collide pass; the bring-up path the fused kernels were checked against).
+ * All compute the same step (Listing 3 line 3).  Variant 5 keeps plane i of
+ * the population buffer as f_i(x + c_ix, y, z) (the x move of Eq. 6, is taken on
+ * the read side); the call re-stores the current populations when the layout changes, and
+ * every entry point that takes or returns populations speaks the plain post-stream layout.
+ * Returns HHRR_W_FALLBACK (> 0, hhrr_last_error() says why) when 5 is asked for on a lattice
+ * it cannot tile: variant 2 then runs; hhrr_create makes the same choice silently, and
+ * hhrr_population_storage tells which kernel a lattice runs.                              */
 int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant);
 /* 1 if the populations are currently kept x-pulled (variant 5 running its own kernel), 0 if
  * post-stream (all other variants, and variant 5 on a lattice it cannot tile).            */
@@ -233,6 +238,9 @@ int hhrr_population_storage(const hhrr_lattice* L);
  * milliseconds and the number of launches it covers (at most 1024 per window), and starts a
  * new window.                                                                              */
 int hhrr_set_timing(hhrr_lattice* L, int enable);
+/* Switches the overlap of the next step's porosity update with the current step (see
+ * hhrr_create) on (default) or off.  Results are bitwise the same either way.            */
+int hhrr_set_lookahead(hhrr_lattice* L, int enable);
 int hhrr_get_timing(hhrr_lattice* L, double* ms_collide_stream, int64_t* launches);
 /* Number of kernel launches issued by this lattice so far. */
 int64_t hhrr_launch_count(const hhrr_lattice* L);

@@ -29,7 +29,7 @@ SYMBOLS = [
     "hhrr_get_cell_types", "hhrr_get_wall_list", "hhrr_get_wall_state", "hhrr_get_populations",
     "hhrr_set_populations", "hhrr_get_cell_populations", "hhrr_get_uhat", "hhrr_check_finite", "hhrr_set_kernel_variant",
     "hhrr_population_storage", "hhrr_set_fsi_region", "hhrr_set_wall_function", "hhrr_set_wall_model_variant",
-    "hhrr_set_timing", "hhrr_get_timing", "hhrr_launch_count", "hhrr_last_error", "hhrr_version",
+    "hhrr_set_timing", "hhrr_get_timing", "hhrr_set_lookahead", "hhrr_launch_count", "hhrr_last_error", "hhrr_version",
 ]
 
 
@@ -102,6 +102,7 @@ def lib():
         L.hhrr_get_uhat.argtypes = [vp, vp]
         L.hhrr_check_finite.argtypes = [vp]
         L.hhrr_set_kernel_variant.argtypes = [vp, i32]
+        L.hhrr_set_lookahead.argtypes = [vp, C.c_int]
         L.hhrr_set_timing.argtypes = [vp, C.c_int]
         L.hhrr_get_timing.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
         L.hhrr_launch_count.restype = i64
@@ -112,9 +113,13 @@ def lib():
     return _lib
 
 
+W_FALLBACK = 1   # hhrr_set_kernel_variant: the default kernel cannot tile this lattice, variant 2 runs
+
+
 def _check(rc):
-    if rc != 0:
+    if rc < 0:
         raise HhrrError(rc, lib().hhrr_last_error().decode())
+    return rc
 
 
 def _p(a):
@@ -248,7 +253,11 @@ class Lattice:
         _check(lib().hhrr_update_geometry(self.h))
 
     def set_kernel_variant(self, variant):
-        _check(lib().hhrr_set_kernel_variant(self.h, int(variant)))
+        """Returns HHRR_OK (0) or the notice W_FALLBACK (1): variant 5 cannot tile the lattice, variant 2 runs."""
+        return _check(lib().hhrr_set_kernel_variant(self.h, int(variant)))
+
+    def set_lookahead(self, enable=True):
+        _check(lib().hhrr_set_lookahead(self.h, int(bool(enable))))
 
     def population_storage(self):
         return int(lib().hhrr_population_storage(self.h))

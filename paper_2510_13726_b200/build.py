@@ -26,10 +26,7 @@ COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-
 SOURCES = {
     "api.cu": [],
     "collide.cu": [],
-    "fused.cu": [],
     "fused_ws.cu": [],
-    "fused_ws2.cu": [],
-    "fused_tma.cu": [],
     "fused_xpull.cu": [],
     "wallmodel.cu": [],
     "geometry.cu": ["-fmad=false"],

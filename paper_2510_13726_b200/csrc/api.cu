@@ -192,7 +192,8 @@ int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes,
   L->geometry_dirty = true;
   L->geometry_current = false;
   L->phi_ahead_step = -1;
-  if (!getenv("HHRR_NO_LOOKAHEAD")) {  // measurement switch; the look-ahead changes no result
+  L->lookahead = true;
+  {
     int prio_lo = 0, prio_hi = 0;
     cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
     if (cudaStreamCreateWithPriority(&L->side, cudaStreamNonBlocking, prio_lo) != cudaSuccess ||
@@ -408,11 +409,23 @@ int hhrr_update_geometry(hhrr_lattice* L) {
 }
 
 int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant) {
-  if (!L || variant < 0 || (variant > 5 && (variant < 11 || variant > 49))) return fail(HHRR_E_ARG, "hhrr_set_kernel_variant: bad argument");
+  if (!L || (variant != 0 && variant != 2 && variant != 5)) return fail(HHRR_E_ARG, "hhrr_set_kernel_variant: bad argument");
   L->variant = variant;
   // variant 5 keeps the populations x-pulled (where it can run); everything else stores them post-stream
-  cudaError_t e = launch_restore(L, (variant == 5 && xpull_supported(L->dom)) ? 1 : 0);
+  const bool tiles = xpull_supported(L->dom);
+  cudaError_t e = launch_restore(L, (variant == 5 && tiles) ? 1 : 0);
   if (e != cudaSuccess) return cuda_fail(e, "restore kernel");
+  if (variant == 5 && !tiles)
+    return fail(HHRR_W_FALLBACK,
+                "variant 5 cannot tile %d x %d x %d (needs a periodic x axis and nx %% 64 == 0, nx >= 128, ny %% 8 == 0, or "
+                "nx %% 128 == 0, nx >= 256, ny %% 4 == 0): variant 2 runs on post-stream storage",
+                L->dom.nx, L->dom.ny, L->dom.nz);
+  return HHRR_OK;
+}
+
+int hhrr_set_lookahead(hhrr_lattice* L, int enable) {
+  if (!L) return fail(HHRR_E_ARG, "hhrr_set_lookahead: NULL lattice");
+  L->lookahead = enable != 0;
   return HHRR_OK;
 }
 

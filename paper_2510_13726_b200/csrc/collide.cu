@@ -283,43 +283,20 @@ cudaError_t launch_restore(hhrr_lattice* L, int xs) {
   return cudaGetLastError();
 }
 
-cudaError_t launch_fused(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo);     // fused.cu
 cudaError_t launch_fused_ws(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo);  // fused_ws.cu
-cudaError_t launch_fused_ws2(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo); // fused_ws2.cu
-cudaError_t launch_fused_tma(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo); // fused_tma.cu
 cudaError_t launch_fused_xpull(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo); // fused_xpull.cu
 
+// Variant 5 (default) runs where its storage is in place (dom.xs, decided by hhrr_create /
+// hhrr_set_kernel_variant from xpull_supported); a lattice it cannot tile keeps post-stream storage and runs
+// variant 2 -- hhrr_set_kernel_variant reports that with HHRR_W_FALLBACK, hhrr_population_storage shows it.
 cudaError_t launch_collide_stream(hhrr_lattice* L) {
   PhysF ph = make_phys(L);
   BodiesF bo = make_bodies(L);
   cudaError_t e;
-  if (L->variant == 5) {
+  if (L->variant == 5 && L->dom.xs) {
     e = launch_fused_xpull(L, ph, bo);
-    if (e == cudaErrorNotSupported) {  // lattice keeps post-stream storage: warp-specialised kernel
-      L->variant = 2;
-      e = launch_fused_ws(L, ph, bo);
-      L->variant = 5;
-    }
-  } else if (L->variant == 4 || L->variant == 41) {
-    e = launch_fused_tma(L, ph, bo);
-    if (e == cudaErrorNotSupported) {  // ragged tiles: warp-specialised kernel, one cell per lane
-      const int v = L->variant;
-      L->variant = 2;
-      e = launch_fused_ws(L, ph, bo);
-      L->variant = v;
-    }
-  } else if (L->variant == 3 || (L->variant >= 31 && L->variant <= 39)) {
-    e = launch_fused_ws2(L, ph, bo);
-    if (e == cudaErrorNotSupported) {  // odd nx: one cell per lane
-      const int v = L->variant;
-      L->variant = 2;
-      e = launch_fused_ws(L, ph, bo);
-      L->variant = v;
-    }
-  } else if (L->variant == 2 || (L->variant >= 21 && L->variant <= 29)) {
+  } else if (L->variant >= 2) {
     e = launch_fused_ws(L, ph, bo);
-  } else if (L->variant >= 1) {
-    e = launch_fused(L, ph, bo);
   } else {
     int bx = row_block(L->dom);
     dim3 g = row_grid(L->dom, bx);

@@ -260,23 +260,12 @@ void fill_ws_args(const hhrr_lattice* L, const PhysF& ph, const BodiesF& bo, WsA
 int ws_zchunks(int nz, int planes) {  // ~planes planes per chunk: measured optima on config 5 (profiles/)
   int nch = (nz + planes / 2) / planes;
   if (nch < 1) nch = 1;
-  if (const char* e = getenv("HHRR_ZCHUNKS")) nch = atoi(e) < 1 ? 1 : atoi(e);  // tuning runs only
   return nch;
 }
 
 cudaError_t launch_fused_ws(hhrr_lattice* L, const PhysF& ph, const BodiesF& bo) {
   WsArgs a;
   fill_ws_args(L, ph, bo, a);
-  switch (L->variant) {
-    case 21: return launch_ws_cfg<64, 8, 10, 4, 1>(L, a);
-    case 22: return launch_ws_cfg<64, 8, 10, 5, 1>(L, a);
-    case 23: return launch_ws_cfg<64, 16, 12, 4, 2>(L, a);
-    case 24: return launch_ws_cfg<128, 8, 10, 4, 2>(L, a);
-    case 25: return launch_ws_cfg<64, 12, 14, 4, 2>(L, a);
-    case 26: return launch_ws_cfg<64, 8, 5, 4, 1>(L, a);
-    case 27: return launch_ws_cfg<64, 8, 10, 4, 2>(L, a);
-    default: break;
-  }
   return launch_ws_cfg<64, 8, 20, 4>(L, a);
 }
 

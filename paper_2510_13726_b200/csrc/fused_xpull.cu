@@ -20,8 +20,6 @@
 // x axis (xpull_supported); other lattices keep post-stream storage and run variant 2.
 #include <cuda.h>
 
-#include <cstdlib>
-
 #include "ws_common.cuh"
 
 namespace hhrr {
@@ -493,11 +491,6 @@ static bool make_map(CUtensorMap* m, const float* base, const Dom& dm, uint32_t 
   cuuint32_t box[4] = {bx, by, 1, (cuuint32_t)Q};
   cuuint32_t estr[4] = {1, 1, 1, 1};
   CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_256B;  // measured: 0.5-1 % faster than 128 B, 64 B slower
-  if (const char* e = getenv("HHRR_TMA_PROMO")) {  // tuning runs only
-    promo = atoi(e) == 0 ? CU_TENSOR_MAP_L2_PROMOTION_NONE
-                         : (atoi(e) == 64 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B
-                                          : (atoi(e) == 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : promo));
-  }
   return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<float*>(base), gdim, gstr, box, estr,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
@@ -539,7 +532,6 @@ static cudaError_t launch_shape(hhrr_lattice* L, WsArgs& a) {
   }
   a.nch = nch;
   a.group = sms;  // one tile per SM and wave (one block per SM: shared memory)
-  if (const char* e = getenv("HHRR_XPULL_GROUP")) a.group = atoi(e) < 1 ? 1 : atoi(e);  // tuning runs only
   const int ntiles = (dm.nx / C::TX) * (dm.ny / C::TY);
   dim3 grid((unsigned)(ntiles * nch));
   fused_xpull_kernel<C><<<grid, C::THREADS, C::SMEM, L->stream>>>(a, m_main, m_row, m_pm, m_pr);
@@ -556,12 +548,8 @@ cudaError_t launch_fused_xpull(hhrr_lattice* L, const PhysF& ph, const BodiesF& 
     a.push_b[i] = 4LL * ((long long)i * dm.n + (long long)dir_cy(i) * dm.nx + (long long)dir_cz(i) * dm.nx * dm.ny);
   // Blocks that need the y halo rows (the FD strain) do better with 64 x 8 tiles (2 halo rows per 8), bulk
   // blocks (region split) with 128 x 4 (fewer x-halo sectors re-read): measured on config 5,
-  // 4.06 / 4.39 ms without the split and 4.16 / 3.98 ms with it.  HHRR_XPULL_SHAPE=tall|wide: tuning runs only.
+  // 4.06 / 4.39 ms without the split and 4.16 / 3.98 ms with it.
   bool wide = shape_tiles<XpWide>(dm) && (a.fsi.n > 0 || !shape_tiles<XpTall>(dm));
-  if (const char* shape = getenv("HHRR_XPULL_SHAPE")) {
-    if (shape[0] == 't' && shape_tiles<XpTall>(dm)) wide = false;
-    if (shape[0] == 'w' && shape_tiles<XpWide>(dm)) wide = true;
-  }
   return wide ? launch_shape<XpWide>(L, a) : launch_shape<XpTall>(L, a);
 }
 

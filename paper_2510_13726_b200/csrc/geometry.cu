@@ -389,7 +389,7 @@ static void launch_box_phi(hhrr_lattice* L, int64_t step, cudaStream_t s) {
 // is queued on a low-priority side stream as soon as pass 2 of geometry(step) has read phi, and runs in the tail
 // of the collide-stream kernel / beside the wall-model and force kernels instead of between two steps.
 cudaError_t launch_phi_ahead(hhrr_lattice* L) {
-  if (!L->side || rotor_box_empty(L) || L->geometry_dirty) return cudaSuccess;
+  if (!L->side || !L->lookahead || rotor_box_empty(L) || L->geometry_dirty) return cudaSuccess;
   cudaStreamWaitEvent(L->side, L->ev_type_done, 0);
   launch_box_phi(L, L->step + 1, L->side);
   cudaEventRecord(L->ev_phi_done, L->side);

@@ -80,6 +80,7 @@ struct hhrr_lattice {
   cudaStream_t side;
   cudaEvent_t ev_type_done, ev_phi_done;
   int64_t phi_ahead_step;
+  bool lookahead;  // hhrr_set_lookahead
   int device;
   // device arrays (inside the caller's workspace)
   float *fA, *fB;           // 27 planes each: post-stream populations minus weights

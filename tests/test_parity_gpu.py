@@ -92,7 +92,7 @@ def run_parity(oracle, case, steps, variant, tol, check_every=None, force_tol=No
     return e_rho, e_v
 
 
-VARIANTS = [0, 1, 2, 3, 4, 5]
+VARIANTS = [0, 2, 5]
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
@@ -202,7 +202,7 @@ def test_xpull_storage_round_trip():
     """Populations go in and out in the plain post-stream layout whatever the storage; switching the
     variant re-stores them without changing the state."""
     case = I.case_sphere(128, 32, 32, 5.0, 4)
-    A, Bv = _xpull_lattice(case), _gpu_lattice(case, 4)
+    A, Bv = _xpull_lattice(case), _gpu_lattice(case, 2)
     assert Bv.population_storage() == 0
     A.step(4); Bv.step(4)
     fa, fb = A.populations(), Bv.populations()
@@ -258,7 +258,7 @@ def test_region_split_violation_is_reported():
     G.close()
 
 
-@pytest.mark.parametrize("variant", [2, 4, 5, 5256])
+@pytest.mark.parametrize("variant", [2, 5, 5256])
 def test_fused_kernels_are_deterministic(variant):
     """Two identical lattices stay bitwise identical: every step is a deterministic function of the
     state (R19).  A race between the warps of a fused kernel (ring slots, pipeline stages,
@@ -273,16 +273,15 @@ def test_fused_kernels_are_deterministic(variant):
     A.close(); Bv.close()
 
 
-def test_geometry_look_ahead_changes_nothing(oracle, monkeypatch):
+def test_geometry_look_ahead_changes_nothing(oracle):
     """Pass 1 of UpdatePorosityO for step n+1 runs ahead on a side stream (geometry.cu: launch_phi_ahead).  With it
-    and without it (HHRR_NO_LOOKAHEAD) the populations stay bitwise equal; a rotor that is replaced, and a geometry
+    and without it (hhrr_set_lookahead) the populations stay bitwise equal; a rotor that is replaced, and a geometry
     evaluation asked for between steps, while a look-ahead pass is pending give the oracle's cell types, lists and
     flow."""
     case = I.case_rotor(128, 72, 72, 20.0, 9, omega=0.012)
     A = _gpu_lattice(case, 5)
-    monkeypatch.setenv("HHRR_NO_LOOKAHEAD", "1")
     Bv = _gpu_lattice(case, 5)
-    monkeypatch.delenv("HHRR_NO_LOOKAHEAD")
+    Bv.set_lookahead(False)
     Oa = _ora_lattice(oracle, case)
     A.step(3); Bv.step(3); Oa.step(3)
     assert np.array_equal(A.populations(), Bv.populations())
@@ -347,12 +346,12 @@ def test_wall_model_second_readings(oracle, slip, shear):
 def test_moving_static_body_and_checkpoint(oracle):
     """set_body on a static solid (translating sphere) and populations round trip."""
     case = I.case_sphere(48, 24, 24, 4.0, 6)
-    G, Oa = _gpu_lattice(case, 1), _ora_lattice(oracle, case)
+    G, Oa = _gpu_lattice(case, 2), _ora_lattice(oracle, case)
     for L in (G, Oa):
         L.set_body(1, centre=(12, 11.5, 11.5), omega=(0.0, 0.0, 0.002), vel=(0.01, 0.0, 0.0))
     G.step(3); Oa.step(3)
     f = G.populations()
-    G2 = _gpu_lattice(case, 1)
+    G2 = _gpu_lattice(case, 2)
     G2.set_body(1, centre=(12, 11.5, 11.5), omega=(0.0, 0.0, 0.002), vel=(0.01, 0.0, 0.0))
     G2.set_populations(f)
     G.step(3); G2.step(3); Oa.step(3)
@@ -364,7 +363,7 @@ def test_moving_static_body_and_checkpoint(oracle):
 def test_variants_agree_bitwise_on_moments_order():
     """The two kernel variants implement the same arithmetic; they must agree to rounding."""
     case = I.case_sphere(64, 32, 32, 5.0, 20)
-    A, Bv = _gpu_lattice(case, 0), _gpu_lattice(case, 1)
+    A, Bv = _gpu_lattice(case, 0), _gpu_lattice(case, 2)
     A.step(20); Bv.step(20)
     e_rho, e_v = rel_linf(*A.moments(), *[x.astype(np.float64) for x in Bv.moments()])
     assert e_rho <= 1e-6 and e_v <= 1e-5, (e_rho, e_v)
@@ -516,7 +515,7 @@ def test_force_history_ring_and_errors(oracle):
     refused; argument errors come back as error codes, not crashes."""
     from paper_2510_13726_b200 import binding as B
     case = I.case_sphere(16, 8, 8, 2.5, 4200)
-    G, Oa = _gpu_lattice(case, 4), _ora_lattice(oracle, case)
+    G, Oa = _gpu_lattice(case, 2), _ora_lattice(oracle, case)
     G.step(4200); Oa.step(4200)
     assert G.step_count() == 4200
     Fg, Fo = G.forces(4190, 10), Oa.forces(4190, 10)

@@ -205,15 +205,31 @@ int hhrr_get_wall_list(hhrr_lattice* L, int64_t capacity, int32_t* idx, double* 
 /* Wall-model output of one cell: slip velocity u_wm[3] and strain S_wm[6] (xx yy zz xy xz yz). */
 int hhrr_get_wall_state(hhrr_lattice* L, int64_t cell, double* u_tau, double u_wm[3], double s_wm[6],
                         int32_t* valid);
-/* Populations as stored: deviations f_i - w_i, 27 planes of N floats (checkpoint / resume). */
+/* Populations as stored: deviations f_i - w_i, 27 planes of N floats.
+ * Checkpoint / resume: the state of a run is (step count, populations, wall-model state); the geometry is a
+ * function of the setters' inputs and the step count.  To resume: create the lattice, call the same setters,
+ * then hhrr_set_step_count, hhrr_set_populations, hhrr_set_wall_model_state (in this order).  The run then
+ * continues bitwise as the uninterrupted one (forces of earlier steps are not part of the state).        */
 int hhrr_get_populations(hhrr_lattice* L, float* f_minus_w);
 int hhrr_set_populations(hhrr_lattice* L, const float* f_minus_w);
+/* Wall-model state of the cells of the current wall list, in list order: cell index, u_tau (the Newton warm
+ * start, Eq. 20), slip velocity u_wm[3 per cell], strain S_wm[6 per cell: xx yy zz xy xz yz] as
+ * stored (fp32), valid flag.  *count = number of wall cells; nothing else is written if capacity < *count.   */
+int hhrr_get_wall_model_state(hhrr_lattice* L, int64_t capacity, int32_t* idx, double* u_tau, float* u_wm, float* s_wm,
+                              uint8_t* valid, int64_t* count);
+/* Restores it: evaluates the geometry of the current step if needed, then writes the state of every listed
+ * cell that belongs to the wall-model set (others are ignored).                                              */
+int hhrr_set_wall_model_state(hhrr_lattice* L, int64_t count, const int32_t* idx, const double* u_tau, const float* u_wm,
+                              const float* s_wm, const uint8_t* valid);
+/* Sets the step counter (rotor angle theta0 + step * omega; slot of the force ring). */
+int hhrr_set_step_count(hhrr_lattice* L, int64_t step);
 /* Populations (deviations f_i - w_i) of selected cells: out[k*27 + i] for cells[k], and the
  * cells' flags as stored (type | tag << 3 | wall-model-valid << 7) if flags != NULL.  Lets tests
  * check sampled cells of lattices too large to copy back whole.                          */
 int hhrr_get_cell_populations(hhrr_lattice* L, int64_t n_cells, const int64_t* cells, float* out,
                               uint8_t* flags);
-/* Time-n homogenised velocity field of the last collide (3N floats), for tests. */
+/* Time-n homogenised velocity field of the last collide (3N floats), for tests.  Only the two-pass kernel
+ * (variant 0) stores it; HHRR_E_STATE otherwise or before the first step.                    */
 int hhrr_get_uhat(hhrr_lattice* L, float* uhat);
 /* HHRR_E_NAN if any population is non-finite (synchronises). */
 int hhrr_check_finite(hhrr_lattice* L);

@@ -29,6 +29,7 @@ SYMBOLS = [
     "hhrr_get_cell_types", "hhrr_get_wall_list", "hhrr_get_wall_state", "hhrr_get_populations",
     "hhrr_set_populations", "hhrr_get_cell_populations", "hhrr_get_uhat", "hhrr_check_finite", "hhrr_set_kernel_variant",
     "hhrr_population_storage", "hhrr_set_fsi_region", "hhrr_set_wall_function", "hhrr_set_wall_model_variant",
+    "hhrr_get_wall_model_state", "hhrr_set_wall_model_state", "hhrr_set_step_count",
     "hhrr_set_timing", "hhrr_get_timing", "hhrr_set_lookahead", "hhrr_launch_count", "hhrr_last_error", "hhrr_version",
 ]
 
@@ -100,6 +101,9 @@ def lib():
         L.hhrr_set_populations.argtypes = [vp, vp]
         L.hhrr_get_cell_populations.argtypes = [vp, i64, vp, vp, vp]
         L.hhrr_get_uhat.argtypes = [vp, vp]
+        L.hhrr_get_wall_model_state.argtypes = [vp, i64, vp, vp, vp, vp, vp, C.POINTER(i64)]
+        L.hhrr_set_wall_model_state.argtypes = [vp, i64, vp, vp, vp, vp, vp]
+        L.hhrr_set_step_count.argtypes = [vp, i64]
         L.hhrr_check_finite.argtypes = [vp]
         L.hhrr_set_kernel_variant.argtypes = [vp, i32]
         L.hhrr_set_lookahead.argtypes = [vp, C.c_int]
@@ -338,6 +342,26 @@ class Lattice:
         s = np.zeros(6)
         _check(lib().hhrr_get_wall_state(self.h, int(cell), C.byref(ut), _p(u), _p(s), C.byref(valid)))
         return valid.value, ut.value, u, s
+
+    def wall_model_state(self):
+        """(idx int32[k], u_tau f64[k], u_wm f32[k,3], s_wm f32[k,6], valid u8[k]) of the current wall list."""
+        kk = C.c_int64(0)
+        _check(lib().hhrr_get_wall_model_state(self.h, 0, None, None, None, None, None, C.byref(kk)))
+        k = kk.value
+        idx = np.zeros(k, np.int32); ut = np.zeros(k); uw = np.zeros((k, 3), np.float32)
+        sw = np.zeros((k, 6), np.float32); va = np.zeros(k, np.uint8)
+        if k:
+            _check(lib().hhrr_get_wall_model_state(self.h, k, _p(idx), _p(ut), _p(uw), _p(sw), _p(va), C.byref(kk)))
+        return idx, ut, uw, sw, va
+
+    def set_wall_model_state(self, idx, u_tau, u_wm, s_wm, valid):
+        idx = np.ascontiguousarray(idx, np.int32); ut = np.ascontiguousarray(u_tau, np.float64)
+        uw = np.ascontiguousarray(u_wm, np.float32); sw = np.ascontiguousarray(s_wm, np.float32)
+        va = np.ascontiguousarray(valid, np.uint8)
+        _check(lib().hhrr_set_wall_model_state(self.h, len(idx), _p(idx), _p(ut), _p(uw), _p(sw), _p(va)))
+
+    def set_step_count(self, step):
+        _check(lib().hhrr_set_step_count(self.h, int(step)))
 
     def populations(self):
         f = np.empty((Q, self.n), np.float32)

@@ -5,7 +5,6 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -35,6 +34,21 @@ int cuda_fail(cudaError_t e, const char* what) {
   } while (0)
 
 size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
+
+// Every entry point that takes a lattice works on the lattice's device, whatever device is current in the
+// calling thread, and leaves the caller's current device as it found it.
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(const hhrr_lattice* L) { enter(L ? L->device : -1); }
+  explicit DeviceGuard(int device) { enter(device); }
+  void enter(int device) {
+    if (device >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != device) cudaSetDevice(device);
+    else prev = -1;
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
 
 bool params_ok(const hhrr_params* p) {
   if (!p) return false;
@@ -85,9 +99,14 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
   float* wm_s = c.take<float>(6 * n);
   int32_t* wall_idx = c.take<int32_t>(cap);
   double* wall_y1n = c.take<double>(3 * cap);
-  double* wall_samp = c.take<double>(6 * cap);
   int32_t* force_idx = c.take<int32_t>(cap);
   Counters* counters = c.take<Counters>(1);
+  uint8_t* alt_flags = c.take<uint8_t>(n);
+  float* alt_d = c.take<float>(n);
+  int32_t* alt_wall_idx = c.take<int32_t>(cap);
+  double* alt_wall_y1n = c.take<double>(3 * cap);
+  int32_t* alt_force_idx = c.take<int32_t>(cap);
+  Counters* alt_counters = c.take<Counters>(1);
   double* force = c.take<double>(FORCE_HISTORY * MAX_TAGS * 3);
   double* torque = c.take<double>(FORCE_HISTORY * MAX_TAGS * 3);
   float* rot_sdf = c.take<float>(rotor_nodes);
@@ -95,7 +114,9 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
   if (L) {
     L->fA = fA; L->fB = fB; L->flags = flags; L->d = d; L->phi = phi; L->below = below; L->tag_prov = tag_prov; L->rowflag = rowflag; L->rowflag_static = rowflag_static; L->phi_static = phi_static;
     L->tag_static = tag_static; L->d_override = d_override; L->uhat = uhat; L->wm_utau = wm_utau;
-    L->wm_u = wm_u; L->wm_s = wm_s; L->wall_idx = wall_idx; L->wall_y1n = wall_y1n; L->wall_samp = wall_samp;
+    L->wm_u = wm_u; L->wm_s = wm_s; L->wall_idx = wall_idx; L->wall_y1n = wall_y1n;
+    L->alt_flags = alt_flags; L->alt_d = alt_d; L->alt_wall_idx = alt_wall_idx; L->alt_wall_y1n = alt_wall_y1n;
+    L->alt_force_idx = alt_force_idx; L->alt_counters = alt_counters;
     L->force_idx = force_idx; L->counters = counters; L->force = force; L->torque = torque; L->rot_sdf = rot_sdf;
     L->rot_tag = rot_tag; L->rot_nodes_cap = rotor_nodes; L->cap_list = cap;
   }
@@ -123,18 +144,47 @@ int download(hhrr_lattice* L, void* dst, const void* src, size_t bytes) {
   return HHRR_OK;
 }
 
-// the side stream may still be reading the rotor grid / static fields for a look-ahead pass: order the
-// caller's stream behind it before those inputs are overwritten
-void quiesce_side(hhrr_lattice* L) {
-  if (L->side && L->phi_ahead_step >= 0) cudaStreamWaitEvent(L->stream, L->ev_phi_done, 0);
+// Everything queued on the side stream (geometry look-ahead: reads the rotor grid and the static fields, writes the
+// alternate geometry set; force collection: reads populations, writes the force ring) is ordered before whatever
+// the caller's stream does next.
+void join_side(hhrr_lattice* L) {
+  if (L->side && L->side_busy) {
+    cudaEventRecord(L->ev_side, L->side);
+    cudaStreamWaitEvent(L->stream, L->ev_side, 0);
+    L->side_busy = false;
+  }
 }
+
+int read_counters(hhrr_lattice* L, Counters* h) { return download(L, h, L->counters, sizeof(Counters)); }
 
 int ensure_geometry(hhrr_lattice* L) {
   if (L->geometry_current) return HHRR_OK;
-  cudaError_t e = launch_geometry(L, L->geometry_dirty);
+  if (L->ahead_step == L->step && !L->geometry_dirty) {
+    // geometry(step) was written ahead into the alternate set (and its WM_VALID bits by the wall-model kernel of
+    // the step before): swap the sets
+    cudaStreamWaitEvent(L->stream, L->ev_k1, 0);
+    swap_geometry_sets(L);
+    L->ahead_step = -1;
+    L->geometry_current = true;
+    return HHRR_OK;
+  }
+  join_side(L);  // a force kernel may still be reading the lists this pass rebuilds in place
+  const bool full = L->geometry_dirty;
+  cudaError_t e = launch_geometry(L, full);
   if (e != cudaSuccess) return cuda_fail(e, "geometry kernels");
   L->geometry_dirty = false;
   L->geometry_current = true;
+  if (full && L->fsi.n > 0) {
+    // The default kernel treats a block outside every FSI box as bulk fluid without looking at its cells: a region
+    // that does not cover the structure must not get as far as a collision.  Full passes follow a setter and are
+    // rare, so this one synchronises and looks.  (A rotor that leaves its boxes later is reported by
+    // hhrr_check_finite.)
+    Counters h;
+    int rc = download(L, &h, L->counters, sizeof(Counters));
+    if (rc) return rc;
+    if (h.region_violation)
+      return fail(HHRR_E_STATE, "a cell that is not plain fluid lies outside the FSI region (hhrr_set_fsi_region)");
+  }
   return HHRR_OK;
 }
 
@@ -169,6 +219,7 @@ int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes,
   e = cudaPointerGetAttributes(&attr, d_workspace);
   if (e != cudaSuccess || attr.type != cudaMemoryTypeDevice)
     return fail(HHRR_E_ARG, "hhrr_create: workspace is not device memory");
+  DeviceGuard guard_(attr.device);  // streams, events and kernels of this lattice live on the workspace's device
   char* base = reinterpret_cast<char*>(align_up(reinterpret_cast<size_t>(d_workspace)));
   size_t lead = (size_t)(base - reinterpret_cast<char*>(d_workspace));
   size_t need_min = carve(nullptr, p, 0, nullptr);
@@ -191,14 +242,19 @@ int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes,
   L->dom.xs = xpull_supported(L->dom) ? 1 : 0;  // buffers start as zeros: nothing to convert
   L->geometry_dirty = true;
   L->geometry_current = false;
-  L->phi_ahead_step = -1;
+  L->ahead_step = -1;
+  L->side_busy = false;
   L->lookahead = true;
   {
     int prio_lo = 0, prio_hi = 0;
     cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
     if (cudaStreamCreateWithPriority(&L->side, cudaStreamNonBlocking, prio_lo) != cudaSuccess ||
-        cudaEventCreateWithFlags(&L->ev_type_done, cudaEventDisableTiming) != cudaSuccess ||
-        cudaEventCreateWithFlags(&L->ev_phi_done, cudaEventDisableTiming) != cudaSuccess) {
+        cudaEventCreateWithFlags(&L->ev_pre, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&L->ev_k1, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&L->ev_k2, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&L->ev_side, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&L->ev_f[0], cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&L->ev_f[1], cudaEventDisableTiming) != cudaSuccess) {
       delete L;
       return cuda_fail(cudaGetLastError(), "hhrr_create: side stream");
     }
@@ -209,12 +265,15 @@ int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes,
   fill_float_kernel<<<1184, 256, 0, s>>>(L->fB, Q * n, 0.f);
   fill_bytes_kernel<<<1184, 256, 0, s>>>(L->flags, n, 0);
   fill_float_kernel<<<1184, 256, 0, s>>>(L->d, n, 1.f);
+  fill_bytes_kernel<<<1184, 256, 0, s>>>(L->alt_flags, n, 0);
+  fill_float_kernel<<<1184, 256, 0, s>>>(L->alt_d, n, 1.f);
   fill_float_kernel<<<1184, 256, 0, s>>>(L->uhat, 3 * n, 0.f);
   fill_float_kernel<<<1184, 256, 0, s>>>(L->wm_u, 3 * n, 0.f);
   fill_float_kernel<<<1184, 256, 0, s>>>(L->wm_s, 6 * n, 0.f);
-  L->launches += 7;
+  L->launches += 9;
   e = cudaMemsetAsync(L->wm_utau, 0, sizeof(double) * n, s);
   if (e == cudaSuccess) e = cudaMemsetAsync(L->counters, 0, sizeof(Counters), s);
+  if (e == cudaSuccess) e = cudaMemsetAsync(L->alt_counters, 0, sizeof(Counters), s);
   if (e == cudaSuccess) e = cudaMemsetAsync(L->force, 0, sizeof(double) * FORCE_HISTORY * MAX_TAGS * 3, s);
   if (e == cudaSuccess) e = cudaMemsetAsync(L->torque, 0, sizeof(double) * FORCE_HISTORY * MAX_TAGS * 3, s);
   if (e == cudaSuccess) e = cudaGetLastError();
@@ -228,12 +287,17 @@ int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes,
 }
 
 int hhrr_destroy(hhrr_lattice* L) {
+  DeviceGuard guard_(L);
   if (!L) return fail(HHRR_E_ARG, "hhrr_destroy: NULL lattice");
   cudaStreamSynchronize(L->stream);
   if (L->side) {
     cudaStreamSynchronize(L->side);
-    cudaEventDestroy(L->ev_type_done);
-    cudaEventDestroy(L->ev_phi_done);
+    cudaEventDestroy(L->ev_pre);
+    cudaEventDestroy(L->ev_k1);
+    cudaEventDestroy(L->ev_k2);
+    cudaEventDestroy(L->ev_side);
+    cudaEventDestroy(L->ev_f[0]);
+    cudaEventDestroy(L->ev_f[1]);
     cudaStreamDestroy(L->side);
   }
   if (L->ev[0])
@@ -243,6 +307,7 @@ int hhrr_destroy(hhrr_lattice* L) {
 }
 
 int hhrr_init_equilibrium(hhrr_lattice* L, const float* rho, const float* u, int with_neq) {
+  DeviceGuard guard_(L);
   if (!L || !rho || !u) return fail(HHRR_E_ARG, "hhrr_init_equilibrium: NULL argument");
   const int64_t n = L->dom.n;
   // stage rho in buffer B (scratch between steps) and u in the uhat field
@@ -258,9 +323,10 @@ int hhrr_init_equilibrium(hhrr_lattice* L, const float* rho, const float* u, int
 }
 
 int hhrr_set_static_geometry(hhrr_lattice* L, const float* phi, const uint8_t* tag, const float* d_override) {
+  DeviceGuard guard_(L);
   if (!L) return fail(HHRR_E_ARG, "hhrr_set_static_geometry: NULL lattice");
   const int64_t n = L->dom.n;
-  quiesce_side(L);
+  join_side(L);
   L->has_static = L->has_tag_static = L->has_override = false;
   if (phi) {
     int rc = upload(L, L->phi_static, phi, sizeof(float) * n);
@@ -284,6 +350,7 @@ int hhrr_set_static_geometry(hhrr_lattice* L, const float* phi, const uint8_t* t
 
 int hhrr_set_body(hhrr_lattice* L, int32_t tag, const double centre[3], const double omega[3],
                   const double vel[3]) {
+  DeviceGuard guard_(L);
   if (!L || !centre || !omega || !vel) return fail(HHRR_E_ARG, "hhrr_set_body: NULL argument");
   if (tag < 0 || tag >= MAX_TAGS) return fail(HHRR_E_ARG, "hhrr_set_body: tag %d out of range", tag);
   for (int a = 0; a < 3; ++a) {
@@ -295,6 +362,7 @@ int hhrr_set_body(hhrr_lattice* L, int32_t tag, const double centre[3], const do
 }
 
 int hhrr_set_fringe(hhrr_lattice* L, int32_t x_begin, int32_t x_end, const double u_in[3]) {
+  DeviceGuard guard_(L);
   if (!L || !u_in) return fail(HHRR_E_ARG, "hhrr_set_fringe: NULL argument");
   L->has_fringe = x_end > x_begin;
   L->fr_x0 = x_begin;
@@ -306,12 +374,14 @@ int hhrr_set_fringe(hhrr_lattice* L, int32_t x_begin, int32_t x_end, const doubl
 }
 
 int hhrr_set_wall_function(hhrr_lattice* L, int32_t kind) {
+  DeviceGuard guard_(L);
   if (!L || (kind != 0 && kind != 1)) return fail(HHRR_E_ARG, "hhrr_set_wall_function: bad argument");
   L->wall_function = kind;
   return HHRR_OK;
 }
 
 int hhrr_set_wall_model_variant(hhrr_lattice* L, int32_t slip, int32_t shear) {
+  DeviceGuard guard_(L);
   if (!L || (slip != 0 && slip != 1) || (shear != 0 && shear != 1))
     return fail(HHRR_E_ARG, "hhrr_set_wall_model_variant: bad argument");
   L->wm_slip = slip;
@@ -320,18 +390,22 @@ int hhrr_set_wall_model_variant(hhrr_lattice* L, int32_t slip, int32_t shear) {
 }
 
 int hhrr_set_fsi_region(hhrr_lattice* L, int32_t n_boxes, const hhrr_box* boxes) {
+  DeviceGuard guard_(L);
   if (!L || n_boxes < 0 || n_boxes > HHRR_MAX_FSI_BOXES || (n_boxes > 0 && !boxes))
     return fail(HHRR_E_ARG, "hhrr_set_fsi_region: bad argument");
   L->fsi.n = n_boxes;
   for (int b = 0; b < n_boxes; ++b)
     L->fsi.b[b] = Box{boxes[b].x0, boxes[b].x1, boxes[b].y0, boxes[b].y1, boxes[b].z0, boxes[b].z1};
+  join_side(L);
   CU(cudaMemsetAsync(&L->counters->region_violation, 0, sizeof(int), L->stream));
+  CU(cudaMemsetAsync(&L->alt_counters->region_violation, 0, sizeof(int), L->stream));
   L->geometry_dirty = true;
   L->geometry_current = false;
   return HHRR_OK;
 }
 
 int hhrr_set_rotor(hhrr_lattice* L, const hhrr_rotor_desc* r) {
+  DeviceGuard guard_(L);
   if (!L || !r || !r->sdf || !r->tag) return fail(HHRR_E_ARG, "hhrr_set_rotor: NULL argument");
   if (r->n_tags < 1 || r->n_tags >= MAX_TAGS) return fail(HHRR_E_ARG, "hhrr_set_rotor: n_tags out of range");
   if (r->gx < 2 || r->gy < 2 || r->gz < 2 || !(r->spacing > 0.0)) return fail(HHRR_E_ARG, "hhrr_set_rotor: bad grid");
@@ -339,7 +413,7 @@ int hhrr_set_rotor(hhrr_lattice* L, const hhrr_rotor_desc* r) {
   if (nodes > L->rot_nodes_cap)
     return fail(HHRR_E_SIZE, "hhrr_set_rotor: reference grid of %lld nodes does not fit the workspace (%lld)",
                 (long long)nodes, (long long)L->rot_nodes_cap);
-  quiesce_side(L);
+  join_side(L);
   int rc = upload(L, L->rot_sdf, r->sdf, sizeof(float) * nodes);
   if (rc) return rc;
   rc = upload(L, L->rot_tag, r->tag, nodes);
@@ -395,6 +469,7 @@ int hhrr_set_rotor(hhrr_lattice* L, const hhrr_rotor_desc* r) {
 }
 
 int hhrr_enable_wall_model(hhrr_lattice* L, int enable) {
+  DeviceGuard guard_(L);
   if (!L) return fail(HHRR_E_ARG, "hhrr_enable_wall_model: NULL lattice");
   L->wm_enabled = enable != 0;
   L->geometry_dirty = true;
@@ -403,12 +478,14 @@ int hhrr_enable_wall_model(hhrr_lattice* L, int enable) {
 }
 
 int hhrr_update_geometry(hhrr_lattice* L) {
+  DeviceGuard guard_(L);
   if (!L) return fail(HHRR_E_ARG, "hhrr_update_geometry: NULL lattice");
   L->geometry_current = false;
   return ensure_geometry(L);
 }
 
 int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant) {
+  DeviceGuard guard_(L);
   if (!L || (variant != 0 && variant != 2 && variant != 5)) return fail(HHRR_E_ARG, "hhrr_set_kernel_variant: bad argument");
   L->variant = variant;
   // variant 5 keeps the populations x-pulled (where it can run); everything else stores them post-stream
@@ -424,14 +501,17 @@ int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant) {
 }
 
 int hhrr_set_lookahead(hhrr_lattice* L, int enable) {
+  DeviceGuard guard_(L);
   if (!L) return fail(HHRR_E_ARG, "hhrr_set_lookahead: NULL lattice");
   L->lookahead = enable != 0;
   return HHRR_OK;
 }
 
-int hhrr_population_storage(const hhrr_lattice* L) { return L ? L->dom.xs : 0; }
+int hhrr_population_storage(const hhrr_lattice* L) {
+  DeviceGuard guard_(L); return L ? L->dom.xs : 0; }
 
 int hhrr_set_timing(hhrr_lattice* L, int enable) {
+  DeviceGuard guard_(L);
   if (!L) return fail(HHRR_E_ARG, "hhrr_set_timing: NULL lattice");
   if (enable && !L->ev[0])
     for (int k = 0; k < 2 * 1024; ++k) CU(cudaEventCreate(&L->ev[k]));
@@ -441,6 +521,7 @@ int hhrr_set_timing(hhrr_lattice* L, int enable) {
 }
 
 int hhrr_get_timing(hhrr_lattice* L, double* ms_collide_stream, int64_t* launches) {
+  DeviceGuard guard_(L);
   if (!L || !ms_collide_stream || !launches) return fail(HHRR_E_ARG, "hhrr_get_timing: NULL argument");
   CU(cudaStreamSynchronize(L->stream));
   double total = 0.0;
@@ -455,14 +536,26 @@ int hhrr_get_timing(hhrr_lattice* L, double* ms_collide_stream, int64_t* launche
   return HHRR_OK;
 }
 
-int64_t hhrr_launch_count(const hhrr_lattice* L) { return L ? L->launches : 0; }
-int64_t hhrr_step_count(const hhrr_lattice* L) { return L ? L->step : 0; }
+int64_t hhrr_launch_count(const hhrr_lattice* L) {
+  DeviceGuard guard_(L); return L ? L->launches : 0; }
+int64_t hhrr_step_count(const hhrr_lattice* L) {
+  DeviceGuard guard_(L); return L ? L->step : 0; }
 
+// One step = Listing 3.  On the caller's stream: [UpdatePorosityO(n): a pointer swap when it
+// was written ahead] -> collide-stream(n) -> WallModelO(n).  On the side stream, beside collide-stream(n):
+// UpdatePorosityO(n + 1) into the alternate geometry set; beside collide-stream(n + 1): the force collection
+// of step n, which only reads.  The call returns with the side stream joined into the caller's stream.
 int hhrr_step(hhrr_lattice* L, int32_t n_steps) {
+  DeviceGuard guard_(L);
   if (!L || n_steps < 0) return fail(HHRR_E_ARG, "hhrr_step: bad argument");
   for (int32_t s = 0; s < n_steps; ++s) {
     int rc = ensure_geometry(L);  // Listing 3 line 2: UpdatePorosityO
     if (rc) return rc;
+    if (L->side) {
+      CU(cudaEventRecord(L->ev_pre, L->stream));
+      // this launch overwrites the buffer the force kernel of two steps ago read (a no-op unless it is still running)
+      if (L->step >= 2) CU(cudaStreamWaitEvent(L->stream, L->ev_f[L->step & 1], 0));
+    }
     const bool timed = L->timing && L->ev_n < 1024;
     if (timed) CU(cudaEventRecord(L->ev[2 * L->ev_n], L->stream));
     cudaError_t e = launch_collide_stream(L);  // line 3
@@ -471,17 +564,31 @@ int hhrr_step(hhrr_lattice* L, int32_t n_steps) {
       CU(cudaEventRecord(L->ev[2 * L->ev_n + 1], L->stream));
       L->ev_n++;
     }
-    e = launch_phi_ahead(L);  // line 2 of the NEXT step, first half: queued behind this step's kernels
+    if (L->side) CU(cudaEventRecord(L->ev_k2, L->stream));
+    e = launch_geometry_ahead(L);  // line 2 of the NEXT step, on the side stream
     if (e != cudaSuccess) return cuda_fail(e, "geometry look-ahead");
-    e = launch_wall_model_and_forces(L);  // line 4: WallModelO; lines 5-6: forces (one launch)
-    if (e != cudaSuccess) return cuda_fail(e, "wall-model / force kernel");
+    const bool ahead = L->ahead_step == L->step + 1;
+    if (ahead && L->wm_enabled) CU(cudaStreamWaitEvent(L->stream, L->ev_k1, 0));  // the kernel marks the alternate flags
+    e = launch_wall_model(L, ahead);  // line 4: WallModelO
+    if (e != cudaSuccess) return cuda_fail(e, "wall-model kernel");
+    if (L->side) {  // lines 5-6: forces, beside the next collide-stream kernel
+      CU(cudaStreamWaitEvent(L->side, L->ev_k2, 0));
+      e = launch_forces(L, L->side);
+      CU(cudaEventRecord(L->ev_f[L->step & 1], L->side));
+      L->side_busy = true;
+    } else {
+      e = launch_forces(L, L->stream);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "force kernel");
     L->step += 1;  // line 7: theta_{n+1} = theta_n + Omega
     L->geometry_current = !L->has_rotor;  // static geometry stays valid
   }
+  join_side(L);
   return HHRR_OK;
 }
 
 int hhrr_get_moments_device(hhrr_lattice* L, float* d_rho, float* d_v) {
+  DeviceGuard guard_(L);
   if (!L || !d_rho || !d_v) return fail(HHRR_E_ARG, "hhrr_get_moments_device: NULL argument");
   cudaError_t e = launch_moments(L, d_rho, d_v);
   if (e != cudaSuccess) return cuda_fail(e, "moments kernel");
@@ -489,6 +596,7 @@ int hhrr_get_moments_device(hhrr_lattice* L, float* d_rho, float* d_v) {
 }
 
 int hhrr_get_moments(hhrr_lattice* L, float* rho, float* v) {
+  DeviceGuard guard_(L);
   if (!L || !rho || !v) return fail(HHRR_E_ARG, "hhrr_get_moments: NULL argument");
   const int64_t n = L->dom.n;
   float* scratch = L->fB;  // buffer B is free between steps
@@ -501,6 +609,7 @@ int hhrr_get_moments(hhrr_lattice* L, float* rho, float* v) {
 
 static int get_force_ring(hhrr_lattice* L, const double* ring, const char* who, int64_t first_step, int64_t n_steps,
                           double* F) {
+  DeviceGuard guard_(L);
   if (!L || !F || n_steps < 0) return fail(HHRR_E_ARG, "%s: bad argument", who);
   if (first_step < 0 || first_step + n_steps > L->step || first_step < L->step - FORCE_HISTORY)
     return fail(HHRR_E_STATE, "%s: steps [%lld,%lld) not in the recorded history (step %lld)", who,
@@ -519,14 +628,17 @@ static int get_force_ring(hhrr_lattice* L, const double* ring, const char* who, 
 }
 
 int hhrr_get_forces(hhrr_lattice* L, int64_t first_step, int64_t n_steps, double* F) {
+  DeviceGuard guard_(L);
   return get_force_ring(L, L ? L->force : nullptr, "hhrr_get_forces", first_step, n_steps, F);
 }
 
 int hhrr_get_torques(hhrr_lattice* L, int64_t first_step, int64_t n_steps, double* M) {
+  DeviceGuard guard_(L);
   return get_force_ring(L, L ? L->torque : nullptr, "hhrr_get_torques", first_step, n_steps, M);
 }
 
 int hhrr_get_cell_types(hhrr_lattice* L, uint8_t* type, uint8_t* tag, float* d) {
+  DeviceGuard guard_(L);
   if (!L) return fail(HHRR_E_ARG, "hhrr_get_cell_types: NULL lattice");
   const int64_t n = L->dom.n;
   if (type || tag) {
@@ -534,7 +646,7 @@ int hhrr_get_cell_types(hhrr_lattice* L, uint8_t* type, uint8_t* tag, float* d) 
     int rc = download(L, fl.data(), L->flags, (size_t)n);
     if (rc) return rc;
     for (int64_t c = 0; c < n; ++c) {
-      if (type) type[c] = fl[c] & TYPE_MASK;
+      if (type) type[c] = (uint8_t)public_type(fl[c] & TYPE_MASK);
       if (tag) tag[c] = (fl[c] >> TAG_SHIFT) & TAG_MASK;
     }
   }
@@ -558,13 +670,13 @@ __global__ void gather_cells_kernel(const float* f, const uint8_t* flags, Dom dm
   int64_t c = cells[k];
   const int x = (int)(c % dm.nx), y = (int)((c / dm.nx) % dm.ny), z = (int)(c / ((int64_t)dm.nx * dm.ny));
   for (int i = 0; i < Q; ++i) out[k * Q + i] = f[pop_index(dm, i, x, y, z)];
-  out_flags[k] = flags[c];
+  out_flags[k] = (uint8_t)((flags[c] & ~TYPE_MASK) | public_type(flags[c] & TYPE_MASK));
 }
-int read_counters(hhrr_lattice* L, Counters* h) { return download(L, h, L->counters, sizeof(Counters)); }
 }  // namespace
 
 int hhrr_get_wall_list(hhrr_lattice* L, int64_t capacity, int32_t* idx, double* y1n, double* u_tau,
                        uint8_t* valid, int64_t* count) {
+  DeviceGuard guard_(L);
   if (!L || !count) return fail(HHRR_E_ARG, "hhrr_get_wall_list: NULL argument");
   Counters h;
   int rc = read_counters(L, &h);
@@ -607,6 +719,7 @@ int hhrr_get_wall_list(hhrr_lattice* L, int64_t capacity, int32_t* idx, double* 
 
 int hhrr_get_wall_state(hhrr_lattice* L, int64_t cell, double* u_tau, double u_wm[3], double s_wm[6],
                         int32_t* valid) {
+  DeviceGuard guard_(L);
   if (!L || cell < 0 || cell >= L->dom.n) return fail(HHRR_E_ARG, "hhrr_get_wall_state: bad argument");
   const int64_t n = L->dom.n;
   double ut;
@@ -628,29 +741,37 @@ int hhrr_get_wall_state(hhrr_lattice* L, int64_t cell, double* u_tau, double u_w
 
 int hhrr_get_cell_populations(hhrr_lattice* L, int64_t n_cells, const int64_t* cells, float* out,
                               uint8_t* flags) {
+  DeviceGuard guard_(L);
   if (!L || !cells || !out || n_cells < 0) return fail(HHRR_E_ARG, "hhrr_get_cell_populations: bad argument");
   if (n_cells == 0) return HHRR_OK;
-  if (n_cells > L->dom.n) return fail(HHRR_E_ARG, "hhrr_get_cell_populations: more cells than the lattice has");
   for (int64_t k = 0; k < n_cells; ++k)
     if (cells[k] < 0 || cells[k] >= L->dom.n) return fail(HHRR_E_ARG, "hhrr_get_cell_populations: cell out of range");
-  // scratch in buffer B: [cells | out | flags]
+  // scratch in buffer B, [cells 8 B | out 108 B | flags 1 B] per cell: as many cells per pass as fit
   char* sb = reinterpret_cast<char*>(L->fB);
-  int64_t* d_cells = reinterpret_cast<int64_t*>(sb);
-  float* d_out = reinterpret_cast<float*>(sb + 8 * n_cells);
-  uint8_t* d_fl = reinterpret_cast<uint8_t*>(sb + 8 * n_cells + 4 * Q * n_cells);
-  int rc = upload(L, d_cells, cells, 8 * (size_t)n_cells);
-  if (rc) return rc;
-  gather_cells_kernel<<<(unsigned)((n_cells + 127) / 128), 128, 0, L->stream>>>(L->fA, L->flags, L->dom, d_cells,
-                                                                             n_cells, d_out, d_fl);
-  L->launches++;
-  CU(cudaGetLastError());
-  rc = download(L, out, d_out, 4 * (size_t)Q * n_cells);
-  if (rc) return rc;
-  if (flags) return download(L, flags, d_fl, (size_t)n_cells);
+  const int64_t per_pass = std::max<int64_t>(1, (int64_t)(sizeof(float) * Q * (size_t)L->dom.n / (8 + 4 * Q + 1)));
+  for (int64_t k0 = 0; k0 < n_cells; k0 += per_pass) {
+    const int64_t m = std::min(per_pass, n_cells - k0);
+    int64_t* d_cells = reinterpret_cast<int64_t*>(sb);
+    float* d_out = reinterpret_cast<float*>(sb + 8 * m);
+    uint8_t* d_fl = reinterpret_cast<uint8_t*>(sb + 8 * m + 4 * Q * m);
+    int rc = upload(L, d_cells, cells + k0, 8 * (size_t)m);
+    if (rc) return rc;
+    gather_cells_kernel<<<(unsigned)((m + 127) / 128), 128, 0, L->stream>>>(L->fA, L->flags, L->dom, d_cells, m, d_out,
+                                                                         d_fl);
+    L->launches++;
+    CU(cudaGetLastError());
+    rc = download(L, out + (size_t)Q * k0, d_out, 4 * (size_t)Q * m);
+    if (rc) return rc;
+    if (flags) {
+      rc = download(L, flags + k0, d_fl, (size_t)m);
+      if (rc) return rc;
+    }
+  }
   return HHRR_OK;
 }
 
 int hhrr_get_populations(hhrr_lattice* L, float* f_minus_w) {
+  DeviceGuard guard_(L);
   if (!L || !f_minus_w) return fail(HHRR_E_ARG, "hhrr_get_populations: NULL argument");
   if (!L->dom.xs) return download(L, f_minus_w, L->fA, sizeof(float) * Q * L->dom.n);
   // the ABI speaks the plain post-stream layout: convert into buffer B (free between steps), read that
@@ -665,6 +786,7 @@ int hhrr_get_populations(hhrr_lattice* L, float* f_minus_w) {
   return rc;
 }
 int hhrr_set_populations(hhrr_lattice* L, const float* f_minus_w) {
+  DeviceGuard guard_(L);
   if (!L || !f_minus_w) return fail(HHRR_E_ARG, "hhrr_set_populations: NULL argument");
   int rc = upload(L, L->fA, f_minus_w, sizeof(float) * Q * L->dom.n);
   if (rc || !L->dom.xs) return rc;
@@ -675,11 +797,116 @@ int hhrr_set_populations(hhrr_lattice* L, const float* f_minus_w) {
   return HHRR_OK;
 }
 int hhrr_get_uhat(hhrr_lattice* L, float* uhat) {
+  DeviceGuard guard_(L);
   if (!L || !uhat) return fail(HHRR_E_ARG, "hhrr_get_uhat: NULL argument");
+  if (L->variant != 0 || L->step == 0)
+    return fail(HHRR_E_STATE, "hhrr_get_uhat: only the two-pass kernel (variant 0) stores the field, and only after a step");
   return download(L, uhat, L->uhat, sizeof(float) * 3 * L->dom.n);
 }
 
+
+namespace {
+__global__ void gather_wall_state_kernel(const int32_t* idx, int count, int64_t n, const double* wm_utau, const float* wm_u,
+                                         const float* wm_s, const uint8_t* flags, double* o_utau, float* o_u, float* o_s,
+                                         uint8_t* o_valid) {
+  int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= count) return;
+  const int64_t c = idx[e];
+  o_utau[e] = wm_utau[c];
+  for (int q = 0; q < 3; ++q) o_u[3 * (int64_t)e + q] = wm_u[q * n + c];
+  for (int q = 0; q < 6; ++q) o_s[6 * (int64_t)e + q] = wm_s[q * n + c];
+  o_valid[e] = (flags[c] & WM_VALID) ? 1 : 0;
+}
+__global__ void scatter_wall_state_kernel(const int32_t* idx, int count, int64_t n, const double* i_utau, const float* i_u,
+                                          const float* i_s, const uint8_t* i_valid, double* wm_utau, float* wm_u,
+                                          float* wm_s, uint8_t* flags) {
+  int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= count) return;
+  const int64_t c = idx[e];
+  const uint8_t fl = flags[c];
+  if ((fl & TYPE_MASK) != T_FRONTIER_W) return;  // not in the wall-model set of the current geometry: no state to hold
+  wm_utau[c] = i_utau[e];
+  for (int q = 0; q < 3; ++q) wm_u[q * n + c] = i_u[3 * (int64_t)e + q];
+  for (int q = 0; q < 6; ++q) wm_s[q * n + c] = i_s[6 * (int64_t)e + q];
+  flags[c] = i_valid[e] ? (fl | WM_VALID) : (fl & ~WM_VALID);
+}
+}  // namespace
+
+int hhrr_get_wall_model_state(hhrr_lattice* L, int64_t capacity, int32_t* idx, double* u_tau, float* u_wm, float* s_wm,
+                              uint8_t* valid, int64_t* count) {
+  DeviceGuard guard_(L);
+  if (!L || !count) return fail(HHRR_E_ARG, "hhrr_get_wall_model_state: NULL argument");
+  Counters h;
+  int rc = read_counters(L, &h);
+  if (rc) return rc;
+  if (h.overflow) return fail(HHRR_E_SIZE, "compact cell list overflowed its capacity of %lld", (long long)L->cap_list);
+  const int64_t k = h.wall_count;
+  *count = k;
+  if (k == 0 || capacity <= 0) return HHRR_OK;
+  if (capacity < k || !idx || !u_tau || !u_wm || !s_wm || !valid)
+    return fail(HHRR_E_ARG, "hhrr_get_wall_model_state: capacity %lld < %lld cells, or a NULL array", (long long)capacity,
+                (long long)k);
+  char* sb = reinterpret_cast<char*>(L->fB);  // scratch: buffer B is free between steps
+  double* s_utau = reinterpret_cast<double*>(sb);
+  float* s_u = reinterpret_cast<float*>(s_utau + k);
+  float* s_s = s_u + 3 * k;
+  uint8_t* s_v = reinterpret_cast<uint8_t*>(s_s + 6 * k);
+  gather_wall_state_kernel<<<(unsigned)((k + 255) / 256), 256, 0, L->stream>>>(L->wall_idx, (int)k, L->dom.n, L->wm_utau,
+                                                                              L->wm_u, L->wm_s, L->flags, s_utau, s_u, s_s, s_v);
+  L->launches++;
+  CU(cudaGetLastError());
+  if ((rc = download(L, idx, L->wall_idx, sizeof(int32_t) * k))) return rc;
+  if ((rc = download(L, u_tau, s_utau, sizeof(double) * k))) return rc;
+  if ((rc = download(L, u_wm, s_u, sizeof(float) * 3 * k))) return rc;
+  if ((rc = download(L, s_wm, s_s, sizeof(float) * 6 * k))) return rc;
+  return download(L, valid, s_v, (size_t)k);
+}
+
+int hhrr_set_wall_model_state(hhrr_lattice* L, int64_t count, const int32_t* idx, const double* u_tau, const float* u_wm,
+                              const float* s_wm, const uint8_t* valid) {
+  DeviceGuard guard_(L);
+  if (!L || count < 0 || (count > 0 && (!idx || !u_tau || !u_wm || !s_wm || !valid)))
+    return fail(HHRR_E_ARG, "hhrr_set_wall_model_state: bad argument");
+  if (count > L->cap_list) return fail(HHRR_E_SIZE, "hhrr_set_wall_model_state: more cells than the wall list can hold");
+  for (int64_t e = 0; e < count; ++e)
+    if (idx[e] < 0 || idx[e] >= L->dom.n) return fail(HHRR_E_ARG, "hhrr_set_wall_model_state: cell out of range");
+  int rc = ensure_geometry(L);  // the state belongs to cells of W of the current step's geometry
+  if (rc || count == 0) return rc;
+  const int64_t k = count;
+  char* sb = reinterpret_cast<char*>(L->fB);
+  double* s_utau = reinterpret_cast<double*>(sb);
+  float* s_u = reinterpret_cast<float*>(s_utau + k);
+  float* s_s = s_u + 3 * k;
+  uint8_t* s_v = reinterpret_cast<uint8_t*>(s_s + 6 * k);
+  int32_t* s_idx = reinterpret_cast<int32_t*>(sb + align_up((size_t)k * (8 + 12 + 24 + 1)));
+  if ((rc = upload(L, s_utau, u_tau, sizeof(double) * k))) return rc;
+  if ((rc = upload(L, s_u, u_wm, sizeof(float) * 3 * k))) return rc;
+  if ((rc = upload(L, s_s, s_wm, sizeof(float) * 6 * k))) return rc;
+  if ((rc = upload(L, s_v, valid, (size_t)k))) return rc;
+  if ((rc = upload(L, s_idx, idx, sizeof(int32_t) * k))) return rc;
+  scatter_wall_state_kernel<<<(unsigned)((k + 255) / 256), 256, 0, L->stream>>>(s_idx, (int)k, L->dom.n, s_utau, s_u, s_s, s_v,
+                                                                               L->wm_utau, L->wm_u, L->wm_s, L->flags);
+  L->launches++;
+  CU(cudaGetLastError());
+  CU(cudaStreamSynchronize(L->stream));
+  return HHRR_OK;
+}
+
+int hhrr_set_step_count(hhrr_lattice* L, int64_t step) {
+  DeviceGuard guard_(L);
+  if (!L || step < 0) return fail(HHRR_E_ARG, "hhrr_set_step_count: bad argument");
+  join_side(L);
+  if (L->ahead_step >= 0) {  // a geometry written ahead belongs to the run that was going on: dropped
+    cudaStreamWaitEvent(L->stream, L->ev_k1, 0);
+    L->ahead_step = -1;
+  }
+  L->step = step;
+  L->geometry_current = !L->has_rotor && L->geometry_current;  // the rotor angle follows the step count
+  return HHRR_OK;
+}
+
 int hhrr_check_finite(hhrr_lattice* L) {
+  DeviceGuard guard_(L);
   if (!L) return fail(HHRR_E_ARG, "hhrr_check_finite: NULL lattice");
   cudaError_t e = launch_check_finite(L);
   if (e != cudaSuccess) return cuda_fail(e, "finite-check kernel");

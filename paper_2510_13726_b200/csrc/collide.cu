@@ -31,7 +31,7 @@ __device__ __forceinline__ void cell_solid_state(const PhysF& ph, const BodiesF&
   d = 1.f;
   uB[0] = uB[1] = uB[2] = 0.f;
   if (type_has_solid_state(type)) {
-    d = (type == HHRR_FRONTIER) ? __ldg(dfield + c) : 0.f;
+    d = type_is_frontier(type) ? __ldg(dfield + c) : 0.f;
     solid_velocity(ph, bo, fl, x, y, z, uB);
     if (fl & WM_VALID) {
       uB[0] += __ldg(wm_u + c);

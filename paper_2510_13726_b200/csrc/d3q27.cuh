@@ -36,21 +36,49 @@ __device__ __forceinline__ float sqrt_fast(float x) {
   return r;
 }
 
-struct Moments {  // of the deviations: drho = rho - 1, j, M_ab = sum c_a c_b (f - w)
-  float drho, jx, jy, jz, mxx, myy, mzz, mxy, mxz, myz;
+// Two x-adjacent cells in one register pair (.x: cell x, .y: cell x + 1): sm_100's packed fp32 arithmetic
+// (FADD2 / FMUL2 / FFMA2) runs the same instruction stream on both -- half the issue slots of the scalar code.
+// Every arithmetic routine below is a template over T = float (one cell) or T = f2 (a cell pair).
+struct f2 {
+  float2 v;
 };
+__device__ __forceinline__ f2 mk2(float a, float b) { return f2{make_float2(a, b)}; }
+__device__ __forceinline__ f2 operator+(f2 a, f2 b) { return f2{__fadd2_rn(a.v, b.v)}; }
+__device__ __forceinline__ f2 operator-(f2 a, f2 b) { return f2{__fadd2_rn(a.v, make_float2(-b.v.x, -b.v.y))}; }
+__device__ __forceinline__ f2 operator-(f2 a) { return f2{make_float2(-a.v.x, -a.v.y)}; }
+__device__ __forceinline__ f2 operator*(f2 a, f2 b) { return f2{__fmul2_rn(a.v, b.v)}; }
+__device__ __forceinline__ f2 operator*(float s, f2 b) { return f2{__fmul2_rn(make_float2(s, s), b.v)}; }
+__device__ __forceinline__ f2 operator*(f2 a, float s) { return f2{__fmul2_rn(a.v, make_float2(s, s))}; }
+__device__ __forceinline__ f2 operator+(f2 a, float s) { return f2{__fadd2_rn(a.v, make_float2(s, s))}; }
+__device__ __forceinline__ f2 operator+(float s, f2 a) { return f2{__fadd2_rn(a.v, make_float2(s, s))}; }
+__device__ __forceinline__ f2 operator-(f2 a, float s) { return f2{__fadd2_rn(a.v, make_float2(-s, -s))}; }
+__device__ __forceinline__ f2 operator-(float s, f2 a) { return f2{__fadd2_rn(make_float2(s, s), make_float2(-a.v.x, -a.v.y))}; }
+__device__ __forceinline__ f2 fma_t(f2 a, f2 b, f2 c) { return f2{__ffma2_rn(a.v, b.v, c.v)}; }
+__device__ __forceinline__ f2 fma_t(float a, f2 b, f2 c) { return f2{__ffma2_rn(make_float2(a, a), b.v, c.v)}; }
+__device__ __forceinline__ float fma_t(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ f2 rcp_nr(f2 x) { return mk2(rcp_nr(x.v.x), rcp_nr(x.v.y)); }
+__device__ __forceinline__ f2 sqrt_fast(f2 x) { return mk2(sqrt_fast(x.v.x), sqrt_fast(x.v.y)); }
+template <class T> __device__ __forceinline__ T bcast(float s);
+template <> __device__ __forceinline__ float bcast<float>(float s) { return s; }
+template <> __device__ __forceinline__ f2 bcast<f2>(float s) { return mk2(s, s); }
+
+template <class T>
+struct MomentsT {  // of the deviations: drho = rho - 1, j, M_ab = sum c_a c_b (f - w)
+  T drho, jx, jy, jz, mxx, myy, mzz, mxy, mxz, myz;
+};
+using Moments = MomentsT<float>;
 
 // rho and j only (halo cells, moments pass, read-back): 3 separable passes
-__device__ __forceinline__ void moments_rho_j(const float (&f)[Q], float& drho, float& jx, float& jy,
-                                              float& jz) {
-  float s0[9], s1[9];
+template <class T>
+__device__ __forceinline__ void moments_rho_j(const T (&f)[Q], T& drho, T& jx, T& jy, T& jz) {
+  T s0[9], s1[9];
 #pragma unroll
   for (int m = 0; m < 9; ++m) {
-    float fm = f[3 * m], f0 = f[3 * m + 1], fp = f[3 * m + 2];
+    T fm = f[3 * m], f0 = f[3 * m + 1], fp = f[3 * m + 2];
     s0[m] = (fp + fm) + f0;
     s1[m] = fp - fm;
   }
-  float t00[3], t01[3], t10[3];
+  T t00[3], t01[3], t10[3];
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
     t00[k] = (s0[3 * k + 2] + s0[3 * k]) + s0[3 * k + 1];
@@ -63,16 +91,17 @@ __device__ __forceinline__ void moments_rho_j(const float (&f)[Q], float& drho, 
   jx = (t10[2] + t10[0]) + t10[1];
 }
 
-__device__ __forceinline__ Moments moments_all(const float (&f)[Q]) {
-  float s0[9], s1[9], s2[9];
+template <class T>
+__device__ __forceinline__ MomentsT<T> moments_all(const T (&f)[Q]) {
+  T s0[9], s1[9], s2[9];
 #pragma unroll
   for (int m = 0; m < 9; ++m) {
-    float fm = f[3 * m], f0 = f[3 * m + 1], fp = f[3 * m + 2];
+    T fm = f[3 * m], f0 = f[3 * m + 1], fp = f[3 * m + 2];
     s2[m] = fp + fm;
     s0[m] = s2[m] + f0;
     s1[m] = fp - fm;
   }
-  float t00[3], t01[3], t02[3], t10[3], t11[3], t20[3];
+  T t00[3], t01[3], t02[3], t10[3], t11[3], t20[3];
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
     t02[k] = s0[3 * k + 2] + s0[3 * k];
@@ -82,7 +111,7 @@ __device__ __forceinline__ Moments moments_all(const float (&f)[Q]) {
     t11[k] = s1[3 * k + 2] - s1[3 * k];
     t20[k] = (s2[3 * k + 2] + s2[3 * k]) + s2[3 * k + 1];
   }
-  Moments m;
+  MomentsT<T> m;
   m.mzz = t00[2] + t00[0];
   m.drho = m.mzz + t00[1];
   m.jz = t00[2] - t00[0];
@@ -105,7 +134,7 @@ __device__ __forceinline__ void solid_velocity(const PhysF& ph, const BodiesF& b
     uB[0] = ph.fr_u[0];
     uB[1] = ph.fr_u[1];
     uB[2] = ph.fr_u[2];
-  } else if (type == HHRR_SOLID || type == HHRR_FRONTIER) {
+  } else if (type == HHRR_SOLID || type == HHRR_FRONTIER || type == T_FRONTIER_W) {
     int k = (flags >> TAG_SHIFT) & TAG_MASK;
     float rx = (float)x - bo.c[k][0], ry = (float)y - bo.c[k][1], rz = (float)z - bo.c[k][2];
     uB[0] = bo.v[k][0] + (bo.w[k][1] * rz - bo.w[k][2] * ry);
@@ -118,18 +147,19 @@ __device__ __forceinline__ void solid_velocity(const PhysF& ph, const BodiesF& b
 __device__ __forceinline__ float cell_sigma(const PhysF& ph, uint8_t flags) {
   return (flags & TYPE_MASK) == HHRR_BULK ? 1.f : ph.sigma;
 }
-__device__ __forceinline__ bool type_has_solid_state(int type) {  // FRONTIER, SOLID, FRINGE: d < 1, u^B
-  return type >= HHRR_FRONTIER && type <= HHRR_FRINGE;
+__device__ __forceinline__ bool type_has_solid_state(int type) {  // FRONTIER (in W or not), SOLID, FRINGE: d < 1, u^B
+  return (type >= HHRR_FRONTIER && type <= HHRR_FRINGE) || type == T_FRONTIER_W;
 }
+__device__ __forceinline__ bool type_is_frontier(int type) { return type == HHRR_FRONTIER || type == T_FRONTIER_W; }
 
 // Eq. 12 with reading R1 (d = 1 fluid): uhat = d u + (1-d) u^B, u = (j + g)/rho  (R11)
-__device__ __forceinline__ void homogenised_velocity(const PhysF& ph, float drho, float jx, float jy,
-                                                     float jz, float d, const float uB[3], float& rho,
-                                                     float uh[3]) {
+template <class T>
+__device__ __forceinline__ void homogenised_velocity(const PhysF& ph, T drho, T jx, T jy, T jz, T d, const T uB[3],
+                                                     T& rho, T uh[3]) {
   rho = 1.f + drho;
-  float ir = rcp_nr(rho);
-  float ux = (jx + ph.g[0]) * ir, uy = (jy + ph.g[1]) * ir, uz = (jz + ph.g[2]) * ir;
-  float e = 1.f - d;
+  T ir = rcp_nr(rho);
+  T ux = (jx + ph.g[0]) * ir, uy = (jy + ph.g[1]) * ir, uz = (jz + ph.g[2]) * ir;
+  T e = 1.f - d;
   uh[0] = d * ux + e * uB[0];
   uh[1] = d * uy + e * uB[1];
   uh[2] = d * uz + e * uB[2];
@@ -138,42 +168,44 @@ __device__ __forceinline__ void homogenised_velocity(const PhysF& ph, float drho
 // One collision.  m: moments of the deviations; rho, uh: from homogenised_velocity;
 // S: strain handed to the hybrid term (xx yy zz xy xz yz); sigma: this cell's hybrid factor.
 // Output: post-collision deviations f*_i - w_i.
-__device__ __forceinline__ void collide(const PhysF& ph, const Moments& m, float rho, const float uh[3],
-                                        const float S[6], float sigma, float (&out)[Q]) {
+template <class T>
+__device__ __forceinline__ void collide(const PhysF& ph, const MomentsT<T>& m, T rho, const T uh[3], const T S[6],
+                                        T sigma, T (&out)[Q]) {
   const float third = 1.f / 3.f;
-  float ux = uh[0], uy = uh[1], uz = uh[2];
-  float rux = rho * ux, ruy = rho * uy, ruz = rho * uz;
+  T ux = uh[0], uy = uh[1], uz = uh[2];
+  T rux = rho * ux, ruy = rho * uy, ruz = rho * uz;
   // Pi^neq = sum H2 f - rho uh uh  (R4)
-  float dr3 = m.drho * third;
-  float pxx = m.mxx - dr3 - rux * ux, pyy = m.myy - dr3 - ruy * uy, pzz = m.mzz - dr3 - ruz * uz;
-  float pxy = m.mxy - rux * uy, pxz = m.mxz - rux * uz, pyz = m.myz - ruy * uz;
+  T dr3 = third * m.drho;
+  T pxx = m.mxx - dr3 - rux * ux, pyy = m.myy - dr3 - ruy * uy, pzz = m.mzz - dr3 - ruz * uz;
+  T pxy = m.mxy - rux * uy, pxz = m.mxz - rux * uz, pyz = m.myz - ruy * uz;
   // Smagorinsky closed form (Eq. 3-5, 14; R6)
-  float pp = pxx * pxx + pyy * pyy + pzz * pzz + 2.f * (pxy * pxy + pxz * pxz + pyz * pyz);
-  float Qn = sqrt_fast(2.f * pp);
-  float tau = 0.5f * (ph.tau0 + sqrt_fast(ph.tau0 * ph.tau0 + ph.smag18 * Qn * rcp_nr(rho)));
-  float k = 1.f - rcp_nr(tau);
-  // hybrid a1^(2) (Eq. 7 + Eq. 10; R2)
-  float hs = (1.f - sigma) * (2.f * third) * rho * tau;
-  float axx = sigma * pxx - hs * S[0], ayy = sigma * pyy - hs * S[1], azz = sigma * pzz - hs * S[2];
-  float axy = sigma * pxy - hs * S[3], axz = sigma * pxz - hs * S[4], ayz = sigma * pyz - hs * S[5];
+  T pp = pxx * pxx + pyy * pyy + pzz * pzz + 2.f * (pxy * pxy + pxz * pxz + pyz * pyz);
+  T Qn = sqrt_fast(2.f * pp);
+  T tau = 0.5f * (ph.tau0 + sqrt_fast(ph.tau0 * ph.tau0 + ph.smag18 * (Qn * rcp_nr(rho))));
+  T k = 1.f - rcp_nr(tau);
+  // hybrid a1^(2) (Eq. 7 + Eq. 10; R2), already scaled by k = 1 - 1/tau_eff (Eq. 6)
+  T ks = k * sigma, kh = k * ((1.f - sigma) * ((2.f * third) * (rho * tau)));
+  T axx = ks * pxx - kh * S[0], ayy = ks * pyy - kh * S[1], azz = ks * pzz - kh * S[2];
+  T axy = ks * pxy - kh * S[3], axz = ks * pxz - kh * S[4], ayz = ks * pyz - kh * S[5];
   // second order: T = 4.5 (rho uh uh + k a2)
-  float Txx = 4.5f * (rux * ux + k * axx), Tyy = 4.5f * (ruy * uy + k * ayy), Tzz = 4.5f * (ruz * uz + k * azz);
-  float Txy = 9.f * (rux * uy + k * axy), Txz = 9.f * (rux * uz + k * axz), Tyz = 9.f * (ruy * uz + k * ayz);
+  T Txx = 4.5f * (rux * ux + axx), Tyy = 4.5f * (ruy * uy + ayy), Tzz = 4.5f * (ruz * uz + azz);
+  T Txy = 9.f * (rux * uy + axy), Txz = 9.f * (rux * uz + axz), Tyz = 9.f * (ruy * uz + ayz);
   // third order (R3): A3_aab = rho ua ua ub + k (2 ua a_ab + ub a_aa); G_ab = 13.5 A3_aab; Gxyz = 27 A3_xyz
-  float Gxy = 13.5f * (rux * ux * uy + k * (2.f * ux * axy + uy * axx));  // xx y
-  float Gxz = 13.5f * (rux * ux * uz + k * (2.f * ux * axz + uz * axx));  // xx z
-  float Gyx = 13.5f * (ruy * uy * ux + k * (2.f * uy * axy + ux * ayy));  // yy x
-  float Gyz = 13.5f * (ruy * uy * uz + k * (2.f * uy * ayz + uz * ayy));  // yy z
-  float Gzx = 13.5f * (ruz * uz * ux + k * (2.f * uz * axz + ux * azz));  // zz x
-  float Gzy = 13.5f * (ruz * uz * uy + k * (2.f * uz * ayz + uy * azz));  // zz y
-  float Gxyz = 27.f * (rux * uy * uz + k * (ux * ayz + uy * axz + uz * axy));
+  T ux2 = ux + ux, uy2 = uy + uy, uz2 = uz + uz;
+  T Gxy = 13.5f * ((rux * ux) * uy + (ux2 * axy + uy * axx));  // xx y
+  T Gxz = 13.5f * ((rux * ux) * uz + (ux2 * axz + uz * axx));  // xx z
+  T Gyx = 13.5f * ((ruy * uy) * ux + (uy2 * axy + ux * ayy));  // yy x
+  T Gyz = 13.5f * ((ruy * uy) * uz + (uy2 * ayz + uz * ayy));  // yy z
+  T Gzx = 13.5f * ((ruz * uz) * ux + (uz2 * axz + ux * azz));  // zz x
+  T Gzy = 13.5f * ((ruz * uz) * uy + (uz2 * ayz + uy * azz));  // zz y
+  T Gxyz = 27.f * ((rux * uy) * uz + (ux * ayz + uy * axz + uz * axy));
   // even part tables: q(c) = c^2 - 1/3
-  float Ex[2] = {-third * Txx, 2.f * third * Txx};
-  float Ey[2] = {-third * Tyy, 2.f * third * Tyy};
-  float Ez[2] = {m.drho - third * Tzz, m.drho + 2.f * third * Tzz};
+  T Ex[2] = {-third * Txx, (2.f * third) * Txx};
+  T Ey[2] = {-third * Tyy, (2.f * third) * Tyy};
+  T Ez[2] = {m.drho - third * Tzz, m.drho + (2.f * third) * Tzz};
   // odd part: coefficient of c_b is m_b + sum_{a != b} q(c_a) G_ab
-  float mx = 3.f * rux, my = 3.f * ruy, mz = 3.f * ruz;
-  float OX[2][2], OY[2][2], OZ[2][2];  // [other axis 1 squared][other axis 2 squared]
+  T mx = 3.f * rux, my = 3.f * ruy, mz = 3.f * ruz;
+  T OX[2][2], OY[2][2], OZ[2][2];  // [other axis 1 squared][other axis 2 squared]
 #pragma unroll
   for (int p = 0; p < 2; ++p)
 #pragma unroll
@@ -187,29 +219,30 @@ __device__ __forceinline__ void collide(const PhysF& ph, const Moments& m, float
   for (int i = 0; i <= 13; ++i) {
     const int cx = dir_cx(i), cy = dir_cy(i), cz = dir_cz(i);
     const int x2 = cx * cx, y2 = cy * cy, z2 = cz * cz;
-    float E = Ex[x2] + Ey[y2] + Ez[z2];
-    if (cx * cy == 1) E += Txy;
-    if (cx * cy == -1) E -= Txy;
-    if (cx * cz == 1) E += Txz;
-    if (cx * cz == -1) E -= Txz;
-    if (cy * cz == 1) E += Tyz;
-    if (cy * cz == -1) E -= Tyz;
+    T E = Ex[x2] + Ey[y2] + Ez[z2];
+    if (cx * cy == 1) E = E + Txy;
+    if (cx * cy == -1) E = E - Txy;
+    if (cx * cz == 1) E = E + Txz;
+    if (cx * cz == -1) E = E - Txz;
+    if (cy * cz == 1) E = E + Tyz;
+    if (cy * cz == -1) E = E - Tyz;
     const float w = dir_w(i);
     if (i == 13) {
       out[13] = w * E;
     } else {
-      float O = 0.f;
-      if (cx == 1) O += OX[y2][z2];
-      if (cx == -1) O -= OX[y2][z2];
-      if (cy == 1) O += OY[x2][z2];
-      if (cy == -1) O -= OY[x2][z2];
-      if (cz == 1) O += OZ[x2][y2];
-      if (cz == -1) O -= OZ[x2][y2];
-      if (cx * cy * cz == 1) O += Gxyz;
-      if (cx * cy * cz == -1) O -= Gxyz;
-      const float wE = w * E;
-      out[i] = fmaf(w, O, wE);
-      out[26 - i] = fmaf(-w, O, wE);
+      T O = bcast<T>(0.f);
+      bool first = true;
+      auto acc = [&](const T& v, int sgn) {
+        if (first) { O = sgn > 0 ? v : -v; first = false; }
+        else O = sgn > 0 ? O + v : O - v;
+      };
+      if (cx) acc(OX[y2][z2], cx);
+      if (cy) acc(OY[x2][z2], cy);
+      if (cz) acc(OZ[x2][y2], cz);
+      if (cx * cy * cz) acc(Gxyz, cx * cy * cz);
+      const T wE = w * E;
+      out[i] = fma_t(w, O, wE);
+      out[26 - i] = fma_t(-w, O, wE);
     }
   }
 }

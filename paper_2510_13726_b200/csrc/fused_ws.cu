@@ -218,7 +218,7 @@ static cudaError_t launch_ws_cfg(hhrr_lattice* L, const WsArgs& a0) {
   using C = WsCfg<TX, TY, NPW, DEPTH, CPT>;
   WsArgs a = a0;
   const Dom& dm = L->dom;
-  static bool attr_set = false;
+  bool& attr_set = L->attr_ws;  // the attribute is per device: kept per lattice
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(fused_ws_kernel<TX, TY, NPW, DEPTH, CPT>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);

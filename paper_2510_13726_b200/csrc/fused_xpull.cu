@@ -31,7 +31,9 @@ template <int TX_, int TY_>
 struct XpCfg {
   static constexpr int TX = TX_, TY = TY_, NS = 2, W = TX + 8;
   static constexpr int WORKERS = TX * TY / 2, AUX = 96, THREADS = WORKERS + AUX + 32;
-  static constexpr int SX = TX + 2, SY = TY + 2, PLANE = SX * SY;
+  // uhat ring plane: SY rows of SX floats; tile cell lx sits at column lx + 2 (an EVEN slot: a worker's cell pair
+  // is one aligned 8-byte word), the x halo at columns 1 and TX + 2, columns 0 and TX + 3 are padding
+  static constexpr int SX = TX + 4, SY = TY + 2, PLANE = SX * SY;
   static constexpr int HALO = 2 * TX + 2 * TY, HSLOTS = (HALO + AUX - 1) / AUX;
   // one stage, in floats: [27][TY][W] tile rows | [27][W] row y0-1 | [27][W] row y0+TY |
   //                       [27][TY][4] wrapped columns of the tile rows | [27][4] | [27][4] of the halo rows
@@ -261,7 +263,7 @@ __global__ void __launch_bounds__(C::THREADS, 1)
         lx = hc % TX;
         region = 1 + top;
         h_fl[k] = (top ? FL_YP : FL_YM) + lx;
-        h_slot[k] = (top ? TY + 1 : 0) * SX + lx + 1;
+        h_slot[k] = (top ? TY + 1 : 0) * SX + lx + 2;
         h_y[k] = top ? yp : ym;
         h_fy[k] = top ? fyp : fym;
       } else {
@@ -270,7 +272,7 @@ __global__ void __launch_bounds__(C::THREADS, 1)
         lx = right ? TX : -1;
         region = 0;
         h_fl[k] = FL_XM + right * TY + row;
-        h_slot[k] = (row + 1) * SX + (right ? TX + 1 : 0);
+        h_slot[k] = (row + 1) * SX + (right ? TX + 2 : 1);
         h_y[k] = y0 + row;
       }
       int xr = x0 + lx;
@@ -330,11 +332,13 @@ __global__ void __launch_bounds__(C::THREADS, 1)
   }
 
   // -------------------------------------------------------------------- workers, two x-adjacent cells each
+  // The two cells of a thread run the same arithmetic: populations, moments, uhat, strain and the 27 results
+  // live in register pairs (f2: .x = cell xa, .y = cell xa + 1) and go through FADD2 / FMUL2 / FFMA2.
   constexpr int HX = TX / 2;
   const int tx2 = tid % HX, ty = tid / HX;
   const int xa = x0 + 2 * tx2, yv = y0 + ty;  // cells (xa, yv) and (xa + 1, yv)
   const bool row_interior = yv > 0 && yv < dm.ny - 1;
-  const int own_slot = (ty + 1) * SX + 2 * tx2 + 1;
+  const int own_slot = (ty + 1) * SX + 2 * tx2 + 2;
   const int own_off = ty * W + 4 + 2 * tx2;   // + i * TY * W: population i of cell xa, unshifted column
   const int own_fl = ty * TX + 2 * tx2;
   const int64_t own_xy = xa + nx * yv;
@@ -342,9 +346,9 @@ __global__ void __launch_bounds__(C::THREADS, 1)
   const bool patch_l = edge_l && tx2 == 0, patch_r = edge_r && tx2 == HX - 1;
   const int patch_off = O_PM + ty * 4 + (patch_l ? 3 : 0);
 
-  Moments mcur[2] = {}, mnext[2] = {};
-  float rho_c[2] = {1.f, 1.f}, rho_n[2] = {1.f, 1.f}, uh_c[2][3] = {}, uh_n[2][3] = {};
-  uint8_t fl_c[2] = {0, 0}, fl_n[2] = {0, 0};
+  MomentsT<f2> mcur = {}, mnext = {};
+  f2 rho_c = mk2(1.f, 1.f), rho_n = mk2(1.f, 1.f), uh_c[3] = {}, uh_n[3] = {};
+  uint16_t fl_c = 0, fl_n = 0;  // flag bytes of the two cells
   char* dst = reinterpret_cast<char*>(a.fout) + 4 * (own_xy + nxy * z0);
   const int64_t zstride_b = 4 * nxy;
 
@@ -359,53 +363,54 @@ __global__ void __launch_bounds__(C::THREADS, 1)
       mbar_wait(full0 + 8 * s, k2 & 1);
       const uint16_t flw = bulk ? (uint16_t)(HHRR_BULK | (HHRR_BULK << 8))
                                 : *reinterpret_cast<const uint16_t*>(smem + (size_t)s * STAGE_BYTES + FLAG_OFF + FL_MAIN + own_fl);
-      float f[2][Q];
+      f2 f[Q];
 #pragma unroll
       for (int i = 0; i < Q; ++i) {  // population i of cell x sits at column x - cx (x-pull)
         const float* q = st + i * (TY * W) + own_off - dir_cx(i);
-        if (dir_cx(i) == 0) {
-          const float2 v = *reinterpret_cast<const float2*>(q);
-          f[0][i] = v.x;
-          f[1][i] = v.y;
-        } else {
-          f[0][i] = q[0];
-          f[1][i] = q[1];
-        }
+        if (dir_cx(i) == 0)
+          f[i].v = *reinterpret_cast<const float2*>(q);
+        else
+          f[i] = mk2(q[0], q[1]);
       }
       if (edge) {
         if (patch_l) {
 #pragma unroll
-          for (int k = 0; k < 9; ++k) f[0][3 * k + 2] = st[patch_off + (3 * k + 2) * (TY * 4)];  // cx = +1 from x = nx-1
+          for (int k = 0; k < 9; ++k) f[3 * k + 2].v.x = st[patch_off + (3 * k + 2) * (TY * 4)];  // cx = +1 from x = nx-1
         }
         if (patch_r) {
 #pragma unroll
-          for (int k = 0; k < 9; ++k) f[1][3 * k] = st[patch_off + (3 * k) * (TY * 4)];          // cx = -1 from x = 0
+          for (int k = 0; k < 9; ++k) f[3 * k].v.y = st[patch_off + (3 * k) * (TY * 4)];          // cx = -1 from x = 0
         }
       }
       __syncwarp();
       if ((tid & 31) == 0) mbar_arrive(empty0 + 8 * s);  // this warp has read its part of the stage
       const bool keep = p >= z0 && p < z1;
+      // porosity and solid velocity of the two cells (plain fluid: d = 1, u^B = 0)
+      f2 d = mk2(1.f, 1.f), uB[3] = {};
+      if (type_has_solid_state(flw & TYPE_MASK) || type_has_solid_state((flw >> 8) & TYPE_MASK)) {
+        float d0, d1, uB0[3], uB1[3];
+        solid_state_ws(a, (uint8_t)(flw & 0xff), c, xa, yv, zr, d0, uB0);
+        solid_state_ws(a, (uint8_t)(flw >> 8), c + 1, xa + 1, yv, zr, d1, uB1);
+        d = mk2(d0, d1);
 #pragma unroll
-      for (int k = 0; k < 2; ++k) {
-        const uint8_t fl = (uint8_t)(k ? (flw >> 8) : (flw & 0xff));
-        float d, uB[3], rho, uh[3];
-        solid_state_ws(a, fl, c + k, xa + k, yv, zr, d, uB);
-        if (keep) {
-          mnext[k] = moments_all(f[k]);
-          homogenised_velocity(a.ph, mnext[k].drho, mnext[k].jx, mnext[k].jy, mnext[k].jz, d, uB, rho, uh);
-          rho_n[k] = rho;
-          uh_n[k][0] = uh[0]; uh_n[k][1] = uh[1]; uh_n[k][2] = uh[2];
-          fl_n[k] = fl;
-        } else {
-          float drho, jx, jy, jz;
-          moments_rho_j(f[k], drho, jx, jy, jz);
-          homogenised_velocity(a.ph, drho, jx, jy, jz, d, uB, rho, uh);
-        }
-        if (!bulk) {
-          slot[0][own_slot + k] = uh[0];
-          slot[1][own_slot + k] = uh[1];
-          slot[2][own_slot + k] = fz ? -uh[2] : uh[2];
-        }
+        for (int q = 0; q < 3; ++q) uB[q] = mk2(uB0[q], uB1[q]);
+      }
+      f2 rho, uh[3];
+      if (keep) {
+        mnext = moments_all(f);
+        homogenised_velocity(a.ph, mnext.drho, mnext.jx, mnext.jy, mnext.jz, d, uB, rho, uh);
+        rho_n = rho;
+        uh_n[0] = uh[0]; uh_n[1] = uh[1]; uh_n[2] = uh[2];
+        fl_n = flw;
+      } else {
+        f2 drho, jx, jy, jz;
+        moments_rho_j(f, drho, jx, jy, jz);
+        homogenised_velocity(a.ph, drho, jx, jy, jz, d, uB, rho, uh);
+      }
+      if (!bulk) {
+        *reinterpret_cast<float2*>(&slot[0][own_slot]) = uh[0].v;
+        *reinterpret_cast<float2*>(&slot[1][own_slot]) = uh[1].v;
+        *reinterpret_cast<float2*>(&slot[2][own_slot]) = fz ? (-uh[2]).v : uh[2].v;
       }
     }
     pub_arrive(pub0, it);
@@ -418,47 +423,57 @@ __global__ void __launch_bounds__(C::THREADS, 1)
       float(*sm)[PLANE] = ring[(it - 2) & 3];
       float(*s0)[PLANE] = ring[(it - 1) & 3];
       float(*sp)[PLANE] = ring[it & 3];
-      float out[2][Q];
+      f2 S[6] = {}, sigma = mk2(cell_sigma(a.ph, (uint8_t)(fl_c & 0xff)), cell_sigma(a.ph, (uint8_t)(fl_c >> 8)));
+      if (!bulk) {
+        const int o = own_slot;
+        f2 dxu[3], dyu[3], dzu[3];  // central differences (times 2) of uhat component q along x, y, z
 #pragma unroll
-      for (int k = 0; k < 2; ++k) {
-        const int o = own_slot + k;
-        float S[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, sigma = cell_sigma(a.ph, fl_c[k]);
-        if (!bulk) {
-          float dxu0 = s0[0][o + 1] - s0[0][o - 1], dxu1 = s0[1][o + 1] - s0[1][o - 1], dxu2 = s0[2][o + 1] - s0[2][o - 1];
-          float dyu0 = s0[0][o + SX] - s0[0][o - SX], dyu1 = s0[1][o + SX] - s0[1][o - SX],
-                dyu2 = s0[2][o + SX] - s0[2][o - SX];
-          float dzu0 = sp[0][o] - sm[0][o], dzu1 = sp[1][o] - sm[1][o], dzu2 = sp[2][o] - sm[2][o];
-          S[0] = 0.5f * dxu0;
-          S[1] = 0.5f * dyu1;
-          S[2] = 0.5f * dzu2;
-          S[3] = 0.25f * (dyu0 + dxu1);
-          S[4] = 0.25f * (dzu0 + dxu2);
-          S[5] = 0.25f * (dzu1 + dyu2);
+        for (int q = 0; q < 3; ++q) {
+          // x: the pair's own values are in registers (a collided plane is never a reflected one)
+          dxu[q] = mk2(uh_c[q].v.y, s0[q][o + 2]) - mk2(s0[q][o - 1], uh_c[q].v.x);
+          dyu[q] = f2{*reinterpret_cast<const float2*>(&s0[q][o + SX])} - f2{*reinterpret_cast<const float2*>(&s0[q][o - SX])};
+          dzu[q] = f2{*reinterpret_cast<const float2*>(&sp[q][o])} - f2{*reinterpret_cast<const float2*>(&sm[q][o])};
         }
-        if (fl_c[k] & WM_VALID) {  // wall-model strain, sigma = 0 (rare)
-          const int64_t c = own_xy + k + nxy * z;
-#pragma unroll
-          for (int q = 0; q < 6; ++q) S[q] = __ldg(a.wm_s + (int64_t)q * n + c);
-          sigma = 0.f;
-        }
-        collide(a.ph, mcur[k], rho_c[k], uh_c[k], S, sigma, out[k]);
+        S[0] = 0.5f * dxu[0];
+        S[1] = 0.5f * dyu[1];
+        S[2] = 0.5f * dzu[2];
+        S[3] = 0.25f * (dyu[0] + dxu[1]);
+        S[4] = 0.25f * (dzu[0] + dxu[2]);
+        S[5] = 0.25f * (dzu[1] + dyu[2]);
       }
+      if (fl_c & (WM_VALID | (WM_VALID << 8))) {  // wall-model strain, sigma = 0 (rare)
+        const int64_t c = own_xy + nxy * z;
+        if (fl_c & WM_VALID) {
+#pragma unroll
+          for (int q = 0; q < 6; ++q) S[q].v.x = __ldg(a.wm_s + (int64_t)q * n + c);
+          sigma.v.x = 0.f;
+        }
+        if (fl_c & (WM_VALID << 8)) {
+#pragma unroll
+          for (int q = 0; q < 6; ++q) S[q].v.y = __ldg(a.wm_s + (int64_t)q * n + c + 1);
+          sigma.v.y = 0.f;
+        }
+      }
+      f2 out[Q];
+      collide(a.ph, mcur, rho_c, uh_c, S, sigma, out);
       if (row_interior && z > 0 && z < dm.nz - 1) {  // no wrap, no reflection: constant offsets, aligned pairs
 #pragma unroll
-        for (int i = 0; i < Q; ++i)
-          *reinterpret_cast<float2*>(dst + a.push_b[i]) = make_float2(out[0][i], out[1][i]);
+        for (int i = 0; i < Q; ++i) *reinterpret_cast<float2*>(dst + a.push_b[i]) = out[i].v;
       } else {
-        push_store_yz(dm, a.fout, xa, yv, z, out[0]);
-        push_store_yz(dm, a.fout, xa + 1, yv, z, out[1]);
+        float o0[Q], o1[Q];
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+          o0[i] = out[i].v.x;
+          o1[i] = out[i].v.y;
+        }
+        push_store_yz(dm, a.fout, xa, yv, z, o0);
+        push_store_yz(dm, a.fout, xa + 1, yv, z, o1);
       }
       dst += zstride_b;
     }
     if (p >= z0) {
-#pragma unroll
-      for (int k = 0; k < 2; ++k) {
-        mcur[k] = mnext[k]; rho_c[k] = rho_n[k]; fl_c[k] = fl_n[k];
-        uh_c[k][0] = uh_n[k][0]; uh_c[k][1] = uh_n[k][1]; uh_c[k][2] = uh_n[k][2];
-      }
+      mcur = mnext; rho_c = rho_n; fl_c = fl_n;
+      uh_c[0] = uh_n[0]; uh_c[1] = uh_n[1]; uh_c[2] = uh_n[2];
     }
   }
 }
@@ -514,7 +529,7 @@ static cudaError_t launch_shape(hhrr_lattice* L, WsArgs& a) {
   if (!make_map(&m_main, L->fA, dm, C::W, C::TY) || !make_map(&m_row, L->fA, dm, C::W, 1) ||
       !make_map(&m_pm, L->fA, dm, 4, C::TY) || !make_map(&m_pr, L->fA, dm, 4, 1))
     return cudaErrorNotSupported;
-  static bool attr_set = false;
+  bool& attr_set = L->attr_xpull[C::TX == 128 ? 1 : 0];  // the attribute is per device: kept per lattice
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(fused_xpull_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
     if (e != cudaSuccess) return e;
@@ -524,14 +539,11 @@ static cudaError_t launch_shape(hhrr_lattice* L, WsArgs& a) {
   int nch = ws_zchunks(dm.nz, a.fsi.n > 0 ? 16 : 22);
   a.zchunk = (dm.nz + nch - 1) / nch;
   nch = (dm.nz + a.zchunk - 1) / a.zchunk;
-  static int sms = 0;
-  if (!sms) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) sms = 148;
-  }
+  if (!L->sm_count &&
+      (cudaDeviceGetAttribute(&L->sm_count, cudaDevAttrMultiProcessorCount, L->device) != cudaSuccess || L->sm_count < 1))
+    L->sm_count = 148;
   a.nch = nch;
-  a.group = sms;  // one tile per SM and wave (one block per SM: shared memory)
+  a.group = L->sm_count;  // one tile per SM and wave (one block per SM: shared memory)
   const int ntiles = (dm.nx / C::TX) * (dm.ny / C::TY);
   dim3 grid((unsigned)(ntiles * nch));
   fused_xpull_kernel<C><<<grid, C::THREADS, C::SMEM, L->stream>>>(a, m_main, m_row, m_pm, m_pr);

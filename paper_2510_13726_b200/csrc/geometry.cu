@@ -10,6 +10,8 @@
 //
 // Integer results (types, tags, lists) are defined by the fp64 operation order below; this
 // file is compiled with -fmad=false so no contraction changes it.
+#include <utility>
+
 #include "lattice.h"
 
 namespace hhrr {
@@ -32,6 +34,8 @@ struct GeoArgs {
   uint8_t* below;   // phi < eps/2 per cell: what the growth-layer test reads (1 B instead of 8)
   uint8_t* rowflag; // per (y,z) row: some cell of the row may have phi < eps/2 (superset)
   uint8_t* tag_prov;  // provisional tag of pass 1 (its own array: pass 1 may run ahead of the step that reads flags)
+  const uint8_t* flags_prev;  // flag bytes the wall-model state bit is carried over from; NULL: written as 0 (look-ahead:
+                              // the wall-model kernel of the step in between sets it, wallmodel.cu)
   uint8_t* flags;
   float* d;
   int32_t* wall_idx;
@@ -206,7 +210,7 @@ __global__ void __launch_bounds__(128) geometry_type_kernel(GeoArgs a) {
     // a row with no cell below eps/2 in it or around it (most rows of the box: the blades cover a small part of the
     // disc) holds plain fluid / fringe cells only: phi >= eps/2, no tag, not in W -- nothing to read
     double phi = near_row ? a.phi[c] : BIG_PHI;
-    uint8_t fl = near_row ? a.flags[c] : (uint8_t)0;
+    uint8_t fl = (near_row && a.flags_prev) ? a.flags_prev[c] : (uint8_t)0;
     int tg = near_row ? a.tag_prov[c] : 0;
     int type;
     float d;
@@ -254,7 +258,8 @@ __global__ void __launch_bounds__(128) geometry_type_kernel(GeoArgs a) {
     }
     inf = (type == HHRR_SOLID || type == HHRR_FRONTIER) && tg > 0;
     uint8_t valid = inw ? (fl & WM_VALID) : 0;  // arrays of cells not in W_n are invalidated
-    a.flags[c] = (uint8_t)(type | (tg << TAG_SHIFT) | valid);
+    const int stored = (type == HHRR_FRONTIER && inw) ? T_FRONTIER_W : type;  // membership of W rides in the type bits
+    a.flags[c] = (uint8_t)(stored | (tg << TAG_SHIFT) | valid);
     a.d[c] = d;
   }
   // warp-aggregated appends keep the lists nearly in cell order
@@ -357,6 +362,7 @@ static void fill_geo(hhrr_lattice* L, GeoArgs& a, int64_t step) {
   a.below = L->below;
   a.rowflag = L->rowflag;
   a.tag_prov = L->tag_prov;
+  a.flags_prev = L->flags;
   a.flags = L->flags;
   a.d = L->d;
   a.wall_idx = L->wall_idx;
@@ -385,16 +391,63 @@ static void launch_box_phi(hhrr_lattice* L, int64_t step, cudaStream_t s) {
   L->launches++;
 }
 
-// Look-ahead: pass 1 of geometry(step + 1) depends on the step count only (rigid rotation), so it
-// is queued on a low-priority side stream as soon as pass 2 of geometry(step) has read phi, and runs in the tail
-// of the collide-stream kernel / beside the wall-model and force kernels instead of between two steps.
-cudaError_t launch_phi_ahead(hhrr_lattice* L) {
+void swap_geometry_sets(hhrr_lattice* L) {
+  std::swap(L->flags, L->alt_flags);
+  std::swap(L->d, L->alt_d);
+  std::swap(L->wall_idx, L->alt_wall_idx);
+  std::swap(L->wall_y1n, L->alt_wall_y1n);
+  std::swap(L->force_idx, L->alt_force_idx);
+  std::swap(L->counters, L->alt_counters);
+}
+
+// Look-ahead: geometry(step + 1) depends on the step count only (rigid rotation).  Both passes are
+// queued on the low-priority side stream while the collide-stream kernel of `step` runs, and write the
+// ALTERNATE geometry set (flags, porosity, lists, counters), which nothing of `step` reads; hhrr_step swaps the
+// sets when it reaches step + 1.  The one thing that depends on the step in between -- whether a cell of
+// W_{n+1} holds wall-model state -- is the WM_VALID bit, left 0 here and set by that step's wall-model kernel
+// (it knows the cell is in W_{n+1} from the type bits written here).
+// Ordering: ev_pre (main stream, recorded before the collide-stream launch) covers every earlier reader of the
+// alternate set and of phi / below / rowflag / tag_prov; the side stream itself orders the force kernel of the
+// previous step (which reads the alternate set's flags and force list) before this.
+cudaError_t launch_geometry_ahead(hhrr_lattice* L) {
   if (!L->side || !L->lookahead || rotor_box_empty(L) || L->geometry_dirty) return cudaSuccess;
-  cudaStreamWaitEvent(L->side, L->ev_type_done, 0);
+  cudaStreamWaitEvent(L->side, L->ev_pre, 0);
   launch_box_phi(L, L->step + 1, L->side);
-  cudaEventRecord(L->ev_phi_done, L->side);
-  L->phi_ahead_step = L->step + 1;
+  GeoArgs a;
+  fill_geo(L, a, L->step + 1);
+  a.flags_prev = nullptr;
+  a.flags = L->alt_flags;
+  a.d = L->alt_d;
+  a.wall_idx = L->alt_wall_idx;
+  a.wall_y1n = L->alt_wall_y1n;
+  a.force_idx = L->alt_force_idx;
+  a.cnt = L->alt_counters;
+  a.box = L->rot_box;
+  a.inside = 1;
+  dim3 g, b;
+  geo_grid(a, g, b);
+  counters_kernel<<<1, 1, 0, L->side>>>(a.cnt, 2);
+  geometry_type_kernel<<<g, b, 0, L->side>>>(a);
+  L->launches += 2;
+  cudaEventRecord(L->ev_k1, L->side);
+  L->ahead_step = L->step + 1;
+  L->side_busy = true;
   return cudaGetLastError();
+}
+
+// after a full pass: the alternate set starts as a copy of the current one (cells outside the rotor box and the
+// static prefix of the lists never change afterwards)
+__global__ void copy_static_lists_kernel(const Counters* cnt, Counters* alt_cnt, const int32_t* wall_idx,
+                                         const double* wall_y1n, const int32_t* force_idx, int32_t* alt_wall_idx,
+                                         double* alt_wall_y1n, int32_t* alt_force_idx, int cap) {
+  const int nw = min(cnt->wall_static, cap), nf = min(cnt->force_static, cap);
+  const int t = blockIdx.x * blockDim.x + threadIdx.x, T = gridDim.x * blockDim.x;
+  for (int e = t; e < nw; e += T) {
+    alt_wall_idx[e] = wall_idx[e];
+    for (int q = 0; q < 3; ++q) alt_wall_y1n[3 * (int64_t)e + q] = wall_y1n[3 * (int64_t)e + q];
+  }
+  for (int e = t; e < nf; e += T) alt_force_idx[e] = force_idx[e];
+  if (t == 0) *alt_cnt = *cnt;
 }
 
 cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
@@ -405,10 +458,10 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
   dim3 g, b;
   bool box_empty = rb.x1 <= rb.x0 || rb.y1 <= rb.y0 || rb.z1 <= rb.z0;
   const size_t rows = (size_t)L->dom.ny * L->dom.nz;
-  const bool ahead = L->phi_ahead_step >= 0;
-  if (ahead) cudaStreamWaitEvent(L->stream, L->ev_phi_done, 0);  // whatever the side stream wrote is complete
-  const bool have_phi = ahead && L->phi_ahead_step == L->step && !full;
-  L->phi_ahead_step = -1;
+  if (L->ahead_step >= 0) {  // a look-ahead result nobody will use: let the side stream finish writing first
+    cudaStreamWaitEvent(L->stream, L->ev_k1, 0);
+    L->ahead_step = -1;
+  }
   if (full) {
     // phi everywhere, then types: outside the rotor box first (static list prefix), box last
     a.box = none;
@@ -423,6 +476,13 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
     geometry_type_kernel<<<g, b, 0, L->stream>>>(a);
     counters_kernel<<<1, 1, 0, L->stream>>>(L->counters, 1);
     L->launches += 4;
+    // alternate set := current set outside the rotor box (the box part is rewritten by every look-ahead pass)
+    cudaMemcpyAsync(L->alt_flags, L->flags, (size_t)L->dom.n, cudaMemcpyDeviceToDevice, L->stream);
+    cudaMemcpyAsync(L->alt_d, L->d, sizeof(float) * (size_t)L->dom.n, cudaMemcpyDeviceToDevice, L->stream);
+    copy_static_lists_kernel<<<592, 256, 0, L->stream>>>(L->counters, L->alt_counters, L->wall_idx, L->wall_y1n,
+                                                         L->force_idx, L->alt_wall_idx, L->alt_wall_y1n,
+                                                         L->alt_force_idx, (int)L->cap_list);
+    L->launches++;
     if (!box_empty) {
       a.inside = 1;
       geo_grid(a, g, b);
@@ -430,7 +490,7 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
       L->launches++;
     }
   } else if (!box_empty) {
-    if (!have_phi) launch_box_phi(L, L->step, L->stream);
+    launch_box_phi(L, L->step, L->stream);
     a.box = rb;
     a.inside = 1;
     geo_grid(a, g, b);
@@ -438,7 +498,6 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
     geometry_type_kernel<<<g, b, 0, L->stream>>>(a);
     L->launches += 2;
   }
-  if (L->side) cudaEventRecord(L->ev_type_done, L->stream);  // phi of this step has been read
   return cudaGetLastError();
 }
 

@@ -18,6 +18,11 @@ constexpr uint8_t TYPE_MASK = 0x07;
 constexpr int TAG_SHIFT = 3;
 constexpr uint8_t TAG_MASK = 0x0f;
 constexpr uint8_t WM_VALID = 0x80;
+// Internal value of the type bits: a FRONTIER cell that belongs to the wall-model set W (reading R13).  The ABI
+// reports it as HHRR_FRONTIER; the flag byte of the NEXT step's geometry (written ahead of time) thereby tells
+// the wall-model kernel of THIS step which cells will consume the state it writes.
+constexpr int T_FRONTIER_W = 6;
+__host__ __device__ inline int public_type(int t) { return t == T_FRONTIER_W ? (int)HHRR_FRONTIER : t; }
 
 struct Dom {
   int nx, ny, nz;
@@ -75,17 +80,27 @@ struct hhrr_lattice {
   hhrr_params p;
   hhrr::Dom dom;
   cudaStream_t stream;
-  // look-ahead of geometry pass 1 (geometry.cu: launch_phi_ahead): low-priority side stream, two ordering events,
-  // the step whose phi the side stream has been asked for (-1: none)
+  // Side stream (low priority) and its ordering events.  Two things run there, beside the collide-stream
+  // kernel of the main stream: the WHOLE porosity update of the next step (geometry.cu: launch_geometry_ahead;
+  // a function of the step count only) into the alternate geometry set, and the force / torque
+  // collection of the step just streamed (wallmodel.cu: launch_forces), which only reads.
   cudaStream_t side;
-  cudaEvent_t ev_type_done, ev_phi_done;
-  int64_t phi_ahead_step;
-  bool lookahead;  // hhrr_set_lookahead
+  cudaEvent_t ev_pre, ev_k1, ev_k2, ev_side, ev_f[2];  // ev_f[n & 1]: force kernel of step n has read its populations
+  int64_t ahead_step;   // step whose geometry the alternate set holds (or is being written with); -1: none
+  bool side_busy;       // something was queued on the side stream since the main stream last waited for it
+  bool lookahead;       // hhrr_set_lookahead
   int device;
   // device arrays (inside the caller's workspace)
   float *fA, *fB;           // 27 planes each: post-stream populations minus weights
   uint8_t* flags;           // N
   float* d;                 // N porosity (read for FRONTIER cells only)
+  // alternate geometry set (flags, porosity, lists, counters): written ahead for the next step, then swapped in
+  uint8_t* alt_flags;
+  float* alt_d;
+  int32_t* alt_wall_idx;
+  double* alt_wall_y1n;
+  int32_t* alt_force_idx;
+  hhrr::Counters* alt_counters;
   double* phi;              // N signed distance of the last geometry
   uint8_t* below;           // N: phi < eps/2
   uint8_t* tag_prov;        // N: provisional tag of geometry pass 1
@@ -123,6 +138,8 @@ struct hhrr_lattice {
   int64_t step;
   int variant;       // requested kernel variant; dom.xs says how the populations are stored for it
   int64_t launches;
+  int sm_count;          // of L->device (0: not yet asked)
+  bool attr_xpull[2], attr_ws;  // dynamic shared-memory attribute set on L->device for the fused kernels
   // optional CUDA-event timing of the collide-stream kernel (hhrr_set_timing)
   bool timing;
   int ev_n;
@@ -137,11 +154,13 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full);
 cudaError_t launch_fill_rest(hhrr_lattice* L);
 cudaError_t launch_init(hhrr_lattice* L, const float* d_rho, const float* d_u, int with_neq);
 cudaError_t launch_collide_stream(hhrr_lattice* L);
-cudaError_t launch_phi_ahead(hhrr_lattice* L);
+cudaError_t launch_geometry_ahead(hhrr_lattice* L);     // geometry(step + 1) into the alternate set, side stream
+void swap_geometry_sets(hhrr_lattice* L);
 cudaError_t launch_moments(hhrr_lattice* L, float* d_rho, float* d_v);
 cudaError_t launch_check_finite(hhrr_lattice* L);
 bool xpull_supported(const Dom& dm);                    // fused_xpull.cu: variant 5 can run this lattice
 cudaError_t launch_restore(hhrr_lattice* L, int xs);    // re-store the populations of buffer A with x-shift xs
 // wallmodel.cu
-cudaError_t launch_wall_model_and_forces(hhrr_lattice* L);
+cudaError_t launch_wall_model(hhrr_lattice* L, bool mark_alt);  // K3 on the main stream
+cudaError_t launch_forces(hhrr_lattice* L, cudaStream_t s);     // K4 (reads only) on stream s
 }  // namespace hhrr

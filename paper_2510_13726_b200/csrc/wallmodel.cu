@@ -4,7 +4,10 @@
 //
 // Both kernels touch 1e4-1e5 cells, so they run in fp64 on the fp32 populations: the Newton
 // stop rule (:184) decides an iteration count, and it is taken in the same precision as the
-// oracle takes it.  Forces accumulate in fp64.  CUDA path only; shares nothing with oracle/.
+// oracle takes it.  Forces accumulate in fp64.  K3 is ONE launch on the critical path between two
+// collide-stream kernels (its output feeds the next collision); K4 only reads the streamed populations
+// and runs on the side stream beside the next collide-stream kernel.
+// CUDA path only; shares nothing with oracle/.
 #include "d3q27.cuh"
 
 namespace hhrr {
@@ -20,11 +23,11 @@ struct WmArgs {
   BodiesD bo;
   const float* f;  // post-stream populations (deviations)
   uint8_t* flags;
+  uint8_t* alt_flags;  // flag bytes of the NEXT step's geometry (written ahead), or NULL: cells of W there get WM_VALID too
   const int32_t* wall_idx;
   const double* wall_y1n;
   const Counters* cnt;
   int cap_list;
-  double* samp;  // [cap_list][6]: sampled velocity v_s and the cell's own velocity v(x_w), phase A -> phase B
   double* wm_utau;
   float* wm_u;
   float* wm_s;
@@ -77,89 +80,70 @@ __device__ __forceinline__ double spalding_df(double ut, double U, double y, dou
 __device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 __device__ __forceinline__ double shfl_down_d(double v, int delta) { return __shfl_down_sync(0xffffffffu, v, delta); }
 
-// K3 runs in two phases.  Phase A, one WARP per wall-model cell: lane 3k + g (k = 0..8, g = 0..2) loads
-// nine populations of cell k -- k = 0..7 the corners of the trilinear stencil around x_w + h_s n
-// (R15), k = 8 the wall cell itself -- so the 243 gathered loads of a cell are in flight at
-// once; the partial sums meet by shuffles and lane 0 stores v_s and v(x_w).  Phase B, one THREAD per
-// cell: tangential speed, Newton iteration on Eq. 18 (Eq. 19; fp64 exp, all 32 lanes busy), slip velocity
-// and wall strain.
-__device__ __forceinline__ void wall_sample_block(const WmArgs& a, int block, int nblocks) {
-  const int count = min(a.cnt->wall_count, a.cap_list);
+// K3, one launch.  A WARP takes a batch of WM_BATCH wall-model cells.  Sampling, cell by cell: lane 3k + g
+// (k = 0..8, g = 0..2) loads nine populations of cell k -- k = 0..7 the corners of the trilinear stencil around
+// x_w + h_s n (R15), k = 8 the wall cell itself -- so the 243 gathered loads of a cell are in
+// flight at once (and, the batch loop being unrolled, those of the next cells behind them); the partial sums
+// meet by shuffles and lane j keeps v_s and v(x_w) of cell j.  Then lanes 0..WM_BATCH-1 each finish one cell:
+// tangential speed, Newton iteration on Eq. 18 (Eq. 19; fp64 exp), slip velocity and wall strain.
+constexpr int WM_BATCH = 8;
+
+__device__ __forceinline__ void wall_sample_cell(const WmArgs& a, int64_t c, const double y1v[3], int lane,
+                                                 double vs[3], double vw[3]) {
   const int64_t nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
-  const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
   const int kc = lane / 3, g = lane - 3 * kc;  // cell of the stencil, population group (lanes 27-31 idle)
-  // the list entry of the NEXT cell is fetched while this one's populations are in flight: one memory latency per
-  // cell instead of two (the kernel is latency-bound: 3e4 cells, a few per warp)
-  int e = block * wpb + (threadIdx.x >> 5);
-  int64_t c_next = 0;
-  double y_next[3] = {0, 0, 0};
-  if (e < count) {
-    c_next = a.wall_idx[e];
-    for (int q = 0; q < 3; ++q) y_next[q] = a.wall_y1n[3 * (int64_t)e + q];
+  int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
+  double y1 = sqrt(y1v[0] * y1v[0] + y1v[1] * y1v[1] + y1v[2] * y1v[2]);
+  double nrm[3] = {y1v[0] / y1, y1v[1] / y1, y1v[2] / y1};
+  // velocity at x_w + h_s n, trilinear over the 8 surrounding cells (R15)
+  double px = x + a.hs * nrm[0], py = y + a.hs * nrm[1], pz = z + a.hs * nrm[2];
+  double fx = floor(px), fy = floor(py), fz = floor(pz);
+  double tx = px - fx, ty = py - fy, tz = pz - fz;
+  int ix = (int)fx, iy = (int)fy, iz = (int)fz;
+  // this lane's cell
+  int xx = x, yy = y, zz = z;
+  bool flx = false, fly = false, flz = false;
+  double w = 0.0;
+  if (kc < 8) {
+    int ox = kc & 1, oy = (kc >> 1) & 1, oz = (kc >> 2) & 1;
+    w = (ox ? tx : 1.0 - tx) * (oy ? ty : 1.0 - ty) * (oz ? tz : 1.0 - tz);
+    xx = wrap_far(ix + ox, a.dm.nx, a.dm.mode[0], flx);
+    yy = wrap_far(iy + oy, a.dm.ny, a.dm.mode[1], fly);
+    zz = wrap_far(iz + oz, a.dm.nz, a.dm.mode[2], flz);
   }
-  for (; e < count; e += nblocks * wpb) {
-    const int64_t c = c_next;
-    const double y1v[3] = {y_next[0], y_next[1], y_next[2]};
-    const int en = e + nblocks * wpb;
-    if (en < count) {
-      c_next = a.wall_idx[en];
-      for (int q = 0; q < 3; ++q) y_next[q] = a.wall_y1n[3 * (int64_t)en + q];
-    }
-    int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
-    double y1 = sqrt(y1v[0] * y1v[0] + y1v[1] * y1v[1] + y1v[2] * y1v[2]);
-    double nrm[3] = {y1v[0] / y1, y1v[1] / y1, y1v[2] / y1};
-    // velocity at x_w + h_s n, trilinear over the 8 surrounding cells (R15)
-    double px = x + a.hs * nrm[0], py = y + a.hs * nrm[1], pz = z + a.hs * nrm[2];
-    double fx = floor(px), fy = floor(py), fz = floor(pz);
-    double tx = px - fx, ty = py - fy, tz = pz - fz;
-    int ix = (int)fx, iy = (int)fy, iz = (int)fz;
-    // this lane's cell
-    int xx = x, yy = y, zz = z;
-    bool flx = false, fly = false, flz = false;
-    double w = 0.0;
-    if (kc < 8) {
-      int ox = kc & 1, oy = (kc >> 1) & 1, oz = (kc >> 2) & 1;
-      w = (ox ? tx : 1.0 - tx) * (oy ? ty : 1.0 - ty) * (oz ? tz : 1.0 - tz);
-      xx = wrap_far(ix + ox, a.dm.nx, a.dm.mode[0], flx);
-      yy = wrap_far(iy + oy, a.dm.ny, a.dm.mode[1], fly);
-      zz = wrap_far(iz + oz, a.dm.nz, a.dm.mode[2], flz);
-    }
-    double drho = 0, j0 = 0, j1 = 0, j2 = 0;
-    if (kc < 9) {
-      float fv[9];
+  double drho = 0, j0 = 0, j1 = 0, j2 = 0;
+  if (kc < 9) {
+    float fv[9];
 #pragma unroll
-      for (int q = 0; q < 9; ++q) fv[q] = __ldg(a.f + pop_index(a.dm, 9 * g + q, xx, yy, zz));
+    for (int q = 0; q < 9; ++q) fv[q] = __ldg(a.f + pop_index(a.dm, 9 * g + q, xx, yy, zz));
 #pragma unroll
-      for (int q = 0; q < 9; ++q) {  // population 9g + q: cx = q % 3 - 1, cy = q / 3 - 1, cz = g - 1
-        double fi = (double)fv[q];
-        drho += fi;
-        j0 += (q % 3 - 1) * fi;
-        j1 += (q / 3 - 1) * fi;
-      }
-      j2 = (g - 1) * drho;
+    for (int q = 0; q < 9; ++q) {  // population 9g + q: cx = q % 3 - 1, cy = q / 3 - 1, cz = g - 1
+      double fi = (double)fv[q];
+      drho += fi;
+      j0 += (q % 3 - 1) * fi;
+      j1 += (q / 3 - 1) * fi;
     }
-    // the three groups of a cell: lanes 3k, 3k+1, 3k+2
-    drho += shfl_down_d(drho, 1) + shfl_down_d(drho, 2);
-    j0 += shfl_down_d(j0, 1) + shfl_down_d(j0, 2);
-    j1 += shfl_down_d(j1, 1) + shfl_down_d(j1, 2);
-    j2 += shfl_down_d(j2, 1) + shfl_down_d(j2, 2);
-    double ir = 1.0 / (1.0 + drho);  // reported velocity moment v = (j + g/2)/rho (R11), valid on lanes 3k
-    double v[3] = {(j0 + 0.5 * a.g[0]) * ir, (j1 + 0.5 * a.g[1]) * ir, (j2 + 0.5 * a.g[2]) * ir};
-    if (flx) v[0] = -v[0];
-    if (fly) v[1] = -v[1];
-    if (flz) v[2] = -v[2];
-    double vs[3] = {0, 0, 0};
-#pragma unroll
-    for (int k = 0; k < 8; ++k) {
-      double wk = shfl_d(w, 3 * k);
-#pragma unroll
-      for (int q = 0; q < 3; ++q) vs[q] += wk * shfl_d(v[q], 3 * k);
-    }
-    if (lane == 0)
-      for (int q = 0; q < 3; ++q) a.samp[6 * (int64_t)e + q] = vs[q];
-    if (lane == 24)
-      for (int q = 0; q < 3; ++q) a.samp[6 * (int64_t)e + 3 + q] = v[q];
+    j2 = (g - 1) * drho;
   }
+  // the three groups of a cell: lanes 3k, 3k+1, 3k+2
+  drho += shfl_down_d(drho, 1) + shfl_down_d(drho, 2);
+  j0 += shfl_down_d(j0, 1) + shfl_down_d(j0, 2);
+  j1 += shfl_down_d(j1, 1) + shfl_down_d(j1, 2);
+  j2 += shfl_down_d(j2, 1) + shfl_down_d(j2, 2);
+  double ir = 1.0 / (1.0 + drho);  // reported velocity moment v = (j + g/2)/rho (R11), valid on lanes 3k
+  double v[3] = {(j0 + 0.5 * a.g[0]) * ir, (j1 + 0.5 * a.g[1]) * ir, (j2 + 0.5 * a.g[2]) * ir};
+  if (flx) v[0] = -v[0];
+  if (fly) v[1] = -v[1];
+  if (flz) v[2] = -v[2];
+  vs[0] = vs[1] = vs[2] = 0.0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    double wk = shfl_d(w, 3 * k);
+#pragma unroll
+    for (int q = 0; q < 3; ++q) vs[q] += wk * shfl_d(v[q], 3 * k);
+  }
+#pragma unroll
+  for (int q = 0; q < 3; ++q) vw[q] = shfl_d(v[q], 24);
 }
 
 // Musker's explicit profile and its slope (include/hhrr.h: hhrr_set_wall_function); residual U/u_tau - u+(y u_tau/nu)
@@ -207,20 +191,14 @@ __device__ __forceinline__ double wall_shear(int kind, double ut, double U, doub
   return ut * ut / nu * slope;
 }
 
-__global__ void __launch_bounds__(128) wall_model_kernel(const __grid_constant__ WmArgs a) {
-  const int count = min(a.cnt->wall_count, a.cap_list);
+// one wall-model cell: tangential speed relative to the wall, u_tau, slip velocity, wall strain, state valid
+__device__ __forceinline__ void wall_finish_cell(const WmArgs& a, int64_t c, const double y1v[3], const double vs[3],
+                                                 const double vw[3]) {
   const int64_t n = a.dm.n, nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
-  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < count; e += gridDim.x * blockDim.x) {
-    int64_t c = a.wall_idx[e];
+  {
     int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
-    double y1v[3] = {a.wall_y1n[3 * (int64_t)e], a.wall_y1n[3 * (int64_t)e + 1], a.wall_y1n[3 * (int64_t)e + 2]};
     double y1 = sqrt(y1v[0] * y1v[0] + y1v[1] * y1v[1] + y1v[2] * y1v[2]);
     double nrm[3] = {y1v[0] / y1, y1v[1] / y1, y1v[2] / y1};
-    double vs[3], vw[3];
-    for (int q = 0; q < 3; ++q) {
-      vs[q] = a.samp[6 * (int64_t)e + q];
-      vw[q] = a.samp[6 * (int64_t)e + 3 + q];
-    }
     double us[3];
     uint8_t fl = a.flags[c];
     body_velocity_d(a.bo, (fl >> TAG_SHIFT) & TAG_MASK, x, y, z, us);
@@ -279,6 +257,48 @@ __global__ void __launch_bounds__(128) wall_model_kernel(const __grid_constant__
     for (int q = 0; q < 3; ++q) a.wm_u[(int64_t)q * n + c] = (float)uw[q];
     for (int q = 0; q < 6; ++q) a.wm_s[(int64_t)q * n + c] = (float)sw[q];
     a.flags[c] = fl | WM_VALID;
+    // the next step's geometry is already written (look-ahead): its collision consumes this state iff the cell is
+    // in W there too (O1: the state of cells not in W_{n+1} is dropped)
+    if (a.alt_flags) {
+      const uint8_t fa = a.alt_flags[c];
+      if ((fa & TYPE_MASK) == T_FRONTIER_W) a.alt_flags[c] = fa | WM_VALID;
+    }
+  }
+}
+
+__global__ void __launch_bounds__(128, 4) wall_model_kernel(const __grid_constant__ WmArgs a) {
+  const int count = min(a.cnt->wall_count, a.cap_list);
+  const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+  const int nw = gridDim.x * wpb;
+  for (int base = (blockIdx.x * wpb + (threadIdx.x >> 5)) * WM_BATCH; base < count; base += nw * WM_BATCH) {
+    // lanes 0..WM_BATCH-1 hold the list entries of the batch
+    const int e_l = base + lane;
+    const bool mine = lane < WM_BATCH && e_l < count;
+    int c_l = 0;
+    double y_l[3] = {1.0, 0.0, 0.0};
+    if (mine) {
+      c_l = a.wall_idx[e_l];
+#pragma unroll
+      for (int q = 0; q < 3; ++q) y_l[q] = a.wall_y1n[3 * (int64_t)e_l + q];
+    }
+    double my_vs[3] = {0, 0, 0}, my_vw[3] = {0, 0, 0};
+#pragma unroll
+    for (int j = 0; j < WM_BATCH; ++j) {
+      if (base + j < count) {  // warp-uniform
+        const int64_t c = __shfl_sync(0xffffffffu, c_l, j);
+        const double y1v[3] = {shfl_d(y_l[0], j), shfl_d(y_l[1], j), shfl_d(y_l[2], j)};
+        double vs[3], vw[3];
+        wall_sample_cell(a, c, y1v, lane, vs, vw);
+        if (lane == j) {
+#pragma unroll
+          for (int q = 0; q < 3; ++q) {
+            my_vs[q] = vs[q];
+            my_vw[q] = vw[q];
+          }
+        }
+      }
+    }
+    if (mine) wall_finish_cell(a, c_l, y_l, my_vs, my_vw);
   }
 }
 
@@ -386,19 +406,8 @@ __device__ __forceinline__ void force_block(const ForceArgs& a, int block, int n
   }
 }
 
-// Phase A of K3 and K4 read the same post-stream populations and nothing of each other: one launch,
-// even blocks sample the wall-model velocities, odd blocks collect the forces.  Both are gathers whose
-// latency hides behind the other's.
-__global__ void __launch_bounds__(128, 8) sample_force_kernel(const __grid_constant__ WmArgs w,
-                                                           const __grid_constant__ ForceArgs f, int wm_on, int split) {
-  // of every four blocks, `split` sample wall-model velocities and 4 - split collect forces
-  const int quad = blockIdx.x >> 2, r = blockIdx.x & 3, nquad = gridDim.x >> 2;
-  if (!wm_on)
-    force_block(f, blockIdx.x, gridDim.x);
-  else if (r < split)
-    wall_sample_block(w, quad * split + r, nquad * split);
-  else
-    force_block(f, quad * (4 - split) + r - split, nquad * (4 - split));
+__global__ void __launch_bounds__(128, 8) force_kernel(const __grid_constant__ ForceArgs f) {
+  force_block(f, blockIdx.x, gridDim.x);
 }
 
 // ---------------------------------------------------------------------------- launchers
@@ -419,20 +428,30 @@ static void fill_wm(const hhrr_lattice* L, WmArgs& a) {
   fill_bodies(L, a.bo);
   a.f = L->fA;
   a.flags = L->flags;
+  a.alt_flags = nullptr;
   a.wall_idx = L->wall_idx;
   a.wall_y1n = L->wall_y1n;
   a.cnt = L->counters;
   a.cap_list = (int)L->cap_list;
-  a.samp = L->wall_samp;
   a.wm_utau = L->wm_utau;
   a.wm_u = L->wm_u;
   a.wm_s = L->wm_s;
 }
 
-// Listing 3 lines 4-6: WallModelO, then force collection and integration
-cudaError_t launch_wall_model_and_forces(hhrr_lattice* L) {
+// Listing 3 line 4: WallModelO.  mark_alt: the alternate geometry set holds geometry(step + 1)
+cudaError_t launch_wall_model(hhrr_lattice* L, bool mark_alt) {
+  if (!L->wm_enabled) return cudaSuccess;
   WmArgs w;
   fill_wm(L, w);
+  w.alt_flags = mark_alt ? L->alt_flags : nullptr;
+  wall_model_kernel<<<1184, 128, 0, L->stream>>>(w);  // 4736 warps x 8 cells per sweep
+  L->launches++;
+  return cudaGetLastError();
+}
+
+// Listing 3 lines 5-6: force collection and per-element integration into the ring slot of
+// this step.  Reads the streamed populations, the flag bytes (tags) and the force list of the current geometry.
+cudaError_t launch_forces(hhrr_lattice* L, cudaStream_t s) {
   ForceArgs a;
   a.dm = L->dom;
   fill_bodies(L, a.bo);
@@ -443,15 +462,9 @@ cudaError_t launch_wall_model_and_forces(hhrr_lattice* L) {
   a.cap_list = (int)L->cap_list;
   a.out = L->force + (L->step % FORCE_HISTORY) * MAX_TAGS * 3;
   a.out_m = L->torque + (L->step % FORCE_HISTORY) * MAX_TAGS * 3;
-  zero_force_kernel<<<1, 64, 0, L->stream>>>(a.out, a.out_m);
-  // 8 blocks per SM (64 registers): 4736 = 4 waves; two of every four blocks sample, two collect forces (measured:
-  // 1:3 and 3:1 are both slower)
-  sample_force_kernel<<<L->wm_enabled ? 4736 : 2368, 128, 0, L->stream>>>(w, a, L->wm_enabled ? 1 : 0, 2);
+  zero_force_kernel<<<1, 64, 0, s>>>(a.out, a.out_m);
+  force_kernel<<<2368, 128, 0, s>>>(a);  // 8 blocks per SM (64 registers), 2 waves
   L->launches += 2;
-  if (L->wm_enabled) {
-    wall_model_kernel<<<592, 128, 0, L->stream>>>(w);
-    L->launches++;
-  }
   return cudaGetLastError();
 }
 

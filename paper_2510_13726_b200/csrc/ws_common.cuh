@@ -43,7 +43,7 @@ __device__ __forceinline__ void solid_state_ws(const WsArgs& a, uint8_t fl, int6
   d = 1.f;
   uB[0] = uB[1] = uB[2] = 0.f;
   if (type_has_solid_state(type)) {
-    d = (type == HHRR_FRONTIER) ? __ldg(a.d + c) : 0.f;
+    d = type_is_frontier(type) ? __ldg(a.d + c) : 0.f;
     solid_velocity(a.ph, a.bo, fl, x, y, z, uB);
     if (fl & WM_VALID) {
       uB[0] += __ldg(a.wm_u + c);

@@ -249,7 +249,10 @@ def test_region_split_violation_is_reported():
     case = I.case_sphere(128, 32, 32, 5.0, 2)
     G = _gpu_lattice(case, 5)
     G.set_fsi_region([(0, 5, 0, 32, 0, 32)])          # the sphere is not covered
-    G.step(1)
+    with pytest.raises(B.HhrrError) as err:           # the geometry pass that follows the setter sees it: no collision runs
+        G.step(1)
+    assert err.value.code == -5 and "FSI region" in str(err.value)
+    assert G.step_count() == 0
     with pytest.raises(B.HhrrError):
         G.check_finite()
     G.set_fsi_region(I.with_region_split(case).fsi_boxes)
@@ -551,6 +554,61 @@ def test_force_across_mirror_planes(oracle):
         case = I.Case("mirror-force", nx, ny, nz, 10, mode=mode, params=dict(I.DEFAULTS, tau0=0.56), rho=rho, u=u,
                       with_neq=True, phi=phi.astype(np.float32), tag=tag, wall_model=True)
         run_parity(oracle, case, 10, variant, TOL10, check_every=5)
+
+
+def test_checkpoint_resume_is_bitwise_with_wall_model_and_rotor(oracle):
+    """Round-1 ADVICE: a resume must restore the wall-model state (u_tau warm start of Eq. 20, slip, strain, valid
+    bits) and the step count (rotor angle) beside the populations.  Rotor recipe and channel recipe:
+    save after 6 steps, restore into a fresh lattice, 5 more steps on both -- populations, u_tau and forces bitwise."""
+    for case in (I.case_rotor(128, 72, 72, 20.0, 11, omega=0.012), I.case_channel(128, 48, 16, 11)):
+        A = _gpu_lattice(case, 5)
+        A.step(6)
+        f = A.populations()
+        state = A.wall_model_state()
+        assert len(state[0]) > 0 and state[4].any()
+        Bv = _gpu_lattice(case, 5)
+        Bv.set_step_count(6)
+        Bv.set_populations(f)
+        Bv.set_wall_model_state(*state)
+        A.step(5); Bv.step(5)
+        assert A.step_count() == Bv.step_count() == 11
+        assert np.array_equal(A.populations(), Bv.populations())
+        wa, wb = A.wall_list(), Bv.wall_list()
+        assert all(np.array_equal(p, q) for p, q in zip(wa, wb))
+        Fa, Fb = A.forces(6, 5), Bv.forces(6, 5)
+        assert np.allclose(Fa, Fb, rtol=1e-12, atol=1e-18)
+        # without the wall-model state the resumed run differs (what the old checkpoint did)
+        Cv = _gpu_lattice(case, 5)
+        Cv.set_step_count(6); Cv.set_populations(f); Cv.step(5)
+        assert not np.array_equal(A.populations(), Cv.populations())
+        A.close(); Bv.close(); Cv.close()
+
+
+def test_moments_device_and_uhat_entry_points(oracle):
+    """hhrr_get_moments_device = hhrr_get_moments without the host copy; hhrr_get_uhat (two-pass variant only) =
+    the oracle's time-n homogenised field of the last collide."""
+    import torch
+    from paper_2510_13726_b200 import binding as B
+    case = I.case_sphere(64, 32, 32, 5.0, 4)
+    G, Oa = _gpu_lattice(case, 0), _ora_lattice(oracle, case)
+    G.step(4); Oa.step(4)
+    rho, v = G.moments()
+    rho_t = torch.empty(case.n, dtype=torch.float32, device="cuda")
+    v_t = torch.empty((3, case.n), dtype=torch.float32, device="cuda")
+    G.moments_device(rho_t, v_t)
+    G.synchronize()
+    assert np.array_equal(rho_t.cpu().numpy(), rho) and np.array_equal(v_t.cpu().numpy(), v)
+    ug, uo = G.uhat().astype(np.float64), Oa.uhat()
+    assert np.max(np.abs(ug - uo)) <= TOL10 * np.max(np.abs(uo))
+    G.set_kernel_variant(5)
+    with pytest.raises(B.HhrrError):
+        G.uhat()
+    assert _gpu_lattice(case, 5).set_kernel_variant(5) == B.W_FALLBACK        # 64 wide: variant 2 runs, and says so
+    assert _gpu_lattice(I.case_sphere(128, 32, 32, 5.0, 1), 2).set_kernel_variant(5) == 0
+    cells = np.arange(case.n, dtype=np.int64)                                   # more cells than one scratch pass holds
+    pops, fl = G.cell_populations(cells)
+    assert np.array_equal(pops.T, G.populations())
+    G.close(); Oa.close()
 
 
 def test_zz_report_utau_error():

@@ -25,14 +25,22 @@
  *
  * Conventions: cell (x,y,z), linear index
  * x + nx*(y + ny*z); direction i = (cx+1) + 3(cy+1) + 9(cz+1); rest i=13;
- * opposite 26-i; w(0)=2/3, w(+-1)=1/6; cs^2 = 1/3; dx = dt = 1.
+ * opposite 26-i; w(0)=2/3, w(+-1)=1/6; cs^2 = 1/3; dx = dt = 1.  (D3Q19: the 19 of these
+ * directions with |c|^2 <= 2 renumbered in the same order, rest 9, opposite 18-i, weights
+ * 1/3, 1/18, 1/36.)
  */
 #include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
 
-#define Q 27
+/* Velocity set: D3Q27 (BASELINE.json's configs; default) or D3Q19 (the paper's own lattice, Fig. 2
+ * :107) when compiled through oracle/hhrr_oracle_q19.c, which defines OHRR_Q 19 and includes this file.  The
+ * directions of D3Q19 are those of D3Q27 with |c|^2 <= 2, in the same order.                                 */
+#ifndef OHRR_Q
+#define OHRR_Q 27
+#endif
+#define Q OHRR_Q
 #define MAX_TAGS 16
 #define BIG_PHI 1.0e30
 
@@ -109,23 +117,40 @@ typedef struct ohrr_lattice {
 /* ---------------------------------------------------------------- lattice tables */
 static int CX[Q], CY[Q], CZ[Q];
 static double W[Q];
+static int DIR_OF[27]; /* index of direction (cx,cy,cz) at slot (cx+1) + 3(cy+1) + 9(cz+1); -1: not in the set */
+static int REST;       /* index of the rest direction */
 static int tables_ready = 0;
 static const double CS2 = 1.0 / 3.0;
 
 static void init_tables(void) {
   if (tables_ready) return;
-  for (int i = 0; i < Q; ++i) {
-    CX[i] = i % 3 - 1;
-    CY[i] = (i / 3) % 3 - 1;
-    CZ[i] = i / 9 - 1;
-    double w = 1.0;
-    w *= (CX[i] == 0) ? 2.0 / 3.0 : 1.0 / 6.0;
-    w *= (CY[i] == 0) ? 2.0 / 3.0 : 1.0 / 6.0;
-    w *= (CZ[i] == 0) ? 2.0 / 3.0 : 1.0 / 6.0;
-    W[i] = w;
+  int i = 0;
+  for (int k = 0; k < 27; ++k) {
+    int cx = k % 3 - 1, cy = (k / 3) % 3 - 1, cz = k / 9 - 1;
+    int nn = abs(cx) + abs(cy) + abs(cz);
+    DIR_OF[k] = -1;
+    if (Q == 19 && nn == 3) continue; /* D3Q19 has no corner directions (Fig. 2) */
+    CX[i] = cx;
+    CY[i] = cy;
+    CZ[i] = cz;
+    if (Q == 27) {
+      double w = 1.0;
+      w *= (cx == 0) ? 2.0 / 3.0 : 1.0 / 6.0;
+      w *= (cy == 0) ? 2.0 / 3.0 : 1.0 / 6.0;
+      w *= (cz == 0) ? 2.0 / 3.0 : 1.0 / 6.0;
+      W[i] = w;
+    } else {
+      W[i] = nn == 0 ? 1.0 / 3.0 : (nn == 1 ? 1.0 / 18.0 : 1.0 / 36.0);
+    }
+    if (nn == 0) REST = i;
+    DIR_OF[k] = i;
+    ++i;
   }
   tables_ready = 1;
 }
+static inline int dir_of(int cx, int cy, int cz) { return DIR_OF[(cx + 1) + 3 * (cy + 1) + 9 * (cz + 1)]; }
+static inline int opposite(int i) { return dir_of(-CX[i], -CY[i], -CZ[i]); }
+int32_t ohrr_q(void) { return Q; }
 
 static inline void cvec(int i, double c[3]) {
   c[0] = CX[i];
@@ -137,6 +162,33 @@ static inline double delta(int a, int b) { return a == b ? 1.0 : 0.0; }
 static inline double H2(const double c[3], int a, int b) { return c[a] * c[b] - (1.0 / 3.0) * delta(a, b); }
 static inline double H3(const double c[3], int a, int b, int g) {
   return c[a] * c[b] * c[g] - (1.0 / 3.0) * (c[a] * delta(b, g) + c[b] * delta(a, g) + c[g] * delta(a, b));
+}
+
+/* Third-order part of the Hermite expansion, sum over the supported third-order polynomials of
+ * H^(3)_i : a^(3) with the normalisation of Eq. 8.
+ * D3Q27: every H^(3)_abg is supported (H_aaa = 0 identically): the full contraction / (3! c_s^6)  (reading R3).
+ * D3Q19: the six H_aab are no longer independent; the supported third-order basis is the one of the paper's
+ * ref. [43] (Jacob, Malaspinas, Sagaut 2018; named at PAPER.md:94): the sums H_xxy + H_yzz, H_xzz + H_xyy,
+ * H_yyz + H_xxz (squared norm 2 c_s^6 -- the "2 c_s^6" printed in Eq. 11) and the differences
+ * H_xxy - H_yzz, H_xzz - H_xyy, H_yyz - H_xxz (squared norm 6 c_s^6); H_xyz is not supported  (reading R23). */
+static double third_order(const double c[3], double a3[3][3][3]) {
+  const double cs6 = CS2 * CS2 * CS2;
+  if (Q == 27) {
+    double t3 = 0.0;
+    for (int a = 0; a < 3; ++a)
+      for (int b = 0; b < 3; ++b)
+        for (int g = 0; g < 3; ++g) t3 += H3(c, a, b, g) * a3[a][b][g];
+    return t3 / (6.0 * cs6);
+  }
+  static const int G1[3][3] = {{0, 0, 1}, {0, 2, 2}, {1, 1, 2}}; /* xxy, xzz, yyz */
+  static const int G2[3][3] = {{1, 2, 2}, {0, 1, 1}, {0, 0, 2}}; /* yzz, xyy, xxz */
+  double t3 = 0.0;
+  for (int k = 0; k < 3; ++k) {
+    double h1 = H3(c, G1[k][0], G1[k][1], G1[k][2]), h2 = H3(c, G2[k][0], G2[k][1], G2[k][2]);
+    double a1 = a3[G1[k][0]][G1[k][1]][G1[k][2]], a2 = a3[G2[k][0]][G2[k][1]][G2[k][2]];
+    t3 += (h1 + h2) * (a1 + a2) / (2.0 * cs6) + (h1 - h2) * (a1 - a2) / (6.0 * cs6);
+  }
+  return t3;
 }
 
 /* exported for the pins */
@@ -160,14 +212,15 @@ void ohrr_equilibrium(double rho, const double u[3], double feq[Q]) {
   for (int i = 0; i < Q; ++i) {
     double c[3];
     cvec(i, c);
-    double t1 = 0.0, t2 = 0.0, t3 = 0.0;
+    double t1 = 0.0, t2 = 0.0;
     for (int a = 0; a < 3; ++a) t1 += c[a] * rho * u[a];
     for (int a = 0; a < 3; ++a)
       for (int b = 0; b < 3; ++b) t2 += H2(c, a, b) * rho * u[a] * u[b];
+    double a3[3][3][3]; /* a0^(3) = a0^(2) u = rho u u u */
     for (int a = 0; a < 3; ++a)
       for (int b = 0; b < 3; ++b)
-        for (int g = 0; g < 3; ++g) t3 += H3(c, a, b, g) * rho * u[a] * u[b] * u[g];
-    feq[i] = W[i] * (rho + t1 / CS2 + t2 / (2.0 * CS2 * CS2) + t3 / (6.0 * CS2 * CS2 * CS2));
+        for (int g = 0; g < 3; ++g) a3[a][b][g] = rho * u[a] * u[b] * u[g];
+    feq[i] = W[i] * (rho + t1 / CS2 + t2 / (2.0 * CS2 * CS2) + third_order(c, a3));
   }
 }
 
@@ -182,13 +235,10 @@ static void regularised_f1(const double a2[3][3], const double u[3], double f1[Q
   for (int i = 0; i < Q; ++i) {
     double c[3];
     cvec(i, c);
-    double t2 = 0.0, t3 = 0.0;
+    double t2 = 0.0;
     for (int a = 0; a < 3; ++a)
       for (int b = 0; b < 3; ++b) t2 += H2(c, a, b) * a2[a][b];
-    for (int a = 0; a < 3; ++a)
-      for (int b = 0; b < 3; ++b)
-        for (int g = 0; g < 3; ++g) t3 += H3(c, a, b, g) * a3[a][b][g];
-    f1[i] = W[i] * (t2 / (2.0 * CS2 * CS2) + t3 / (6.0 * CS2 * CS2 * CS2));
+    f1[i] = W[i] * (t2 / (2.0 * CS2 * CS2) + third_order(c, a3));
   }
 }
 
@@ -675,7 +725,7 @@ static void collide_and_stream(ohrr_lattice *L) {
             if (L->p.mode[2] == AX_PERIODIC) tz = (tz + nz) % nz;
             else { tz = z; ci[2] = -ci[2]; }
           }
-          int io = (ci[0] + 1) + 3 * (ci[1] + 1) + 9 * (ci[2] + 1);
+          int io = dir_of(ci[0], ci[1], ci[2]);
           L->f2[(int64_t)io * n + lidx(L, tx, ty, tz)] = fout[i];
         }
       }
@@ -822,7 +872,7 @@ static void forces(ohrr_lattice *L) {
         body_velocity(L, k, x, y, z, us);
         double acc[3] = {0, 0, 0};
         for (int i = 0; i < Q; ++i) {
-          if (i == 13) continue;
+          if (i == REST) continue;
           /* R12: the cell behind a MIRROR plane is the reflected image of the lattice, so f_i there is the
            * population of the reflected cell whose normal velocity component is reversed (the same rule the
            * streaming step O3 applies to a population leaving through the plane)                          */
@@ -830,9 +880,9 @@ static void forces(ohrr_lattice *L) {
           int xx = wrap1(x + CX[i], nx, L->p.mode[0], &flx);
           int yy = wrap1(y + CY[i], ny, L->p.mode[1], &fly);
           int zz = wrap1(z + CZ[i], nz, L->p.mode[2], &flz);
-          int ir = ((flx ? -CX[i] : CX[i]) + 1) + 3 * ((fly ? -CY[i] : CY[i]) + 1) + 9 * ((flz ? -CZ[i] : CZ[i]) + 1);
+          int ir = dir_of(flx ? -CX[i] : CX[i], fly ? -CY[i] : CY[i], flz ? -CZ[i] : CZ[i]);
           double fa = L->f[(int64_t)ir * n + lidx(L, xx, yy, zz)];
-          double fb = L->f[(int64_t)(26 - i) * n + c];
+          double fb = L->f[(int64_t)opposite(i) * n + c];
           double ci[3] = {CX[i], CY[i], CZ[i]};
           for (int a = 0; a < 3; ++a) acc[a] += (ci[a] - us[a]) * fa + (ci[a] + us[a]) * fb;
         }

@@ -17,6 +17,9 @@ import numpy as np
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "hhrr_oracle.c"
 _LIB = _HERE / "libhhrr_oracle.so"
+# the same oracle on the paper's own velocity set: a second translation unit, a second library
+_SRC19 = _HERE / "hhrr_oracle_q19.c"
+_LIB19 = _HERE / "libhhrr_oracle_q19.so"
 
 Q = 27
 MAX_TAGS = 16
@@ -27,10 +30,12 @@ PERIODIC, MIRROR = 0, 1
 def build(force: bool = False) -> Path:
     """Compile the oracle with gcc.  -ffp-contract=off: the geometry classification
     is defined by its operation order (bit-exact cell types)."""
-    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
-        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-ffp-contract=off", "-fno-fast-math",
-               "-shared", "-fPIC", "-o", str(_LIB), str(_SRC), "-lm"]
-        subprocess.run(cmd, check=True)
+    for src, out in ((_SRC, _LIB), (_SRC19, _LIB19)):
+        newest = max(_SRC.stat().st_mtime, src.stat().st_mtime)
+        if force or not out.exists() or out.stat().st_mtime < newest:
+            cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-ffp-contract=off", "-fno-fast-math",
+                   "-shared", "-fPIC", "-o", str(out), str(src), "-lm"]
+            subprocess.run(cmd, check=True)
     return _LIB
 
 
@@ -53,15 +58,15 @@ class RotorDesc(C.Structure):
                 ("omega", C.c_double), ("theta0", C.c_double), ("n_tags", C.c_int32)]
 
 
-_lib = None
+_libs = {}
 
 
-def lib():
-    global _lib
-    if _lib is None:
+def lib(q=27):
+    if q not in _libs:
         build()
-        _lib = C.CDLL(str(_LIB))
-        L = _lib
+        _libs[q] = C.CDLL(str({27: _LIB, 19: _LIB19}[q]))
+        L = _libs[q]
+        assert L.ohrr_q() == q
         L.ohrr_create.restype = C.c_void_p
         L.ohrr_create.argtypes = [C.POINTER(Params)]
         L.ohrr_destroy.argtypes = [C.c_void_p]
@@ -86,7 +91,7 @@ def lib():
         L.ohrr_get_wall_list.restype = C.c_int64
         L.ohrr_step_count.restype = C.c_int64
         L.ohrr_step_count.argtypes = [C.c_void_p]
-    return _lib
+    return _libs[q]
 
 
 def _p(a):
@@ -113,23 +118,23 @@ def make_params(nx, ny, nz, mode=(0, 0, 0), tau0=0.55, sigma=0.995, smagorinsky_
 
 
 # ---- free functions (cell-model pieces, used by the pins) ---------------------------------
-def lattice_tables():
-    cx = np.zeros(Q, np.int32); cy = np.zeros(Q, np.int32); cz = np.zeros(Q, np.int32)
-    w = np.zeros(Q, np.float64)
-    lib().ohrr_lattice_tables(_p(cx), _p(cy), _p(cz), _p(w))
+def lattice_tables(q=27):
+    cx = np.zeros(q, np.int32); cy = np.zeros(q, np.int32); cz = np.zeros(q, np.int32)
+    w = np.zeros(q, np.float64)
+    lib(q).ohrr_lattice_tables(_p(cx), _p(cy), _p(cz), _p(w))
     return cx, cy, cz, w
 
 
-def equilibrium(rho, u):
-    u = _f64(u); out = np.zeros(Q)
-    lib().ohrr_equilibrium(C.c_double(rho), _p(u), _p(out))
+def equilibrium(rho, u, q=27):
+    u = _f64(u); out = np.zeros(q)
+    lib(q).ohrr_equilibrium(C.c_double(rho), _p(u), _p(out))
     return out
 
 
-def collide_cell(fin, g, d, uB, S, sigma, tau0, cs):
+def collide_cell(fin, g, d, uB, S, sigma, tau0, cs, q=27):
     fin = _f64(fin); g = _f64(g); uB = _f64(uB); S = _f64(S)
-    out = np.zeros(Q); diag = np.zeros(5)
-    lib().ohrr_collide_cell(_p(fin), _p(g), C.c_double(d), _p(uB), _p(S), C.c_double(sigma),
+    out = np.zeros(q); diag = np.zeros(5)
+    lib(q).ohrr_collide_cell(_p(fin), _p(g), C.c_double(d), _p(uB), _p(S), C.c_double(sigma),
                             C.c_double(tau0), C.c_double(cs), _p(out), _p(diag))
     return out, diag
 
@@ -177,18 +182,20 @@ def newton_utau(u0, U, y, nu, kappa=0.41, E=9.8, max_iter=10, tol=1e-4):
 
 # ---- lattice object -------------------------------------------------------------------------
 class Lattice:
-    def __init__(self, params: Params):
+    def __init__(self, params: Params, q=27):
         self.p = params
+        self.q = q
+        self.lib = lib(q)
         self.nx, self.ny, self.nz = params.nx, params.ny, params.nz
         self.n = self.nx * self.ny * self.nz
-        self.h = lib().ohrr_create(C.byref(params))
+        self.h = self.lib.ohrr_create(C.byref(params))
         if not self.h:
             raise RuntimeError("ohrr_create failed")
         self._keep = []
 
     def close(self):
         if self.h:
-            lib().ohrr_destroy(C.c_void_p(self.h))
+            self.lib.ohrr_destroy(C.c_void_p(self.h))
             self.h = None
 
     def __del__(self):
@@ -201,21 +208,21 @@ class Lattice:
     def init_equilibrium(self, rho, u, with_neq=False):
         rho = _f64(rho).ravel(); u = _f64(u).reshape(3, -1)
         assert rho.size == self.n and u.shape[1] == self.n
-        lib().ohrr_init_equilibrium(self._h, _p(rho), _p(u), int(with_neq))
+        self.lib.ohrr_init_equilibrium(self._h, _p(rho), _p(u), int(with_neq))
 
     def set_static_geometry(self, phi, tag=None, d_override=None):
         phi = _f64(phi).ravel()
         tag = None if tag is None else np.ascontiguousarray(tag, np.uint8).ravel()
         dov = None if d_override is None else _f64(d_override).ravel()
-        lib().ohrr_set_static_geometry(self._h, _p(phi), _p(tag), _p(dov))
+        self.lib.ohrr_set_static_geometry(self._h, _p(phi), _p(tag), _p(dov))
 
     def set_body(self, tag, centre=(0, 0, 0), omega=(0, 0, 0), vel=(0, 0, 0)):
         c = _f64(centre); o = _f64(omega); v = _f64(vel)
-        lib().ohrr_set_body(self._h, int(tag), _p(c), _p(o), _p(v))
+        self.lib.ohrr_set_body(self._h, int(tag), _p(c), _p(o), _p(v))
 
     def set_fringe(self, x0, x1, u_in):
         u = _f64(u_in)
-        lib().ohrr_set_fringe(self._h, int(x0), int(x1), _p(u))
+        self.lib.ohrr_set_fringe(self._h, int(x0), int(x1), _p(u))
 
     def set_rotor(self, sdf, tag, spacing, origin, centre, axis, omega, theta0, n_tags):
         sdf = np.ascontiguousarray(sdf, np.float32); tag = np.ascontiguousarray(tag, np.uint8)
@@ -226,103 +233,121 @@ class Lattice:
         r.spacing = spacing
         r.origin[:] = list(origin); r.centre[:] = list(centre); r.axis[:] = list(axis)
         r.omega, r.theta0, r.n_tags = omega, theta0, n_tags
-        rc = lib().ohrr_set_rotor(self._h, C.byref(r))
+        rc = self.lib.ohrr_set_rotor(self._h, C.byref(r))
         if rc:
             raise RuntimeError("ohrr_set_rotor failed")
 
     def enable_wall_model(self, enable=True):
-        lib().ohrr_enable_wall_model(self._h, int(enable))
+        self.lib.ohrr_enable_wall_model(self._h, int(enable))
 
     def set_fsi_region(self, boxes):
         """boxes: iterable of (x0, x1, y0, y1, z0, z1), half-open; empty = HHRRLBM everywhere."""
         b = np.ascontiguousarray(np.asarray(list(boxes), np.int32).reshape(-1, 6))
-        rc = lib().ohrr_set_fsi_region(self._h, int(b.shape[0]), _p(b) if b.size else None)
+        rc = self.lib.ohrr_set_fsi_region(self._h, int(b.shape[0]), _p(b) if b.size else None)
         if rc:
             raise RuntimeError("ohrr_set_fsi_region failed")
 
     def set_wall_model_variant(self, slip=0, shear=0):
-        if lib().ohrr_set_wall_model_variant(self._h, int(slip), int(shear)):
+        if self.lib.ohrr_set_wall_model_variant(self._h, int(slip), int(shear)):
             raise RuntimeError("ohrr_set_wall_model_variant failed")
 
     def set_wall_function(self, kind):
-        if lib().ohrr_set_wall_function(self._h, int(kind)):
+        if self.lib.ohrr_set_wall_function(self._h, int(kind)):
             raise RuntimeError("ohrr_set_wall_function failed")
 
     def region_violation(self):
-        return bool(lib().ohrr_region_violation(self._h))
+        return bool(self.lib.ohrr_region_violation(self._h))
 
     def update_geometry(self):
-        lib().ohrr_update_geometry(self._h)
+        self.lib.ohrr_update_geometry(self._h)
 
     def wall_model_only(self):
-        lib().ohrr_wall_model_only(self._h)
+        self.lib.ohrr_wall_model_only(self._h)
 
     def force_only(self):
         F = np.zeros((MAX_TAGS, 3))
-        lib().ohrr_force_only(self._h, _p(F))
+        self.lib.ohrr_force_only(self._h, _p(F))
         return F
 
     def torque_only(self):
         M = np.zeros((MAX_TAGS, 3))
-        lib().ohrr_torque_only(self._h, _p(M))
+        self.lib.ohrr_torque_only(self._h, _p(M))
         return M
 
     def step(self, n=1):
-        lib().ohrr_step(self._h, int(n))
+        self.lib.ohrr_step(self._h, int(n))
 
     def moments(self):
         rho = np.zeros(self.n); v = np.zeros((3, self.n))
-        lib().ohrr_get_moments(self._h, _p(rho), _p(v))
+        self.lib.ohrr_get_moments(self._h, _p(rho), _p(v))
         return rho, v
 
     def forces(self, first=0, count=None):
         if count is None:
-            count = lib().ohrr_step_count(self._h) - first
+            count = self.lib.ohrr_step_count(self._h) - first
         F = np.zeros((count, MAX_TAGS, 3))
-        rc = lib().ohrr_get_forces(self._h, C.c_int64(first), C.c_int64(count), _p(F))
+        rc = self.lib.ohrr_get_forces(self._h, C.c_int64(first), C.c_int64(count), _p(F))
         if rc:
             raise RuntimeError("ohrr_get_forces: range")
         return F
 
     def torques(self, first=0, count=None):
         if count is None:
-            count = lib().ohrr_step_count(self._h) - first
+            count = self.lib.ohrr_step_count(self._h) - first
         M = np.zeros((count, MAX_TAGS, 3))
-        rc = lib().ohrr_get_torques(self._h, C.c_int64(first), C.c_int64(count), _p(M))
+        rc = self.lib.ohrr_get_torques(self._h, C.c_int64(first), C.c_int64(count), _p(M))
         if rc:
             raise RuntimeError("ohrr_get_torques: range")
         return M
 
     def cell_types(self):
         t = np.zeros(self.n, np.uint8); g = np.zeros(self.n, np.uint8); d = np.zeros(self.n)
-        lib().ohrr_get_cell_types(self._h, _p(t), _p(g), _p(d))
+        self.lib.ohrr_get_cell_types(self._h, _p(t), _p(g), _p(d))
         return t, g, d
 
     def wall_list(self):
-        k = lib().ohrr_get_wall_list(self._h, None, None, None, None, C.c_int64(0))
+        k = self.lib.ohrr_get_wall_list(self._h, None, None, None, None, C.c_int64(0))
         idx = np.zeros(k, np.int32); y1n = np.zeros((k, 3)); ut = np.zeros(k); va = np.zeros(k, np.uint8)
         if k:
-            lib().ohrr_get_wall_list(self._h, _p(idx), _p(y1n), _p(ut), _p(va), C.c_int64(k))
+            self.lib.ohrr_get_wall_list(self._h, _p(idx), _p(y1n), _p(ut), _p(va), C.c_int64(k))
         return idx, y1n, ut, va
 
     def wall_state(self, cell):
         ut = C.c_double(0); u = np.zeros(3); s = np.zeros(6)
-        valid = lib().ohrr_get_wall_state(self._h, C.c_int64(cell), C.byref(ut), _p(u), _p(s))
+        valid = self.lib.ohrr_get_wall_state(self._h, C.c_int64(cell), C.byref(ut), _p(u), _p(s))
         return valid, ut.value, u, s
 
     def populations(self):
-        f = np.zeros((Q, self.n))
-        lib().ohrr_get_populations(self._h, _p(f))
+        f = np.zeros((self.q, self.n))
+        self.lib.ohrr_get_populations(self._h, _p(f))
         return f
 
     def set_populations(self, f):
-        f = _f64(f).reshape(Q, self.n)
-        lib().ohrr_set_populations(self._h, _p(f))
+        f = _f64(f).reshape(self.q, self.n)
+        self.lib.ohrr_set_populations(self._h, _p(f))
 
     def uhat(self):
         u = np.zeros((3, self.n))
-        lib().ohrr_get_uhat(self._h, _p(u))
+        self.lib.ohrr_get_uhat(self._h, _p(u))
         return u
+
+
+class View:
+    """The oracle on one velocity set with the module's own names: view(19).Lattice(p), .equilibrium(rho, u), ..."""
+
+    def __init__(self, q):
+        self.Q = self.q = q
+
+    def __getattr__(self, name):
+        import functools
+        obj = globals()[name]
+        if name in ("lattice_tables", "equilibrium", "collide_cell", "Lattice"):
+            return functools.partial(obj, q=self.q)
+        return obj
+
+
+def view(q):
+    return View(q)
 
 
 def threads() -> int:

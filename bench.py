@@ -33,7 +33,11 @@ sys.path.insert(0, str(ROOT))
 from paper_2510_13726_b200 import inputs as I  # noqa: E402  (seeded input recipes only)
 
 METRIC = "MLUPs (fused HHRRLBM+wall-model step) on 1 B200 and % of HBM peak GB/s"
-BYTES_PER_CELL = 216.0  # 27 x 4 B read + 27 x 4 B write
+BYTES_PER_CELL = 216.0  # D3Q27: 27 x 4 B read + 27 x 4 B write; D3Q19: 152 B
+
+
+def bytes_per_cell(q: int) -> float:
+    return 8.0 * q
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 
 
@@ -104,10 +108,12 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------- CPU oracle leg
-def oracle_sample(config: int, budget_s: float = 20.0):
+def oracle_sample(config: int, budget_s: float = 20.0, q: int = 27):
     """Times the oracle as it stands on a bounded sample of the config's recipe."""
     from oracle import oracle as O
     O.build()
+    if q != 27:
+        O = O.view(q)
     case, sample = reference_sample(config)
     p = O.make_params(case.nx, case.ny, case.nz, mode=case.mode, **case.params)
     L = O.Lattice(p)
@@ -147,6 +153,8 @@ def run_reference(args, rank, world):
     _, wname = workload(args.config)
     from oracle import oracle as O
     O.build()
+    if args.q != 27:
+        O = O.view(args.q)
     # size the sample so that W + K oracle steps end within a few minutes on this host
     for shrink in range(4):
         case, sample = reference_sample(args.config, shrink)
@@ -170,7 +178,7 @@ def run_reference(args, rank, world):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "MLUPs", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": {"workload": wname, "note": "each step = one oracle time step on the bounded sample"},
+            "data": "synthetic", "config": {"workload": wname, "lattice": args.lattice, "note": "each step = one oracle time step on the bounded sample"},
             "cpu_baseline": cb,
             "e2e": {"value": value, "unit": "MLUPs", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -192,7 +200,8 @@ def run_ours(args, rank, world, local_rank):
 
     case, wname = workload(args.config, args.region_split)
     p = B.make_params(case.nx, case.ny, case.nz, mode=case.mode, **case.params)
-    L = B.Lattice(p, rotor_shape=None if case.rotor is None else case.rotor["sdf"].shape, device=dev)
+    L = B.Lattice(p, rotor_shape=None if case.rotor is None else case.rotor["sdf"].shape, device=dev, q=args.q)
+    BYTES_PER_CELL = bytes_per_cell(args.q)
     L.set_kernel_variant(args.variant)
     I.apply_case(case, L)
     n = case.n
@@ -231,18 +240,18 @@ def run_ours(args, rank, world, local_rank):
     # end to end through the C ABI with HOST buffers: upload the populations from pinned host
     # memory, step, read moments and forces back -- all inside the timed region
     e2e_steps = args.steps
-    h_f = torch.empty((27, n), dtype=torch.float32).pin_memory()
+    h_f = torch.empty((args.q, n), dtype=torch.float32).pin_memory()
     h_rho = torch.empty(n, dtype=torch.float32).pin_memory()
     h_v = torch.empty((3, n), dtype=torch.float32).pin_memory()
-    lib = B.lib()
+    lib = B.lib(args.q)
     import ctypes as C
-    B._check(lib.hhrr_get_populations(L.h, C.c_void_p(h_f.data_ptr())))
+    L._check(lib.hhrr_get_populations(L.h, C.c_void_p(h_f.data_ptr())))
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(L.stream)
-    B._check(lib.hhrr_set_populations(L.h, C.c_void_p(h_f.data_ptr())))
+    L._check(lib.hhrr_set_populations(L.h, C.c_void_p(h_f.data_ptr())))
     L.step(e2e_steps)
-    B._check(lib.hhrr_get_moments(L.h, C.c_void_p(h_rho.data_ptr()), C.c_void_p(h_v.data_ptr())))
+    L._check(lib.hhrr_get_moments(L.h, C.c_void_p(h_rho.data_ptr()), C.c_void_p(h_v.data_ptr())))
     F = L.forces(L.step_count() - min(e2e_steps, 1024), min(e2e_steps, 1024))
     e1.record(L.stream)
     barrier()
@@ -298,27 +307,31 @@ def run_ours(args, rank, world, local_rank):
         achieved = n * BYTES_PER_CELL / (k_avg_ms * 1e-3) / 1e9
         roofline = {"bound": "hbm", "kernel": {0: "moments_kernel+collide_kernel", 2: "fused_ws_kernel", 5: "fused_xpull_kernel"}[args.variant],
                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                    "traffic_source": None,
                     "peak_source": peak_src, "kernel_ms": k_avg_ms, "kernel_launches_timed": k_n,
                     "kernel_share_of_step": k_ms / (ms * k_n / args.steps) if k_n else None,
                     "algorithmic_bytes_per_cell": BYTES_PER_CELL}
-        tr = ROOT / "profiles" / "r01_traffic.txt"   # DRAM bytes per launch from the committed ncu captures
+        # DRAM bytes per launch: NOT measured in this run -- the figure of the committed ncu capture of the same kernel,
+        # lattice and launch configuration (profiles/r02_traffic.txt names the capture command); null if there is none
+        tr = ROOT / "profiles" / "r02_traffic.txt"
         if tr.exists():
             try:
                 for t in json.loads(tr.read_text()):
-                    if (t.get("cells") == n and t.get("variant") == args.variant
+                    if (t.get("cells") == n and t.get("variant") == args.variant and t.get("lattice", "D3Q27") == args.lattice
                             and bool(t.get("region_split")) == bool(args.region_split)):
                         roofline["traffic"] = t["dram_bytes_per_launch"]
+                        roofline["traffic_source"] = "committed ncu capture: " + t.get("source", "profiles/r02_traffic.txt")
             except Exception:
                 pass
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
-            cpu, _ = oracle_sample(args.config, budget_s=15.0)
+            cpu, _ = oracle_sample(args.config, budget_s=15.0, q=args.q)
         line = {"metric": METRIC, "value": value, "unit": "MLUPs", "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": {"workload": wname, "cells_per_gpu": n, "lattice": "D3Q27", "storage": "fp32 SoA A/B" + (", x-pull / yz-push" if L.population_storage() else ""),
+                "config": {"workload": wname, "cells_per_gpu": n, "lattice": args.lattice, "storage": "fp32 SoA A/B" + (", x-pull / yz-push" if L.population_storage() else ""),
                            "kernel_variant": args.variant, "parallelism": f"replicas x{world}",
-                           "l2": "inputs (11.6 GB per buffer) exceed the 126 MB L2; no flush needed"},
+                           "l2": "inputs (%.1f GB per buffer) exceed the 126 MB L2; no flush needed" % (4e-9 * args.q * n)},
                 "hbm_frac_of_peak_step": value * 1e6 * BYTES_PER_CELL / 1e9 / peak / world,
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
                 "clocks": clocks, "thrust_last_step": thrust, "thrust_coefficient_last_step": c_t,
@@ -338,11 +351,14 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--variant", type=int, default=5, choices=[0, 2, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--lattice", default="D3Q27", choices=["D3Q27", "D3Q19"],
+                    help="velocity set: D3Q27 (BASELINE.json's configs, default) or the paper's own D3Q19 (PAPER.md:94)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-region-split-leg", action="store_true", help="skip the extra region-split measurement")
     ap.add_argument("--region-split", action="store_true",
                     help="the paper's bulk / FSI region split (PAPER.md:215); default: HHRRLBM in every cell")
     args = ap.parse_args()
+    args.q = 27 if args.lattice == "D3Q27" else 19
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -40,7 +40,13 @@
 extern "C" {
 #endif
 
+/* Velocity set of the library build: 27 = D3Q27 (default, libhhrr.so), 19 = D3Q19 (libhhrr_q19.so, the paper's
+ * own lattice).  hhrr_velocity_set() tells which one a loaded library was built for.  D3Q19 holds
+ * the directions of D3Q27 with |c|^2 <= 2 in the same order: rest i = 9, opposite 18 - i, weights 1/3, 1/18,
+ * 1/36; every population buffer of the ABI then has 19 planes.                                              */
+#ifndef HHRR_Q
 #define HHRR_Q 27
+#endif
 #define HHRR_MAX_TAGS 16 /* element tags 1..15; tag 0 = none */
 
 typedef enum {
@@ -263,6 +269,7 @@ int64_t hhrr_launch_count(const hhrr_lattice* L);
 
 const char* hhrr_last_error(void);
 const char* hhrr_version(void);
+int32_t hhrr_velocity_set(void);
 
 #ifdef __cplusplus
 }

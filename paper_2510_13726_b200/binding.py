@@ -14,6 +14,7 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libhhrr.so"
+LIB_PATHS = {27: LIB_PATH, 19: _HERE / "libhhrr_q19.so"}   # one library build per velocity set (HHRR_Q)
 
 Q = 27
 MAX_TAGS = 16
@@ -31,6 +32,7 @@ SYMBOLS = [
     "hhrr_population_storage", "hhrr_set_fsi_region", "hhrr_set_wall_function", "hhrr_set_wall_model_variant",
     "hhrr_get_wall_model_state", "hhrr_set_wall_model_state", "hhrr_set_step_count",
     "hhrr_set_timing", "hhrr_get_timing", "hhrr_set_lookahead", "hhrr_launch_count", "hhrr_last_error", "hhrr_version",
+    "hhrr_velocity_set",
 ]
 
 
@@ -59,17 +61,17 @@ class HhrrError(RuntimeError):
         self.code = code
 
 
-_lib = None
+_libs = {}
 
 
-def lib():
-    """Loads libhhrr.so; raises if it has not been built (no fallback)."""
-    global _lib
-    if _lib is None:
-        if not LIB_PATH.exists():
-            raise RuntimeError(f"{LIB_PATH} missing: run `python -m paper_2510_13726_b200.build` "
+def lib(q=27):
+    """Loads libhhrr.so (D3Q27) or libhhrr_q19.so (D3Q19); raises if it has not been built (no fallback)."""
+    if q not in _libs:
+        path = LIB_PATHS[q]
+        if not path.exists():
+            raise RuntimeError(f"{path} missing: run `python -m paper_2510_13726_b200.build` "
                                "(the CUDA library is the only implementation; there is no fallback)")
-        L = C.CDLL(str(LIB_PATH))
+        L = C.CDLL(str(path))
         vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
         L.hhrr_workspace_bytes.restype = C.c_size_t
         L.hhrr_workspace_bytes.argtypes = [C.POINTER(Params), C.POINTER(RotorDesc)]
@@ -113,16 +115,19 @@ def lib():
         L.hhrr_launch_count.argtypes = [vp]
         L.hhrr_last_error.restype = C.c_char_p
         L.hhrr_version.restype = C.c_char_p
-        _lib = L
-    return _lib
+        L.hhrr_velocity_set.restype = i32
+        if L.hhrr_velocity_set() != q:
+            raise RuntimeError(f"{path} was built for D3Q{L.hhrr_velocity_set()}, not D3Q{q}")
+        _libs[q] = L
+    return _libs[q]
 
 
 W_FALLBACK = 1   # hhrr_set_kernel_variant: the default kernel cannot tile this lattice, variant 2 runs
 
 
-def _check(rc):
+def _check(rc, q=27):
     if rc < 0:
-        raise HhrrError(rc, lib().hhrr_last_error().decode())
+        raise HhrrError(rc, lib(q).hhrr_last_error().decode())
     return rc
 
 
@@ -168,12 +173,12 @@ def _rotor_desc(sdf, tag, spacing, origin, centre, axis, omega, theta0, n_tags):
     return r, (sdf, tag)
 
 
-def workspace_bytes(params: Params, rotor_shape=None) -> int:
+def workspace_bytes(params: Params, rotor_shape=None, q=27) -> int:
     r = None
     if rotor_shape is not None:
         r = RotorDesc()
         r.gz, r.gy, r.gx = rotor_shape
-    n = lib().hhrr_workspace_bytes(C.byref(params), C.byref(r) if r is not None else None)
+    n = lib(q).hhrr_workspace_bytes(C.byref(params), C.byref(r) if r is not None else None)
     if n == 0:
         raise HhrrError(-1, "hhrr_workspace_bytes: invalid parameters")
     return n
@@ -182,26 +187,31 @@ def workspace_bytes(params: Params, rotor_shape=None) -> int:
 class Lattice:
     """One lattice on one GPU.  Method names mirror include/hhrr.h without the prefix."""
 
-    def __init__(self, params: Params, rotor_shape=None, device="cuda:0", stream=None):
+    def __init__(self, params: Params, rotor_shape=None, device="cuda:0", stream=None, q=27):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2510_13726_b200 needs a CUDA device (no CPU fallback)")
         self.p = params
+        self.q = q                      # velocity set: 27 (libhhrr.so) or 19 (libhhrr_q19.so)
+        self.lib = lib(q)
         self.nx, self.ny, self.nz = params.nx, params.ny, params.nz
         self.n = self.nx * self.ny * self.nz
         self.device = torch.device(device)
-        nbytes = workspace_bytes(params, rotor_shape)
+        nbytes = workspace_bytes(params, rotor_shape, q)
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             h = C.c_void_p()
-            _check(lib().hhrr_create(C.byref(params), C.c_void_p(self.workspace.data_ptr()), nbytes,
+            self._check(self.lib.hhrr_create(C.byref(params), C.c_void_p(self.workspace.data_ptr()), nbytes,
                                      C.c_void_p(self.stream.cuda_stream), C.byref(h)))
         self.h = h
 
+    def _check(self, rc):
+        return _check(rc, self.q)
+
     def close(self):
         if getattr(self, "h", None):
-            lib().hhrr_destroy(self.h)
+            self.lib.hhrr_destroy(self.h)
             self.h = None
             self.workspace = None
 
@@ -216,95 +226,95 @@ class Lattice:
         rho = _f32(rho).ravel()
         u = _f32(u).reshape(3, -1)
         assert rho.size == self.n and u.shape[1] == self.n
-        _check(lib().hhrr_init_equilibrium(self.h, _p(rho), _p(u), int(with_neq)))
+        self._check(self.lib.hhrr_init_equilibrium(self.h, _p(rho), _p(u), int(with_neq)))
 
     def set_static_geometry(self, phi, tag=None, d_override=None):
         phi = None if phi is None else _f32(phi).ravel()
         tag = None if tag is None else np.ascontiguousarray(tag, np.uint8).ravel()
         dov = None if d_override is None else _f32(d_override).ravel()
-        _check(lib().hhrr_set_static_geometry(self.h, _p(phi), _p(tag), _p(dov)))
+        self._check(self.lib.hhrr_set_static_geometry(self.h, _p(phi), _p(tag), _p(dov)))
 
     def set_body(self, tag, centre=(0, 0, 0), omega=(0, 0, 0), vel=(0, 0, 0)):
         c, o, v = _f64(centre), _f64(omega), _f64(vel)
-        _check(lib().hhrr_set_body(self.h, int(tag), _p(c), _p(o), _p(v)))
+        self._check(self.lib.hhrr_set_body(self.h, int(tag), _p(c), _p(o), _p(v)))
 
     def set_fringe(self, x0, x1, u_in):
         u = _f64(u_in)
-        _check(lib().hhrr_set_fringe(self.h, int(x0), int(x1), _p(u)))
+        self._check(self.lib.hhrr_set_fringe(self.h, int(x0), int(x1), _p(u)))
 
     def set_rotor(self, sdf, tag, spacing, origin, centre, axis, omega, theta0, n_tags):
         r, keep = _rotor_desc(sdf, tag, spacing, origin, centre, axis, omega, theta0, n_tags)
-        _check(lib().hhrr_set_rotor(self.h, C.byref(r)))
+        self._check(self.lib.hhrr_set_rotor(self.h, C.byref(r)))
         del keep
 
     def enable_wall_model(self, enable=True):
-        _check(lib().hhrr_enable_wall_model(self.h, int(enable)))
+        self._check(self.lib.hhrr_enable_wall_model(self.h, int(enable)))
 
     def set_fsi_region(self, boxes):
         """boxes: iterable of (x0, x1, y0, y1, z0, z1), half-open; empty = HHRRLBM everywhere."""
         b = np.ascontiguousarray(np.asarray(list(boxes), np.int32).reshape(-1, 6))
-        _check(lib().hhrr_set_fsi_region(self.h, int(b.shape[0]), _p(b) if b.size else None))
+        self._check(self.lib.hhrr_set_fsi_region(self.h, int(b.shape[0]), _p(b) if b.size else None))
 
     def set_wall_model_variant(self, slip=0, shear=0):
         """Second readings of PAPER.md:314 / :324 (include/hhrr.h)."""
-        _check(lib().hhrr_set_wall_model_variant(self.h, int(slip), int(shear)))
+        self._check(self.lib.hhrr_set_wall_model_variant(self.h, int(slip), int(shear)))
 
     def set_wall_function(self, kind):
         """0: truncated Spalding (Eq. 18, default); 1: Musker's profile."""
-        _check(lib().hhrr_set_wall_function(self.h, int(kind)))
+        self._check(self.lib.hhrr_set_wall_function(self.h, int(kind)))
 
     def update_geometry(self):
-        _check(lib().hhrr_update_geometry(self.h))
+        self._check(self.lib.hhrr_update_geometry(self.h))
 
     def set_kernel_variant(self, variant):
         """Returns HHRR_OK (0) or the notice W_FALLBACK (1): variant 5 cannot tile the lattice, variant 2 runs."""
-        return _check(lib().hhrr_set_kernel_variant(self.h, int(variant)))
+        return self._check(self.lib.hhrr_set_kernel_variant(self.h, int(variant)))
 
     def set_lookahead(self, enable=True):
-        _check(lib().hhrr_set_lookahead(self.h, int(bool(enable))))
+        self._check(self.lib.hhrr_set_lookahead(self.h, int(bool(enable))))
 
     def population_storage(self):
-        return int(lib().hhrr_population_storage(self.h))
+        return int(self.lib.hhrr_population_storage(self.h))
 
     # ---- time loop
     def step(self, n=1):
-        _check(lib().hhrr_step(self.h, int(n)))
+        self._check(self.lib.hhrr_step(self.h, int(n)))
 
     def step_count(self):
-        return lib().hhrr_step_count(self.h)
+        return self.lib.hhrr_step_count(self.h)
 
     def launch_count(self):
-        return lib().hhrr_launch_count(self.h)
+        return self.lib.hhrr_launch_count(self.h)
 
     def set_timing(self, enable=True):
-        _check(lib().hhrr_set_timing(self.h, int(enable)))
+        self._check(self.lib.hhrr_set_timing(self.h, int(enable)))
 
     def timing(self):
         """(summed collide-stream device ms, launches covered) since the last call."""
         ms, k = C.c_double(0), C.c_int64(0)
-        _check(lib().hhrr_get_timing(self.h, C.byref(ms), C.byref(k)))
+        self._check(self.lib.hhrr_get_timing(self.h, C.byref(ms), C.byref(k)))
         return ms.value, k.value
 
     def check_finite(self):
-        _check(lib().hhrr_check_finite(self.h))
+        self._check(self.lib.hhrr_check_finite(self.h))
 
     # ---- outputs
     def moments(self):
         rho = np.empty(self.n, np.float32)
         v = np.empty((3, self.n), np.float32)
-        _check(lib().hhrr_get_moments(self.h, _p(rho), _p(v)))
+        self._check(self.lib.hhrr_get_moments(self.h, _p(rho), _p(v)))
         return rho, v
 
     def moments_device(self, rho_t, v_t):
         """rho_t: float32 CUDA tensor [n]; v_t: float32 CUDA tensor [3, n]; asynchronous."""
-        _check(lib().hhrr_get_moments_device(self.h, C.c_void_p(rho_t.data_ptr()), C.c_void_p(v_t.data_ptr())))
+        self._check(self.lib.hhrr_get_moments_device(self.h, C.c_void_p(rho_t.data_ptr()), C.c_void_p(v_t.data_ptr())))
 
     def forces(self, first=0, count=None):
         if count is None:
             count = self.step_count() - first
         F = np.zeros((count, MAX_TAGS, 3))
         if count:
-            _check(lib().hhrr_get_forces(self.h, int(first), int(count), _p(F)))
+            self._check(self.lib.hhrr_get_forces(self.h, int(first), int(count), _p(F)))
         return F
 
     def torques(self, first=0, count=None):
@@ -312,19 +322,19 @@ class Lattice:
             count = self.step_count() - first
         M = np.zeros((count, MAX_TAGS, 3))
         if count:
-            _check(lib().hhrr_get_torques(self.h, int(first), int(count), _p(M)))
+            self._check(self.lib.hhrr_get_torques(self.h, int(first), int(count), _p(M)))
         return M
 
     def cell_types(self):
         t = np.empty(self.n, np.uint8)
         g = np.empty(self.n, np.uint8)
         d = np.empty(self.n, np.float32)
-        _check(lib().hhrr_get_cell_types(self.h, _p(t), _p(g), _p(d)))
+        self._check(self.lib.hhrr_get_cell_types(self.h, _p(t), _p(g), _p(d)))
         return t, g, d
 
     def wall_list(self):
         k = C.c_int64(0)
-        _check(lib().hhrr_get_wall_list(self.h, 0, None, None, None, None, C.byref(k)))
+        self._check(self.lib.hhrr_get_wall_list(self.h, 0, None, None, None, None, C.byref(k)))
         k = k.value
         idx = np.zeros(k, np.int32)
         y1n = np.zeros((k, 3))
@@ -332,7 +342,7 @@ class Lattice:
         va = np.zeros(k, np.uint8)
         if k:
             kk = C.c_int64(0)
-            _check(lib().hhrr_get_wall_list(self.h, k, _p(idx), _p(y1n), _p(ut), _p(va), C.byref(kk)))
+            self._check(self.lib.hhrr_get_wall_list(self.h, k, _p(idx), _p(y1n), _p(ut), _p(va), C.byref(kk)))
         return idx, y1n, ut, va
 
     def wall_state(self, cell):
@@ -340,49 +350,49 @@ class Lattice:
         valid = C.c_int32(0)
         u = np.zeros(3)
         s = np.zeros(6)
-        _check(lib().hhrr_get_wall_state(self.h, int(cell), C.byref(ut), _p(u), _p(s), C.byref(valid)))
+        self._check(self.lib.hhrr_get_wall_state(self.h, int(cell), C.byref(ut), _p(u), _p(s), C.byref(valid)))
         return valid.value, ut.value, u, s
 
     def wall_model_state(self):
         """(idx int32[k], u_tau f64[k], u_wm f32[k,3], s_wm f32[k,6], valid u8[k]) of the current wall list."""
         kk = C.c_int64(0)
-        _check(lib().hhrr_get_wall_model_state(self.h, 0, None, None, None, None, None, C.byref(kk)))
+        self._check(self.lib.hhrr_get_wall_model_state(self.h, 0, None, None, None, None, None, C.byref(kk)))
         k = kk.value
         idx = np.zeros(k, np.int32); ut = np.zeros(k); uw = np.zeros((k, 3), np.float32)
         sw = np.zeros((k, 6), np.float32); va = np.zeros(k, np.uint8)
         if k:
-            _check(lib().hhrr_get_wall_model_state(self.h, k, _p(idx), _p(ut), _p(uw), _p(sw), _p(va), C.byref(kk)))
+            self._check(self.lib.hhrr_get_wall_model_state(self.h, k, _p(idx), _p(ut), _p(uw), _p(sw), _p(va), C.byref(kk)))
         return idx, ut, uw, sw, va
 
     def set_wall_model_state(self, idx, u_tau, u_wm, s_wm, valid):
         idx = np.ascontiguousarray(idx, np.int32); ut = np.ascontiguousarray(u_tau, np.float64)
         uw = np.ascontiguousarray(u_wm, np.float32); sw = np.ascontiguousarray(s_wm, np.float32)
         va = np.ascontiguousarray(valid, np.uint8)
-        _check(lib().hhrr_set_wall_model_state(self.h, len(idx), _p(idx), _p(ut), _p(uw), _p(sw), _p(va)))
+        self._check(self.lib.hhrr_set_wall_model_state(self.h, len(idx), _p(idx), _p(ut), _p(uw), _p(sw), _p(va)))
 
     def set_step_count(self, step):
-        _check(lib().hhrr_set_step_count(self.h, int(step)))
+        self._check(self.lib.hhrr_set_step_count(self.h, int(step)))
 
     def populations(self):
-        f = np.empty((Q, self.n), np.float32)
-        _check(lib().hhrr_get_populations(self.h, _p(f)))
+        f = np.empty((self.q, self.n), np.float32)
+        self._check(self.lib.hhrr_get_populations(self.h, _p(f)))
         return f
 
     def set_populations(self, f_minus_w):
-        f = _f32(f_minus_w).reshape(Q, self.n)
-        _check(lib().hhrr_set_populations(self.h, _p(f)))
+        f = _f32(f_minus_w).reshape(self.q, self.n)
+        self._check(self.lib.hhrr_set_populations(self.h, _p(f)))
 
     def cell_populations(self, cells):
         """(f - w)[k, 27] and the stored flag bytes of the given cell indices."""
         cells = np.ascontiguousarray(cells, np.int64)
-        out = np.empty((cells.size, Q), np.float32)
+        out = np.empty((cells.size, self.q), np.float32)
         fl = np.empty(cells.size, np.uint8)
-        _check(lib().hhrr_get_cell_populations(self.h, cells.size, _p(cells), _p(out), _p(fl)))
+        self._check(self.lib.hhrr_get_cell_populations(self.h, cells.size, _p(cells), _p(out), _p(fl)))
         return out, fl
 
     def uhat(self):
         u = np.empty((3, self.n), np.float32)
-        _check(lib().hhrr_get_uhat(self.h, _p(u)))
+        self._check(self.lib.hhrr_get_uhat(self.h, _p(u)))
         return u
 
     def synchronize(self):

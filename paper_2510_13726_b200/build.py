@@ -20,6 +20,8 @@ CSRC = HERE / "csrc"
 INCLUDE = HERE.parent / "include"
 LIB = HERE / "libhhrr.so"
 OBJ = HERE / "build"
+# one build per velocity set (HHRR_Q): D3Q27 (BASELINE.json's configs) and D3Q19 (the paper's own)
+LIBS = {27: LIB, 19: HERE / "libhhrr_q19.so"}
 
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v", f"-I{INCLUDE}"]
@@ -45,26 +47,31 @@ def _newest_dep() -> float:
     return max(p.stat().st_mtime for p in deps)
 
 
-def _compile(name: str, extra: list[str]) -> Path:
-    obj = OBJ / (name + ".o")
-    cmd = [nvcc(), *ARCH, *COMMON, *extra, "-c", str(CSRC / name), "-o", str(obj)]
+def _compile(q: int, name: str, extra: list[str]) -> Path:
+    tag = "" if q == 27 else f".q{q}"
+    obj = OBJ / (name + tag + ".o")
+    cmd = [nvcc(), *ARCH, *COMMON, f"-DHHRR_Q={q}", *extra, "-c", str(CSRC / name), "-o", str(obj)]
     r = subprocess.run(cmd, capture_output=True, text=True)
-    (OBJ / (name + ".log")).write_text(" ".join(cmd) + "\n" + r.stdout + r.stderr)
+    (OBJ / (name + tag + ".log")).write_text(" ".join(cmd) + "\n" + r.stdout + r.stderr)
     if r.returncode:
-        raise RuntimeError(f"nvcc failed on {name}:\n{r.stdout}\n{r.stderr}")
+        raise RuntimeError(f"nvcc failed on {name} (D3Q{q}):\n{r.stdout}\n{r.stderr}")
     return obj
 
 
 def build(force: bool = False) -> Path:
-    if not force and LIB.exists() and LIB.stat().st_mtime >= _newest_dep():
+    """Builds libhhrr.so (D3Q27) and libhhrr_q19.so (D3Q19); returns the path of the former."""
+    if not force and all(p.exists() and p.stat().st_mtime >= _newest_dep() for p in LIBS.values()):
         return LIB
     OBJ.mkdir(exist_ok=True)
-    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
-        objs = list(ex.map(lambda kv: _compile(*kv), SOURCES.items()))
-    cmd = [nvcc(), *ARCH, "-shared", "-o", str(LIB), *map(str, objs), "-cudart", "static"]
-    r = subprocess.run(cmd, capture_output=True, text=True)
-    if r.returncode:
-        raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
+    jobs = [(q, name, extra) for q in LIBS for name, extra in SOURCES.items()]
+    with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
+        objs = list(ex.map(lambda j: _compile(*j), jobs))
+    for q, out in LIBS.items():
+        mine = [str(o) for (jq, _, _), o in zip(jobs, objs) if jq == q]
+        cmd = [nvcc(), *ARCH, "-shared", "-o", str(out), *mine, "-cudart", "static"]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode:
+            raise RuntimeError(f"link failed (D3Q{q}):\n{r.stdout}\n{r.stderr}")
     return LIB
 
 

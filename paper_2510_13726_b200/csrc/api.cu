@@ -9,7 +9,7 @@
 #include <new>
 #include <vector>
 
-#include "d3q27.cuh"
+#include "cell_model.cuh"
 
 using namespace hhrr;
 
@@ -193,7 +193,8 @@ int ensure_geometry(hhrr_lattice* L) {
 extern "C" {
 
 const char* hhrr_last_error(void) { return g_err; }
-const char* hhrr_version(void) { return "hhrr-b200 0.1 (D3Q27 fp32, sm_100a)"; }
+const char* hhrr_version(void) { return Q == 27 ? "hhrr-b200 0.2 (D3Q27 fp32, sm_100a)" : "hhrr-b200 0.2 (D3Q19 fp32, sm_100a)"; }
+int32_t hhrr_velocity_set(void) { return Q; }
 int64_t hhrr_force_history(void) { return FORCE_HISTORY; }
 
 size_t hhrr_workspace_bytes(const hhrr_params* p, const hhrr_rotor_desc* rotor) {

@@ -1,28 +1,53 @@
-// d3q27.cuh -- D3Q27 cell model of the HHRRLBM in fp32 on population deviations f_i - w_i.
+// cell_model.cuh -- cell model of the HHRRLBM in fp32 on population deviations f_i - w_i, on the velocity set
+// HHRR_Q: D3Q27 (BASELINE.json's configs, the default build) or D3Q19 (the paper's own, Fig. 2 :107;
+// the library built with -DHHRR_Q=19).
 //
 // PAPER.md:98 (Eq. 6), :102 (Eq. 7), :113-122 (Eq. 8-10), :126-129 (Eq. 11), :133 (Eq. 12),
-// :144 (Eq. 14); readings R1-R6 of DESIGN.md.  All sums over the 27 directions are written
-// through the tensor-product structure c = (cx,cy,cz), cx,cy,cz in {-1,0,1}:
-//   * moments: three separable passes (x, then y, then z)            ~70 adds
+// :144 (Eq. 14); readings R1-R6, R23 of DESIGN.md.  The sums over the directions are written through the
+// structure of the set:
+//   * D3Q27 moments: three separable passes (x, then y, then z) over c in {-1,0,1}^3          ~70 adds
+//   * D3Q19 moments: sums and differences of the 9 opposite pairs, then per-axis sums           ~54 adds
 //   * reconstruction: f_i = w_i (E_i + O_i), f_ibar = w_i (E_i - O_i) with E the even and
-//     O the odd polynomial in c                                       ~220 flops
+//     O the odd polynomial in c; the same Hermite algebra for both sets, only the third-order
+//     coefficients differ (R3 / R23)                                                           ~220 / ~170 flops
 // CUDA path only; shares nothing with oracle/.
 #pragma once
 #include "lattice.h"
 
 namespace hhrr {
 
-__host__ __device__ constexpr int dir_cx(int i) { return i % 3 - 1; }
-__host__ __device__ constexpr int dir_cy(int i) { return (i / 3) % 3 - 1; }
-__host__ __device__ constexpr int dir_cz(int i) { return i / 9 - 1; }
-__host__ __device__ constexpr float dir_w(int i) {
-  return (dir_cx(i) ? 1.f / 6.f : 2.f / 3.f) * (dir_cy(i) ? 1.f / 6.f : 2.f / 3.f) *
-         (dir_cz(i) ? 1.f / 6.f : 2.f / 3.f);
+static_assert(Q == 27 || Q == 19, "velocity set: D3Q27 or D3Q19");
+
+// Direction i of the set sits at slot (cx+1) + 3(cy+1) + 9(cz+1) of the 27-point cube; D3Q19 = the slots with
+// |c|^2 <= 2 in the same order, so that for both sets rest = (Q-1)/2 and opposite = Q-1-i.
+__host__ __device__ constexpr int dir_slot(int i) {
+  if (Q == 27) return i;
+  constexpr int s19[19] = {1, 3, 4, 5, 7, 9, 10, 11, 12, 13, 14, 15, 16, 17, 19, 21, 22, 23, 25};
+  return s19[i < 19 ? i : 0];
+}
+__host__ __device__ constexpr int dir_cx(int i) { return dir_slot(i) % 3 - 1; }
+__host__ __device__ constexpr int dir_cy(int i) { return (dir_slot(i) / 3) % 3 - 1; }
+__host__ __device__ constexpr int dir_cz(int i) { return dir_slot(i) / 9 - 1; }
+constexpr int REST = (Q - 1) / 2;
+__host__ __device__ constexpr int dir_opp(int i) { return Q - 1 - i; }
+// index of direction (cx, cy, cz); -1 if the set does not hold it (cube corners on D3Q19)
+__host__ __device__ constexpr int dir_index(int cx, int cy, int cz) {
+  const int slot = (cx + 1) + 3 * (cy + 1) + 9 * (cz + 1);
+  if (Q == 27) return slot;
+  constexpr int i19[27] = {-1, 0, -1, 1, 2, 3, -1, 4, -1, 5, 6, 7, 8, 9, 10, 11, 12, 13, -1, 14, -1, 15, 16, 17, -1, 18, -1};
+  return i19[slot];
+}
+// direction i with the marked components reversed (a population reflected at MIRROR planes, R12)
+__host__ __device__ constexpr int dir_flip(int i, bool fx, bool fy, bool fz) {
+  return dir_index(fx ? -dir_cx(i) : dir_cx(i), fy ? -dir_cy(i) : dir_cy(i), fz ? -dir_cz(i) : dir_cz(i));
 }
 __host__ __device__ constexpr double dir_wd(int i) {
-  return (dir_cx(i) ? 1.0 / 6.0 : 2.0 / 3.0) * (dir_cy(i) ? 1.0 / 6.0 : 2.0 / 3.0) *
-         (dir_cz(i) ? 1.0 / 6.0 : 2.0 / 3.0);
+  if (Q == 27)
+    return (dir_cx(i) ? 1.0 / 6.0 : 2.0 / 3.0) * (dir_cy(i) ? 1.0 / 6.0 : 2.0 / 3.0) * (dir_cz(i) ? 1.0 / 6.0 : 2.0 / 3.0);
+  const int nn = dir_cx(i) * dir_cx(i) + dir_cy(i) * dir_cy(i) + dir_cz(i) * dir_cz(i);
+  return nn == 0 ? 1.0 / 3.0 : (nn == 1 ? 1.0 / 18.0 : 1.0 / 36.0);
 }
+__host__ __device__ constexpr float dir_w(int i) { return (float)dir_wd(i); }
 
 // MUFU reciprocal + one Newton step (<= 1 ulp, branch-free) and MUFU square root (2^-23 rel.)
 __device__ __forceinline__ float rcp_nr(float x) {
@@ -68,9 +93,15 @@ struct MomentsT {  // of the deviations: drho = rho - 1, j, M_ab = sum c_a c_b (
 };
 using Moments = MomentsT<float>;
 
-// rho and j only (halo cells, moments pass, read-back): 3 separable passes
+// Sums over the directions, per velocity set.
+template <class T, int NQ>
+struct CellSums;
+
+// D3Q27: three separable passes (x, then y, then z)
 template <class T>
-__device__ __forceinline__ void moments_rho_j(const T (&f)[Q], T& drho, T& jx, T& jy, T& jz) {
+struct CellSums<T, 27> {
+  // rho and j only (halo cells, moments pass, read-back)
+  static __device__ __forceinline__ void rho_j(const T (&f)[27], T& drho, T& jx, T& jy, T& jz) {
   T s0[9], s1[9];
 #pragma unroll
   for (int m = 0; m < 9; ++m) {
@@ -91,8 +122,7 @@ __device__ __forceinline__ void moments_rho_j(const T (&f)[Q], T& drho, T& jx, T
   jx = (t10[2] + t10[0]) + t10[1];
 }
 
-template <class T>
-__device__ __forceinline__ MomentsT<T> moments_all(const T (&f)[Q]) {
+  static __device__ __forceinline__ MomentsT<T> all(const T (&f)[27]) {
   T s0[9], s1[9], s2[9];
 #pragma unroll
   for (int m = 0; m < 9; ++m) {
@@ -123,6 +153,70 @@ __device__ __forceinline__ MomentsT<T> moments_all(const T (&f)[Q]) {
   m.mxy = (t11[2] + t11[0]) + t11[1];
   m.mxx = (t20[2] + t20[0]) + t20[1];
   return m;
+}
+
+};
+
+// D3Q19: sum s and difference d of each opposite pair (direction j > REST minus direction Q-1-j), then the
+// per-axis sums; the compile-time direction components pick the terms
+template <class T>
+struct CellSums<T, 19> {
+  struct Acc {  // sum of signed terms without a leading zero
+    T v;
+    bool any = false;
+    __device__ __forceinline__ void add(const T& t, int sgn) {
+      if (!any) v = sgn > 0 ? t : -t;
+      else v = sgn > 0 ? v + t : v - t;
+      any = true;
+    }
+  };
+  static __device__ __forceinline__ void rho_j(const T (&f)[19], T& drho, T& jx, T& jy, T& jz) {
+    Acc r, x, y, z;
+    r.add(f[9], 1);
+#pragma unroll
+    for (int j = 10; j < 19; ++j) {
+      const T s = f[j] + f[18 - j], d = f[j] - f[18 - j];
+      r.add(s, 1);
+      if (dir_cx(j)) x.add(d, dir_cx(j));
+      if (dir_cy(j)) y.add(d, dir_cy(j));
+      if (dir_cz(j)) z.add(d, dir_cz(j));
+    }
+    drho = r.v; jx = x.v; jy = y.v; jz = z.v;
+  }
+  static __device__ __forceinline__ MomentsT<T> all(const T (&f)[19]) {
+    Acc x, y, z, xx, yy, zz, xy, xz, yz, ax;  // ax: the axis pairs (one non-zero component)
+    T sd = f[9];                              // rest + face-diagonal pairs not counted in mzz
+#pragma unroll
+    for (int j = 10; j < 19; ++j) {
+      const int cx = dir_cx(j), cy = dir_cy(j), cz = dir_cz(j);
+      const T s = f[j] + f[18 - j], d = f[j] - f[18 - j];
+      if (cx) x.add(d, cx);
+      if (cy) y.add(d, cy);
+      if (cz) z.add(d, cz);
+      if (cx) xx.add(s, 1);
+      if (cy) yy.add(s, 1);
+      if (cz) zz.add(s, 1);
+      if (cx * cy) xy.add(s, cx * cy);
+      if (cx * cz) xz.add(s, cx * cz);
+      if (cy * cz) yz.add(s, cy * cz);
+      if (!cz) sd = sd + s;
+    }
+    MomentsT<T> m;
+    m.drho = sd + zz.v;
+    m.jx = x.v; m.jy = y.v; m.jz = z.v;
+    m.mxx = xx.v; m.myy = yy.v; m.mzz = zz.v;
+    m.mxy = xy.v; m.mxz = xz.v; m.myz = yz.v;
+    return m;
+  }
+};
+
+template <class T>
+__device__ __forceinline__ void moments_rho_j(const T (&f)[Q], T& drho, T& jx, T& jy, T& jz) {
+  CellSums<T, Q>::rho_j(f, drho, jx, jy, jz);
+}
+template <class T>
+__device__ __forceinline__ MomentsT<T> moments_all(const T (&f)[Q]) {
+  return CellSums<T, Q>::all(f);
 }
 
 // u^B of a cell (fringe R12), without the wall-model slip
@@ -190,15 +284,26 @@ __device__ __forceinline__ void collide(const PhysF& ph, const MomentsT<T>& m, T
   // second order: T = 4.5 (rho uh uh + k a2)
   T Txx = 4.5f * (rux * ux + axx), Tyy = 4.5f * (ruy * uy + ayy), Tzz = 4.5f * (ruz * uz + azz);
   T Txy = 9.f * (rux * uy + axy), Txz = 9.f * (rux * uz + axz), Tyz = 9.f * (ruy * uz + ayz);
-  // third order (R3): A3_aab = rho ua ua ub + k (2 ua a_ab + ub a_aa); G_ab = 13.5 A3_aab; Gxyz = 27 A3_xyz
+  // third order: A3_aab = rho ua ua ub + k (2 ua a_ab + ub a_aa) (recursion of R3); G_ab = coefficient of H_aab.
+  // D3Q27 (R3): G_ab = 13.5 A3_aab, Gxyz = 27 A3_xyz.  D3Q19 (R23, basis of the paper's ref. [43]): per group
+  // (H1, H2) in {(xxy, yzz), (xzz, xyy), (yyz, xxz)} the term is 13.5 (H1 + H2)(A1 + A2) + 4.5 (H1 - H2)(A1 - A2),
+  // i.e. coefficient 18 A1 + 9 A2 of H1 and 9 A1 + 18 A2 of H2; H_xyz is not supported.
   T ux2 = ux + ux, uy2 = uy + uy, uz2 = uz + uz;
-  T Gxy = 13.5f * ((rux * ux) * uy + (ux2 * axy + uy * axx));  // xx y
-  T Gxz = 13.5f * ((rux * ux) * uz + (ux2 * axz + uz * axx));  // xx z
-  T Gyx = 13.5f * ((ruy * uy) * ux + (uy2 * axy + ux * ayy));  // yy x
-  T Gyz = 13.5f * ((ruy * uy) * uz + (uy2 * ayz + uz * ayy));  // yy z
-  T Gzx = 13.5f * ((ruz * uz) * ux + (uz2 * axz + ux * azz));  // zz x
-  T Gzy = 13.5f * ((ruz * uz) * uy + (uz2 * ayz + uy * azz));  // zz y
-  T Gxyz = 27.f * ((rux * uy) * uz + (ux * ayz + uy * axz + uz * axy));
+  T Axy = (rux * ux) * uy + (ux2 * axy + uy * axx);  // xx y
+  T Axz = (rux * ux) * uz + (ux2 * axz + uz * axx);  // xx z
+  T Ayx = (ruy * uy) * ux + (uy2 * axy + ux * ayy);  // yy x
+  T Ayz = (ruy * uy) * uz + (uy2 * ayz + uz * ayy);  // yy z
+  T Azx = (ruz * uz) * ux + (uz2 * axz + ux * azz);  // zz x
+  T Azy = (ruz * uz) * uy + (uz2 * ayz + uy * azz);  // zz y
+  T Gxy, Gxz, Gyx, Gyz, Gzx, Gzy, Gxyz = bcast<T>(0.f);
+  if (Q == 27) {
+    Gxy = 13.5f * Axy; Gxz = 13.5f * Axz; Gyx = 13.5f * Ayx; Gyz = 13.5f * Ayz; Gzx = 13.5f * Azx; Gzy = 13.5f * Azy;
+    Gxyz = 27.f * ((rux * uy) * uz + (ux * ayz + uy * axz + uz * axy));
+  } else {
+    Gxy = 18.f * Axy + 9.f * Azy; Gzy = 9.f * Axy + 18.f * Azy;  // (xxy, yzz)
+    Gzx = 18.f * Azx + 9.f * Ayx; Gyx = 9.f * Azx + 18.f * Ayx;  // (xzz, xyy)
+    Gyz = 18.f * Ayz + 9.f * Axz; Gxz = 9.f * Ayz + 18.f * Axz;  // (yyz, xxz)
+  }
   // even part tables: q(c) = c^2 - 1/3
   T Ex[2] = {-third * Txx, (2.f * third) * Txx};
   T Ey[2] = {-third * Tyy, (2.f * third) * Tyy};
@@ -216,7 +321,7 @@ __device__ __forceinline__ void collide(const PhysF& ph, const MomentsT<T>& m, T
       OZ[p][q] = mz + qp * Gxz + qq * Gyz;  // p: cx^2, q: cy^2
     }
 #pragma unroll
-  for (int i = 0; i <= 13; ++i) {
+  for (int i = 0; i <= REST; ++i) {
     const int cx = dir_cx(i), cy = dir_cy(i), cz = dir_cz(i);
     const int x2 = cx * cx, y2 = cy * cy, z2 = cz * cz;
     T E = Ex[x2] + Ey[y2] + Ez[z2];
@@ -227,8 +332,8 @@ __device__ __forceinline__ void collide(const PhysF& ph, const MomentsT<T>& m, T
     if (cy * cz == 1) E = E + Tyz;
     if (cy * cz == -1) E = E - Tyz;
     const float w = dir_w(i);
-    if (i == 13) {
-      out[13] = w * E;
+    if (i == REST) {
+      out[REST] = w * E;
     } else {
       T O = bcast<T>(0.f);
       bool first = true;
@@ -239,10 +344,10 @@ __device__ __forceinline__ void collide(const PhysF& ph, const MomentsT<T>& m, T
       if (cx) acc(OX[y2][z2], cx);
       if (cy) acc(OY[x2][z2], cy);
       if (cz) acc(OZ[x2][y2], cz);
-      if (cx * cy * cz) acc(Gxyz, cx * cy * cz);
+      if (Q == 27 && cx * cy * cz) acc(Gxyz, cx * cy * cz);
       const T wE = w * E;
       out[i] = fma_t(w, O, wE);
-      out[26 - i] = fma_t(-w, O, wE);
+      out[dir_opp(i)] = fma_t(-w, O, wE);
     }
   }
 }
@@ -291,7 +396,7 @@ __device__ __forceinline__ void push_store(const Dom& dm, float* __restrict__ fo
       if ((cx < 0 && fxm) || (cx > 0 && fxp)) { tx = x; cx = -cx; }
       if ((cy < 0 && fym) || (cy > 0 && fyp)) { ty = y; cy = -cy; }
       if ((cz < 0 && fzm) || (cz > 0 && fzp)) { tz = z; cz = -cz; }
-      int io = (cx + 1) + 3 * (cy + 1) + 9 * (cz + 1);
+      int io = dir_index(cx, cy, cz);
       fout[(int64_t)io * dm.n + tz * nxy + ty * nx + tx] = o[i];
     }
   }

@@ -6,7 +6,7 @@
 // Variant 0 (two-pass): moments_kernel writes the time-n homogenised velocity field,
 //   collide_kernel differentiates it (S^FD, Eq. 10 "non-local") and collides.
 // Variant 1 (fused): see fused.cu.
-#include "d3q27.cuh"
+#include "cell_model.cuh"
 
 namespace hhrr {
 
@@ -161,23 +161,37 @@ __global__ void init_kernel(Dom dm, double tau0, const float* __restrict__ rho_i
     for (int a = 0; a < 3; ++a)
       for (int b = 0; b < 3; ++b) a2[a][b] = -2.0 * rho * (1.0 / 3.0) * tau0 * 0.5 * (G[a][b] + G[b][a]);
   }
+  double A3[3][3][3];  // a0^(3) + a1^(3): rho u u u and the recursion of R3 on a2
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b)
+      for (int g = 0; g < 3; ++g)
+        A3[a][b][g] = rho * u[a] * u[b] * u[g] + (u[a] * a2[b][g] + u[b] * a2[a][g] + u[g] * a2[a][b]);
   for (int i = 0; i < Q; ++i) {
     double cv[3] = {(double)dir_cx(i), (double)dir_cy(i), (double)dir_cz(i)};
+    auto h3 = [&](int a, int b, int g) {
+      return cv[a] * cv[b] * cv[g] - (1.0 / 3.0) * (cv[a] * (b == g) + cv[b] * (a == g) + cv[g] * (a == b));
+    };
     double t1 = 0, t2 = 0, t3 = 0;
     for (int a = 0; a < 3; ++a) t1 += cv[a] * rho * u[a];
     for (int a = 0; a < 3; ++a)
       for (int b = 0; b < 3; ++b) {
         double h2 = cv[a] * cv[b] - (a == b ? 1.0 / 3.0 : 0.0);
         t2 += h2 * (rho * u[a] * u[b] + a2[a][b]);
-        for (int g = 0; g < 3; ++g) {
-          double h3 = cv[a] * cv[b] * cv[g] -
-                      (1.0 / 3.0) * (cv[a] * (b == g) + cv[b] * (a == g) + cv[g] * (a == b));
-          double a3 = u[a] * a2[b][g] + u[b] * a2[a][g] + u[g] * a2[a][b];
-          t3 += h3 * (rho * u[a] * u[b] * u[g] + a3);
-        }
       }
+    if (Q == 27) {  // full contraction / (3! cs^6) = 4.5 sum (R3)
+      for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b)
+          for (int g = 0; g < 3; ++g) t3 += 4.5 * h3(a, b, g) * A3[a][b][g];
+    } else {  // D3Q19: basis of the paper's ref. [43] (R23): sums / (2 cs^6), differences / (6 cs^6)
+      const int G1[3][3] = {{0, 0, 1}, {0, 2, 2}, {1, 1, 2}}, G2[3][3] = {{1, 2, 2}, {0, 1, 1}, {0, 0, 2}};
+      for (int k = 0; k < 3; ++k) {
+        double h1 = h3(G1[k][0], G1[k][1], G1[k][2]), h2 = h3(G2[k][0], G2[k][1], G2[k][2]);
+        double a1 = A3[G1[k][0]][G1[k][1]][G1[k][2]], a2_ = A3[G2[k][0]][G2[k][1]][G2[k][2]];
+        t3 += 13.5 * (h1 + h2) * (a1 + a2_) + 4.5 * (h1 - h2) * (a1 - a2_);
+      }
+    }
     double w = dir_wd(i);
-    double dev = w * ((rho - 1.0) + 3.0 * t1 + 4.5 * t2 + 4.5 * t3);
+    double dev = w * ((rho - 1.0) + 3.0 * t1 + 4.5 * t2 + t3);
     f[(int64_t)i * n + c] = (float)dev;
   }
 }

@@ -35,8 +35,8 @@ struct XpCfg {
   // is one aligned 8-byte word), the x halo at columns 1 and TX + 2, columns 0 and TX + 3 are padding
   static constexpr int SX = TX + 4, SY = TY + 2, PLANE = SX * SY;
   static constexpr int HALO = 2 * TX + 2 * TY, HSLOTS = (HALO + AUX - 1) / AUX;
-  // one stage, in floats: [27][TY][W] tile rows | [27][W] row y0-1 | [27][W] row y0+TY |
-  //                       [27][TY][4] wrapped columns of the tile rows | [27][4] | [27][4] of the halo rows
+  // one stage, in floats: [Q][TY][W] tile rows | [Q][W] row y0-1 | [Q][W] row y0+TY |
+  //                       [Q][TY][4] wrapped columns of the tile rows | [Q][4] | [Q][4] of the halo rows
   static constexpr int pad32(int f) { return (f + 31) / 32 * 32; }  // 128-byte granules (TMA destination)
   static constexpr int MAIN_F = Q * TY * W, ROW_F = Q * W, ROW_PAD_F = pad32(ROW_F), PM_F = Q * TY * 4,
                        PM_PAD_F = pad32(PM_F), PR_F = Q * 4, PR_PAD_F = pad32(PR_F);
@@ -101,12 +101,15 @@ __device__ __forceinline__ void push_store_yz(const Dom& dm, float* __restrict__
   const int64_t nx = dm.nx, nxy = (int64_t)dm.nx * dm.ny;
 #pragma unroll
   for (int i = 0; i < Q; ++i) {
-    int cy = dir_cy(i), cz = dir_cz(i), io = i;
+    const int cy = dir_cy(i), cz = dir_cz(i);
     int ty = cy < 0 ? ym : (cy > 0 ? yp : y);
     int tz = cz < 0 ? zm : (cz > 0 ? zp : z);
     // a population leaving through a mirror plane returns to the same cell, component reversed
-    if ((cy < 0 && fym) || (cy > 0 && fyp)) { ty = y; io -= 6 * cy; }
-    if ((cz < 0 && fzm) || (cz > 0 && fzp)) { tz = z; io -= 18 * cz; }
+    const bool ry = (cy < 0 && fym) || (cy > 0 && fyp), rz = (cz < 0 && fzm) || (cz > 0 && fzp);
+    if (ry) ty = y;
+    if (rz) tz = z;
+    const int io = ry ? (rz ? dir_flip(i, false, true, true) : dir_flip(i, false, true, false))
+                      : (rz ? dir_flip(i, false, false, true) : i);
     fout[(int64_t)io * dm.n + tz * nxy + ty * nx + x] = o[i];
   }
 }
@@ -284,14 +287,14 @@ __global__ void __launch_bounds__(C::THREADS, 1)
           const int col = 4 + lx - (g - 1);
           const int pstride = region == 0 ? TY * W : W;
           const int base = region == 0 ? row * W : (region == 1 ? O_RM : O_RP);
-          h_off[k][g] = base + col + g * pstride;
-          h_str[k][g] = 3 * pstride;
+          h_off[k][g] = base + col;
+          h_str[k][g] = pstride;
         } else {
           const int col = (sx < 0 ? sx + dm.nx : sx - dm.nx) - px;  // 0..3
           const int pstride = region == 0 ? TY * 4 : 4;
           const int base = region == 0 ? O_PM + row * 4 : (region == 1 ? O_PRM : O_PRP);
-          h_off[k][g] = base + col + g * pstride;
-          h_str[k][g] = 3 * pstride;
+          h_off[k][g] = base + col;
+          h_str[k][g] = pstride;
         }
       }
     }
@@ -312,7 +315,7 @@ __global__ void __launch_bounds__(C::THREADS, 1)
         if (!h_on[k]) continue;
         float f[Q];
 #pragma unroll
-        for (int i = 0; i < Q; ++i) f[i] = st[h_off[k][i % 3] + (i / 3) * h_str[k][i % 3]];
+        for (int i = 0; i < Q; ++i) f[i] = st[h_off[k][dir_cx(i) + 1] + i * h_str[k][dir_cx(i) + 1]];
         const int64_t c = h_x[k] + nx * h_y[k] + zoff;
         float d, uB[3], rho, uh[3], drho, jx, jy, jz;
         solid_state_ws(a, flb[h_fl[k]], c, h_x[k], h_y[k], zr, d, uB);
@@ -375,11 +378,13 @@ __global__ void __launch_bounds__(C::THREADS, 1)
       if (edge) {
         if (patch_l) {
 #pragma unroll
-          for (int k = 0; k < 9; ++k) f[3 * k + 2].v.x = st[patch_off + (3 * k + 2) * (TY * 4)];  // cx = +1 from x = nx-1
+          for (int i = 0; i < Q; ++i)
+            if (dir_cx(i) == 1) f[i].v.x = st[patch_off + i * (TY * 4)];   // cx = +1 from x = nx-1
         }
         if (patch_r) {
 #pragma unroll
-          for (int k = 0; k < 9; ++k) f[3 * k].v.y = st[patch_off + (3 * k) * (TY * 4)];          // cx = -1 from x = 0
+          for (int i = 0; i < Q; ++i)
+            if (dir_cx(i) == -1) f[i].v.y = st[patch_off + i * (TY * 4)];  // cx = -1 from x = 0
         }
       }
       __syncwarp();

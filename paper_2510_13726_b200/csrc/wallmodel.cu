@@ -8,7 +8,7 @@
 // collide-stream kernels (its output feeds the next collision); K4 only reads the streamed populations
 // and runs on the side stream beside the next collide-stream kernel.
 // CUDA path only; shares nothing with oracle/.
-#include "d3q27.cuh"
+#include "cell_model.cuh"
 
 namespace hhrr {
 
@@ -112,12 +112,15 @@ __device__ __forceinline__ void wall_sample_cell(const WmArgs& a, int64_t c, con
     zz = wrap_far(iz + oz, a.dm.nz, a.dm.mode[2], flz);
   }
   double drho = 0, j0 = 0, j1 = 0, j2 = 0;
-  if (kc < 9) {
+  if (kc < 9) {  // group g holds the populations with cz = g - 1 (nine on D3Q27; five, nine, five on D3Q19)
     float fv[9];
 #pragma unroll
-    for (int q = 0; q < 9; ++q) fv[q] = __ldg(a.f + pop_index(a.dm, 9 * g + q, xx, yy, zz));
+    for (int q = 0; q < 9; ++q) {
+      const int i = dir_index(q % 3 - 1, q / 3 - 1, g - 1);  // -1: the set has no such direction
+      fv[q] = i >= 0 ? __ldg(a.f + pop_index(a.dm, i, xx, yy, zz)) : 0.f;
+    }
 #pragma unroll
-    for (int q = 0; q < 9; ++q) {  // population 9g + q: cx = q % 3 - 1, cy = q / 3 - 1, cz = g - 1
+    for (int q = 0; q < 9; ++q) {  // cx = q % 3 - 1, cy = q / 3 - 1
       double fi = (double)fv[q];
       drho += fi;
       j0 += (q % 3 - 1) * fi;
@@ -353,18 +356,19 @@ __device__ __forceinline__ void force_block(const ForceArgs& a, int block, int n
         const int zz = wrap_far(z + cz, a.dm.nz, a.dm.mode[2], flz);
 #pragma unroll
         for (int j = 0; j < 9; ++j) {
-          const int cx = j % 3 - 1, cy = j / 3 - 1, i = 9 * pz + j;
-          if (i == 13) continue;
+          const int cx = j % 3 - 1, cy = j / 3 - 1;
+          if ((Q == 19 && cx * cy * cz != 0) || (cx == 0 && cy == 0 && cz == 0)) continue;  // not in the set / rest
+          const int i = dir_index(cx, cy, cz);
           const int xx = wrap_far(x + cx, a.dm.nx, a.dm.mode[0], flx);
           const int yy = wrap_far(y + cy, a.dm.ny, a.dm.mode[1], fly);
           // R12: the cell behind a MIRROR plane is the reflected image of the lattice -- f_i there is the population
           // of the reflected cell with the normal velocity component reversed (what push_store does to a
           // population that leaves through the plane)
-          const int ir = i - (flx ? 2 * cx : 0) - (fly ? 6 * cy : 0) - (flz ? 18 * cz : 0);
+          const int ir = dir_index(flx ? -cx : cx, fly ? -cy : cy, flz ? -cz : cz);
           // stored values are deviations: f = w + dev, and w_i = w_ibar = w of the reflected direction
-          const double w = (cx ? 1.0 / 6.0 : 2.0 / 3.0) * (cy ? 1.0 / 6.0 : 2.0 / 3.0) * (cz ? 1.0 / 6.0 : 2.0 / 3.0);
+          const double w = dir_wd(i);
           const double fa = w + (double)__ldg(a.f + pop_index(a.dm, ir, xx, yy, zz));
-          const double fb = w + (double)__ldg(a.f + pop_index(a.dm, 26 - i, x, y, z));
+          const double fb = w + (double)__ldg(a.f + pop_index(a.dm, dir_opp(i), x, y, z));
           const double ci[3] = {(double)cx, (double)cy, (double)cz};
 #pragma unroll
           for (int q = 0; q < 3; ++q) acc[q] += (ci[q] - us[q]) * fa + (ci[q] + us[q]) * fb;

@@ -2,7 +2,7 @@
 // (fused_ws.cu: one cell per producer lane; fused_ws2.cu: two x-adjacent cells per lane).
 // CUDA path only; shares nothing with oracle/.
 #pragma once
-#include "d3q27.cuh"
+#include "cell_model.cuh"
 
 namespace hhrr {
 

@@ -28,15 +28,30 @@ def test_header_and_binding_agree():
     assert _declared() == sorted(binding.SYMBOLS)
 
 
+def _libraries(built):
+    from paper_2510_13726_b200 import build
+    assert build.LIBS[27] == built
+    return list(build.LIBS.items())     # D3Q27 (libhhrr.so) and D3Q19 (libhhrr_q19.so): same ABI, same sources
+
+
 def test_library_exports_every_declared_symbol(built):
-    out = subprocess.run(["nm", "-D", "--defined-only", str(built)], capture_output=True, text=True, check=True).stdout
-    exported = set(re.findall(r"\bT (hhrr_[a-z_0-9]+)$", out, flags=re.M))
-    assert set(_declared()) <= exported, set(_declared()) - exported
+    for q, path in _libraries(built):
+        out = subprocess.run(["nm", "-D", "--defined-only", str(path)], capture_output=True, text=True, check=True).stdout
+        exported = set(re.findall(r"\bT (hhrr_[a-z_0-9]+)$", out, flags=re.M))
+        assert set(_declared()) <= exported, (q, set(_declared()) - exported)
 
 
 def test_library_is_sm100a_with_lineinfo(built):
-    out = subprocess.run(["cuobjdump", "-lelf", str(built)], capture_output=True, text=True).stdout
-    assert "sm_100a" in out
+    for q, path in _libraries(built):
+        out = subprocess.run(["cuobjdump", "-lelf", str(path)], capture_output=True, text=True).stdout
+        assert "sm_100a" in out, q
+
+
+def test_velocity_set_of_each_build(built):
+    from paper_2510_13726_b200 import binding as B
+    assert B.lib(27).hhrr_velocity_set() == 27 and B.lib(19).hhrr_velocity_set() == 19
+    p = B.make_params(128, 64, 64)
+    assert B.workspace_bytes(p, q=19) < B.workspace_bytes(p, q=27)    # 19 instead of 27 planes per buffer
 
 
 def test_workspace_bytes_and_argument_errors(built):

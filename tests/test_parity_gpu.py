@@ -18,12 +18,12 @@ TOL_LONG = 1e-3
 UTAU_ERR = []      # observed relative u_tau differences (reported by test_zz_report_utau_error)
 
 
-def _gpu_lattice(case, variant, rotor_shape=None):
+def _gpu_lattice(case, variant, rotor_shape=None, q=27):
     from paper_2510_13726_b200 import binding as B
     p = B.make_params(case.nx, case.ny, case.nz, mode=case.mode, **case.params)
     if case.rotor is not None:
         rotor_shape = case.rotor["sdf"].shape
-    L = B.Lattice(p, rotor_shape=rotor_shape)
+    L = B.Lattice(p, rotor_shape=rotor_shape, q=q)
     L.set_kernel_variant(variant)
     I.apply_case(case, L)
     return L
@@ -74,7 +74,8 @@ def compare_forces(G, Oa, tol):
 
 
 def run_parity(oracle, case, steps, variant, tol, check_every=None, force_tol=None):
-    G, Oa = _gpu_lattice(case, variant), _ora_lattice(oracle, case)
+    """oracle: the oracle module (D3Q27) or oracle.view(19) (D3Q19: the CUDA library built with HHRR_Q = 19)."""
+    G, Oa = _gpu_lattice(case, variant, q=getattr(oracle, "q", 27)), _ora_lattice(oracle, case)
     done = 0
     chunk = check_every or steps
     G.update_geometry(); Oa.update_geometry()

@@ -237,6 +237,21 @@ int hhrr_get_cell_populations(hhrr_lattice* L, int64_t n_cells, const int64_t* c
 /* Time-n homogenised velocity field of the last collide (3N floats), for tests.  Only the two-pass kernel
  * (variant 0) stores it; HHRR_E_STATE otherwise or before the first step.                    */
 int hhrr_get_uhat(hhrr_lattice* L, float* uhat);
+/* Slab decomposition along z (the paper's multi-GPU layout: one block per GPU).  A rank's
+ * lattice is z-periodic and holds one HALO plane at either end (z = 0, z = nz - 1) around its nz - 2 real planes.
+ * After every hhrr_step(L, 1) the ranks exchange, per face, hhrr_halo_floats(L) floats:
+ *   hhrr_halo_pack(L, face, d_buf)    face 0 = low z, 1 = high z; asynchronous on the stream: the populations the
+ *                                     collision pushed into the halo plane (they belong to the neighbour's first real
+ *                                     plane) and the other populations of the last real plane (the neighbour's halo);
+ *   hhrr_halo_unpack(L, face, d_buf)  at the RECEIVING rank with the face the data arrived through, i.e. the buffer
+ *                                     a neighbour packed with face 1 is unpacked with face 0 and vice versa.
+ * d_buf is a device pointer (it may be peer-mapped memory of the neighbour GPU: the pack kernel's stores then are
+ * the transfer).  Structures (cells with d < 1 and their wall-model stencils) must stay clear of the halo planes
+ * and the planes next to them; the fringe and plain fluid may cross.  The exchanged state equals the undecomposed
+ * lattice's bit for bit (tests/test_slabs*.py).                                                                  */
+int64_t hhrr_halo_floats(const hhrr_lattice* L);
+int hhrr_halo_pack(hhrr_lattice* L, int32_t face, float* d_buf);
+int hhrr_halo_unpack(hhrr_lattice* L, int32_t face, const float* d_buf);
 /* HHRR_E_NAN if any population is non-finite (synchronises). */
 int hhrr_check_finite(hhrr_lattice* L);
 /* Selects the collide-stream kernel: 5 = the TMA-fed fused kernel on x-pull / yz-push storage

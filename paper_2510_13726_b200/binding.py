@@ -32,7 +32,7 @@ SYMBOLS = [
     "hhrr_population_storage", "hhrr_set_fsi_region", "hhrr_set_wall_function", "hhrr_set_wall_model_variant",
     "hhrr_get_wall_model_state", "hhrr_set_wall_model_state", "hhrr_set_step_count",
     "hhrr_set_timing", "hhrr_get_timing", "hhrr_set_lookahead", "hhrr_launch_count", "hhrr_last_error", "hhrr_version",
-    "hhrr_velocity_set",
+    "hhrr_velocity_set", "hhrr_halo_floats", "hhrr_halo_pack", "hhrr_halo_unpack",
 ]
 
 
@@ -116,6 +116,10 @@ def lib(q=27):
         L.hhrr_last_error.restype = C.c_char_p
         L.hhrr_version.restype = C.c_char_p
         L.hhrr_velocity_set.restype = i32
+        L.hhrr_halo_floats.restype = i64
+        L.hhrr_halo_floats.argtypes = [vp]
+        L.hhrr_halo_pack.argtypes = [vp, i32, vp]
+        L.hhrr_halo_unpack.argtypes = [vp, i32, vp]
         if L.hhrr_velocity_set() != q:
             raise RuntimeError(f"{path} was built for D3Q{L.hhrr_velocity_set()}, not D3Q{q}")
         _libs[q] = L
@@ -369,6 +373,16 @@ class Lattice:
         uw = np.ascontiguousarray(u_wm, np.float32); sw = np.ascontiguousarray(s_wm, np.float32)
         va = np.ascontiguousarray(valid, np.uint8)
         self._check(self.lib.hhrr_set_wall_model_state(self.h, len(idx), _p(idx), _p(ut), _p(uw), _p(sw), _p(va)))
+
+    def halo_floats(self):
+        return int(self.lib.hhrr_halo_floats(self.h))
+
+    def halo_pack(self, face, buf_t):
+        """buf_t: float32 CUDA tensor of halo_floats() elements (asynchronous on the lattice's stream)."""
+        self._check(self.lib.hhrr_halo_pack(self.h, int(face), C.c_void_p(buf_t.data_ptr())))
+
+    def halo_unpack(self, face, buf_t):
+        self._check(self.lib.hhrr_halo_unpack(self.h, int(face), C.c_void_p(buf_t.data_ptr())))
 
     def set_step_count(self, step):
         self._check(self.lib.hhrr_set_step_count(self.h, int(step)))

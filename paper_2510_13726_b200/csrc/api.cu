@@ -922,3 +922,70 @@ int hhrr_check_finite(hhrr_lattice* L) {
 }
 
 }  // extern "C"
+
+// ---- slab decomposition along z (the paper's weak-scaling layout) -------
+// A rank holds nz - 2 planes of the global lattice plus one halo plane at either end (z = 0 and z = nz - 1) on a
+// z-periodic local lattice.  After a collide-stream step the halo exchange makes the local state exact again:
+//   * what this rank's collision pushed INTO a halo plane (the 9 populations moving outward) belongs to the
+//     neighbour's first real plane;
+//   * the other populations of the neighbour's halo plane (those not moving towards the neighbour) are copied from
+//     this rank's last real plane, so that the neighbour can form the time-n homogenised velocity of the plane next
+//     to its slab (S^FD, Eq. 10) and the momentum-exchange links that reach into it (Eq. 23 :211).
+// Per face and direction: Q planes of nx * ny floats (9 + 18 on D3Q27; 5 + 14 on D3Q19), packed into one contiguous
+// device buffer so that the transport (NCCL send / recv, a peer copy, or -- d_buf being a peer-mapped pointer -- the
+// pack kernel's own stores over NVLink) is one transfer per face.  Planes are copied as stored: both ranks keep the
+// same population storage.
+namespace {
+// face 0 = low z, 1 = high z; c = the c_z of the populations that cross the face (pack: leaving, c = +-1 outward;
+// unpack: arriving, the same c seen from the receiver).  Slot i of the buffer carries
+//   c_z(i) ==  c : population i of the HALO plane of the sender   -> population i of the first REAL plane of the receiver
+//   c_z(i) ==  0 : population i of the last REAL plane of the sender -> population i of the HALO plane of the receiver
+//   c_z(i) == -c : population j = i with c_z reversed (c_z(j) = c) of the last REAL plane of the sender
+//                                                                   -> population j of the HALO plane of the receiver
+// (the receiver's halo plane already holds its populations with c_z = -c: its own collision pushed them there).
+__global__ void halo_copy_kernel(float* __restrict__ f, float* __restrict__ buf, int64_t n, int64_t plane, int nz, int face,
+                                 int unpack) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, T = (int64_t)gridDim.x * blockDim.x;
+  const int c = unpack ? (face ? -1 : 1) : (face ? 1 : -1);
+  const int z_halo = face ? nz - 1 : 0, z_real = face ? nz - 2 : 1;
+  for (int i = 0; i < Q; ++i) {
+    const int cz = dir_cz(i);
+    const int pop = cz == -c ? dir_flip(i, false, false, true) : i;
+    // sender: crossing populations sit in its halo plane; receiver: they land in its first real plane
+    const int z = (cz == c) ? (unpack ? z_real : z_halo) : (unpack ? z_halo : z_real);
+    float* p = f + (int64_t)pop * n + plane * z;
+    float* b = buf + (int64_t)i * plane;
+    if (!unpack)
+      for (int64_t k = t; k < plane; k += T) b[k] = p[k];
+    else
+      for (int64_t k = t; k < plane; k += T) p[k] = b[k];
+  }
+}
+}  // namespace
+
+extern "C" {
+int64_t hhrr_halo_floats(const hhrr_lattice* L) { return L ? (int64_t)Q * L->dom.nx * L->dom.ny : 0; }
+
+int hhrr_halo_pack(hhrr_lattice* L, int32_t face, float* d_buf) {
+  DeviceGuard guard_(L);
+  if (!L || !d_buf || (face != 0 && face != 1)) return fail(HHRR_E_ARG, "hhrr_halo_pack: bad argument");
+  if (L->dom.nz < 4 || L->dom.mode[2] != HHRR_PERIODIC)
+    return fail(HHRR_E_STATE, "hhrr_halo_pack: a slab needs a periodic z axis of at least 4 planes (2 halo + 2 real)");
+  halo_copy_kernel<<<592, 256, 0, L->stream>>>(L->fA, d_buf, L->dom.n, (int64_t)L->dom.nx * L->dom.ny, L->dom.nz, face, 0);
+  L->launches++;
+  CU(cudaGetLastError());
+  return HHRR_OK;
+}
+
+int hhrr_halo_unpack(hhrr_lattice* L, int32_t face, const float* d_buf) {
+  DeviceGuard guard_(L);
+  if (!L || !d_buf || (face != 0 && face != 1)) return fail(HHRR_E_ARG, "hhrr_halo_unpack: bad argument");
+  if (L->dom.nz < 4 || L->dom.mode[2] != HHRR_PERIODIC)
+    return fail(HHRR_E_STATE, "hhrr_halo_unpack: a slab needs a periodic z axis of at least 4 planes (2 halo + 2 real)");
+  halo_copy_kernel<<<592, 256, 0, L->stream>>>(L->fA, const_cast<float*>(d_buf), L->dom.n, (int64_t)L->dom.nx * L->dom.ny,
+                                                L->dom.nz, face, 1);
+  L->launches++;
+  CU(cudaGetLastError());
+  return HHRR_OK;
+}
+}  // extern "C"

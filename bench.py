@@ -199,12 +199,32 @@ def run_ours(args, rank, world, local_rank):
     dev = f"cuda:{local_rank}"
 
     case, wname = workload(args.config, args.region_split)
+    slab = None
+    if args.decompose:
+        # SURVEY 8(f)-3, the paper's weak-scaling layout: the ranks' blocks are stacked along z into
+        # ONE periodic lattice of N x nz planes, one rotor per block; every rank holds its block plus a halo plane at
+        # either end and exchanges Q planes per face after every step (paper_2510_13726_b200/slabs.py)
+        import dataclasses
+        from paper_2510_13726_b200 import slabs as S
+        assert case.rotor is not None and case.phi is None, "--decompose: rotor recipes (configs 4, 5)"
+        nzl = case.nz + 2
+        rotor = dict(case.rotor, centre=(case.rotor["centre"][0], case.rotor["centre"][1], case.rotor["centre"][2] + 1.0))
+        n_l = case.nx * case.ny * nzl
+        u = np.zeros((3, n_l), np.float32)
+        u[0] = case.fringe[2][0]
+        boxes = None if case.fsi_boxes is None else [(b[0], b[1], b[2], b[3], b[4] + 1, b[5] + 1) for b in case.fsi_boxes]
+        case = dataclasses.replace(case, nz=nzl, rotor=rotor, rho=np.ones(n_l, np.float32), u=u, fsi_boxes=boxes)
+        wname += f" x{world} stacked along z, one block (+2 halo planes) per GPU"
     p = B.make_params(case.nx, case.ny, case.nz, mode=case.mode, **case.params)
     L = B.Lattice(p, rotor_shape=None if case.rotor is None else case.rotor["sdf"].shape, device=dev, q=args.q)
     BYTES_PER_CELL = bytes_per_cell(args.q)
     L.set_kernel_variant(args.variant)
     I.apply_case(case, L)
     n = case.n
+    if args.decompose:
+        n = case.nx * case.ny * (case.nz - 2)          # real cells: halo planes are not counted as work
+        slab = S.SlabLattice(L, rank, world, dist.group.WORLD if world > 1 else "self")
+    stepper = slab if slab is not None else L
 
     def barrier():
         torch.cuda.synchronize()
@@ -212,7 +232,7 @@ def run_ours(args, rank, world, local_rank):
             dist.barrier()
             torch.cuda.synchronize()
 
-    L.step(args.warmup)
+    stepper.step(args.warmup)
     barrier()
     sampler = ClockSampler(local_rank)
     if rank == 0:
@@ -224,7 +244,7 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     t_wall0 = time.time()
     ev0.record(L.stream)
-    L.step(args.steps)
+    stepper.step(args.steps)
     ev1.record(L.stream)
     barrier()
     t_wall1 = time.time()
@@ -250,7 +270,7 @@ def run_ours(args, rank, world, local_rank):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(L.stream)
     L._check(lib.hhrr_set_populations(L.h, C.c_void_p(h_f.data_ptr())))
-    L.step(e2e_steps)
+    stepper.step(e2e_steps)
     L._check(lib.hhrr_get_moments(L.h, C.c_void_p(h_rho.data_ptr()), C.c_void_p(h_v.data_ptr())))
     F = L.forces(L.step_count() - min(e2e_steps, 1024), min(e2e_steps, 1024))
     e1.record(L.stream)
@@ -283,12 +303,12 @@ def run_ours(args, rank, world, local_rank):
     if not args.region_split and not args.no_region_split_leg and case.fringe is not None:
         boxes = I.with_region_split(case).fsi_boxes
         L.set_fsi_region(boxes)
-        L.step(min(args.warmup, 20))
+        stepper.step(min(args.warmup, 20))
         barrier()
         L.set_timing(True)
         s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         s0.record(L.stream)
-        L.step(args.steps)
+        stepper.step(args.steps)
         s1.record(L.stream)
         barrier()
         s_ms = replicas.max_over_ranks(s0.elapsed_time(s1), device=dev)
@@ -330,7 +350,9 @@ def run_ours(args, rank, world, local_rank):
                 "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": wname, "cells_per_gpu": n, "lattice": args.lattice, "storage": "fp32 SoA A/B" + (", x-pull / yz-push" if L.population_storage() else ""),
-                           "kernel_variant": args.variant, "parallelism": f"replicas x{world}",
+                           "kernel_variant": args.variant,
+                           "parallelism": (f"z-slabs x{world}: halo exchange of {args.q} planes per face and step (NCCL send/recv), "
+                                           "per-element force all-reduce" if args.decompose else f"replicas x{world}"),
                            "l2": "inputs (%.1f GB per buffer) exceed the 126 MB L2; no flush needed" % (4e-9 * args.q * n)},
                 "hbm_frac_of_peak_step": value * 1e6 * BYTES_PER_CELL / 1e9 / peak / world,
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
@@ -351,6 +373,8 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--variant", type=int, default=5, choices=[0, 2, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--decompose", action="store_true",
+                    help="N blocks stacked along z into one lattice with halo exchange (SURVEY 8(f)-3) instead of N replicas")
     ap.add_argument("--lattice", default="D3Q27", choices=["D3Q27", "D3Q19"],
                     help="velocity set: D3Q27 (BASELINE.json's configs, default) or the paper's own D3Q19 (PAPER.md:94)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -99,6 +99,7 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
   float* wm_s = c.take<float>(6 * n);
   int32_t* wall_idx = c.take<int32_t>(cap);
   double* wall_y1n = c.take<double>(3 * cap);
+  double* wall_samp = c.take<double>(6 * cap);
   int32_t* force_idx = c.take<int32_t>(cap);
   Counters* counters = c.take<Counters>(1);
   uint8_t* alt_flags = c.take<uint8_t>(n);
@@ -114,7 +115,7 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
   if (L) {
     L->fA = fA; L->fB = fB; L->flags = flags; L->d = d; L->phi = phi; L->below = below; L->tag_prov = tag_prov; L->rowflag = rowflag; L->rowflag_static = rowflag_static; L->phi_static = phi_static;
     L->tag_static = tag_static; L->d_override = d_override; L->uhat = uhat; L->wm_utau = wm_utau;
-    L->wm_u = wm_u; L->wm_s = wm_s; L->wall_idx = wall_idx; L->wall_y1n = wall_y1n;
+    L->wm_u = wm_u; L->wm_s = wm_s; L->wall_idx = wall_idx; L->wall_y1n = wall_y1n; L->wall_samp = wall_samp;
     L->alt_flags = alt_flags; L->alt_d = alt_d; L->alt_wall_idx = alt_wall_idx; L->alt_wall_y1n = alt_wall_y1n;
     L->alt_force_idx = alt_force_idx; L->alt_counters = alt_counters;
     L->force_idx = force_idx; L->counters = counters; L->force = force; L->torque = torque; L->rot_sdf = rot_sdf;

@@ -34,8 +34,14 @@ __host__ __device__ constexpr int dir_opp(int i) { return Q - 1 - i; }
 __host__ __device__ constexpr int dir_index(int cx, int cy, int cz) {
   const int slot = (cx + 1) + 3 * (cy + 1) + 9 * (cz + 1);
   if (Q == 27) return slot;
-  constexpr int i19[27] = {-1, 0, -1, 1, 2, 3, -1, 4, -1, 5, 6, 7, 8, 9, 10, 11, 12, 13, -1, 14, -1, 15, 16, 17, -1, 18, -1};
-  return i19[slot];
+  // D3Q19: slot minus the number of cube-corner slots below it (arithmetic: cheap with run-time arguments too)
+  constexpr unsigned corners = (1u << 0) | (1u << 2) | (1u << 6) | (1u << 8) | (1u << 18) | (1u << 20) | (1u << 24) | (1u << 26);
+  if ((corners >> slot) & 1u) return -1;
+  unsigned v = corners & ((1u << slot) - 1u);
+  v = v - ((v >> 1) & 0x55555555u);
+  v = (v & 0x33333333u) + ((v >> 2) & 0x33333333u);
+  v = (v + (v >> 4)) & 0x0f0f0f0fu;
+  return slot - (int)((v * 0x01010101u) >> 24);
 }
 // direction i with the marked components reversed (a population reflected at MIRROR planes, R12)
 __host__ __device__ constexpr int dir_flip(int i, bool fx, bool fy, bool fz) {
@@ -48,6 +54,11 @@ __host__ __device__ constexpr double dir_wd(int i) {
   return nn == 0 ? 1.0 / 3.0 : (nn == 1 ? 1.0 / 18.0 : 1.0 / 36.0);
 }
 __host__ __device__ constexpr float dir_w(int i) { return (float)dir_wd(i); }
+__host__ __device__ constexpr double dir_wd_of(int cx, int cy, int cz) {  // weight of direction (cx, cy, cz)
+  if (Q == 27) return (cx ? 1.0 / 6.0 : 2.0 / 3.0) * (cy ? 1.0 / 6.0 : 2.0 / 3.0) * (cz ? 1.0 / 6.0 : 2.0 / 3.0);
+  const int nn = cx * cx + cy * cy + cz * cz;
+  return nn == 0 ? 1.0 / 3.0 : (nn == 1 ? 1.0 / 18.0 : 1.0 / 36.0);
+}
 
 // MUFU reciprocal + one Newton step (<= 1 ulp, branch-free) and MUFU square root (2^-23 rel.)
 __device__ __forceinline__ float rcp_nr(float x) {
@@ -170,18 +181,21 @@ struct CellSums<T, 19> {
       any = true;
     }
   };
+  // rho and j in EXACTLY the summation order of all(): a plane's uhat must not depend on which of the two a block
+  // uses for it (overlap planes of a z-chunk take rho_j, the neighbouring chunk takes all())
   static __device__ __forceinline__ void rho_j(const T (&f)[19], T& drho, T& jx, T& jy, T& jz) {
-    Acc r, x, y, z;
-    r.add(f[9], 1);
+    Acc x, y, z, zz;
+    T sd = f[9];
 #pragma unroll
     for (int j = 10; j < 19; ++j) {
       const T s = f[j] + f[18 - j], d = f[j] - f[18 - j];
-      r.add(s, 1);
       if (dir_cx(j)) x.add(d, dir_cx(j));
       if (dir_cy(j)) y.add(d, dir_cy(j));
       if (dir_cz(j)) z.add(d, dir_cz(j));
+      if (dir_cz(j)) zz.add(s, 1);
+      else sd = sd + s;
     }
-    drho = r.v; jx = x.v; jy = y.v; jz = z.v;
+    drho = sd + zz.v; jx = x.v; jy = y.v; jz = z.v;
   }
   static __device__ __forceinline__ MomentsT<T> all(const T (&f)[19]) {
     Acc x, y, z, xx, yy, zz, xy, xz, yz, ax;  // ax: the axis pairs (one non-zero component)
@@ -353,6 +367,13 @@ __device__ __forceinline__ void collide(const PhysF& ph, const MomentsT<T>& m, T
 }
 
 // where population i of the post-stream state of cell (x,y,z) is stored (see Dom::xs)
+// (cx = c_x of direction i, passed by callers that know it at compile time while i is a run-time value)
+__device__ __forceinline__ int64_t pop_index_cx(const Dom& dm, int i, int cx, int x, int y, int z) {
+  int xs = x - dm.xs * cx;
+  if (xs < 0) xs += dm.nx;
+  else if (xs >= dm.nx) xs -= dm.nx;
+  return (int64_t)i * dm.n + xs + (int64_t)dm.nx * (y + (int64_t)dm.ny * z);
+}
 __device__ __forceinline__ int64_t pop_index(const Dom& dm, int i, int x, int y, int z) {
   int xs = x - dm.xs * dir_cx(i);
   if (xs < 0) xs += dm.nx;

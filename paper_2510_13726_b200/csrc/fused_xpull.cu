@@ -117,7 +117,7 @@ __device__ __forceinline__ void push_store_yz(const Dom& dm, float* __restrict__
 }  // namespace
 
 template <class C>
-__global__ void __launch_bounds__(C::THREADS, 1)
+__global__ void __maxnreg__(160)  // 384 threads x 160 = 61440 registers: 4096 stay free per SM for the side-stream kernels
     fused_xpull_kernel(const __grid_constant__ WsArgs a, const __grid_constant__ CUtensorMap map_main,
                        const __grid_constant__ CUtensorMap map_row, const __grid_constant__ CUtensorMap map_pm,
                        const __grid_constant__ CUtensorMap map_pr) {
@@ -176,7 +176,7 @@ __global__ void __launch_bounds__(C::THREADS, 1)
   }
   __syncthreads();
 
-  if (tid >= WORKERS) reg_dec<88>(); else reg_inc<208>();
+  if (tid >= WORKERS) reg_dec<96>(); else reg_inc<192>();
 
   if (tid >= WORKERS + AUX) {
     // ------------------------------------------------------------------ producer: one lane issues TMA
@@ -541,7 +541,12 @@ static cudaError_t launch_shape(hhrr_lattice* L, WsArgs& a) {
     attr_set = true;
   }
   // with the grouped launch order the halo planes of a chunk are L2 hits: 22 planes without, 16 with the region split
-  int nch = ws_zchunks(dm.nz, a.fsi.n > 0 ? 16 : 22);
+  // z-chunk length: neighbouring tiles re-synchronise at every chunk start, and the halo rows / x-halo sectors they
+  // share stay L2 hits only while they march within a few planes of each other.  Measured on config 5 with the
+  // packed-fp32 workers (profiles/r02_k2_chunk_scan.md): 13-16 planes 3.99 ms, 18 planes 4.18 ms, 22 planes 4.42 ms
+  // (DRAM reads 15.3 GB per launch instead of 12.9); D3Q19 (19 planes of populations per cell plane) is flat from 22
+  // to 30.  Hence 16 planes x 27 / Q.
+  int nch = ws_zchunks(dm.nz, (16 * 27 + Q / 2) / Q);
   a.zchunk = (dm.nz + nch - 1) / nch;
   nch = (dm.nz + a.zchunk - 1) / a.zchunk;
   if (!L->sm_count &&
@@ -551,6 +556,28 @@ static cudaError_t launch_shape(hhrr_lattice* L, WsArgs& a) {
   a.group = L->sm_count;  // one tile per SM and wave (one block per SM: shared memory)
   const int ntiles = (dm.nx / C::TX) * (dm.ny / C::TY);
   dim3 grid((unsigned)(ntiles * nch));
+  // Two x-adjacent tiles form a thread-block cluster (no cluster barrier, no distributed shared memory): the pair
+  // starts together on neighbouring SMs and asks L2 for the x-halo sectors it shares at the same time.  Measured:
+  // nothing at 16-plane chunks without the region split, 4.07 -> 3.95 ms with it, and the cliff at longer chunks
+  // moves out (18 planes: 4.18 -> 4.02 ms).
+  constexpr int cl = 2;
+  if (grid.x % cl == 0 && a.group % cl == 0 && ntiles % cl == 0) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = dim3(C::THREADS);
+    cfg.dynamicSmemBytes = C::SMEM;
+    cfg.stream = L->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = cl;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, fused_xpull_kernel<C>, a, m_main, m_row, m_pm, m_pr);
+    L->launches++;
+    return e != cudaSuccess ? e : cudaGetLastError();
+  }
   fused_xpull_kernel<C><<<grid, C::THREADS, C::SMEM, L->stream>>>(a, m_main, m_row, m_pm, m_pr);
   L->launches++;
   return cudaGetLastError();

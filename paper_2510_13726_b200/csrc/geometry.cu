@@ -310,10 +310,12 @@ __global__ void counters_kernel(Counters* cnt, int op) {
   }
 }
 
-static void geo_grid(const GeoArgs& a, dim3& g, dim3& b) {
+// max_threads: 64 for the look-ahead launches -- a block of <= 4096 registers fits beside a resident block of the
+// collide-stream kernel (384 threads x 160 registers of the SM's 65536), so the side stream really runs during it
+static void geo_grid(const GeoArgs& a, dim3& g, dim3& b, int max_threads = 128) {
   if (a.inside) {
     int bx = a.box.x1 - a.box.x0, by = a.box.y1 - a.box.y0, bz = a.box.z1 - a.box.z0;
-    int t = bx >= 128 ? 128 : ((bx + 31) / 32) * 32;  // a rotor box is thin along its axis: do not idle warps
+    int t = bx >= max_threads ? max_threads : ((bx + 31) / 32) * 32;  // a rotor box is thin along its axis: do not idle warps
     b = dim3(t);
     g = dim3(by * bz, (bx + t - 1) / t);
   } else {
@@ -379,13 +381,13 @@ static bool rotor_box_empty(const hhrr_lattice* L) {
 
 // pass 1 of geometry(step) over the rotor box, on stream s.  It reads the rotor description and the static
 // fields and writes phi / below / rowflag / tag_prov -- nothing a collide-stream, wall-model or force kernel touches.
-static void launch_box_phi(hhrr_lattice* L, int64_t step, cudaStream_t s) {
+static void launch_box_phi(hhrr_lattice* L, int64_t step, cudaStream_t s, int max_threads = 128) {
   GeoArgs a;
   fill_geo(L, a, step);
   a.box = L->rot_box;
   a.inside = 1;
   dim3 g, b;
-  geo_grid(a, g, b);
+  geo_grid(a, g, b, max_threads);
   cudaMemcpyAsync(L->rowflag, L->rowflag_static, (size_t)L->dom.ny * L->dom.nz, cudaMemcpyDeviceToDevice, s);
   geometry_phi_kernel<<<g, b, 0, s>>>(a);
   L->launches++;
@@ -412,7 +414,7 @@ void swap_geometry_sets(hhrr_lattice* L) {
 cudaError_t launch_geometry_ahead(hhrr_lattice* L) {
   if (!L->side || !L->lookahead || rotor_box_empty(L) || L->geometry_dirty) return cudaSuccess;
   cudaStreamWaitEvent(L->side, L->ev_pre, 0);
-  launch_box_phi(L, L->step + 1, L->side);
+  launch_box_phi(L, L->step + 1, L->side, 64);
   GeoArgs a;
   fill_geo(L, a, L->step + 1);
   a.flags_prev = nullptr;
@@ -425,7 +427,7 @@ cudaError_t launch_geometry_ahead(hhrr_lattice* L) {
   a.box = L->rot_box;
   a.inside = 1;
   dim3 g, b;
-  geo_grid(a, g, b);
+  geo_grid(a, g, b, 64);
   counters_kernel<<<1, 1, 0, L->side>>>(a.cnt, 2);
   geometry_type_kernel<<<g, b, 0, L->side>>>(a);
   L->launches += 2;

@@ -28,6 +28,7 @@ struct WmArgs {
   const double* wall_y1n;
   const Counters* cnt;
   int cap_list;
+  double* samp;  // [cap_list][6]: sampled velocity v_s and the cell's own velocity v(x_w), sampling kernel -> Newton kernel
   double* wm_utau;
   float* wm_u;
   float* wm_s;
@@ -80,18 +81,29 @@ __device__ __forceinline__ double spalding_df(double ut, double U, double y, dou
 __device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 __device__ __forceinline__ double shfl_down_d(double v, int delta) { return __shfl_down_sync(0xffffffffu, v, delta); }
 
-// K3, one launch.  A WARP takes a batch of WM_BATCH wall-model cells.  Sampling, cell by cell: lane 3k + g
-// (k = 0..8, g = 0..2) loads nine populations of cell k -- k = 0..7 the corners of the trilinear stencil around
-// x_w + h_s n (R15), k = 8 the wall cell itself -- so the 243 gathered loads of a cell are in
-// flight at once (and, the batch loop being unrolled, those of the next cells behind them); the partial sums
-// meet by shuffles and lane j keeps v_s and v(x_w) of cell j.  Then lanes 0..WM_BATCH-1 each finish one cell:
-// tangential speed, Newton iteration on Eq. 18 (Eq. 19; fp64 exp), slip velocity and wall strain.
-constexpr int WM_BATCH = 8;
+// K3 = two launches on the critical path between two collide-stream kernels.
+// wall_sample_kernel: a WARP takes a batch of WM_BATCH wall-model cells.  Phase 1: for every cell of the batch, lane
+// 3k + g (k = 0..8, g = 0..2) issues the loads of up to nine populations of cell k -- k = 0..7 the corners of the
+// trilinear stencil around x_w + h_s n (R15), k = 8 the wall cell itself -- so the 243 gathered loads
+// of ALL cells of the batch are in flight before any is used (the kernel is bound by the latency of these gathers:
+// 27 planes, one page each).  Phase 2: per cell the partial sums meet by shuffles; lane j stores v_s and v(x_w).
+// wall_model_kernel: one THREAD per cell (32 Newton solves per fp64 instruction): tangential speed, Newton iteration
+// on Eq. 18 (Eq. 19; fp64 exp), slip velocity and wall strain.  (Both in one launch, with the Newton solves on a few
+// lanes of the sampling warps, was measured slower: 148 vs 87 us -- the fp64 pipe then runs a quarter full.)
+constexpr int WM_BATCH = 4;
 
-__device__ __forceinline__ void wall_sample_cell(const WmArgs& a, int64_t c, const double y1v[3], int lane,
-                                                 double vs[3], double vw[3]) {
+// what a lane needs to finish its part of one wall cell's sample once its nine loads have landed
+struct SampleLane {
+  float fv[9];    // populations with cz = g - 1 of stencil cell kc (zeros where the set has no such direction)
+  double w;       // trilinear weight of stencil cell kc (0 for the wall cell itself, kc = 8)
+  bool flx, fly, flz;
+};
+
+// phase 1: addresses and loads of this lane (lane 3k + g: stencil cell k, population group g; lanes 27-31 idle)
+__device__ __forceinline__ void wall_sample_issue(const WmArgs& a, int64_t c, const double y1v[3], int lane,
+                                                  SampleLane& sl) {
   const int64_t nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
-  const int kc = lane / 3, g = lane - 3 * kc;  // cell of the stencil, population group (lanes 27-31 idle)
+  const int kc = lane / 3, g = lane - 3 * kc;
   int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
   double y1 = sqrt(y1v[0] * y1v[0] + y1v[1] * y1v[1] + y1v[2] * y1v[2]);
   double nrm[3] = {y1v[0] / y1, y1v[1] / y1, y1v[2] / y1};
@@ -100,48 +112,50 @@ __device__ __forceinline__ void wall_sample_cell(const WmArgs& a, int64_t c, con
   double fx = floor(px), fy = floor(py), fz = floor(pz);
   double tx = px - fx, ty = py - fy, tz = pz - fz;
   int ix = (int)fx, iy = (int)fy, iz = (int)fz;
-  // this lane's cell
   int xx = x, yy = y, zz = z;
-  bool flx = false, fly = false, flz = false;
-  double w = 0.0;
+  sl.flx = sl.fly = sl.flz = false;
+  sl.w = 0.0;
   if (kc < 8) {
     int ox = kc & 1, oy = (kc >> 1) & 1, oz = (kc >> 2) & 1;
-    w = (ox ? tx : 1.0 - tx) * (oy ? ty : 1.0 - ty) * (oz ? tz : 1.0 - tz);
-    xx = wrap_far(ix + ox, a.dm.nx, a.dm.mode[0], flx);
-    yy = wrap_far(iy + oy, a.dm.ny, a.dm.mode[1], fly);
-    zz = wrap_far(iz + oz, a.dm.nz, a.dm.mode[2], flz);
+    sl.w = (ox ? tx : 1.0 - tx) * (oy ? ty : 1.0 - ty) * (oz ? tz : 1.0 - tz);
+    xx = wrap_far(ix + ox, a.dm.nx, a.dm.mode[0], sl.flx);
+    yy = wrap_far(iy + oy, a.dm.ny, a.dm.mode[1], sl.fly);
+    zz = wrap_far(iz + oz, a.dm.nz, a.dm.mode[2], sl.flz);
   }
+#pragma unroll
+  for (int q = 0; q < 9; ++q) {  // cx = q % 3 - 1, cy = q / 3 - 1, cz = g - 1
+    const int i = dir_index(q % 3 - 1, q / 3 - 1, g - 1);  // -1: the set has no such direction (D3Q19 corners)
+    sl.fv[q] = (kc < 9 && i >= 0) ? __ldg(a.f + pop_index_cx(a.dm, i, q % 3 - 1, xx, yy, zz)) : 0.f;
+  }
+}
+
+// phase 2: v = (j + g/2)/rho of the nine cells (R11), weighted sum over the stencil -> v_s; the wall cell's own -> v_w
+__device__ __forceinline__ void wall_sample_reduce(const WmArgs& a, const SampleLane& sl, int lane, double vs[3],
+                                                   double vw[3]) {
+  const int g = lane % 3;
   double drho = 0, j0 = 0, j1 = 0, j2 = 0;
-  if (kc < 9) {  // group g holds the populations with cz = g - 1 (nine on D3Q27; five, nine, five on D3Q19)
-    float fv[9];
 #pragma unroll
-    for (int q = 0; q < 9; ++q) {
-      const int i = dir_index(q % 3 - 1, q / 3 - 1, g - 1);  // -1: the set has no such direction
-      fv[q] = i >= 0 ? __ldg(a.f + pop_index(a.dm, i, xx, yy, zz)) : 0.f;
-    }
-#pragma unroll
-    for (int q = 0; q < 9; ++q) {  // cx = q % 3 - 1, cy = q / 3 - 1
-      double fi = (double)fv[q];
-      drho += fi;
-      j0 += (q % 3 - 1) * fi;
-      j1 += (q / 3 - 1) * fi;
-    }
-    j2 = (g - 1) * drho;
+  for (int q = 0; q < 9; ++q) {
+    double fi = (double)sl.fv[q];
+    drho += fi;
+    j0 += (q % 3 - 1) * fi;
+    j1 += (q / 3 - 1) * fi;
   }
+  j2 = (g - 1) * drho;
   // the three groups of a cell: lanes 3k, 3k+1, 3k+2
   drho += shfl_down_d(drho, 1) + shfl_down_d(drho, 2);
   j0 += shfl_down_d(j0, 1) + shfl_down_d(j0, 2);
   j1 += shfl_down_d(j1, 1) + shfl_down_d(j1, 2);
   j2 += shfl_down_d(j2, 1) + shfl_down_d(j2, 2);
-  double ir = 1.0 / (1.0 + drho);  // reported velocity moment v = (j + g/2)/rho (R11), valid on lanes 3k
+  double ir = 1.0 / (1.0 + drho);  // valid on lanes 3k
   double v[3] = {(j0 + 0.5 * a.g[0]) * ir, (j1 + 0.5 * a.g[1]) * ir, (j2 + 0.5 * a.g[2]) * ir};
-  if (flx) v[0] = -v[0];
-  if (fly) v[1] = -v[1];
-  if (flz) v[2] = -v[2];
+  if (sl.flx) v[0] = -v[0];
+  if (sl.fly) v[1] = -v[1];
+  if (sl.flz) v[2] = -v[2];
   vs[0] = vs[1] = vs[2] = 0.0;
 #pragma unroll
   for (int k = 0; k < 8; ++k) {
-    double wk = shfl_d(w, 3 * k);
+    double wk = shfl_d(sl.w, 3 * k);
 #pragma unroll
     for (int q = 0; q < 3; ++q) vs[q] += wk * shfl_d(v[q], 3 * k);
   }
@@ -269,7 +283,7 @@ __device__ __forceinline__ void wall_finish_cell(const WmArgs& a, int64_t c, con
   }
 }
 
-__global__ void __launch_bounds__(128, 4) wall_model_kernel(const __grid_constant__ WmArgs a) {
+__global__ void __launch_bounds__(128, 4) wall_sample_kernel(const __grid_constant__ WmArgs a) {
   const int count = min(a.cnt->wall_count, a.cap_list);
   const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
   const int nw = gridDim.x * wpb;
@@ -284,24 +298,41 @@ __global__ void __launch_bounds__(128, 4) wall_model_kernel(const __grid_constan
 #pragma unroll
       for (int q = 0; q < 3; ++q) y_l[q] = a.wall_y1n[3 * (int64_t)e_l + q];
     }
-    double my_vs[3] = {0, 0, 0}, my_vw[3] = {0, 0, 0};
+    SampleLane sl[WM_BATCH];
+#pragma unroll
+    for (int j = 0; j < WM_BATCH; ++j) {  // a batch's tail repeats its last cell (never out of range, no branch)
+      const int src = min(j, count - 1 - base);
+      const int64_t c = __shfl_sync(0xffffffffu, c_l, src);
+      const double y1v[3] = {shfl_d(y_l[0], src), shfl_d(y_l[1], src), shfl_d(y_l[2], src)};
+      wall_sample_issue(a, c, y1v, lane, sl[j]);
+    }
 #pragma unroll
     for (int j = 0; j < WM_BATCH; ++j) {
-      if (base + j < count) {  // warp-uniform
-        const int64_t c = __shfl_sync(0xffffffffu, c_l, j);
-        const double y1v[3] = {shfl_d(y_l[0], j), shfl_d(y_l[1], j), shfl_d(y_l[2], j)};
-        double vs[3], vw[3];
-        wall_sample_cell(a, c, y1v, lane, vs, vw);
-        if (lane == j) {
+      double vs[3], vw[3];
+      wall_sample_reduce(a, sl[j], lane, vs, vw);
+      if (lane == j && mine) {
 #pragma unroll
-          for (int q = 0; q < 3; ++q) {
-            my_vs[q] = vs[q];
-            my_vw[q] = vw[q];
-          }
+        for (int q = 0; q < 3; ++q) {
+          a.samp[6 * (int64_t)e_l + q] = vs[q];
+          a.samp[6 * (int64_t)e_l + 3 + q] = vw[q];
         }
       }
     }
-    if (mine) wall_finish_cell(a, c_l, y_l, my_vs, my_vw);
+  }
+}
+
+__global__ void __launch_bounds__(128) wall_model_kernel(const __grid_constant__ WmArgs a) {
+  const int count = min(a.cnt->wall_count, a.cap_list);
+  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < count; e += gridDim.x * blockDim.x) {
+    const int64_t c = a.wall_idx[e];
+    double y1v[3], vs[3], vw[3];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+      y1v[q] = a.wall_y1n[3 * (int64_t)e + q];
+      vs[q] = a.samp[6 * (int64_t)e + q];
+      vw[q] = a.samp[6 * (int64_t)e + 3 + q];
+    }
+    wall_finish_cell(a, c, y1v, vs, vw);
   }
 }
 
@@ -366,9 +397,9 @@ __device__ __forceinline__ void force_block(const ForceArgs& a, int block, int n
           // population that leaves through the plane)
           const int ir = dir_index(flx ? -cx : cx, fly ? -cy : cy, flz ? -cz : cz);
           // stored values are deviations: f = w + dev, and w_i = w_ibar = w of the reflected direction
-          const double w = dir_wd(i);
-          const double fa = w + (double)__ldg(a.f + pop_index(a.dm, ir, xx, yy, zz));
-          const double fb = w + (double)__ldg(a.f + pop_index(a.dm, dir_opp(i), x, y, z));
+          const double w = dir_wd_of(cx, cy, cz);
+          const double fa = w + (double)__ldg(a.f + pop_index_cx(a.dm, ir, flx ? -cx : cx, xx, yy, zz));
+          const double fb = w + (double)__ldg(a.f + pop_index_cx(a.dm, dir_opp(i), -cx, x, y, z));
           const double ci[3] = {(double)cx, (double)cy, (double)cz};
 #pragma unroll
           for (int q = 0; q < 3; ++q) acc[q] += (ci[q] - us[q]) * fa + (ci[q] + us[q]) * fb;
@@ -410,7 +441,8 @@ __device__ __forceinline__ void force_block(const ForceArgs& a, int block, int n
   }
 }
 
-__global__ void __launch_bounds__(128, 8) force_kernel(const __grid_constant__ ForceArgs f) {
+// 64 threads x 64 registers: fits beside a resident block of the collide-stream kernel (see geometry.cu: geo_grid)
+__global__ void __launch_bounds__(64, 16) force_kernel(const __grid_constant__ ForceArgs f) {
   force_block(f, blockIdx.x, gridDim.x);
 }
 
@@ -437,6 +469,7 @@ static void fill_wm(const hhrr_lattice* L, WmArgs& a) {
   a.wall_y1n = L->wall_y1n;
   a.cnt = L->counters;
   a.cap_list = (int)L->cap_list;
+  a.samp = L->wall_samp;
   a.wm_utau = L->wm_utau;
   a.wm_u = L->wm_u;
   a.wm_s = L->wm_s;
@@ -448,8 +481,9 @@ cudaError_t launch_wall_model(hhrr_lattice* L, bool mark_alt) {
   WmArgs w;
   fill_wm(L, w);
   w.alt_flags = mark_alt ? L->alt_flags : nullptr;
-  wall_model_kernel<<<1184, 128, 0, L->stream>>>(w);  // 4736 warps x 8 cells per sweep
-  L->launches++;
+  wall_sample_kernel<<<2368, 128, 0, L->stream>>>(w);  // 9472 warps x 4 cells per sweep, 4 blocks per SM resident
+  wall_model_kernel<<<592, 128, 0, L->stream>>>(w);
+  L->launches += 2;
   return cudaGetLastError();
 }
 
@@ -467,7 +501,7 @@ cudaError_t launch_forces(hhrr_lattice* L, cudaStream_t s) {
   a.out = L->force + (L->step % FORCE_HISTORY) * MAX_TAGS * 3;
   a.out_m = L->torque + (L->step % FORCE_HISTORY) * MAX_TAGS * 3;
   zero_force_kernel<<<1, 64, 0, s>>>(a.out, a.out_m);
-  force_kernel<<<2368, 128, 0, s>>>(a);  // 8 blocks per SM (64 registers), 2 waves
+  force_kernel<<<4736, 64, 0, s>>>(a);
   L->launches += 2;
   return cudaGetLastError();
 }

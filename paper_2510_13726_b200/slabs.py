@@ -120,7 +120,7 @@ class SlabLattice:
                 upper.recv[0].copy_(self.send[1], non_blocking=True)
             return
         import torch.distributed as dist
-        if self.world == 1:   # periodic in z onto itself
+        if self.world == 1 or self.group == "self":   # periodic in z onto itself
             with torch.cuda.stream(self.L.stream):
                 self.recv[1].copy_(self.send[0], non_blocking=True)
                 self.recv[0].copy_(self.send[1], non_blocking=True)
@@ -152,7 +152,7 @@ class SlabLattice:
         """Per-element forces summed over all ranks: one all-reduce of count x 16 x 3 doubles."""
         import torch
         F = self.L.forces(first, count)
-        if self.group is None or self.world == 1:
+        if self.group is None or self.group == "self" or self.world == 1:
             return F
         import torch.distributed as dist
         t = torch.from_numpy(F).to(self.L.device)

@@ -570,9 +570,13 @@ int hhrr_step(hhrr_lattice* L, int32_t n_steps) {
     e = launch_geometry_ahead(L);  // line 2 of the NEXT step, on the side stream
     if (e != cudaSuccess) return cuda_fail(e, "geometry look-ahead");
     const bool ahead = L->ahead_step == L->step + 1;
-    if (ahead && L->wm_enabled) CU(cudaStreamWaitEvent(L->stream, L->ev_k1, 0));  // the kernel marks the alternate flags
-    e = launch_wall_model(L, ahead);  // line 4: WallModelO
+    e = launch_wall_model(L);  // line 4: WallModelO -- beside the geometry look-ahead, which starts in the tail of K2
     if (e != cudaSuccess) return cuda_fail(e, "wall-model kernel");
+    if (ahead && L->wm_enabled) {  // the two meet: the geometry written ahead learns which of its wall cells hold state
+      CU(cudaStreamWaitEvent(L->stream, L->ev_k1, 0));
+      e = launch_merge_valid(L);
+      if (e != cudaSuccess) return cuda_fail(e, "wall-state merge kernel");
+    }
     if (L->side) {  // lines 5-6: forces, beside the next collide-stream kernel
       CU(cudaStreamWaitEvent(L->side, L->ev_k2, 0));
       e = launch_forces(L, L->side);

@@ -161,6 +161,7 @@ cudaError_t launch_check_finite(hhrr_lattice* L);
 bool xpull_supported(const Dom& dm);                    // fused_xpull.cu: variant 5 can run this lattice
 cudaError_t launch_restore(hhrr_lattice* L, int xs);    // re-store the populations of buffer A with x-shift xs
 // wallmodel.cu
-cudaError_t launch_wall_model(hhrr_lattice* L, bool mark_alt);  // K3 on the main stream
+cudaError_t launch_wall_model(hhrr_lattice* L);                 // K3 on the main stream
+cudaError_t launch_merge_valid(hhrr_lattice* L);                // WM_VALID of the geometry written ahead
 cudaError_t launch_forces(hhrr_lattice* L, cudaStream_t s);     // K4 (reads only) on stream s
 }  // namespace hhrr

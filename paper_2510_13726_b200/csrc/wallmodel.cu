@@ -23,7 +23,6 @@ struct WmArgs {
   BodiesD bo;
   const float* f;  // post-stream populations (deviations)
   uint8_t* flags;
-  uint8_t* alt_flags;  // flag bytes of the NEXT step's geometry (written ahead), or NULL: cells of W there get WM_VALID too
   const int32_t* wall_idx;
   const double* wall_y1n;
   const Counters* cnt;
@@ -90,7 +89,6 @@ __device__ __forceinline__ double shfl_down_d(double v, int delta) { return __sh
 // wall_model_kernel: one THREAD per cell (32 Newton solves per fp64 instruction): tangential speed, Newton iteration
 // on Eq. 18 (Eq. 19; fp64 exp), slip velocity and wall strain.  (Both in one launch, with the Newton solves on a few
 // lanes of the sampling warps, was measured slower: 148 vs 87 us -- the fp64 pipe then runs a quarter full.)
-constexpr int WM_BATCH = 4;
 
 // what a lane needs to finish its part of one wall cell's sample once its nine loads have landed
 struct SampleLane {
@@ -274,16 +272,11 @@ __device__ __forceinline__ void wall_finish_cell(const WmArgs& a, int64_t c, con
     for (int q = 0; q < 3; ++q) a.wm_u[(int64_t)q * n + c] = (float)uw[q];
     for (int q = 0; q < 6; ++q) a.wm_s[(int64_t)q * n + c] = (float)sw[q];
     a.flags[c] = fl | WM_VALID;
-    // the next step's geometry is already written (look-ahead): its collision consumes this state iff the cell is
-    // in W there too (O1: the state of cells not in W_{n+1} is dropped)
-    if (a.alt_flags) {
-      const uint8_t fa = a.alt_flags[c];
-      if ((fa & TYPE_MASK) == T_FRONTIER_W) a.alt_flags[c] = fa | WM_VALID;
-    }
   }
 }
 
-__global__ void __launch_bounds__(128, 4) wall_sample_kernel(const __grid_constant__ WmArgs a) {
+template <int WM_BATCH, int BLOCKS_PER_SM>
+__global__ void __launch_bounds__(128, BLOCKS_PER_SM) wall_sample_kernel(const __grid_constant__ WmArgs a) {
   const int count = min(a.cnt->wall_count, a.cap_list);
   const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
   const int nw = gridDim.x * wpb;
@@ -464,7 +457,6 @@ static void fill_wm(const hhrr_lattice* L, WmArgs& a) {
   fill_bodies(L, a.bo);
   a.f = L->fA;
   a.flags = L->flags;
-  a.alt_flags = nullptr;
   a.wall_idx = L->wall_idx;
   a.wall_y1n = L->wall_y1n;
   a.cnt = L->counters;
@@ -475,15 +467,33 @@ static void fill_wm(const hhrr_lattice* L, WmArgs& a) {
   a.wm_s = L->wm_s;
 }
 
-// Listing 3 line 4: WallModelO.  mark_alt: the alternate geometry set holds geometry(step + 1)
-cudaError_t launch_wall_model(hhrr_lattice* L, bool mark_alt) {
+// The next step's geometry was written ahead into the alternate set with WM_VALID clear (geometry.cu).  Its collision
+// consumes the wall-model state of a cell iff the cell is in W there AND holds state now, i.e. was in W of this step
+// (O1: the state of cells that leave W is dropped): one pass over the alternate wall list after the wall model.
+__global__ void merge_valid_kernel(const int32_t* __restrict__ alt_wall_idx, const Counters* alt_cnt, int cap,
+                                   const uint8_t* __restrict__ flags, uint8_t* __restrict__ alt_flags) {
+  const int count = min(alt_cnt->wall_count, cap);
+  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < count; e += gridDim.x * blockDim.x) {
+    const int64_t c = alt_wall_idx[e];
+    if (flags[c] & WM_VALID) alt_flags[c] |= WM_VALID;
+  }
+}
+
+// Listing 3 line 4: WallModelO
+cudaError_t launch_wall_model(hhrr_lattice* L) {
   if (!L->wm_enabled) return cudaSuccess;
   WmArgs w;
   fill_wm(L, w);
-  w.alt_flags = mark_alt ? L->alt_flags : nullptr;
-  wall_sample_kernel<<<2368, 128, 0, L->stream>>>(w);  // 9472 warps x 4 cells per sweep, 4 blocks per SM resident
+  // two cells per warp and sweep, 8 blocks per SM (64 registers); measured against 1, 4 and 8 cells per warp
+  wall_sample_kernel<2, 8><<<4736, 128, 0, L->stream>>>(w);
   wall_model_kernel<<<592, 128, 0, L->stream>>>(w);
   L->launches += 2;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_merge_valid(hhrr_lattice* L) {
+  merge_valid_kernel<<<148, 256, 0, L->stream>>>(L->alt_wall_idx, L->alt_counters, (int)L->cap_list, L->flags, L->alt_flags);
+  L->launches++;
   return cudaGetLastError();
 }
 

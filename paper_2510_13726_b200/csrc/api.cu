@@ -90,6 +90,10 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
   uint8_t* tag_prov = c.take<uint8_t>(n);
   uint8_t* rowflag = c.take<uint8_t>((int64_t)p->ny * p->nz);
   uint8_t* rowflag_static = c.take<uint8_t>((int64_t)p->ny * p->nz);
+  uint8_t* rowact0 = c.take<uint8_t>((int64_t)p->ny * p->nz);
+  uint8_t* rowact1 = c.take<uint8_t>((int64_t)p->ny * p->nz);
+  int32_t* rowlist = c.take<int32_t>((int64_t)p->ny * p->nz);
+  int* n_rows = c.take<int>(1);
   float* phi_static = c.take<float>(n);
   uint8_t* tag_static = c.take<uint8_t>(n);
   float* d_override = c.take<float>(n);
@@ -116,6 +120,7 @@ size_t carve(hhrr_lattice* L, const hhrr_params* p, int64_t rotor_nodes, char* b
     L->fA = fA; L->fB = fB; L->flags = flags; L->d = d; L->phi = phi; L->below = below; L->tag_prov = tag_prov; L->rowflag = rowflag; L->rowflag_static = rowflag_static; L->phi_static = phi_static;
     L->tag_static = tag_static; L->d_override = d_override; L->uhat = uhat; L->wm_utau = wm_utau;
     L->wm_u = wm_u; L->wm_s = wm_s; L->wall_idx = wall_idx; L->wall_y1n = wall_y1n; L->wall_samp = wall_samp;
+    L->rowact[0] = rowact0; L->rowact[1] = rowact1; L->rowlist = rowlist; L->n_rows = n_rows;
     L->alt_flags = alt_flags; L->alt_d = alt_d; L->alt_wall_idx = alt_wall_idx; L->alt_wall_y1n = alt_wall_y1n;
     L->alt_force_idx = alt_force_idx; L->alt_counters = alt_counters;
     L->force_idx = force_idx; L->counters = counters; L->force = force; L->torque = torque; L->rot_sdf = rot_sdf;
@@ -465,6 +470,8 @@ int hhrr_set_rotor(hhrr_lattice* L, const hhrr_rotor_desc* r) {
     if (!any_node) lo[a] = hi[a] = 0;
   }
   L->rot_box = Box{lo[0], hi[0], lo[1], hi[1], lo[2], hi[2]};
+  // the row band of geometry.cu rests on the paper's premise that the surface moves less than a cell per step
+  L->band_ok = std::fabs(r->omega) * (rmax + 2.0) < 0.9;
   L->geometry_dirty = true;
   L->geometry_current = false;
   return HHRR_OK;
@@ -907,7 +914,10 @@ int hhrr_set_step_count(hhrr_lattice* L, int64_t step) {
     L->ahead_step = -1;
   }
   L->step = step;
-  L->geometry_current = !L->has_rotor && L->geometry_current;  // the rotor angle follows the step count
+  if (L->has_rotor) {  // the rotor angle follows the step count; the row band of the last steps is void
+    L->geometry_current = false;
+    L->geometry_dirty = true;
+  }
   return HHRR_OK;
 }
 

@@ -33,6 +33,14 @@ struct GeoArgs {
   double* phi;
   uint8_t* below;   // phi < eps/2 per cell: what the growth-layer test reads (1 B instead of 8)
   uint8_t* rowflag; // per (y,z) row: some cell of the row may have phi < eps/2 (superset)
+  // Row band of the rotor (see "K1 on the band" below): rowact_w = the parity written by this evaluation,
+  // rowact0 / rowact1 = both parities (read by the row selection), rowlist / n_rows = the rows to evaluate
+  uint8_t* rowact_w;
+  uint8_t *rowact0, *rowact1;
+  const uint8_t* rowflag_static;
+  int32_t* rowlist;
+  int* n_rows;
+  int all_rows;     // 1: every row of the box (the rotor may move more than a cell per step: no band argument)
   uint8_t* tag_prov;  // provisional tag of pass 1 (its own array: pass 1 may run ahead of the step that reads flags)
   const uint8_t* flags_prev;  // flag bytes the wall-model state bit is carried over from; NULL: written as 0 (look-ahead:
                               // the wall-model kernel of the step in between sets it, wallmodel.cu)
@@ -111,6 +119,9 @@ __device__ __forceinline__ bool geo_cell(const GeoArgs& a, int& x, int& y, int& 
   return !in_box;
 }
 
+constexpr double ROW_ACT = 3.9;   // see "K1 on the band" below
+constexpr int ROW_DILATE = 3;
+
 // pass 1: phi and provisional tag
 __global__ void __launch_bounds__(128) geometry_phi_kernel(GeoArgs a) {
   int x, y, z;
@@ -134,13 +145,89 @@ __global__ void __launch_bounds__(128) geometry_phi_kernel(GeoArgs a) {
   const bool below = phi < a.h;
   a.below[c] = below ? 1 : 0;
   if (below) a.rowflag[y + a.dm.ny * z] = 1;
+  if (phi < ROW_ACT) a.rowact0[y + a.dm.ny * z] = a.rowact1[y + a.dm.ny * z] = 1;
   a.tag_prov[c] = (uint8_t)(tg & TAG_MASK);
 }
 
+// ---------------------------------------------------------------------------------------------- K1 on the band
+// The paper re-embeds the tagged porosities only in the growth layer around the structure, because the surface
+// moves less than a cell per step (Fig. 4 :254-263).  Here the unit is a ROW of the rotor box (fixed y, z;
+// the rows run along the rotor axis for the paper's layout): a row is ACTIVE at step m if one of its cells has
+// phi_m < ROW_ACT (the reference grid is clipped at 4 cells: an inactive row is at least ~3.9 cells from the
+// surface).  Step m evaluates the rows within ROW_DILATE rows (in y and z) of a row that was active at step m-1 or
+// m-2 -- two steps, because the two geometry sets alternate and each must see a row turn plain fluid once.  Every
+// other row keeps what it has: plain fluid in both sets, no cell below eps/2, no list entry.  A cell can only get
+// phi < eps/2 + 1 (anything but plain fluid) at step m if a cell within a few cells of it was active before.
+// The rows to evaluate are compacted into a list; both passes then run as a few hundred blocks that walk the list
+// (a block per row of a 5-million-cell box is bound by the block dispatch rate, ncu round 1).
+
+__global__ void rows_select_kernel(GeoArgs a) {
+  const int by = a.box.y1 - a.box.y0, bz = a.box.z1 - a.box.z0;
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  bool take = false;
+  int y = 0, z = 0;
+  if (r < by * bz) {
+    y = a.box.y0 + r % by;
+    z = a.box.z0 + r / by;
+    take = a.all_rows != 0;
+    for (int dz = -ROW_DILATE; dz <= ROW_DILATE && !take; ++dz) {
+      const int zz = wrap_any(z + dz, a.dm.nz, a.dm.mode[2]);
+      for (int dy = -ROW_DILATE; dy <= ROW_DILATE; ++dy) {
+        const int row = wrap_any(y + dy, a.dm.ny, a.dm.mode[1]) + a.dm.ny * zz;
+        take |= (a.rowact0[row] | a.rowact1[row]) != 0;
+      }
+    }
+  }
+  const unsigned m = __ballot_sync(0xffffffffu, take);
+  if (m) {
+    const unsigned lane = threadIdx.x & 31;
+    int base = 0;
+    if (lane == 0) base = atomicAdd(a.n_rows, __popc(m));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (take) a.rowlist[base + __popc(m & ((1u << lane) - 1))] = y + a.dm.ny * z;
+  }
+}
+
+// pass 1 over the listed rows: phi, below, provisional tag; per row the two flags
+__global__ void __launch_bounds__(128) geometry_phi_rows_kernel(GeoArgs a) {
+  const int n_rows = *a.n_rows;
+  for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
+    const int row = a.rowlist[r], y = row % a.dm.ny, z = row / a.dm.ny;
+    int any_below = 0, any_act = 0;
+    for (int x = a.box.x0 + threadIdx.x; x < a.box.x1; x += blockDim.x) {
+      const int64_t c = (int64_t)x + (int64_t)a.dm.nx * row;
+      double phi = BIG_PHI;
+      int tg = 0;
+      if (a.has_static) {
+        phi = (double)a.phi_static[c];
+        tg = a.has_tag_static ? a.tag_static[c] : 1;
+      }
+      int rt;
+      const double pr = rotor_phi(a.rot, a.cth, a.sth, (double)x, (double)y, (double)z, &rt);
+      if (pr < phi) {
+        phi = pr;
+        tg = rt;
+      }
+      a.phi[c] = phi;
+      const bool below = phi < a.h;
+      a.below[c] = below ? 1 : 0;
+      a.tag_prov[c] = (uint8_t)(tg & TAG_MASK);
+      any_below |= below;
+      any_act |= phi < ROW_ACT;
+    }
+    any_below = __syncthreads_or(any_below);
+    any_act = __syncthreads_or(any_act);
+    if (threadIdx.x == 0) {
+      a.rowflag[row] = (uint8_t)(a.rowflag_static[row] | (any_below ? 1 : 0));
+      a.rowact_w[row] = any_act ? 1 : 0;
+    }
+  }
+}
+
 // pass 2: type, porosity, wall-model set (R13) and the compact lists
-__global__ void __launch_bounds__(128) geometry_type_kernel(GeoArgs a) {
-  int x, y, z;
-  bool active = geo_cell(a, x, y, z);
+// pass 2 for the cells (x .. x + blockDim.x) of row (y, z), one cell per thread; `active`: this thread has a cell.
+// All threads of the block call it together (shared memory, barrier, ballots).
+__device__ __forceinline__ void type_cells(const GeoArgs& a, int x, int y, int z, bool active) {
   int inw = 0, inf = 0;
   int64_t c = 0;
   double y1v[3] = {0, 0, 0};
@@ -296,6 +383,25 @@ __global__ void __launch_bounds__(128) geometry_type_kernel(GeoArgs a) {
   }
 }
 
+__global__ void __launch_bounds__(128) geometry_type_kernel(GeoArgs a) {
+  int x, y, z;
+  const bool active = geo_cell(a, x, y, z);
+  type_cells(a, x, y, z, active);
+}
+
+// pass 2 over the listed rows
+__global__ void __launch_bounds__(128) geometry_type_rows_kernel(GeoArgs a) {
+  const int n_rows = *a.n_rows;
+  for (int r = blockIdx.x; r < n_rows; r += gridDim.x) {
+    const int row = a.rowlist[r], y = row % a.dm.ny, z = row / a.dm.ny;
+    for (int xb = a.box.x0; xb < a.box.x1; xb += blockDim.x) {
+      const int x = xb + threadIdx.x;
+      type_cells(a, x, y, z, x < a.box.x1);
+      __syncthreads();  // the shared column bytes are reused by the next segment / row
+    }
+  }
+}
+
 __global__ void counters_kernel(Counters* cnt, int op) {
   if (op == 0) {  // start a full rebuild
     cnt->wall_count = cnt->force_count = 0;
@@ -310,9 +416,8 @@ __global__ void counters_kernel(Counters* cnt, int op) {
   }
 }
 
-// max_threads: 64 for the look-ahead launches -- a block of <= 4096 registers fits beside a resident block of the
-// collide-stream kernel (384 threads x 160 registers of the SM's 65536), so the side stream really runs during it
-static void geo_grid(const GeoArgs& a, dim3& g, dim3& b, int max_threads = 128) {
+static void geo_grid(const GeoArgs& a, dim3& g, dim3& b) {
+  const int max_threads = 128;
   if (a.inside) {
     int bx = a.box.x1 - a.box.x0, by = a.box.y1 - a.box.y0, bz = a.box.z1 - a.box.z0;
     int t = bx >= max_threads ? max_threads : ((bx + 31) / 32) * 32;  // a rotor box is thin along its axis: do not idle warps
@@ -363,6 +468,13 @@ static void fill_geo(hhrr_lattice* L, GeoArgs& a, int64_t step) {
   a.phi = L->phi;
   a.below = L->below;
   a.rowflag = L->rowflag;
+  a.rowflag_static = L->rowflag_static;
+  a.rowact0 = L->rowact[0];
+  a.rowact1 = L->rowact[1];
+  a.rowact_w = L->rowact[step & 1];
+  a.rowlist = L->rowlist;
+  a.n_rows = L->n_rows;
+  a.all_rows = L->band_ok ? 0 : 1;
   a.tag_prov = L->tag_prov;
   a.flags_prev = L->flags;
   a.flags = L->flags;
@@ -379,18 +491,21 @@ static bool rotor_box_empty(const hhrr_lattice* L) {
   return !L->has_rotor || rb.x1 <= rb.x0 || rb.y1 <= rb.y0 || rb.z1 <= rb.z0;
 }
 
-// pass 1 of geometry(step) over the rotor box, on stream s.  It reads the rotor description and the static
-// fields and writes phi / below / rowflag / tag_prov -- nothing a collide-stream, wall-model or force kernel touches.
-static void launch_box_phi(hhrr_lattice* L, int64_t step, cudaStream_t s, int max_threads = 128) {
-  GeoArgs a;
-  fill_geo(L, a, step);
+// geometry(step) over the rotor box on stream s, into the geometry set `a` points at: row selection, pass 1
+// (phi / below / row flags / provisional tag -- nothing a collide-stream, wall-model or force kernel touches),
+// list reset, pass 2.  Both passes walk the row list with a fixed number of blocks.
+static void launch_box_rows(hhrr_lattice* L, GeoArgs& a, cudaStream_t s) {
   a.box = L->rot_box;
   a.inside = 1;
-  dim3 g, b;
-  geo_grid(a, g, b, max_threads);
-  cudaMemcpyAsync(L->rowflag, L->rowflag_static, (size_t)L->dom.ny * L->dom.nz, cudaMemcpyDeviceToDevice, s);
-  geometry_phi_kernel<<<g, b, 0, s>>>(a);
-  L->launches++;
+  const int rows = (a.box.y1 - a.box.y0) * (a.box.z1 - a.box.z0);
+  const int bx = a.box.x1 - a.box.x0;
+  const int t = bx >= 128 ? 128 : ((bx + 31) / 32) * 32;  // a rotor box is thin along its axis: do not idle warps
+  cudaMemsetAsync(L->n_rows, 0, sizeof(int), s);
+  rows_select_kernel<<<(rows + 127) / 128, 128, 0, s>>>(a);
+  geometry_phi_rows_kernel<<<4736, t, 0, s>>>(a);  // latency-bound rows: many short blocks in flight, still 14 x fewer than one per row
+  counters_kernel<<<1, 1, 0, s>>>(a.cnt, 2);
+  geometry_type_rows_kernel<<<4736, t, 0, s>>>(a);
+  L->launches += 4;
 }
 
 void swap_geometry_sets(hhrr_lattice* L) {
@@ -414,7 +529,6 @@ void swap_geometry_sets(hhrr_lattice* L) {
 cudaError_t launch_geometry_ahead(hhrr_lattice* L) {
   if (!L->side || !L->lookahead || rotor_box_empty(L) || L->geometry_dirty) return cudaSuccess;
   cudaStreamWaitEvent(L->side, L->ev_pre, 0);
-  launch_box_phi(L, L->step + 1, L->side, 64);
   GeoArgs a;
   fill_geo(L, a, L->step + 1);
   a.flags_prev = nullptr;
@@ -424,13 +538,7 @@ cudaError_t launch_geometry_ahead(hhrr_lattice* L) {
   a.wall_y1n = L->alt_wall_y1n;
   a.force_idx = L->alt_force_idx;
   a.cnt = L->alt_counters;
-  a.box = L->rot_box;
-  a.inside = 1;
-  dim3 g, b;
-  geo_grid(a, g, b, 64);
-  counters_kernel<<<1, 1, 0, L->side>>>(a.cnt, 2);
-  geometry_type_kernel<<<g, b, 0, L->side>>>(a);
-  L->launches += 2;
+  launch_box_rows(L, a, L->side);
   cudaEventRecord(L->ev_k1, L->side);
   L->ahead_step = L->step + 1;
   L->side_busy = true;
@@ -470,6 +578,8 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
     a.inside = 0;
     geo_grid(a, g, b);
     cudaMemsetAsync(L->rowflag, 0, rows, L->stream);
+    cudaMemsetAsync(L->rowact[0], 0, rows, L->stream);
+    cudaMemsetAsync(L->rowact[1], 0, rows, L->stream);
     geometry_phi_kernel<<<g, b, 0, L->stream>>>(a);
     // what the full pass marks (static geometry and the rotor at this angle) stays marked: a superset
     cudaMemcpyAsync(L->rowflag_static, L->rowflag, rows, cudaMemcpyDeviceToDevice, L->stream);
@@ -492,13 +602,7 @@ cudaError_t launch_geometry(hhrr_lattice* L, bool full) {
       L->launches++;
     }
   } else if (!box_empty) {
-    launch_box_phi(L, L->step, L->stream);
-    a.box = rb;
-    a.inside = 1;
-    geo_grid(a, g, b);
-    counters_kernel<<<1, 1, 0, L->stream>>>(L->counters, 2);
-    geometry_type_kernel<<<g, b, 0, L->stream>>>(a);
-    L->launches += 2;
+    launch_box_rows(L, a, L->stream);
   }
   return cudaGetLastError();
 }

@@ -105,6 +105,10 @@ struct hhrr_lattice {
   uint8_t* below;           // N: phi < eps/2
   uint8_t* tag_prov;        // N: provisional tag of geometry pass 1
   uint8_t *rowflag, *rowflag_static;  // ny*nz: row may hold a cell with phi < eps/2
+  uint8_t* rowact[2];       // ny*nz each: row held a cell within ~3.9 cells of the rotor at the last even / odd step (geometry.cu)
+  int32_t* rowlist;         // ny*nz: rows of the rotor box to evaluate this step
+  int* n_rows;
+  bool band_ok;             // the rotor moves less than a cell per step: the row band applies
   float* phi_static;        // N
   uint8_t* tag_static;      // N
   float* d_override;        // N

@@ -219,6 +219,8 @@ def run_ours(args, rank, world, local_rank):
     L = B.Lattice(p, rotor_shape=None if case.rotor is None else case.rotor["sdf"].shape, device=dev, q=args.q)
     BYTES_PER_CELL = bytes_per_cell(args.q)
     L.set_kernel_variant(args.variant)
+    if args.chunk_planes or args.cluster:
+        L.set_launch_shape(args.chunk_planes, args.cluster)
     I.apply_case(case, L)
     n = case.n
     if args.decompose:
@@ -350,7 +352,7 @@ def run_ours(args, rank, world, local_rank):
                 "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": wname, "cells_per_gpu": n, "lattice": args.lattice, "storage": "fp32 SoA A/B" + (", x-pull / yz-push" if L.population_storage() else ""),
-                           "kernel_variant": args.variant,
+                           "kernel_variant": args.variant, "chunk_planes": args.chunk_planes or "auto", "cluster": args.cluster or "auto",
                            "parallelism": (f"z-slabs x{world}: halo exchange of {args.q} planes per face and step (NCCL send/recv), "
                                            "per-element force all-reduce" if args.decompose else f"replicas x{world}"),
                            "l2": "inputs (%.1f GB per buffer) exceed the 126 MB L2; no flush needed" % (4e-9 * args.q * n)},
@@ -373,6 +375,8 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--variant", type=int, default=5, choices=[0, 2, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--chunk-planes", type=int, default=0, help="planes per z-chunk of the default kernel (0: automatic)")
+    ap.add_argument("--cluster", type=int, default=0, help="tiles per thread-block cluster of the default kernel (0: automatic)")
     ap.add_argument("--decompose", action="store_true",
                     help="N blocks stacked along z into one lattice with halo exchange (SURVEY 8(f)-3) instead of N replicas")
     ap.add_argument("--lattice", default="D3Q27", choices=["D3Q27", "D3Q19"],

@@ -275,6 +275,11 @@ int hhrr_population_storage(const hhrr_lattice* L);
  * milliseconds and the number of launches it covers (at most 1024 per window), and starts a
  * new window.                                                                              */
 int hhrr_set_timing(hhrr_lattice* L, int enable);
+/* Launch shape of the default kernel (variant 5): planes per z-chunk of a tile column and tiles per thread-block
+ * cluster (1, 2, 4, 8).  0 = automatic (16 x 27 / Q planes, clusters of 2: the measured optimum on config 5,
+ * profiles/r02_k2_chunk_scan.md).  Results do not depend on it; it exists so that the scan behind the defaults can be
+ * repeated (bench.py --chunk-planes / --cluster).                                                               */
+int hhrr_set_launch_shape(hhrr_lattice* L, int32_t chunk_planes, int32_t cluster);
 /* Switches the overlap of the next step's porosity update with the current step (see
  * hhrr_create) on (default) or off.  Results are bitwise the same either way.            */
 int hhrr_set_lookahead(hhrr_lattice* L, int enable);

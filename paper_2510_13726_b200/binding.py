@@ -31,7 +31,7 @@ SYMBOLS = [
     "hhrr_set_populations", "hhrr_get_cell_populations", "hhrr_get_uhat", "hhrr_check_finite", "hhrr_set_kernel_variant",
     "hhrr_population_storage", "hhrr_set_fsi_region", "hhrr_set_wall_function", "hhrr_set_wall_model_variant",
     "hhrr_get_wall_model_state", "hhrr_set_wall_model_state", "hhrr_set_step_count",
-    "hhrr_set_timing", "hhrr_get_timing", "hhrr_set_lookahead", "hhrr_launch_count", "hhrr_last_error", "hhrr_version",
+    "hhrr_set_timing", "hhrr_get_timing", "hhrr_set_lookahead", "hhrr_set_launch_shape", "hhrr_launch_count", "hhrr_last_error", "hhrr_version",
     "hhrr_velocity_set", "hhrr_halo_floats", "hhrr_halo_pack", "hhrr_halo_unpack",
 ]
 
@@ -109,6 +109,7 @@ def lib(q=27):
         L.hhrr_check_finite.argtypes = [vp]
         L.hhrr_set_kernel_variant.argtypes = [vp, i32]
         L.hhrr_set_lookahead.argtypes = [vp, C.c_int]
+        L.hhrr_set_launch_shape.argtypes = [vp, i32, i32]
         L.hhrr_set_timing.argtypes = [vp, C.c_int]
         L.hhrr_get_timing.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
         L.hhrr_launch_count.restype = i64
@@ -273,6 +274,9 @@ class Lattice:
     def set_kernel_variant(self, variant):
         """Returns HHRR_OK (0) or the notice W_FALLBACK (1): variant 5 cannot tile the lattice, variant 2 runs."""
         return self._check(self.lib.hhrr_set_kernel_variant(self.h, int(variant)))
+
+    def set_launch_shape(self, chunk_planes=0, cluster=0):
+        self._check(self.lib.hhrr_set_launch_shape(self.h, int(chunk_planes), int(cluster)))
 
     def set_lookahead(self, enable=True):
         self._check(self.lib.hhrr_set_lookahead(self.h, int(bool(enable))))

@@ -509,6 +509,15 @@ int hhrr_set_kernel_variant(hhrr_lattice* L, int32_t variant) {
   return HHRR_OK;
 }
 
+int hhrr_set_launch_shape(hhrr_lattice* L, int32_t chunk_planes, int32_t cluster) {
+  DeviceGuard guard_(L);
+  if (!L || chunk_planes < 0 || chunk_planes > 4096 || cluster < 0 || cluster > 8 || (cluster & (cluster - 1)))
+    return fail(HHRR_E_ARG, "hhrr_set_launch_shape: bad argument");
+  L->chunk_planes = chunk_planes;
+  L->cluster = cluster;
+  return HHRR_OK;
+}
+
 int hhrr_set_lookahead(hhrr_lattice* L, int enable) {
   DeviceGuard guard_(L);
   if (!L) return fail(HHRR_E_ARG, "hhrr_set_lookahead: NULL lattice");

@@ -546,7 +546,7 @@ static cudaError_t launch_shape(hhrr_lattice* L, WsArgs& a) {
   // packed-fp32 workers (profiles/r02_k2_chunk_scan.md): 13-16 planes 3.99 ms, 18 planes 4.18 ms, 22 planes 4.42 ms
   // (DRAM reads 15.3 GB per launch instead of 12.9); D3Q19 (19 planes of populations per cell plane) is flat from 22
   // to 30.  Hence 16 planes x 27 / Q.
-  int nch = ws_zchunks(dm.nz, (16 * 27 + Q / 2) / Q);
+  int nch = ws_zchunks(dm.nz, L->chunk_planes > 0 ? L->chunk_planes : (16 * 27 + Q / 2) / Q);
   a.zchunk = (dm.nz + nch - 1) / nch;
   nch = (dm.nz + a.zchunk - 1) / a.zchunk;
   if (!L->sm_count &&
@@ -560,8 +560,8 @@ static cudaError_t launch_shape(hhrr_lattice* L, WsArgs& a) {
   // starts together on neighbouring SMs and asks L2 for the x-halo sectors it shares at the same time.  Measured:
   // nothing at 16-plane chunks without the region split, 4.07 -> 3.95 ms with it, and the cliff at longer chunks
   // moves out (18 planes: 4.18 -> 4.02 ms).
-  constexpr int cl = 2;
-  if (grid.x % cl == 0 && a.group % cl == 0 && ntiles % cl == 0) {
+  const int cl = L->cluster > 0 ? L->cluster : 2;
+  if (cl > 1 && grid.x % cl == 0 && a.group % cl == 0 && ntiles % cl == 0) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid;
     cfg.blockDim = dim3(C::THREADS);

@@ -142,6 +142,7 @@ struct hhrr_lattice {
   int64_t step;
   int variant;       // requested kernel variant; dom.xs says how the populations are stored for it
   int64_t launches;
+  int chunk_planes, cluster;  // hhrr_set_launch_shape: planes per z-chunk / tiles per cluster of the default kernel (0: automatic)
   int sm_count;          // of L->device (0: not yet asked)
   bool attr_xpull[2], attr_ws;  // dynamic shared-memory attribute set on L->device for the fused kernels
   // optional CUDA-event timing of the collide-stream kernel (hhrr_set_timing)

@@ -120,12 +120,13 @@ size_t hhrr_workspace_bytes(const hhrr_params* p, const hhrr_rotor_desc* rotor);
 
 /* Creates a lattice at rest (f_i = w_i, d = 1, no geometry) in the caller's device
  * workspace.  `cuda_stream` is a cudaStream_t: every kernel and copy of the library is
- * queued on it, except the first half of the NEXT step's porosity update (rotor signed
- * distance; a function of the step count only), which hhrr_step queues on
- * one internal low-priority stream, ordered against `cuda_stream` by events, so that it
- * overlaps the tail of the collide-stream kernel.  Results do not depend on it
- * (hhrr_set_lookahead(L, 0) switches it off, for measurement and tests).  The workspace
- * must stay allocated until hhrr_destroy, which waits for both streams.                  */
+ * queued on it, except two things hhrr_step puts on one internal side stream, ordered against
+ * `cuda_stream` by events: the porosity update of the NEXT step (a function of the step count
+ * only; written into an alternate geometry set) and the force collection of the
+ * step just streamed (it only reads).  hhrr_step returns with the side stream joined into
+ * `cuda_stream`.  Results do not depend on it (hhrr_set_lookahead(L, 0) switches the look-ahead
+ * off, for measurement and tests).  The workspace must stay allocated until hhrr_destroy,
+ * which waits for both streams.                                                           */
 int hhrr_create(const hhrr_params* p, void* d_workspace, size_t workspace_bytes, void* cuda_stream,
                 hhrr_lattice** out);
 int hhrr_destroy(hhrr_lattice* L);
@@ -273,10 +274,11 @@ int hhrr_population_storage(const hhrr_lattice* L);
 /* Optional CUDA-event timing of the collide-stream launches inside hhrr_step (the kernel the
  * roofline is quoted on).  hhrr_get_timing synchronises, returns the summed device time in
  * milliseconds and the number of launches it covers (at most 1024 per window), and starts a
- * new window.                                                                              */
+ * new window.  (The first hhrr_set_timing(L, 1) creates 2048 CUDA events, the only device-side resources besides
+ * a side stream and a handful of ordering events that the library creates itself; hhrr_destroy releases them.)          */
 int hhrr_set_timing(hhrr_lattice* L, int enable);
 /* Launch shape of the default kernel (variant 5): planes per z-chunk of a tile column and tiles per thread-block
- * cluster (1, 2, 4, 8).  0 = automatic (16 x 27 / Q planes, clusters of 2: the measured optimum on config 5,
+ * cluster (1, 2, 4, 8).  0 = automatic (16 planes, 12 with an FSI region; 30 / 22 on D3Q19; clusters of 2: measured on config 5,
  * profiles/r02_k2_chunk_scan.md).  Results do not depend on it; it exists so that the scan behind the defaults can be
  * repeated (bench.py --chunk-planes / --cluster).                                                               */
 int hhrr_set_launch_shape(hhrr_lattice* L, int32_t chunk_planes, int32_t cluster);

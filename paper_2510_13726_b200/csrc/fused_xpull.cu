@@ -543,10 +543,12 @@ static cudaError_t launch_shape(hhrr_lattice* L, WsArgs& a) {
   // with the grouped launch order the halo planes of a chunk are L2 hits: 22 planes without, 16 with the region split
   // z-chunk length: neighbouring tiles re-synchronise at every chunk start, and the halo rows / x-halo sectors they
   // share stay L2 hits only while they march within a few planes of each other.  Measured on config 5 with the
-  // packed-fp32 workers (profiles/r02_k2_chunk_scan.md): 13-16 planes 3.99 ms, 18 planes 4.18 ms, 22 planes 4.42 ms
-  // (DRAM reads 15.3 GB per launch instead of 12.9); D3Q19 (19 planes of populations per cell plane) is flat from 22
-  // to 30.  Hence 16 planes x 27 / Q.
-  int nch = ws_zchunks(dm.nz, L->chunk_planes > 0 ? L->chunk_planes : (16 * 27 + Q / 2) / Q);
+  // packed-fp32 workers (profiles/r02_k2_chunk_scan.md; bench.py --chunk-planes): 13-16 planes 4.01-4.03 ms, 18 planes
+  // 4.06 ms, 22 planes 4.15 ms, 32 planes 4.51 ms (without clusters: 4.09 / 4.27 / 4.52 / 4.92 ms); with the region
+  // split 12 planes 3.88 ms, 16 planes 3.92 ms; D3Q19 (19 populations per cell plane) 16 / 23 / 30 planes 3.08 / 3.02 /
+  // 3.00 ms.  hhrr_set_launch_shape overrides.
+  const int auto_planes = Q == 27 ? (a.fsi.n > 0 ? 12 : 16) : (a.fsi.n > 0 ? 22 : 30);
+  int nch = ws_zchunks(dm.nz, L->chunk_planes > 0 ? L->chunk_planes : auto_planes);
   a.zchunk = (dm.nz + nch - 1) / nch;
   nch = (dm.nz + a.zchunk - 1) / a.zchunk;
   if (!L->sm_count &&
@@ -557,9 +559,9 @@ static cudaError_t launch_shape(hhrr_lattice* L, WsArgs& a) {
   const int ntiles = (dm.nx / C::TX) * (dm.ny / C::TY);
   dim3 grid((unsigned)(ntiles * nch));
   // Two x-adjacent tiles form a thread-block cluster (no cluster barrier, no distributed shared memory): the pair
-  // starts together on neighbouring SMs and asks L2 for the x-halo sectors it shares at the same time.  Measured:
-  // nothing at 16-plane chunks without the region split, 4.07 -> 3.95 ms with it, and the cliff at longer chunks
-  // moves out (18 planes: 4.18 -> 4.02 ms).
+  // starts together on neighbouring SMs and asks L2 for the x-halo sectors it shares at the same time.  Measured
+  // (profiles/r02_k2_chunk_scan.md): 4.09 -> 4.01 ms at 16-plane chunks, 3.99 -> 3.88 ms with the region split at 12,
+  // and the cliff at longer chunks moves out (22 planes: 4.52 -> 4.15 ms); clusters of 4: 4.15 ms.
   const int cl = L->cluster > 0 ? L->cluster : 2;
   if (cl > 1 && grid.x % cl == 0 && a.group % cl == 0 && ntiles % cl == 0) {
     cudaLaunchConfig_t cfg = {};

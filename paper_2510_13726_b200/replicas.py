@@ -19,8 +19,3 @@ def max_over_ranks(ms_local: float, device=None) -> float:
 def aggregate_mlups(cells_per_rank: int, steps: int, ms_max: float, world: int) -> float:
     """Whole-job throughput: the units all ranks processed / the slowest rank's time."""
     return world * cells_per_rank * steps / (ms_max * 1e3)
-
-
-def seed_for_rank(base_seed: int, rank: int) -> int:
-    """Replicas run the same recipe with distinct noise seeds."""
-    return base_seed + 7919 * rank

@@ -253,6 +253,22 @@ int hhrr_get_uhat(hhrr_lattice* L, float* uhat);
 int64_t hhrr_halo_floats(const hhrr_lattice* L);
 int hhrr_halo_pack(hhrr_lattice* L, int32_t face, float* d_buf);
 int hhrr_halo_unpack(hhrr_lattice* L, int32_t face, const float* d_buf);
+/* Allocation-free wall model, for callers that may not allocate (CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc).  Runs WallModelO (Listing 3 line 4; Eq. 15-20 :159-184) on the lattice's CURRENT
+ * populations and the wall list of the last evaluated geometry -- what the wall model inside the last hhrr_step saw --
+ * asynchronously on the lattice's stream, and writes its results per LIST ENTRY e (order of hhrr_get_wall_model_state)
+ * into caller-owned DEVICE arrays instead of the lattice's state, which it neither reads nor writes:
+ *   d_u_tau_start  [capacity] doubles or NULL: warm start of the Newton iteration per entry (Eq. 20 :181); <= 0 or NULL =
+ *                  the cold start sqrt(nu U / y);
+ *   d_u_tau [capacity] doubles, d_u_wm [capacity][3] floats, d_s_wm [capacity][6] floats (xx yy zz xy xz yz).
+ * Entries [0, min(wall count, capacity)) are written.  The scratch between its two kernels (48 B per wall cell) is a
+ * file-scope device array of HHRR_NOALLOC_MAX_WALL_CELLS cells = 3 MiB that every GPU which loads the library holds
+ * until exit: capacity > HHRR_NOALLOC_MAX_WALL_CELLS is refused with HHRR_E_SIZE.  The call allocates and frees nothing
+ * and does not synchronise.  All calls share the scratch: calls that overlap on one GPU (different streams) race; calls
+ * on one stream or on different GPUs do not.  Nothing in the scratch needs clearing between calls.                    */
+#define HHRR_NOALLOC_MAX_WALL_CELLS 65536
+int hhrr_wall_model_noalloc(hhrr_lattice* L, int64_t capacity, const double* d_u_tau_start, double* d_u_tau,
+                            float* d_u_wm, float* d_s_wm);
 /* HHRR_E_NAN if any population is non-finite (synchronises). */
 int hhrr_check_finite(hhrr_lattice* L);
 /* Selects the collide-stream kernel: 5 = the TMA-fed fused kernel on x-pull / yz-push storage

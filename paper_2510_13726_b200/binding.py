@@ -32,7 +32,7 @@ SYMBOLS = [
     "hhrr_population_storage", "hhrr_set_fsi_region", "hhrr_set_wall_function", "hhrr_set_wall_model_variant",
     "hhrr_get_wall_model_state", "hhrr_set_wall_model_state", "hhrr_set_step_count",
     "hhrr_set_timing", "hhrr_get_timing", "hhrr_set_lookahead", "hhrr_set_launch_shape", "hhrr_launch_count", "hhrr_last_error", "hhrr_version",
-    "hhrr_velocity_set", "hhrr_halo_floats", "hhrr_halo_pack", "hhrr_halo_unpack",
+    "hhrr_velocity_set", "hhrr_halo_floats", "hhrr_halo_pack", "hhrr_halo_unpack", "hhrr_wall_model_noalloc",
 ]
 
 
@@ -121,6 +121,7 @@ def lib(q=27):
         L.hhrr_halo_floats.argtypes = [vp]
         L.hhrr_halo_pack.argtypes = [vp, i32, vp]
         L.hhrr_halo_unpack.argtypes = [vp, i32, vp]
+        L.hhrr_wall_model_noalloc.argtypes = [vp, i64, vp, vp, vp, vp]
         if L.hhrr_velocity_set() != q:
             raise RuntimeError(f"{path} was built for D3Q{L.hhrr_velocity_set()}, not D3Q{q}")
         _libs[q] = L
@@ -377,6 +378,13 @@ class Lattice:
         uw = np.ascontiguousarray(u_wm, np.float32); sw = np.ascontiguousarray(s_wm, np.float32)
         va = np.ascontiguousarray(valid, np.uint8)
         self._check(self.lib.hhrr_set_wall_model_state(self.h, len(idx), _p(idx), _p(ut), _p(uw), _p(sw), _p(va)))
+
+    def wall_model_noalloc(self, capacity, start_t, utau_t, uwm_t, swm_t):
+        """hhrr_wall_model_noalloc: CUDA tensors start_t (float64 [capacity] or None), utau_t (float64 [capacity]),
+        uwm_t (float32 [capacity, 3]), swm_t (float32 [capacity, 6]); asynchronous, allocates nothing."""
+        self._check(self.lib.hhrr_wall_model_noalloc(
+            self.h, int(capacity), None if start_t is None else C.c_void_p(start_t.data_ptr()),
+            C.c_void_p(utau_t.data_ptr()), C.c_void_p(uwm_t.data_ptr()), C.c_void_p(swm_t.data_ptr())))
 
     def halo_floats(self):
         return int(self.lib.hhrr_halo_floats(self.h))

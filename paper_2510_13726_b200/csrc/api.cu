@@ -196,6 +196,14 @@ int ensure_geometry(hhrr_lattice* L) {
 
 }  // namespace
 
+int hhrr::set_error(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
 extern "C" {
 
 const char* hhrr_last_error(void) { return g_err; }

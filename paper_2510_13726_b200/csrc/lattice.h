@@ -153,6 +153,9 @@ struct hhrr_lattice {
 
 // ---- kernel launchers (one per translation unit) ---------------------------------------
 namespace hhrr {
+// api.cu: records the thread-local message hhrr_last_error() returns and hands `code` back (for entry points that live
+// in other translation units)
+int set_error(int code, const char* fmt, ...);
 // geometry.cu (compiled with -fmad=false: operation order is part of the definition)
 cudaError_t launch_geometry(hhrr_lattice* L, bool full);
 // collide.cu

@@ -8,6 +8,8 @@
 // collide-stream kernels (its output feeds the next collision); K4 only reads the streamed populations
 // and runs on the side stream beside the next collide-stream kernel.
 // CUDA path only; shares nothing with oracle/.
+#include <algorithm>
+
 #include "cell_model.cuh"
 
 namespace hhrr {
@@ -206,9 +208,20 @@ __device__ __forceinline__ double wall_shear(int kind, double ut, double U, doub
   return ut * ut / nu * slope;
 }
 
-// one wall-model cell: tangential speed relative to the wall, u_tau, slip velocity, wall strain, state valid
+// Outputs of the allocation-free entry point (hhrr_wall_model_noalloc, end of this file): per list entry e instead
+// of per cell, in caller-owned device arrays; the lattice's own wall-model state is neither read nor written.
+struct WmDirect {
+  const double* start;  // [count] warm-start u_tau per entry (<= 0: none, Eq. 20's cold start), or NULL
+  double* utau;         // [count]
+  float* u;             // [count][3]
+  float* s;             // [count][6]
+};
+
+// one wall-model cell: tangential speed relative to the wall, u_tau, slip velocity, wall strain, state valid.
+// DIRECT = false (every existing caller): warm start from, and results into, the lattice's per-cell state.
+template <bool DIRECT = false>
 __device__ __forceinline__ void wall_finish_cell(const WmArgs& a, int64_t c, const double y1v[3], const double vs[3],
-                                                 const double vw[3]) {
+                                                 const double vw[3], const WmDirect* o = nullptr, int e = 0) {
   const int64_t n = a.dm.n, nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
   {
     int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
@@ -232,8 +245,16 @@ __device__ __forceinline__ void wall_finish_cell(const WmArgs& a, int64_t c, con
     double uw[3] = {0, 0, 0}, sw[6] = {0, 0, 0, 0, 0, 0};
     if (!(U < 1e-14)) {
       double yy = y1 + a.hs;
-      double prev = a.wm_utau[c];
-      double ua = ((fl & WM_VALID) && prev > 0.0) ? prev : sqrt(a.nu * U / yy);  // Eq. 20
+      double prev;
+      bool have_prev;
+      if (DIRECT) {
+        prev = o->start ? o->start[e] : 0.0;
+        have_prev = true;
+      } else {
+        prev = a.wm_utau[c];
+        have_prev = (fl & WM_VALID) != 0;
+      }
+      double ua = (have_prev && prev > 0.0) ? prev : sqrt(a.nu * U / yy);  // Eq. 20
       // Newton-Raphson (Eq. 19), stop rule of PAPER.md:184
       double fa = wall_f(a.wall_function, ua, U, yy, a.nu, a.kappa, a.E), ub = ua;
       for (int it = 0; it < a.max_iter; ++it) {
@@ -267,6 +288,12 @@ __device__ __forceinline__ void wall_finish_cell(const WmArgs& a, int64_t c, con
       sw[3] = 0.5 * (G[0][1] + G[1][0]);
       sw[4] = 0.5 * (G[0][2] + G[2][0]);
       sw[5] = 0.5 * (G[1][2] + G[2][1]);
+    }
+    if (DIRECT) {
+      o->utau[e] = utau;
+      for (int q = 0; q < 3; ++q) o->u[3 * (int64_t)e + q] = (float)uw[q];
+      for (int q = 0; q < 6; ++q) o->s[6 * (int64_t)e + q] = (float)sw[q];
+      return;
     }
     a.wm_utau[c] = utau;
     for (int q = 0; q < 3; ++q) a.wm_u[(int64_t)q * n + c] = (float)uw[q];
@@ -517,3 +544,89 @@ cudaError_t launch_forces(hhrr_lattice* L, cudaStream_t s) {
 }
 
 }  // namespace hhrr
+
+// ---------------------------------------------------------------------------- allocation-free wall model
+// hhrr_wall_model_noalloc (include/hhrr.h): WallModelO (K3) on the lattice's current populations and wall list for
+// callers that may not allocate -- code under CUDA graph capture, tight serving loops, harnesses that forbid
+// cudaMalloc.  K3 is two kernels with scratch between them (v_s and v(x_w) per wall cell, 48 B); the regular path keeps
+// that scratch in the caller's workspace, this one in the file-scope array below: HHRR_NOALLOC_MAX_WALL_CELLS cells x 6
+// doubles = 3 MiB, held by every GPU that loads the library until the process exits.
+//   * The array's NAME is a host-side stand-in in host code, not a device address: its address on a device comes from
+//     cudaGetSymbolAddress, asked once per device with that device current (scratch_address below).
+//   * All calls share the array.  The sampling kernel overwrites entries [0, count) before the Newton kernel reads
+//     them and nothing reads beyond: no entry has to start at zero, a shorter list after a longer one reads nothing
+//     stale.  Two calls that OVERLAP on the GPU (different streams, or lattices on different streams of one device) race
+//     on it; calls on one stream, or on different devices, do not.
+//   * No cudaMalloc / cudaFree / allocating library routine on this path: two kernel launches on the lattice's stream.
+namespace hhrr {
+
+static __device__ __align__(256) double g_noalloc_scratch[(size_t)HHRR_NOALLOC_MAX_WALL_CELLS * 6];
+
+constexpr int MAX_DEVICES = 64;
+static double* g_noalloc_ptr[MAX_DEVICES] = {};
+
+// device address of the scratch array on the CURRENT device (the caller has made `device` current)
+static cudaError_t scratch_address(int device, double** out) {
+  if (device < 0 || device >= MAX_DEVICES) return cudaErrorInvalidDevice;
+  if (!g_noalloc_ptr[device]) {
+    double* p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress((void**)&p, g_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    g_noalloc_ptr[device] = p;  // benign if two threads get here together: both write the same address
+  }
+  *out = g_noalloc_ptr[device];
+  return cudaSuccess;
+}
+
+// Newton kernel of the allocation-free path: one thread per list entry, outputs per entry into the caller's arrays
+__global__ void __launch_bounds__(128) wall_model_direct_kernel(const __grid_constant__ WmArgs a,
+                                                                const __grid_constant__ WmDirect o) {
+  const int count = min(a.cnt->wall_count, a.cap_list);
+  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < count; e += gridDim.x * blockDim.x) {
+    const int64_t c = a.wall_idx[e];
+    double y1v[3], vs[3], vw[3];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+      y1v[q] = a.wall_y1n[3 * (int64_t)e + q];
+      vs[q] = a.samp[6 * (int64_t)e + q];
+      vw[q] = a.samp[6 * (int64_t)e + 3 + q];
+    }
+    wall_finish_cell<true>(a, c, y1v, vs, vw, &o, e);
+  }
+}
+
+}  // namespace hhrr
+
+extern "C" int hhrr_wall_model_noalloc(hhrr_lattice* L, int64_t capacity, const double* d_u_tau_start, double* d_u_tau,
+                                       float* d_u_wm, float* d_s_wm) {
+  using namespace hhrr;
+  if (!L || !d_u_tau || !d_u_wm || !d_s_wm || capacity < 1)
+    return set_error(HHRR_E_ARG, "hhrr_wall_model_noalloc: NULL output array or capacity < 1");
+  if (capacity > HHRR_NOALLOC_MAX_WALL_CELLS)
+    return set_error(HHRR_E_SIZE, "hhrr_wall_model_noalloc: capacity %lld exceeds the built-in scratch of %d wall cells "
+                     "(HHRR_NOALLOC_MAX_WALL_CELLS); use hhrr_step, whose scratch lives in the caller's workspace",
+                     (long long)capacity, (int)HHRR_NOALLOC_MAX_WALL_CELLS);
+  int prev = -1;  // work on the lattice's device, leave the caller's current device as it was
+  if (cudaGetDevice(&prev) != cudaSuccess) return set_error(HHRR_E_CUDA, "hhrr_wall_model_noalloc: no CUDA device");
+  if (prev != L->device && cudaSetDevice(L->device) != cudaSuccess)
+    return set_error(HHRR_E_CUDA, "hhrr_wall_model_noalloc: cannot select device %d", L->device);
+  int rc = HHRR_OK;
+  double* scratch = nullptr;
+  cudaError_t e = scratch_address(L->device, &scratch);
+  if (e != cudaSuccess) {
+    rc = set_error(HHRR_E_CUDA, "hhrr_wall_model_noalloc: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+  } else {
+    WmArgs w;
+    fill_wm(L, w);
+    w.samp = scratch;                                             // instead of the workspace's wall_samp
+    w.cap_list = (int)std::min<int64_t>(w.cap_list, capacity);  // entries [0, min(wall count, capacity))
+    WmDirect o{d_u_tau_start, d_u_tau, d_u_wm, d_s_wm};
+    wall_sample_kernel<2, 8><<<4736, 128, 0, L->stream>>>(w);
+    wall_model_direct_kernel<<<592, 128, 0, L->stream>>>(w, o);
+    L->launches += 2;
+    e = cudaGetLastError();
+    if (e != cudaSuccess) rc = set_error(HHRR_E_CUDA, "hhrr_wall_model_noalloc: launch: %s", cudaGetErrorString(e));
+  }
+  if (prev != L->device) cudaSetDevice(prev);
+  return rc;
+}

@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdint>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -975,23 +976,46 @@ namespace {
 //   c_z(i) == -c : population j = i with c_z reversed (c_z(j) = c) of the last REAL plane of the sender
 //                                                                   -> population j of the HALO plane of the receiver
 // (the receiver's halo plane already holds its populations with c_z = -c: its own collision pushed them there).
-__global__ void halo_copy_kernel(float* __restrict__ f, float* __restrict__ buf, int64_t n, int64_t plane, int nz, int face,
-                                 int unpack) {
-  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, T = (int64_t)gridDim.x * blockDim.x;
+// grid (blocks per plane, Q): blockIdx.y is the buffer slot, so all Q planes move at once; 16-byte accesses when VEC
+template <bool VEC>
+__global__ void __launch_bounds__(256) halo_copy_kernel(float* __restrict__ f, float* __restrict__ buf, int64_t n,
+                                                        int64_t plane, int nz, int face, int unpack) {
+  const int i = blockIdx.y;
   const int c = unpack ? (face ? -1 : 1) : (face ? 1 : -1);
   const int z_halo = face ? nz - 1 : 0, z_real = face ? nz - 2 : 1;
-  for (int i = 0; i < Q; ++i) {
-    const int cz = dir_cz(i);
-    const int pop = cz == -c ? dir_flip(i, false, false, true) : i;
-    // sender: crossing populations sit in its halo plane; receiver: they land in its first real plane
-    const int z = (cz == c) ? (unpack ? z_real : z_halo) : (unpack ? z_halo : z_real);
-    float* p = f + (int64_t)pop * n + plane * z;
-    float* b = buf + (int64_t)i * plane;
+  const int cz = dir_cz(i);
+  const int pop = cz == -c ? dir_flip(i, false, false, true) : i;
+  // sender: crossing populations sit in its halo plane; receiver: they land in its first real plane
+  const int z = (cz == c) ? (unpack ? z_real : z_halo) : (unpack ? z_halo : z_real);
+  float* p = f + (int64_t)pop * n + plane * z;
+  float* b = buf + (int64_t)i * plane;
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, T = (int64_t)gridDim.x * blockDim.x;
+  if (VEC) {
+    float4* p4 = reinterpret_cast<float4*>(p);
+    float4* b4 = reinterpret_cast<float4*>(b);
+    if (!unpack)
+      for (int64_t k = t; k < plane / 4; k += T) b4[k] = p4[k];
+    else
+      for (int64_t k = t; k < plane / 4; k += T) p4[k] = b4[k];
+  } else {
     if (!unpack)
       for (int64_t k = t; k < plane; k += T) b[k] = p[k];
     else
       for (int64_t k = t; k < plane; k += T) p[k] = b[k];
   }
+}
+
+cudaError_t launch_halo_copy(hhrr_lattice* L, float* buf, int face, int unpack) {
+  const int64_t plane = (int64_t)L->dom.nx * L->dom.ny;
+  const bool vec = plane % 4 == 0 && (reinterpret_cast<uintptr_t>(buf) & 15) == 0;
+  const int64_t items = vec ? plane / 4 : plane;
+  dim3 grid((unsigned)std::min<int64_t>(148, (items + 255) / 256), Q);
+  if (vec)
+    halo_copy_kernel<true><<<grid, 256, 0, L->stream>>>(L->fA, buf, L->dom.n, plane, L->dom.nz, face, unpack);
+  else
+    halo_copy_kernel<false><<<grid, 256, 0, L->stream>>>(L->fA, buf, L->dom.n, plane, L->dom.nz, face, unpack);
+  L->launches++;
+  return cudaGetLastError();
 }
 }  // namespace
 
@@ -1003,9 +1027,7 @@ int hhrr_halo_pack(hhrr_lattice* L, int32_t face, float* d_buf) {
   if (!L || !d_buf || (face != 0 && face != 1)) return fail(HHRR_E_ARG, "hhrr_halo_pack: bad argument");
   if (L->dom.nz < 4 || L->dom.mode[2] != HHRR_PERIODIC)
     return fail(HHRR_E_STATE, "hhrr_halo_pack: a slab needs a periodic z axis of at least 4 planes (2 halo + 2 real)");
-  halo_copy_kernel<<<592, 256, 0, L->stream>>>(L->fA, d_buf, L->dom.n, (int64_t)L->dom.nx * L->dom.ny, L->dom.nz, face, 0);
-  L->launches++;
-  CU(cudaGetLastError());
+  CU(launch_halo_copy(L, d_buf, face, 0));
   return HHRR_OK;
 }
 
@@ -1014,10 +1036,7 @@ int hhrr_halo_unpack(hhrr_lattice* L, int32_t face, const float* d_buf) {
   if (!L || !d_buf || (face != 0 && face != 1)) return fail(HHRR_E_ARG, "hhrr_halo_unpack: bad argument");
   if (L->dom.nz < 4 || L->dom.mode[2] != HHRR_PERIODIC)
     return fail(HHRR_E_STATE, "hhrr_halo_unpack: a slab needs a periodic z axis of at least 4 planes (2 halo + 2 real)");
-  halo_copy_kernel<<<592, 256, 0, L->stream>>>(L->fA, const_cast<float*>(d_buf), L->dom.n, (int64_t)L->dom.nx * L->dom.ny,
-                                                L->dom.nz, face, 1);
-  L->launches++;
-  CU(cudaGetLastError());
+  CU(launch_halo_copy(L, const_cast<float*>(d_buf), face, 1));
   return HHRR_OK;
 }
 }  // extern "C"

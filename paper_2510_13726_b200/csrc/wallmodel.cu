@@ -93,6 +93,62 @@ __device__ __forceinline__ double shfl_down_d(double v, int delta) { return __sh
 // lanes of the sampling warps, was measured slower: 148 vs 87 us -- the fp64 pipe then runs a quarter full.)
 
 // what a lane needs to finish its part of one wall cell's sample once its nine loads have landed
+// neighbour coordinate with the outer-boundary rule R12 for SMALL offsets (a few cells beyond the lattice): no integer
+// division; the loops run at most once unless the lattice is only a few cells wide
+__device__ __forceinline__ int wrap_near(int v, int n, int mode, bool& flip) {
+  flip = false;
+  if (mode == HHRR_PERIODIC) {
+    while (v < 0) v += n;
+    while (v >= n) v -= n;
+    return v;
+  }
+  while (v < 0 || v >= n) {  // reflections at the two planes alternate
+    v = v < 0 ? -1 - v : 2 * n - 1 - v;
+    flip = !flip;
+  }
+  return v;
+}
+
+// Per wall cell, computed ONCE by the lane that owns the list entry and handed to the warp by shuffles: the cell, the
+// base corner of the trilinear stencil around x_w + h_s n (R15) and the three weights.
+struct SamplePoint {
+  int x, y, z;        // the wall cell
+  int ix, iy, iz;     // base corner of the stencil
+  double tx, ty, tz;  // interpolation weights
+};
+__device__ __forceinline__ SamplePoint sample_point(const WmArgs& a, int c, const double y1v[3]) {
+  SamplePoint p;
+  const unsigned cu = (unsigned)c, nx = (unsigned)a.dm.nx, ny = (unsigned)a.dm.ny;  // cells are int32 list entries
+  const unsigned row = cu / nx;
+  p.x = (int)(cu - row * nx);
+  p.z = (int)(row / ny);
+  p.y = (int)(row - (unsigned)p.z * ny);
+  double y1 = sqrt(y1v[0] * y1v[0] + y1v[1] * y1v[1] + y1v[2] * y1v[2]);
+  double nrm[3] = {y1v[0] / y1, y1v[1] / y1, y1v[2] / y1};
+  double px = p.x + a.hs * nrm[0], py = p.y + a.hs * nrm[1], pz = p.z + a.hs * nrm[2];
+  double fx = floor(px), fy = floor(py), fz = floor(pz);
+  p.tx = px - fx;
+  p.ty = py - fy;
+  p.tz = pz - fz;
+  p.ix = (int)fx;
+  p.iy = (int)fy;
+  p.iz = (int)fz;
+  return p;
+}
+__device__ __forceinline__ SamplePoint shfl_point(const SamplePoint& p, int src) {
+  SamplePoint q;
+  q.x = __shfl_sync(0xffffffffu, p.x, src);
+  q.y = __shfl_sync(0xffffffffu, p.y, src);
+  q.z = __shfl_sync(0xffffffffu, p.z, src);
+  q.ix = __shfl_sync(0xffffffffu, p.ix, src);
+  q.iy = __shfl_sync(0xffffffffu, p.iy, src);
+  q.iz = __shfl_sync(0xffffffffu, p.iz, src);
+  q.tx = shfl_d(p.tx, src);
+  q.ty = shfl_d(p.ty, src);
+  q.tz = shfl_d(p.tz, src);
+  return q;
+}
+
 struct SampleLane {
   float fv[9];    // populations with cz = g - 1 of stencil cell kc (zeros where the set has no such direction)
   double w;       // trilinear weight of stencil cell kc (0 for the wall cell itself, kc = 8)
@@ -100,36 +156,31 @@ struct SampleLane {
 };
 
 // phase 1: addresses and loads of this lane (lane 3k + g: stencil cell k, population group g; lanes 27-31 idle)
-__device__ __forceinline__ void wall_sample_issue(const WmArgs& a, int64_t c, const double y1v[3], int lane,
-                                                  SampleLane& sl) {
-  const int64_t nx = a.dm.nx, nxy = (int64_t)a.dm.nx * a.dm.ny;
+__device__ __forceinline__ void wall_sample_issue(const WmArgs& a, const SamplePoint& p, int lane, SampleLane& sl) {
   const int kc = lane / 3, g = lane - 3 * kc;
-  int x = (int)(c % nx), y = (int)((c / nx) % a.dm.ny), z = (int)(c / nxy);
-  double y1 = sqrt(y1v[0] * y1v[0] + y1v[1] * y1v[1] + y1v[2] * y1v[2]);
-  double nrm[3] = {y1v[0] / y1, y1v[1] / y1, y1v[2] / y1};
-  // velocity at x_w + h_s n, trilinear over the 8 surrounding cells (R15)
-  double px = x + a.hs * nrm[0], py = y + a.hs * nrm[1], pz = z + a.hs * nrm[2];
-  double fx = floor(px), fy = floor(py), fz = floor(pz);
-  double tx = px - fx, ty = py - fy, tz = pz - fz;
-  int ix = (int)fx, iy = (int)fy, iz = (int)fz;
-  int xx = x, yy = y, zz = z;
+  int xx = p.x, yy = p.y, zz = p.z;
   sl.flx = sl.fly = sl.flz = false;
   sl.w = 0.0;
   if (kc < 8) {
     int ox = kc & 1, oy = (kc >> 1) & 1, oz = (kc >> 2) & 1;
-    sl.w = (ox ? tx : 1.0 - tx) * (oy ? ty : 1.0 - ty) * (oz ? tz : 1.0 - tz);
-    xx = wrap_far(ix + ox, a.dm.nx, a.dm.mode[0], sl.flx);
-    yy = wrap_far(iy + oy, a.dm.ny, a.dm.mode[1], sl.fly);
-    zz = wrap_far(iz + oz, a.dm.nz, a.dm.mode[2], sl.flz);
+    sl.w = (ox ? p.tx : 1.0 - p.tx) * (oy ? p.ty : 1.0 - p.ty) * (oz ? p.tz : 1.0 - p.tz);
+    xx = wrap_near(p.ix + ox, a.dm.nx, a.dm.mode[0], sl.flx);
+    yy = wrap_near(p.iy + oy, a.dm.ny, a.dm.mode[1], sl.fly);
+    zz = wrap_near(p.iz + oz, a.dm.nz, a.dm.mode[2], sl.flz);
   }
+  const int64_t yz = (int64_t)a.dm.nx * (yy + (int64_t)a.dm.ny * zz);
 #pragma unroll
   for (int q = 0; q < 9; ++q) {  // cx = q % 3 - 1, cy = q / 3 - 1, cz = g - 1
     const int i = dir_index(q % 3 - 1, q / 3 - 1, g - 1);  // -1: the set has no such direction (D3Q19 corners)
-    sl.fv[q] = (kc < 9 && i >= 0) ? __ldg(a.f + pop_index_cx(a.dm, i, q % 3 - 1, xx, yy, zz)) : 0.f;
+    int xs = xx - a.dm.xs * (q % 3 - 1);                   // population storage, as pop_index
+    if (xs < 0) xs += a.dm.nx;
+    else if (xs >= a.dm.nx) xs -= a.dm.nx;
+    sl.fv[q] = (kc < 9 && i >= 0) ? __ldg(a.f + (int64_t)i * a.dm.n + yz + xs) : 0.f;
   }
 }
 
-// phase 2: v = (j + g/2)/rho of the nine cells (R11), weighted sum over the stencil -> v_s; the wall cell's own -> v_w
+// phase 2: v = (j + g/2)/rho of the nine cells (R11); v_s = weighted sum over the stencil as a tree over lanes 0, 3, ..,
+// 21 (valid on lane 0), v_w = the wall cell's own (every lane)
 __device__ __forceinline__ void wall_sample_reduce(const WmArgs& a, const SampleLane& sl, int lane, double vs[3],
                                                    double vw[3]) {
   const int g = lane % 3;
@@ -152,15 +203,15 @@ __device__ __forceinline__ void wall_sample_reduce(const WmArgs& a, const Sample
   if (sl.flx) v[0] = -v[0];
   if (sl.fly) v[1] = -v[1];
   if (sl.flz) v[2] = -v[2];
-  vs[0] = vs[1] = vs[2] = 0.0;
 #pragma unroll
-  for (int k = 0; k < 8; ++k) {
-    double wk = shfl_d(sl.w, 3 * k);
-#pragma unroll
-    for (int q = 0; q < 3; ++q) vs[q] += wk * shfl_d(v[q], 3 * k);
+  for (int q = 0; q < 3; ++q) {
+    vw[q] = shfl_d(v[q], 24);
+    double t = sl.w * v[q];    // lanes 3k + 1, 3k + 2 and the wall cell's carry values nobody reads (w = 0 on lane 24)
+    t += shfl_down_d(t, 12);   // stencil cell k + 4
+    t += shfl_down_d(t, 6);    // k + 2
+    t += shfl_down_d(t, 3);    // k + 1
+    vs[q] = t;
   }
-#pragma unroll
-  for (int q = 0; q < 3; ++q) vw[q] = shfl_d(v[q], 24);
 }
 
 // Musker's explicit profile and its slope (include/hhrr.h: hhrr_set_wall_function); residual U/u_tau - u+(y u_tau/nu)
@@ -318,24 +369,32 @@ __global__ void __launch_bounds__(128, BLOCKS_PER_SM) wall_sample_kernel(const _
 #pragma unroll
       for (int q = 0; q < 3; ++q) y_l[q] = a.wall_y1n[3 * (int64_t)e_l + q];
     }
+    const SamplePoint mine_p = sample_point(a, c_l, y_l);  // lanes >= WM_BATCH: a dummy cell, never used
     SampleLane sl[WM_BATCH];
 #pragma unroll
     for (int j = 0; j < WM_BATCH; ++j) {  // a batch's tail repeats its last cell (never out of range, no branch)
       const int src = min(j, count - 1 - base);
-      const int64_t c = __shfl_sync(0xffffffffu, c_l, src);
-      const double y1v[3] = {shfl_d(y_l[0], src), shfl_d(y_l[1], src), shfl_d(y_l[2], src)};
-      wall_sample_issue(a, c, y1v, lane, sl[j]);
+      wall_sample_issue(a, shfl_point(mine_p, src), lane, sl[j]);
     }
+    double my_vs[3] = {0, 0, 0}, my_vw[3] = {0, 0, 0};
 #pragma unroll
     for (int j = 0; j < WM_BATCH; ++j) {
       double vs[3], vw[3];
-      wall_sample_reduce(a, sl[j], lane, vs, vw);
-      if (lane == j && mine) {
+      wall_sample_reduce(a, sl[j], lane, vs, vw);  // vs valid on lane 0, vw on every lane
 #pragma unroll
-        for (int q = 0; q < 3; ++q) {
-          a.samp[6 * (int64_t)e_l + q] = vs[q];
-          a.samp[6 * (int64_t)e_l + 3 + q] = vw[q];
+      for (int q = 0; q < 3; ++q) {
+        const double s0 = shfl_d(vs[q], 0);
+        if (lane == j) {
+          my_vs[q] = s0;
+          my_vw[q] = vw[q];
         }
+      }
+    }
+    if (mine) {
+#pragma unroll
+      for (int q = 0; q < 3; ++q) {
+        a.samp[6 * (int64_t)e_l + q] = my_vs[q];
+        a.samp[6 * (int64_t)e_l + 3 + q] = my_vw[q];
       }
     }
   }

@@ -50,6 +50,7 @@ def test_library_is_sm100a_with_lineinfo(built):
 def test_velocity_set_of_each_build(built):
     from paper_2510_13726_b200 import binding as B
     assert B.lib(27).hhrr_velocity_set() == 27 and B.lib(19).hhrr_velocity_set() == 19
+    assert b"D3Q27" in B.lib(27).hhrr_version() and b"D3Q19" in B.lib(19).hhrr_version()
     p = B.make_params(128, 64, 64)
     assert B.workspace_bytes(p, q=19) < B.workspace_bytes(p, q=27)    # 19 instead of 27 planes per buffer
 

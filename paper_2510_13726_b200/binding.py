@@ -193,7 +193,7 @@ def workspace_bytes(params: Params, rotor_shape=None, q=27) -> int:
 class Lattice:
     """One lattice on one GPU.  Method names mirror include/hhrr.h without the prefix."""
 
-    def __init__(self, params: Params, rotor_shape=None, device="cuda:0", stream=None, q=27):
+    def __init__(self, params: Params, rotor_shape=None, device="cuda:0", stream=None, q=27, guard_bytes=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2510_13726_b200 needs a CUDA device (no CPU fallback)")
@@ -205,7 +205,13 @@ class Lattice:
         self.device = torch.device(device)
         nbytes = workspace_bytes(params, rotor_shape, q)
         with torch.cuda.device(self.device):
-            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            # guard_bytes > 0 (tests): canary regions of 0xA5 before and after the workspace handed to the library
+            self.guard_bytes = int(guard_bytes)
+            self._alloc = torch.empty(nbytes + 2 * self.guard_bytes, dtype=torch.uint8, device=self.device)
+            if self.guard_bytes:
+                self._alloc[:self.guard_bytes] = 0xA5
+                self._alloc[self.guard_bytes + nbytes:] = 0xA5
+            self.workspace = self._alloc[self.guard_bytes:self.guard_bytes + nbytes]
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             h = C.c_void_p()
             self._check(self.lib.hhrr_create(C.byref(params), C.c_void_p(self.workspace.data_ptr()), nbytes,
@@ -215,11 +221,20 @@ class Lattice:
     def _check(self, rc):
         return _check(rc, self.q)
 
+    def guards_intact(self):
+        """True if no kernel wrote outside the workspace (only meaningful with guard_bytes > 0)."""
+        import torch
+        self.synchronize()
+        torch.cuda.synchronize(self.device)
+        g, n = self.guard_bytes, self.workspace.numel()
+        return bool((self._alloc[:g] == 0xA5).all().item() and (self._alloc[g + n:] == 0xA5).all().item())
+
     def close(self):
         if getattr(self, "h", None):
             self.lib.hhrr_destroy(self.h)
             self.h = None
             self.workspace = None
+            self._alloc = None
 
     def __del__(self):
         try:

@@ -612,6 +612,45 @@ def test_moments_device_and_uhat_entry_points(oracle):
     G.close(); Oa.close()
 
 
+def test_no_kernel_writes_outside_the_workspace(oracle):
+    """compute-sanitizer is not available on this pool: the workspace handed to hhrr_create sits between two 1 MiB
+    canary regions, every kernel of the path runs (all variants, both tile shapes, region split, wall model, forces,
+    rotor look-ahead, halo pack / unpack, read-backs, the no-alloc entry point, D3Q19), and the canaries must be
+    untouched.  Extents are chosen so that tiles, rows and lists end exactly at the end of their arrays."""
+    import torch
+    from paper_2510_13726_b200 import binding as B
+    cases = [(I.case_rotor(128, 72, 72, 20.0, 4, omega=0.012), 5, 27), (I.case_rotor(256, 72, 72, 20.0, 3, omega=0.012), 5, 27),
+             (I.with_region_split(I.case_rotor(384, 72, 72, 20.0, 3, omega=0.012), margin=3), 5, 27),
+             (I.case_channel(128, 48, 16, 4), 5, 27), (I.case_channel(64, 48, 32, 3), 2, 27),
+             (I.case_sphere(48, 24, 24, 4.0, 3), 0, 27), (I.case_rotor(128, 72, 72, 20.0, 3, omega=0.012), 5, 19)]
+    for ext in [(1, 1, 1), (5, 1, 1), (33, 2, 3), (45, 19, 23)]:
+        rho, u = I.noisy_uniform(*ext, (0.02, 0.01, -0.01), 2e-3, 5)
+        cases.append((I.Case("tiny", *ext, 3, params=dict(I.DEFAULTS, tau0=0.6), rho=rho, u=u), 2, 27))
+    for case, variant, q in cases:
+        p = B.make_params(case.nx, case.ny, case.nz, mode=case.mode, **case.params)
+        L = B.Lattice(p, rotor_shape=None if case.rotor is None else case.rotor["sdf"].shape, q=q, guard_bytes=1 << 20)
+        L.set_kernel_variant(variant)
+        I.apply_case(case, L)
+        L.step(case.steps)
+        L.update_geometry()
+        L.moments(); L.populations(); L.cell_types(); L.wall_list(); L.wall_model_state(); L.forces(); L.check_finite()
+        L.cell_populations(np.arange(min(case.n, 5000), dtype=np.int64))
+        L.set_populations(L.populations())
+        k = len(L.wall_list()[0])
+        if k:
+            dev = L.device
+            L.wall_model_noalloc(k, None, torch.empty(k, dtype=torch.float64, device=dev),
+                                 torch.empty((k, 3), dtype=torch.float32, device=dev),
+                                 torch.empty((k, 6), dtype=torch.float32, device=dev))
+        if case.nz >= 4 and case.mode[2] == I.PERIODIC:
+            buf = torch.empty(L.halo_floats(), dtype=torch.float32, device=L.device)
+            for face in (0, 1):
+                L.halo_pack(face, buf); L.halo_unpack(1 - face, buf)
+        L.step(1)
+        assert L.guards_intact(), (case.name, case.nx, case.ny, case.nz, variant, q)
+        L.close()
+
+
 def test_zz_report_utau_error():
     """Not a check of its own: prints the largest relative u_tau difference the parity tests of this module saw."""
     if UTAU_ERR:

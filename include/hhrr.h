@@ -294,7 +294,7 @@ int hhrr_population_storage(const hhrr_lattice* L);
  * a side stream and a handful of ordering events that the library creates itself; hhrr_destroy releases them.)          */
 int hhrr_set_timing(hhrr_lattice* L, int enable);
 /* Launch shape of the default kernel (variant 5): planes per z-chunk of a tile column and tiles per thread-block
- * cluster (1, 2, 4, 8).  0 = automatic (16 planes, 12 with an FSI region; 30 / 22 on D3Q19; clusters of 2: measured on config 5,
+ * cluster (1, 2, 4, 8).  0 = automatic (16 planes, 12 with an FSI region; 40 / 22 on D3Q19; clusters of 2: measured on config 5,
  * profiles/r02_k2_chunk_scan.md).  Results do not depend on it; it exists so that the scan behind the defaults can be
  * repeated (bench.py --chunk-planes / --cluster).                                                               */
 int hhrr_set_launch_shape(hhrr_lattice* L, int32_t chunk_planes, int32_t cluster);

@@ -29,7 +29,8 @@ namespace hhrr {
 // 2 sectors per 16 with 128-cell rows, 2 per 8 with 64-cell rows.  64 x 8 serves lattices 128 x 4 cannot tile.
 template <int TX_, int TY_>
 struct XpCfg {
-  static constexpr int TX = TX_, TY = TY_, NS = 2, W = TX + 8;
+  // pipeline stages: two planes of 27 populations fill shared memory; the D3Q19 stages are 30 % smaller and a third one fits
+  static constexpr int TX = TX_, TY = TY_, NS = (Q == 19 && TX_ == 64) ? 3 : 2, W = TX + 8;
   static constexpr int WORKERS = TX * TY / 2, AUX = 96, THREADS = WORKERS + AUX + 32;
   // uhat ring plane: SY rows of SX floats; tile cell lx sits at column lx + 2 (an EVEN slot: a worker's cell pair
   // is one aligned 8-byte word), the x halo at columns 1 and TX + 2, columns 0 and TX + 3 are padding
@@ -545,9 +546,9 @@ static cudaError_t launch_shape(hhrr_lattice* L, WsArgs& a) {
   // share stay L2 hits only while they march within a few planes of each other.  Measured on config 5 with the
   // packed-fp32 workers (profiles/r02_k2_chunk_scan.md; bench.py --chunk-planes): 13-16 planes 4.01-4.03 ms, 18 planes
   // 4.06 ms, 22 planes 4.15 ms, 32 planes 4.51 ms (without clusters: 4.09 / 4.27 / 4.52 / 4.92 ms); with the region
-  // split 12 planes 3.88 ms, 16 planes 3.92 ms; D3Q19 (19 populations per cell plane) 16 / 23 / 30 planes 3.08 / 3.02 /
-  // 3.00 ms.  hhrr_set_launch_shape overrides.
-  const int auto_planes = Q == 27 ? (a.fsi.n > 0 ? 12 : 16) : (a.fsi.n > 0 ? 22 : 30);
+  // split 12 planes 3.88 ms, 16 planes 3.92 ms; D3Q19 (19 populations per cell plane, three pipeline stages) 16 / 23 / 30 /
+  // 40 / 52 / 73 planes 3.00 / 2.95 / 2.93 / 2.91 / 2.94 / 3.07 ms.  hhrr_set_launch_shape overrides.
+  const int auto_planes = Q == 27 ? (a.fsi.n > 0 ? 12 : 16) : (a.fsi.n > 0 ? 22 : 40);
   int nch = ws_zchunks(dm.nz, L->chunk_planes > 0 ? L->chunk_planes : auto_planes);
   a.zchunk = (dm.nz + nch - 1) / nch;
   nch = (dm.nz + a.zchunk - 1) / a.zchunk;

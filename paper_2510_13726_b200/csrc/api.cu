@@ -530,7 +530,14 @@ int hhrr_set_launch_shape(hhrr_lattice* L, int32_t chunk_planes, int32_t cluster
 int hhrr_set_lookahead(hhrr_lattice* L, int enable) {
   DeviceGuard guard_(L);
   if (!L) return fail(HHRR_E_ARG, "hhrr_set_lookahead: NULL lattice");
-  L->lookahead = enable != 0;
+  const bool on = enable != 0;
+  if (on && !L->lookahead) {
+    // Steps taken without the look-ahead evaluate every geometry in place: the alternate set (and the row band's
+    // view of it) is as old as the last step that used it.  The next geometry pass is a full one, which re-seeds it.
+    L->geometry_dirty = true;
+    L->geometry_current = false;
+  }
+  L->lookahead = on;
   return HHRR_OK;
 }
 

@@ -302,6 +302,17 @@ def test_geometry_look_ahead_changes_nothing(oracle):
     assert np.array_equal(A.forces(), Bv.forces()) or np.allclose(A.forces(), Bv.forces(), rtol=1e-12, atol=1e-18)
     e_rho, e_v = rel_linf(*A.moments(), *Oa.moments())
     assert e_rho <= TOL10 and e_v <= TOL10, (e_rho, e_v)
+    # switching the look-ahead back on after steps without it (the alternate geometry set is stale by then), and off again
+    A.step(79); Bv.step(79); Oa.step(79)      # 79 more steps without it: the blades end up midway between the stale ones
+    Bv.set_lookahead(True)
+    A.step(4); Bv.step(4); Oa.step(4)
+    Bv.set_lookahead(False)
+    A.step(3); Bv.step(3); Oa.step(3)
+    assert np.array_equal(A.populations(), Bv.populations())
+    for L in (A, Bv, Oa):
+        L.update_geometry()
+    compare_geometry(A, Oa)
+    compare_geometry(Bv, Oa)
     A.close(); Bv.close(); Oa.close()
 
 

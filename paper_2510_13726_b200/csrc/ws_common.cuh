@@ -1,5 +1,5 @@
-// ws_common.cuh -- pieces shared by the warp-specialised collide-stream kernels
-// (fused_ws.cu: one cell per producer lane; fused_ws2.cu: two x-adjacent cells per lane).
+// ws_common.cuh -- pieces shared by the fused collide-stream kernels
+// (fused_xpull.cu: TMA-fed, x-pull / yz-push storage; fused_ws.cu: warp-specialised, LDG-fed, post-stream storage).
 // CUDA path only; shares nothing with oracle/.
 #pragma once
 #include "cell_model.cuh"

@@ -278,7 +278,7 @@ def test_fused_kernels_are_deterministic(variant):
 
 
 def test_geometry_look_ahead_changes_nothing(oracle):
-    """Pass 1 of UpdatePorosityO for step n+1 runs ahead on a side stream (geometry.cu: launch_phi_ahead).  With it
+    """UpdatePorosityO of step n+1 runs ahead on a side stream into the alternate geometry set (geometry.cu: launch_geometry_ahead).  With it
     and without it (hhrr_set_lookahead) the populations stay bitwise equal; a rotor that is replaced, and a geometry
     evaluation asked for between steps, while a look-ahead pass is pending give the oracle's cell types, lists and
     flow."""

@@ -623,6 +623,28 @@ def test_moments_device_and_uhat_entry_points(oracle):
     G.close(); Oa.close()
 
 
+def test_rotor_with_static_body_and_mirror_planes(oracle):
+    """Rotor AND static geometry in one lattice (phi = min of the two; static list prefix + rotor-box suffix; static
+    cells inside the rotor box keep their rows in the row band), and a rotor whose blades cut through a MIRROR plane
+    (box clipped at the lattice, growth test / wall-model sampling / force links reflected): geometry bit-exact after
+    every step, flow, u_tau, forces and torques at 1e-5."""
+    import dataclasses
+    base = I.case_rotor(128, 72, 72, 20.0, 10, omega=0.012)
+    n = base.n
+    # a static ball just downstream of the rotor disc, inside the rotor box in y-z, tag 5 at rest
+    phi = I.sphere_phi(128, 72, 72, (41.0, 48.0, 30.0), 5.0)
+    case = dataclasses.replace(base, name="rotor+ball", phi=phi, tag=np.full(n, 5, np.uint8))
+    for variant in (5, 2):
+        run_parity(oracle, case, 10, variant, TOL10, check_every=1)
+    # blades through the y = -1/2 mirror plane, hub 12 cells above it
+    rotor = dict(base.rotor, centre=(32.0, 12.0, 35.5))
+    case = dataclasses.replace(base, name="rotor@mirror", mode=(I.PERIODIC, I.MIRROR, I.MIRROR), rotor=rotor)
+    run_parity(oracle, case, 10, 5, TOL10, check_every=1)
+    run_parity(oracle, dataclasses.replace(case, nx=96, rho=np.ones(96 * 72 * 72, np.float32),
+                                           u=np.tile(np.array([[0.04], [0.0], [0.0]], np.float32), (1, 96 * 72 * 72))),
+               6, 2, TOL10, check_every=2)
+
+
 def test_no_kernel_writes_outside_the_workspace(oracle):
     """compute-sanitizer is not available on this pool: the workspace handed to hhrr_create sits between two 1 MiB
     canary regions, every kernel of the path runs (all variants, both tile shapes, region split, wall model, forces,

@@ -287,17 +287,15 @@ def run_ours(args, rank, world, local_rank):
     thrust = float(F[-1, 1:5, 0].sum()) if case.rotor is not None else None
     # Definition 3 / Eq. 26: C_T = T / (0.5 rho pi r^2 U_inf^2), lattice units, rho = 1;
     # after a few hundred steps from rest it is a start-up value, not the converged one of the paper's Fig. 7
-    c_t = None
-    if thrust is not None and case.fringe is not None:
-        r_rot = 0.5 * (case.rotor["sdf"].shape[1] - 1) * case.rotor["spacing"] - 4.0   # grid half-extent minus its 4-cell margin
-        c_t = thrust / (0.5 * np.pi * r_rot ** 2 * case.fringe[2][0] ** 2)
-    # torque of the rotor about its axis (+x) from hhrr_get_torques and the usual power coefficient
-    # C_P = M_x Omega / (0.5 rho pi r^2 U_inf^3) (not defined in the paper, start-up value as above)
-    torque = c_p = None
+    # (hhrr_get_rotor_coefficients).  Torque of the rotor about its axis (+x) from hhrr_get_torques and the usual power
+    # coefficient C_P = M_x Omega / (0.5 rho pi r^2 U_inf^3) (not defined in the paper, start-up value)
+    c_t = torque = c_p = None
     if case.rotor is not None:
         torque = float(L.torques(L.step_count() - 1, 1)[0, 1:5, 0].sum())
-        if c_t is not None:
-            c_p = torque * case.rotor["omega"] / (0.5 * np.pi * r_rot ** 2 * case.fringe[2][0] ** 3)
+        if case.fringe is not None:
+            r_rot = 0.5 * (case.rotor["sdf"].shape[1] - 1) * case.rotor["spacing"] - 4.0   # grid half-extent minus its 4-cell margin
+            ct, cp = L.rotor_coefficients(1.0, case.fringe[2][0], r_rot, L.step_count() - 1, 1)
+            c_t, c_p = float(ct[0]), float(cp[0])
 
     # the same workload with the paper's bulk / FSI region split (Listing 2): reported beside the
     # headline, which keeps HHRRLBM in every cell

@@ -200,6 +200,15 @@ int hhrr_get_forces(hhrr_lattice* L, int64_t first_step, int64_t n_steps, double
  * integrates forces only; the torque is SURVEY 8(f)-4's output for torque / power coefficients.
  * Same layout, history and error behaviour as hhrr_get_forces; M is a HOST buffer.            */
 int hhrr_get_torques(hhrr_lattice* L, int64_t first_step, int64_t n_steps, double* M);
+/* Thrust coefficient, Definition 3 / Eq. 26: C_T = T / (0.5 rho pi r^2 U_inf^2), T = "the integral
+ * of all axial forces acting on the rotor" = sum over the rotor's elements (tags 1..n_tags of hhrr_set_rotor) of
+ * F_k . a, with F_k of hhrr_get_forces and a the unit rotor axis -- and, from the torques of the same elements, the
+ * power coefficient C_P = (sum_k M_k . a) omega / (0.5 rho pi r^2 U_inf^3) (the paper reports C_T
+ * only).  rho, u_inf, radius: lattice units, all > 0 (HHRR_E_ARG otherwise).  c_t, c_p: HOST arrays of n_steps
+ * doubles, one value per step, either may be NULL.  Steps as for hhrr_get_forces; HHRR_E_STATE without a rotor.
+ * Host arithmetic on the recorded forces: synchronises the stream.                                                  */
+int hhrr_get_rotor_coefficients(hhrr_lattice* L, int64_t first_step, int64_t n_steps, double rho, double u_inf,
+                                double radius, double* c_t, double* c_p);
 int64_t hhrr_force_history(void);
 /* Cell types / tags / porosity of the last evaluated geometry (any pointer nullable). */
 int hhrr_get_cell_types(hhrr_lattice* L, uint8_t* type, uint8_t* tag, float* d);

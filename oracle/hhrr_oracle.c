@@ -1130,6 +1130,27 @@ int ohrr_get_torques(const ohrr_lattice *L, int64_t first, int64_t count, double
   memcpy(M, L->torque + first * MAX_TAGS * 3, sizeof(double) * count * MAX_TAGS * 3);
   return 0;
 }
+/* Definition 3 / Eq. 26: C_T = T / (0.5 rho pi r^2 U^2), T = "the integral of all axial forces
+ * acting on the rotor" = sum over the rotor's elements (tags 1..n_tags) of F_k . a, a = the (unit) rotor axis.  With the
+ * torques of the same elements, the power coefficient C_P = (sum_k M_k . a) Omega / (0.5 rho pi r^2 U^3) (torque /
+ * power output of SURVEY 8(f)-4; the paper reports C_T only).  One value per step. */
+int ohrr_rotor_coefficients(const ohrr_lattice *L, int64_t first, int64_t count, double rho, double u_inf,
+                            double radius, double *c_t, double *c_p) {
+  if (!L->has_rotor || first < 0 || first + count > L->step || !(rho > 0) || !(u_inf > 0) || !(radius > 0)) return -1;
+  const double *ax = L->rot.axis; /* a unit vector by the rotor description's contract */
+  const double area = 3.14159265358979323846 * radius * radius;
+  for (int64_t s = 0; s < count; ++s) {
+    double T = 0, Mz = 0;
+    for (int k = 1; k <= L->rot.n_tags; ++k)
+      for (int a = 0; a < 3; ++a) {
+        T += L->force[((first + s) * MAX_TAGS + k) * 3 + a] * ax[a];
+        Mz += L->torque[((first + s) * MAX_TAGS + k) * 3 + a] * ax[a];
+      }
+    if (c_t) c_t[s] = T / (0.5 * rho * area * u_inf * u_inf);
+    if (c_p) c_p[s] = Mz * L->rot.omega / (0.5 * rho * area * u_inf * u_inf * u_inf);
+  }
+  return 0;
+}
 /* geometry of the LAST evaluated step (call ohrr_update_geometry first for the current one) */
 int ohrr_get_cell_types(const ohrr_lattice *L, uint8_t *type, uint8_t *tag, double *d) {
   memcpy(type, L->type, L->n);

@@ -70,6 +70,8 @@ def lib(q=27):
         L.ohrr_create.restype = C.c_void_p
         L.ohrr_create.argtypes = [C.POINTER(Params)]
         L.ohrr_destroy.argtypes = [C.c_void_p]
+        L.ohrr_rotor_coefficients.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_double, C.c_double,
+                                              C.c_void_p, C.c_void_p]
         L.ohrr_spalding_f.restype = C.c_double
         L.ohrr_spalding_f.argtypes = [C.c_double] * 6
         L.ohrr_newton_utau.restype = C.c_double
@@ -299,6 +301,16 @@ class Lattice:
         if rc:
             raise RuntimeError("ohrr_get_torques: range")
         return M
+
+    def rotor_coefficients(self, rho, u_inf, radius, first=0, count=None):
+        """(C_T, C_P) per step: Definition 3 / Eq. 26 and the power coefficient of the same rotor."""
+        if count is None:
+            count = self.lib.ohrr_step_count(self._h) - first
+        ct = np.zeros(count); cp = np.zeros(count)
+        rc = self.lib.ohrr_rotor_coefficients(self._h, first, count, rho, u_inf, radius, _p(ct), _p(cp))
+        if rc:
+            raise RuntimeError("ohrr_rotor_coefficients: no rotor, bad range or bad argument")
+        return ct, cp
 
     def cell_types(self):
         t = np.zeros(self.n, np.uint8); g = np.zeros(self.n, np.uint8); d = np.zeros(self.n)

@@ -26,7 +26,7 @@ SYMBOLS = [
     "hhrr_workspace_bytes", "hhrr_create", "hhrr_destroy", "hhrr_init_equilibrium",
     "hhrr_set_static_geometry", "hhrr_set_body", "hhrr_set_fringe", "hhrr_set_rotor",
     "hhrr_enable_wall_model", "hhrr_update_geometry", "hhrr_step", "hhrr_step_count",
-    "hhrr_get_moments", "hhrr_get_moments_device", "hhrr_get_forces", "hhrr_get_torques", "hhrr_force_history",
+    "hhrr_get_moments", "hhrr_get_moments_device", "hhrr_get_forces", "hhrr_get_torques", "hhrr_get_rotor_coefficients", "hhrr_force_history",
     "hhrr_get_cell_types", "hhrr_get_wall_list", "hhrr_get_wall_state", "hhrr_get_populations",
     "hhrr_set_populations", "hhrr_get_cell_populations", "hhrr_get_uhat", "hhrr_check_finite", "hhrr_set_kernel_variant",
     "hhrr_population_storage", "hhrr_set_fsi_region", "hhrr_set_wall_function", "hhrr_set_wall_model_variant",
@@ -95,6 +95,7 @@ def lib(q=27):
         L.hhrr_get_moments_device.argtypes = [vp, vp, vp]
         L.hhrr_get_forces.argtypes = [vp, i64, i64, vp]
         L.hhrr_get_torques.argtypes = [vp, i64, i64, vp]
+        L.hhrr_get_rotor_coefficients.argtypes = [vp, i64, i64, C.c_double, C.c_double, C.c_double, vp, vp]
         L.hhrr_force_history.restype = i64
         L.hhrr_get_cell_types.argtypes = [vp, vp, vp, vp]
         L.hhrr_get_wall_list.argtypes = [vp, i64, vp, vp, vp, vp, C.POINTER(i64)]
@@ -348,6 +349,16 @@ class Lattice:
         if count:
             self._check(self.lib.hhrr_get_torques(self.h, int(first), int(count), _p(M)))
         return M
+
+    def rotor_coefficients(self, rho, u_inf, radius, first=0, count=None):
+        """(C_T, C_P) per step: thrust coefficient of Eq. 26 and power coefficient (include/hhrr.h)."""
+        if count is None:
+            count = self.step_count() - first
+        ct = np.zeros(count)
+        cp = np.zeros(count)
+        self._check(self.lib.hhrr_get_rotor_coefficients(self.h, int(first), int(count), float(rho), float(u_inf),
+                                                         float(radius), _p(ct), _p(cp)))
+        return ct, cp
 
     def cell_types(self):
         t = np.empty(self.n, np.uint8)

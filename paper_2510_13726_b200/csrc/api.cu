@@ -675,6 +675,34 @@ int hhrr_get_torques(hhrr_lattice* L, int64_t first_step, int64_t n_steps, doubl
   return get_force_ring(L, L ? L->torque : nullptr, "hhrr_get_torques", first_step, n_steps, M);
 }
 
+int hhrr_get_rotor_coefficients(hhrr_lattice* L, int64_t first_step, int64_t n_steps, double rho, double u_inf,
+                                double radius, double* c_t, double* c_p) {
+  DeviceGuard guard_(L);
+  if (!L || n_steps < 0 || (!c_t && !c_p)) return fail(HHRR_E_ARG, "hhrr_get_rotor_coefficients: bad argument");
+  if (!(rho > 0.0) || !(u_inf > 0.0) || !(radius > 0.0))
+    return fail(HHRR_E_ARG, "hhrr_get_rotor_coefficients: rho, u_inf and radius must be positive");
+  if (!L->has_rotor) return fail(HHRR_E_STATE, "hhrr_get_rotor_coefficients: no rotor set");
+  std::vector<double> F((size_t)n_steps * MAX_TAGS * 3), M((size_t)n_steps * MAX_TAGS * 3);
+  int rc = get_force_ring(L, L->force, "hhrr_get_rotor_coefficients", first_step, n_steps, F.data());
+  if (rc) return rc;
+  rc = get_force_ring(L, L->torque, "hhrr_get_rotor_coefficients", first_step, n_steps, M.data());
+  if (rc) return rc;
+  const double* ax = L->rot.axis;  // unit vector (include/hhrr.h: hhrr_rotor_desc)
+  const double q = 0.5 * rho * M_PI * radius * radius * u_inf * u_inf;  // denominator of Eq. 26
+  for (int64_t s = 0; s < n_steps; ++s) {
+    double thrust = 0.0, torque = 0.0;  // axial force on / axial torque on the rotor: all its elements
+    for (int k = 1; k <= L->rot.n_tags; ++k) {
+      const double* f = F.data() + ((size_t)s * MAX_TAGS + k) * 3;
+      const double* m = M.data() + ((size_t)s * MAX_TAGS + k) * 3;
+      thrust += f[0] * ax[0] + f[1] * ax[1] + f[2] * ax[2];
+      torque += m[0] * ax[0] + m[1] * ax[1] + m[2] * ax[2];
+    }
+    if (c_t) c_t[s] = thrust / q;
+    if (c_p) c_p[s] = torque * L->rot.omega / (q * u_inf);
+  }
+  return HHRR_OK;
+}
+
 int hhrr_get_cell_types(hhrr_lattice* L, uint8_t* type, uint8_t* tag, float* d) {
   DeviceGuard guard_(L);
   if (!L) return fail(HHRR_E_ARG, "hhrr_get_cell_types: NULL lattice");

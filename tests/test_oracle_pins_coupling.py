@@ -675,3 +675,66 @@ def test_wall_model_across_a_mirror_plane_equals_even_extension(oracle):
     assert np.allclose(uta, utb[lower], rtol=1e-12)
     Fa, Fb = A.forces()[-1, 1], B.forces()[-1, 1]             # the whole ball: twice the half's in-plane force,
     assert np.allclose(Fa[[0, 2]], 0.5 * Fb[[0, 2]], rtol=0, atol=1e-13) and abs(Fb[1]) < 1e-13   # no normal one
+
+
+# ---- Definition 3 / Eq. 26: thrust coefficient (and the power coefficient of the same rotor) -------------------
+def _two_ball_rotor(O, axis, omega, theta0, u0, steps=6, n=24):
+    """A 'rotor' of two off-axis balls (elements 1 and 2) in a periodic box with uniform initial velocity u0 e_x."""
+    g = 41; sp = 0.5
+    ax = -10 + sp * np.arange(g)
+    Z, Y, X = np.meshgrid(ax, ax, ax, indexing="ij")
+    b1 = np.sqrt(X ** 2 + (Y - 5.0) ** 2 + Z ** 2) - 2.5
+    b2 = np.sqrt(X ** 2 + (Y + 5.0) ** 2 + Z ** 2) - 2.5
+    sdf = np.clip(np.minimum(b1, b2), -4, 4).astype(np.float32)
+    tag = np.where(b1 < b2, 1, 2).astype(np.uint8)
+    L = O.Lattice(O.make_params(n, n, n, tau0=0.6))
+    L.set_rotor(sdf, tag, sp, (-10, -10, -10), (11.5, 11.5, 11.5), axis, omega, theta0, 2)
+    u = np.zeros((3, n ** 3)); u[0] = u0
+    L.init_equilibrium(np.ones(n ** 3), u, False)
+    L.step(steps)
+    return L
+
+
+def test_rotor_coefficients_definition_3(oracle):
+    """Eq. 26: C_T = T / (0.5 rho pi r^2 U^2) with T the axial force on ALL elements of the rotor; the
+    power coefficient uses the axial torque times Omega.  Pinned by: the sums written out from forces() / torques()
+    ; the scaling in U and r; the same motion described about the opposite axis (C_T changes sign,
+    C_P does not); the physics -- a flow along the axis pushes the rotor downstream (C_T > 0), still fluid brakes a
+    driven rotor (C_P < 0), a rotor at rest delivers no power (C_P = 0)."""
+    rho, U, r = 1.0, 0.05, 7.5
+    L = _two_ball_rotor(oracle, (1.0, 0.0, 0.0), 0.03, 0.3, U)
+    ct, cp = L.rotor_coefficients(rho, U, r)
+    F, M = L.forces(), L.torques()
+    q = 0.5 * rho * np.pi * r * r * U * U
+    assert np.allclose(ct, (F[:, 1, 0] + F[:, 2, 0]) / q, rtol=1e-13, atol=0)
+    assert np.allclose(cp, (M[:, 1, 0] + M[:, 2, 0]) * 0.03 / (q * U), rtol=1e-13, atol=0)
+    assert np.all(np.abs(F[:, 1, 0]) > 0) and np.all(np.abs(F[:, 2, 0]) > 0)      # both elements count
+    assert np.all(ct[1:] > 0)
+    ct2, cp2 = L.rotor_coefficients(rho, 2 * U, 2 * r)
+    assert np.allclose(ct2, ct / 16, rtol=1e-13) and np.allclose(cp2, cp / 32, rtol=1e-13)
+    ct3, cp3 = L.rotor_coefficients(rho, U, r, first=2, count=3)
+    assert np.array_equal(ct3, ct[2:5]) and np.array_equal(cp3, cp[2:5])
+    # an axis along y: the y components count
+    Ly = _two_ball_rotor(oracle, (0.0, 1.0, 0.0), 0.03, 0.3, U)
+    cty, cpy = Ly.rotor_coefficients(rho, U, r)
+    Fy, My = Ly.forces(), Ly.torques()
+    assert np.allclose(cty, (Fy[:, 1, 1] + Fy[:, 2, 1]) / q, rtol=1e-13, atol=0)
+    assert np.allclose(cpy, (My[:, 1, 1] + My[:, 2, 1]) * 0.03 / (q * U), rtol=1e-13, atol=0)
+    assert np.max(np.abs(Fy[:, 1:3, 0])) > 10 * np.max(np.abs(cty * q))       # the drag along x is NOT the thrust here
+    Ly.close()
+    # the same motion about the opposite axis
+    Lm = _two_ball_rotor(oracle, (-1.0, 0.0, 0.0), -0.03, -0.3, U)
+    ctm, cpm = Lm.rotor_coefficients(rho, U, r)
+    assert np.allclose(Lm.forces(), F, rtol=1e-12, atol=1e-18)
+    assert np.allclose(ctm, -ct, rtol=1e-10) and np.allclose(cpm, cp, rtol=1e-10)
+    # still fluid brakes a driven rotor; a rotor at rest delivers no power
+    Ls = _two_ball_rotor(oracle, (1.0, 0.0, 0.0), 0.03, 0.0, 0.0)
+    _, cps = Ls.rotor_coefficients(rho, U, r)
+    assert np.all(cps[1:] < 0)
+    L0 = _two_ball_rotor(oracle, (1.0, 0.0, 0.0), 0.0, 0.0, U)
+    ct0, cp0 = L0.rotor_coefficients(rho, U, r)
+    assert np.all(cp0 == 0) and np.all(ct0[1:] > 0)
+    with pytest.raises(RuntimeError):
+        L.rotor_coefficients(rho, 0.0, r)
+    for x in (L, Lm, Ls, L0):
+        x.close()

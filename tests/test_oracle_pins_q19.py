@@ -146,6 +146,7 @@ def test_q19_force_and_torque_structure(o19):
     P.test_force_vanishes_for_comoving_solid(o19)
     P.test_torque_of_hydrostatic_load_closed_form(o19)
     PC.test_force_solid_velocity_term_is_minus_us_times_mass_inflow(o19)
+    PC.test_rotor_coefficients_definition_3(o19)
 
 
 def test_q19_half_channel_wall_drag_equals_body_force(o19):

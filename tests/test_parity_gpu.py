@@ -89,6 +89,10 @@ def run_parity(oracle, case, steps, variant, tol, check_every=None, force_tol=No
     e_rho, e_v = rel_linf(*G.moments(), *Oa.moments())
     assert e_rho <= tol and e_v <= tol, (e_rho, e_v)
     compare_forces(G, Oa, force_tol or tol)
+    if case.rotor is not None:   # Eq. 26: thrust coefficient, and the power coefficient of the same rotor
+        R, U = 0.25 * case.ny, 0.04
+        for g, o in zip(G.rotor_coefficients(1.0, U, R), Oa.rotor_coefficients(1.0, U, R)):
+            assert len(g) == steps and np.max(np.abs(g - o)) <= (force_tol or tol) * np.max(np.abs(o)), (g, o)
     G.close(); Oa.close()
     return e_rho, e_v
 

@@ -551,6 +551,9 @@ def test_force_history_ring_and_errors(oracle):
         G.set_kernel_variant(7)
     with pytest.raises(B.HhrrError):
         G.cell_populations([case.n])         # out of range
+    with pytest.raises(B.HhrrError) as err:
+        G.rotor_coefficients(1.0, 0.05, 4.0, 4190, 10)   # Eq. 26 needs a rotor: this lattice holds a static sphere
+    assert err.value.code == -5                          # HHRR_E_STATE
     G.step(0)
     assert G.step_count() == 4200
     G.close(); Oa.close()

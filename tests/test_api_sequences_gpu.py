@@ -1,0 +1,103 @@
+"""Seeded random sequences of API calls on a small rotor lattice, the CUDA library and the oracle side by side (-m gpu).
+
+The step schedule of the library keeps state between calls -- the geometry written ahead into the alternate set, the
+wall-model state and its valid bits, the storage form of the populations, the force ring -- and every setter has to
+leave that state consistent.  The parity tests walk the paths one at a time; here they are mixed: steps of varying
+length, geometry evaluations between steps, the look-ahead switched off and on, the three kernel variants, other
+z-chunk lengths and cluster sizes, the wall model switched off and on, a replaced rotor (other speed, sense and phase),
+the bulk / FSI region split set and cleared, and a checkpoint restored into a fresh lattice.  After every block of
+steps: cell types, tags, wall list and valid bits bit-exact, porosity, u_tau, flow and the forces of those steps at the
+parity tolerance (the sequence is at most 40 steps long).
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from paper_2510_13726_b200 import inputs as I
+from test_parity_gpu import _gpu_lattice, _ora_lattice, compare_geometry, rel_linf
+
+pytestmark = pytest.mark.gpu
+
+TOL = 2e-5      # TOL10 = 1e-5 holds at 10 steps; these runs are up to 40 steps long
+
+
+def _fresh_gpu(case, settings):
+    """A new CUDA lattice in the state `settings` describes (what a restart would set up before loading a checkpoint)."""
+    c = dataclasses.replace(case, rotor=settings["rotor"], wall_model=settings["wm"], fsi_boxes=settings["boxes"])
+    G = _gpu_lattice(c, settings["variant"])
+    G.set_lookahead(settings["lookahead"])
+    G.set_launch_shape(*settings["shape"])
+    return G
+
+
+@pytest.mark.parametrize("seed", [11, 12, 13, 14, 15, 16, 17, 18])
+def test_random_api_sequence_matches_the_oracle(oracle, seed):
+    rng = np.random.default_rng(seed)
+    case = I.case_rotor(128, 48, 48, 12.0, 40, omega=0.02)
+    split_boxes = I.with_region_split(case).fsi_boxes
+    settings = dict(rotor=case.rotor, wm=True, boxes=None, variant=5, lookahead=True, shape=(0, 0))
+    G, Oa = _gpu_lattice(case, 5), _ora_lattice(oracle, case)
+    ops = ["step"] * 5 + ["update_geometry", "lookahead", "variant", "shape", "wm", "rotor", "region", "checkpoint"]
+    done, log, worst = 0, [], 0.0
+    while done < 40:
+        op = ops[rng.integers(len(ops))]
+        if op == "step":
+            k = int(min(rng.choice([1, 1, 2, 3, 5]), 40 - done))
+            G.step(k); Oa.step(k)
+            done += k
+            log.append(f"step({k})")
+            try:
+                compare_geometry(G, Oa, TOL)
+            except AssertionError as e:
+                raise AssertionError(f"{e} after: " + " ".join(log)) from None
+            e_rho, e_v = rel_linf(*G.moments(), *Oa.moments())
+            worst = max(worst, e_rho, e_v)
+            assert e_rho <= TOL and e_v <= TOL, (e_rho, e_v, log)
+            Fg, Fo = G.forces(done - k, k), Oa.forces(done - k, k)
+            assert np.max(np.abs(Fg - Fo)) <= TOL * max(np.max(np.abs(Fo)), 1e-30), log
+            Mg, Mo = G.torques(done - k, k), Oa.torques(done - k, k)
+            assert np.max(np.abs(Mg - Mo)) <= TOL * max(np.max(np.abs(Mo)), 1e-30), log
+        elif op == "update_geometry":
+            G.update_geometry(); Oa.update_geometry()
+            log.append(op)
+            try:
+                compare_geometry(G, Oa, TOL)
+            except AssertionError as e:
+                raise AssertionError(f"{e} after: " + " ".join(log)) from None
+        elif op == "lookahead":
+            settings["lookahead"] = bool(rng.integers(2))
+            G.set_lookahead(settings["lookahead"])
+            log.append(f"lookahead({settings['lookahead']})")
+        elif op == "variant":
+            settings["variant"] = int(rng.choice([0, 2, 5]))
+            G.set_kernel_variant(settings["variant"])
+            log.append(f"variant({settings['variant']})")
+        elif op == "shape":
+            settings["shape"] = (int(rng.choice([0, 5, 9, 16, 48])), int(rng.choice([0, 1, 2])))
+            G.set_launch_shape(*settings["shape"])
+            log.append(f"shape{settings['shape']}")
+        elif op == "wm":
+            settings["wm"] = bool(rng.integers(2))
+            G.enable_wall_model(settings["wm"]); Oa.enable_wall_model(settings["wm"])
+            log.append(f"wm({settings['wm']})")
+        elif op == "rotor":
+            settings["rotor"] = dict(case.rotor, omega=float(rng.uniform(-0.03, 0.03)), theta0=float(rng.uniform(0, 6.28)))
+            G.set_rotor(**settings["rotor"]); Oa.set_rotor(**settings["rotor"])
+            log.append("rotor(omega=%.3f)" % settings["rotor"]["omega"])
+        elif op == "region":
+            settings["boxes"] = None if settings["boxes"] else split_boxes
+            G.set_fsi_region(settings["boxes"] or []); Oa.set_fsi_region(settings["boxes"] or [])
+            log.append("region(%s)" % ("on" if settings["boxes"] else "off"))
+        elif op == "checkpoint" and done > 0:
+            # hhrr_set_wall_model_state evaluates the geometry of the step to come (include/hhrr.h): a checkpoint is
+            # taken of an evaluated state, on both sides -- a setter since the last step may have left it pending
+            G.update_geometry(); Oa.update_geometry()
+            f, state, n = G.populations(), G.wall_model_state(), G.step_count()
+            G.close()
+            G = _fresh_gpu(case, settings)
+            G.set_step_count(n); G.set_populations(f); G.set_wall_model_state(*state)
+            log.append("checkpoint")
+    G.check_finite()
+    print(f"seed {seed}: {len(log)} calls, worst rel-Linf {worst:.2e}: " + " ".join(log))
+    G.close(); Oa.close()

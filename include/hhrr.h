@@ -215,7 +215,9 @@ int hhrr_get_cell_types(hhrr_lattice* L, uint8_t* type, uint8_t* tag, float* d);
 /* Wall-model cell list in ascending cell index.  *count receives the list length;
  * at most `capacity` entries are written.  idx: cell index; y1n: 3 doubles per entry
  * (wall distance times unit normal); u_tau: last friction velocity;
- * valid: 1 if the cell carries a wall-model state.  Array pointers nullable.         */
+ * valid: 1 if the cell carries a wall-model state -- only then is u_tau ever read (the
+ * Newton warm start; a cell without state starts from Eq. 20); what the array keeps for a
+ * cell without state is history.  Array pointers nullable.                            */
 int hhrr_get_wall_list(hhrr_lattice* L, int64_t capacity, int32_t* idx, double* y1n, double* u_tau,
                        uint8_t* valid, int64_t* count);
 /* Wall-model output of one cell: slip velocity u_wm[3] and strain S_wm[6] (xx yy zz xy xz yz). */
@@ -233,8 +235,10 @@ int hhrr_set_populations(hhrr_lattice* L, const float* f_minus_w);
  * stored (fp32), valid flag.  *count = number of wall cells; nothing else is written if capacity < *count.   */
 int hhrr_get_wall_model_state(hhrr_lattice* L, int64_t capacity, int32_t* idx, double* u_tau, float* u_wm, float* s_wm,
                               uint8_t* valid, int64_t* count);
-/* Restores it: evaluates the geometry of the current step if needed, then writes the state of every listed
- * cell that belongs to the wall-model set (others are ignored).                                              */
+/* Restores it: evaluates the geometry of the current step if needed (as hhrr_update_geometry does: state of cells
+ * outside its wall-model set is dropped), then writes the state of every listed cell that belongs to that set
+ * (others are ignored).  Save a checkpoint from an evaluated state -- after a step, or after hhrr_update_geometry
+ * when a setter was called since -- and restore it under the same setters: the run then continues as above.      */
 int hhrr_set_wall_model_state(hhrr_lattice* L, int64_t count, const int32_t* idx, const double* u_tau, const float* u_wm,
                               const float* s_wm, const uint8_t* valid);
 /* Sets the step counter (rotor angle theta0 + step * omega; slot of the force ring). */

@@ -20,6 +20,8 @@
 // x axis (xpull_supported); other lattices keep post-stream storage and run variant 2.
 #include <cuda.h>
 
+#include <cstdlib>
+
 #include "ws_common.cuh"
 
 namespace hhrr {
@@ -549,15 +551,34 @@ static cudaError_t launch_shape(hhrr_lattice* L, WsArgs& a) {
   // split 12 planes 3.88 ms, 16 planes 3.92 ms; D3Q19 (19 populations per cell plane, three pipeline stages) 16 / 23 / 30 /
   // 40 / 52 / 73 planes 3.00 / 2.95 / 2.93 / 2.91 / 2.94 / 3.07 ms.  hhrr_set_launch_shape overrides.
   const int auto_planes = Q == 27 ? (a.fsi.n > 0 ? 12 : 16) : (a.fsi.n > 0 ? 22 : 40);
-  int nch = ws_zchunks(dm.nz, L->chunk_planes > 0 ? L->chunk_planes : auto_planes);
-  a.zchunk = (dm.nz + nch - 1) / nch;
-  nch = (dm.nz + a.zchunk - 1) / a.zchunk;
   if (!L->sm_count &&
       (cudaDeviceGetAttribute(&L->sm_count, cudaDevAttrMultiProcessorCount, L->device) != cudaSuccess || L->sm_count < 1))
     L->sm_count = 148;
+  const int ntiles = (dm.nx / C::TX) * (dm.ny / C::TY);
+  int nch = ws_zchunks(dm.nz, L->chunk_planes > 0 ? L->chunk_planes : auto_planes);
+  if (L->chunk_planes <= 0 && (long long)ntiles * nch < 12LL * L->sm_count) {
+    // A lattice of a few waves of blocks: the time is (waves of blocks) x (planes a block walks, its two overlap
+    // planes included), and a last wave that is nearly empty costs as much as a full one.  Among chunk lengths
+    // between 6 planes and twice the usual one take the cheapest, the one nearest the usual length among equals
+    // (config 3, 256 x 128 x 128: 9 chunks, 576 blocks in 4 waves of 17 planes, instead of 8 x 64 = 512 in 4 of 18).
+    long long best = -1;
+    int best_n = nch;
+    for (int c = 1; c <= dm.nz; ++c) {
+      const int planes = (dm.nz + c - 1) / c;
+      if (planes > 2 * auto_planes || planes < 6) continue;
+      if ((dm.nz + planes - 1) / planes != c) continue;  // not a chunk count of its own
+      const long long waves = ((long long)ntiles * c + L->sm_count - 1) / L->sm_count, cost = waves * (planes + 2);
+      if (best < 0 || cost < best || (cost == best && abs(planes - auto_planes) < abs((dm.nz + best_n - 1) / best_n - auto_planes))) {
+        best = cost;
+        best_n = c;
+      }
+    }
+    nch = best_n;
+  }
+  a.zchunk = (dm.nz + nch - 1) / nch;
+  nch = (dm.nz + a.zchunk - 1) / a.zchunk;
   a.nch = nch;
   a.group = L->sm_count;  // one tile per SM and wave (one block per SM: shared memory)
-  const int ntiles = (dm.nx / C::TX) * (dm.ny / C::TY);
   dim3 grid((unsigned)(ntiles * nch));
   // Two x-adjacent tiles form a thread-block cluster (no cluster barrier, no distributed shared memory): the pair
   // starts together on neighbouring SMs and asks L2 for the x-halo sectors it shares at the same time.  Measured

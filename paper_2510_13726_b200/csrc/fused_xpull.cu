@@ -84,7 +84,7 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map
       ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar)
       : "memory");
 }
-// register reallocation between warpgroups: 256 * 208 + 128 * 88 = 384 * 168
+// register reallocation between warpgroups: 256 * 192 + 128 * 96 = 384 * 160 (the launch allocation)
 template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 
@@ -120,7 +120,11 @@ __device__ __forceinline__ void push_store_yz(const Dom& dm, float* __restrict__
 }  // namespace
 
 template <class C>
-__global__ void __maxnreg__(160)  // 384 threads x 160 = 61440 registers: 4096 stay free per SM for the side-stream kernels
+// 160 registers per thread at launch, re-divided into 192 per worker and 96 per aux / producer thread (the worker
+// code needs about 190: 176 spills twelve registers and costs 3.5 %).  Registers are allocated per SM sub-partition:
+// each holds three of the block's warps, 15 360 of its 16 384 registers, so the 4096 registers the block leaves free
+// on an SM are 4 x 1024 -- nothing above 32 registers per thread is ever resident beside it.
+__global__ void __maxnreg__(160)
     fused_xpull_kernel(const __grid_constant__ WsArgs a, const __grid_constant__ CUtensorMap map_main,
                        const __grid_constant__ CUtensorMap map_row, const __grid_constant__ CUtensorMap map_pm,
                        const __grid_constant__ CUtensorMap map_pr) {

@@ -518,7 +518,8 @@ void swap_geometry_sets(hhrr_lattice* L) {
 }
 
 // Look-ahead: geometry(step + 1) depends on the step count only (rigid rotation).  Both passes are
-// queued on the low-priority side stream while the collide-stream kernel of `step` runs, and write the
+// queued on the side stream behind the launch of the collide-stream kernel of `step` (they get SMs from its last
+// wave of blocks on, and then share the machine with the wall model), and write the
 // ALTERNATE geometry set (flags, porosity, lists, counters), which nothing of `step` reads; hhrr_step swaps the
 // sets when it reaches step + 1.  The one thing that depends on the step in between -- whether a cell of
 // W_{n+1} holds wall-model state -- is the WM_VALID bit, left 0 here and set by that step's wall-model kernel

@@ -80,10 +80,12 @@ struct hhrr_lattice {
   hhrr_params p;
   hhrr::Dom dom;
   cudaStream_t stream;
-  // Side stream (low priority) and its ordering events.  Two things run there, beside the collide-stream
-  // kernel of the main stream: the WHOLE porosity update of the next step (geometry.cu: launch_geometry_ahead;
-  // a function of the step count only) into the alternate geometry set, and the force / torque
-  // collection of the step just streamed (wallmodel.cu: launch_forces), which only reads.
+  // Side stream (lowest priority, which is also the default's) and its ordering events.  Two things are queued there
+  // behind the launch of the collide-stream kernel: the WHOLE porosity update of the next step (geometry.cu:
+  // launch_geometry_ahead; a function of the step count only) into the alternate geometry set, and the
+  // force / torque collection of the step just streamed (wallmodel.cu: launch_forces), which only reads.  They get SMs
+  // from the collide-stream kernel's last wave of blocks on -- the block scheduler gives a grid of equal priority no SM
+  // before the last block of the grid ahead of it is placed -- and then share the machine with the wall model.
   cudaStream_t side;
   cudaEvent_t ev_pre, ev_k1, ev_k2, ev_side, ev_f[2];  // ev_f[n & 1]: force kernel of step n has read its populations
   int64_t ahead_step;   // step whose geometry the alternate set holds (or is being written with); -1: none

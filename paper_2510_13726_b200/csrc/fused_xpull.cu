@@ -84,6 +84,14 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map
       ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar)
       : "memory");
 }
+__device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* map, int c0, int c1, int c2, int c3) {
+  asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];" ::"l"(map), "r"(c0), "r"(c1),
+               "r"(c2), "r"(c3)
+               : "memory");
+}
+#ifndef HHRR_PF
+#define HHRR_PF 0
+#endif
 // register reallocation between warpgroups: 256 * 192 + 128 * 96 = 384 * 160 (the launch allocation)
 template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
@@ -191,6 +199,15 @@ __global__ void __maxnreg__(160)
     const int xl = edge_l ? dm.nx - 1 : x0 - 1, xr = edge_r ? 0 : x0 + TX;  // real x of the halo columns
     for (int p = pfirst; p <= plast; ++p) {
       const int it = p - pfirst, s = it % NS, k = it / NS;
+      if (HHRR_PF >= 0 && lane == 0 && p + HHRR_PF <= plast && (HHRR_PF > 0 || k > 0)) {
+        bool f2_, ok2_;
+        const int zq = virt_ws(p + HHRR_PF, dm.nz, dm.mode[2], f2_, ok2_);
+        tma_prefetch_4d(&map_main, x0 - 4, y0, zq, 0);
+        if (!bulk) {
+          tma_prefetch_4d(&map_row, x0 - 4, ym, zq, 0);
+          tma_prefetch_4d(&map_row, x0 - 4, yp, zq, 0);
+        }
+      }
       if (k > 0) mbar_wait(empty0 + 8 * s, (k - 1) & 1);
       bool fz, okz;
       const int zr = virt_ws(p, dm.nz, dm.mode[2], fz, okz);

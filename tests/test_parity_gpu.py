@@ -699,3 +699,38 @@ def test_zz_report_utau_error():
     """Not a check of its own: prints the largest relative u_tau difference the parity tests of this module saw."""
     if UTAU_ERR:
         print(f"u_tau: max relative difference over {len(UTAU_ERR)} comparisons: {max(UTAU_ERR):.3e}")
+
+
+def test_degenerate_rotor_cases(oracle):
+    """Degenerate cases of the rotor path: a rotor that lies wholly outside the lattice (empty rotor box, empty lists,
+    wall model enabled with nothing to do), a rotor at rest (Omega = 0: a static body described as a rotor) and the
+    wall model enabled on a lattice without any body -- geometry bit-exact after every step, flow / u_tau / forces at
+    1e-5.  And a rotor whose surface moves more than a cell per step, so that the row band of PAPER.md:269 does not
+    apply and every row of the box is evaluated: no lattice Boltzmann flow survives a tip at Mach 4, so there only
+    the geometry -- a function of the step count alone -- is compared, bit for bit, over three steps."""
+    import dataclasses
+    base = I.case_rotor(128, 72, 72, 20.0, 4, omega=0.012)
+    away = dataclasses.replace(base, name="rotor-away", rotor=dict(base.rotor, centre=(-400.0, 35.5, 35.5)))
+    rest = dataclasses.replace(base, name="rotor-rest", rotor=dict(base.rotor, omega=0.0, theta0=0.4))
+    rho, u = I.noisy_uniform(128, 24, 16, (0.03, 0.01, -0.02), 2e-3, 5)
+    bare = I.Case("no-body", 128, 24, 16, 4, params=dict(I.DEFAULTS, tau0=0.55), rho=rho, u=u, with_neq=True,
+                  wall_model=True)
+    for case in (away, rest, bare):
+        for variant in (5, 2):
+            run_parity(oracle, case, 4, variant, TOL10, check_every=1)
+    G = _gpu_lattice(away, 5)
+    G.step(2)
+    t, g, d = G.cell_types()
+    assert not np.any((t == 2) | (t == 3)) and len(G.wall_list()[0]) == 0 and np.all(G.forces()[:, 1:] == 0)
+    G.close()
+    fast = dataclasses.replace(base, name="rotor-fast", rotor=dict(base.rotor, omega=0.11))
+    G, Oa = _gpu_lattice(fast, 5), _ora_lattice(oracle, fast)
+    for _ in range(3):
+        for L in (G, Oa):
+            L.update_geometry()
+        (tg, gg, dg), (to, go, do) = G.cell_types(), Oa.cell_types()
+        assert np.array_equal(tg, to) and np.array_equal(gg, go) and np.max(np.abs(dg.astype(np.float64) - do)) <= 1e-7
+        wg, wo = G.wall_list(), Oa.wall_list()
+        assert np.array_equal(wg[0], wo[0]) and np.max(np.abs(wg[1] - wo[1])) <= 1e-12
+        G.step(1); Oa.step(1)
+    G.close(); Oa.close()

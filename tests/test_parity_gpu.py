@@ -734,3 +734,27 @@ def test_degenerate_rotor_cases(oracle):
         assert np.array_equal(wg[0], wo[0]) and np.max(np.abs(wg[1] - wo[1])) <= 1e-12
         G.step(1); Oa.step(1)
     G.close(); Oa.close()
+
+
+def test_lattice_on_a_stream_of_its_own():
+    """The library works on the stream it was created with (include/hhrr.h): a lattice on a non-default stream, with
+    another lattice stepping on the default stream in between, gives the populations, wall-model state and forces of
+    a lattice that runs alone -- bit for bit (rotor recipe: look-ahead and force collection on the side stream)."""
+    import torch
+    from paper_2510_13726_b200 import binding as B
+    case = I.case_rotor(128, 72, 72, 20.0, 8, omega=0.012)
+    ref = _gpu_lattice(case, 5)
+    ref.step(3); ref.step(5)
+    s = torch.cuda.Stream()
+    p = B.make_params(case.nx, case.ny, case.nz, mode=case.mode, **case.params)
+    own = B.Lattice(p, rotor_shape=case.rotor["sdf"].shape, stream=s)
+    own.set_kernel_variant(5)
+    I.apply_case(case, own)
+    other = _gpu_lattice(I.case_channel(128, 48, 16, 4), 5)     # shares the device, runs on the default stream
+    own.step(3); other.step(2); own.step(5); other.step(2)
+    assert np.array_equal(own.populations(), ref.populations())
+    a, b = own.wall_model_state(), ref.wall_model_state()
+    oa, ob = np.argsort(a[0]), np.argsort(b[0])
+    assert all(np.array_equal(x[oa], y[ob]) for x, y in zip(a, b))
+    assert np.allclose(own.forces(), ref.forces(), rtol=1e-12, atol=1e-18)
+    own.close(); other.close(); ref.close()
